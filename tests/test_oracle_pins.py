@@ -1,0 +1,269 @@
+"""Pins of the CPU oracle: what the paper and the mathematics fix.
+
+The paper prints no value of I(n,k) (PAPER.md has no worked numeric example), so the oracle is
+pinned by brute force on tiny inputs, closed forms, invariants and special cases that reduce to a
+library routine.  None of these tests touches the CUDA path.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from ephc_inputs import make_problem, fermi_dirac, bose_einstein
+from oracle import brute
+from helpers import exact_energy_problem, manual_problem
+
+HBAR = 0.6582119569
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    p = make_problem("tiny")
+    return p, oracle.OracleList(p)
+
+
+@pytest.fixture(scope="module")
+def small_win():
+    # 4x4x4, 2 bands, 3 modes, a window that cuts states out, a g2 cut-off, low hw so that q=0 diagonals exist
+    p = make_problem("tiny", grid=(4, 4, 4), window=(0.08, 0.22), seed=99)
+    p.g2_cut = float(np.quantile(p.g2, 0.2))
+    p.hw[...] = p.hw * 0.5                                   # hw in [2.5, 30) meV, still even in q
+    p.N = bose_einstein(p.hw, 300.0).reshape(-1)
+    return p, oracle.OracleList(p)
+
+
+# ----------------------------------------------------------------------------- P0: brute force
+def test_p0_list_equals_brute_force_tiny(tiny):
+    p, L = tiny
+    IB = L.collision(p.f, p.N)
+    IA, nterms = brute.collision_brute(p, p.f, p.N)
+    assert nterms == 2 * L.nch + L.ndiag                       # every channel = two ordered terms
+    assert np.abs(IA - IB).max() <= 1e-13 * np.abs(IA).max()
+    assert 3e5 < L.nch < 7e5                                   # ~5e5 unordered channels
+
+
+def test_p0_list_equals_brute_force_window_cut_diag(small_win):
+    p, L = small_win
+    assert p.nk < 64 and L.ndiag > 0 and L.nch > 100
+    IA, nterms = brute.collision_brute(p, p.f, p.N)
+    assert nterms == 2 * L.nch + L.ndiag
+    IB = L.collision(p.f, p.N)
+    assert np.abs(IA - IB).max() <= 1e-13 * np.abs(IA).max()
+    # out-of-window states never receive a contribution
+    out = ~((p.E.reshape(-1) >= p.emin) & (p.E.reshape(-1) <= p.emax))
+    assert out.any() and np.all(IB[out] == 0.0)
+
+
+def test_sampled_definition_equals_list(small_win, tiny):
+    for p, L in (small_win, tiny):
+        IB = L.collision(p.f, p.N)
+        st = np.arange(0, p.ns, max(1, p.ns // 37), dtype=np.int32)
+        Is = oracle.collision_sampled(p, p.f, p.N, st)
+        assert np.abs(Is - IB[st]).max() <= 1e-13 * np.abs(IB).max()
+
+
+def test_canonical_list_structure(tiny):
+    p, L = tiny
+    ch = L.export()
+    key = np.stack([ch["ik"], ch["ikq"], ch["nu"], ch["m"], ch["n"]]).astype(np.int64)
+    # strictly increasing lexicographic order (ik, ikq, nu, m, n): unique and sorted
+    d = np.diff(key, axis=1)
+    first = (d != 0).argmax(axis=0)
+    assert np.all(d[first, np.arange(d.shape[1])] > 0)
+    assert np.all((ch["ik"] < ch["ikq"]) | ((ch["ik"] == ch["ikq"]) & (ch["n"] < ch["m"])))
+    assert np.all((ch["w_abs"] > 0) | (ch["w_em"] > 0))
+    # q index: kfull[ikq] - kfull[ik] on the 8x8x8 grid (all k active, kfull = identity)
+    n = 8
+    kf, kqf = ch["ik"].astype(np.int64), ch["ikq"].astype(np.int64)
+    q = [((kqf // (n * n) - kf // (n * n)) % n), (((kqf // n) % n - (kf // n) % n) % n), ((kqf % n - kf % n) % n)]
+    assert np.array_equal(ch["iq"], (q[0] * n + q[1]) * n + q[2])
+
+
+# ----------------------------------------------------------------------------- P1: one channel by hand
+def test_p1_single_channel_worked_example():
+    # tests/golden/p1_single_channel.txt: Eq. 2 for one absorption channel with exact energy
+    vals = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "p1_single_channel.txt")) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split("=")
+                vals[k.strip()] = float(v)
+    hw = 0.03
+    p = manual_problem((1, 1, 1), E=[[0.0, hw]], hw=[[hw]], pairs=[(0, 0)], g2=[[[[0.0, 1e-4], [1e-4, 0.0]]]],
+                       sigma=0.010, f=[0.5, 0.25], N=[1.0])
+    L = oracle.OracleList(p)
+    assert L.nch == 1 and L.ndiag == 0
+    ch = L.export()
+    assert (ch["n"][0], ch["m"][0]) == (0, 1) and ch["w_em"][0] == 0.0
+    I = L.collision(p.f, p.N)
+    assert I[0] == pytest.approx(vals["I_a"], rel=1e-11)
+    assert I[1] == -I[0]
+    # the same number from the formula, written out: -(2 pi/hbar) g2 delta_sigma(0) F_abs
+    expect = -(2 * math.pi / HBAR) * 1e-4 * (1.0 / (0.010 * math.sqrt(2 * math.pi))) * 0.125
+    assert I[0] == pytest.approx(expect, rel=1e-14)
+
+
+# ----------------------------------------------------------------------------- P2: f == c closed form
+def test_p2_constant_occupation_closed_form(tiny):
+    p, L = tiny
+    ch = L.export()
+    a = ch["ik"] * p.nb + ch["n"]
+    b = ch["ikq"] * p.nb + ch["m"]
+    # ordered terms of a: (w_abs, w_em); of b (mirror): (w_em, w_abs)  ->  I_s = -c(1-c) * S_s
+    S = np.zeros(p.ns)
+    np.add.at(S, a, ch["w_em"] - ch["w_abs"])
+    np.add.at(S, b, ch["w_abs"] - ch["w_em"])
+    for c in (0.3, 0.9):
+        for Nscale in (1.0, 3.0):                      # independent of N
+            I = L.collision(np.full(p.ns, c), p.N * Nscale)
+            assert np.abs(I + c * (1 - c) * S).max() <= 1e-12 * np.abs(c * (1 - c) * S).max()
+    assert np.all(L.collision(np.zeros(p.ns), p.N) == 0.0)
+    assert np.abs(L.collision(np.ones(p.ns), p.N)).max() <= 1e-18
+
+
+# ----------------------------------------------------------------------------- P3: particle number
+def test_p3_particle_number_conservation(tiny, small_win):
+    rng = np.random.default_rng(5)
+    for p, L in (tiny, small_win):
+        for _ in range(2):
+            f = rng.uniform(0, 1, p.ns)
+            N = rng.uniform(0, 3, p.nq * p.nnu)
+            I = L.collision(f, N)
+            assert abs(I.sum()) <= 1e-13 * np.abs(I).sum()
+            assert np.abs(I).max() > 0
+
+
+# ----------------------------------------------------------------------------- P4: detailed balance
+def test_p4_detailed_balance_on_exact_energy_channels():
+    p = exact_energy_problem()
+    L = oracle.OracleList(p)
+    assert L.nch > 500
+    ch = L.export()
+    # every surviving delta has argument exactly zero: weight = C g2 / (sigma sqrt(2 pi))
+    I_eq = L.collision(p.f, p.N)
+    scale = np.zeros(p.ns)
+    a = ch["ik"] * p.nb + ch["n"]
+    b = ch["ikq"] * p.nb + ch["m"]
+    np.add.at(scale, a, ch["w_abs"] + ch["w_em"])
+    np.add.at(scale, b, ch["w_abs"] + ch["w_em"])
+    assert np.abs(I_eq).max() <= 1e-14 * scale.max()
+    # ... and it is not zero away from equilibrium (the pin would pass trivially otherwise)
+    f2 = p.f.copy(); f2[::3] *= 0.5
+    assert np.abs(L.collision(f2, p.N)).max() > 1e-3 * scale.max() * 0.01
+    # wrong phonon temperature breaks it
+    N2 = bose_einstein(p.hw, 800.0).reshape(-1)
+    assert np.abs(L.collision(p.f, N2)).max() > 1e-6 * scale.max()
+    IA, _ = brute.collision_brute(p, p.f, p.N)
+    assert np.abs(IA).max() <= 1e-14 * scale.max()
+
+
+# ----------------------------------------------------------------------------- P5: structure
+def test_p5_quadratic_in_f_linear_in_g2(small_win):
+    p, L = small_win
+    rng = np.random.default_rng(11)
+    d = rng.uniform(-0.05, 0.05, p.ns)
+    I = [L.collision(p.f + t * d, p.N) for t in range(4)]
+    third = I[0] - 3 * I[1] + 3 * I[2] - I[3]
+    second = I[0] - 2 * I[1] + I[2]
+    assert np.abs(second).max() > 1e-9 * np.abs(I[0]).max()          # genuinely quadratic
+    assert np.abs(third).max() <= 1e-12 * np.abs(I[0]).max()
+    p2 = make_problem("tiny", grid=(4, 4, 4), window=(0.08, 0.22), seed=99)
+    p2.hw[...] = p.hw; p2.N = p.N; p2.g2 = p.g2 * 2.0; p2.g2_cut = p.g2_cut * 2.0
+    assert np.array_equal(oracle.OracleList(p2).collision(p.f, p.N), 2.0 * I[0])   # power of two: bit exact
+
+
+# ----------------------------------------------------------------------------- P6: Gamma = -dI_a/df_a
+def test_p6_gamma_is_minus_diagonal_derivative(small_win):
+    p, L = small_win
+    G = L.transport_setup(p.f0, p.N)
+    h = 1e-3
+    rng = np.random.default_rng(3)
+    inw = np.nonzero(G > 0)[0]
+    for s in rng.choice(inw, size=12, replace=False):
+        fp, fm = p.f0.copy(), p.f0.copy()
+        fp[s] += h; fm[s] -= h
+        dIds = (L.collision(fp, p.N)[s] - L.collision(fm, p.N)[s]) / (2 * h)   # exact for a quadratic
+        # the q=0, n==m diagonal term enters Gamma_a but cancels in I (W_aa F_a on both sides): remove it
+        dg = L.export_diag()
+        Wd = 0.0
+        for j in np.nonzero(dg["s"] == s)[0]:
+            Nq = p.N[dg["iq"][j] * p.nnu + dg["nu"][j]]
+            Wd += dg["w_em"][j] * (1 + Nq - p.f0[s]) + dg["w_abs"][j] * (Nq + p.f0[s])
+        assert -dIds == pytest.approx(G[s] - Wd, rel=1e-9)
+
+
+# ----------------------------------------------------------------------------- P7: transport
+def test_p7_transport_iteration_is_dense_matvec(small_win):
+    p, L = small_win
+    W = brute.transport_matrix_brute(p, p.f0, p.N)
+    G = L.transport_setup(p.f0, p.N)
+    assert np.abs(W.sum(axis=1) - G).max() <= 1e-13 * G.max()
+    tau = np.where(G > 0, 1.0 / np.where(G > 0, G, 1.0), 0.0)
+    rng = np.random.default_rng(8)
+    F = rng.normal(size=(3, p.ns)); v = rng.normal(size=(3, p.ns))
+    Fo = L.transport_iter(p.f0, p.N, F, v, tau)
+    ref = tau[None, :] * (v + F @ W.T)
+    assert np.abs(Fo - ref).max() <= 1e-12 * np.abs(ref).max()
+    # F == const c  =>  F' = tau v + c  on every state that scatters (row sums of W are Gamma)
+    c = 0.37
+    Fc = L.transport_iter(p.f0, p.N, np.full((3, p.ns), c), v, tau)
+    on = G > 0
+    assert np.abs(Fc[:, on] - (tau[on] * v[:, on] + c)).max() <= 1e-12
+
+
+def test_p7_detailed_balance_symmetry_of_W():
+    p = exact_energy_problem(seed=21)
+    W = brute.transport_matrix_brute(p, p.f, p.N)
+    w = p.f * (1 - p.f)
+    A = W * w[:, None]            # W(a<-b) f0_a (1 - f0_a) = W(b<-a) f0_b (1 - f0_b)
+    assert np.abs(A - A.T).max() <= 1e-13 * np.abs(A).max() and np.abs(A).max() > 0
+    L = oracle.OracleList(p)
+    G = L.transport_setup(p.f, p.N)
+    assert np.abs(W.sum(axis=1) - G).max() <= 1e-13 * G.max()
+
+
+# ----------------------------------------------------------------------------- P8: two-state logistic
+def _two_state(f_a, f_b, Nph):
+    hw = 0.03
+    p = manual_problem((1, 1, 1), E=[[0.0, hw]], hw=[[hw]], pairs=[(0, 0)], g2=[[[[0.0, 4e-3], [4e-3, 0.0]]]],
+                       sigma=0.010, f=[f_a, f_b], N=[Nph])
+    return p, oracle.OracleList(p)
+
+
+def _logistic(fa0, c, Nph, R, t):
+    # df/dt = R (f - r1)(f - r2),  r1,2 roots of f^2 - (2N+1+c) f + c(N+1)
+    bq = 2 * Nph + 1 + c
+    disc = math.sqrt(bq * bq - 4 * c * (Nph + 1))
+    r1, r2 = (bq - disc) / 2, (bq + disc) / 2
+    K = (fa0 - r1) / (fa0 - r2)
+    e = K * math.exp(R * (r1 - r2) * t)
+    return (r1 - r2 * e) / (1 - e)
+
+
+def test_p8_rk4_two_state_closed_form():
+    fa0, fb0, Nph = 0.8, 0.1, 0.6
+    p, L = _two_state(fa0, fb0, Nph)
+    R = L.export()["w_abs"][0]
+    assert R == pytest.approx((2 * math.pi / HBAR) * 4e-3 / (0.010 * math.sqrt(2 * math.pi)), rel=1e-14)
+    T = 2.0   # fs; R ~ 1.5 / fs, so the relaxation is well under way
+    errs = []
+    for nsteps in (20, 40, 80):
+        f, sumf = L.rt_step(p.f, p.N, T / nsteps, nsteps)
+        exact = _logistic(fa0, fa0 + fb0, Nph, R, T)
+        errs.append(abs(f[0] - exact))
+        assert f[0] + f[1] == pytest.approx(fa0 + fb0, abs=1e-15)
+        assert np.abs(sumf - (fa0 + fb0)).max() <= 1e-15
+    assert errs[0] < 1e-4 and 12 < errs[0] / errs[1] < 20 and 12 < errs[1] / errs[2] < 20   # 4th order
+    assert abs(fa0 - _logistic(fa0, fa0 + fb0, Nph, R, T)) > 0.05
+
+
+# ----------------------------------------------------------------------------- P9: conservation over many steps
+def test_p9_rt_conserves_particle_number_and_is_reproducible(small_win):
+    p, L = small_win
+    f1, s1 = L.rt_step(p.f, p.N, 1.0, 200)
+    f2, s2 = L.rt_step(p.f, p.N, 1.0, 200)
+    assert np.array_equal(f1, f2) and np.array_equal(s1, s2)
+    assert np.abs(s1 - s1[0]).max() <= 1e-12 * abs(s1[0])
+    assert np.abs(f1 - p.f).max() > 1e-4          # the state did evolve
