@@ -1,0 +1,168 @@
+/*
+ * ephc.h -- C ABI of the B200-native electron-phonon collision-integral library
+ *           (hot path of arxiv 2511.03683; citations are PAPER.md:LINE).
+ *
+ * What the library computes
+ * -------------------------
+ *   PAPER.md:51 (II.B, Eq. 2)   I(n,k) = -(2 pi/hbar)(1/N_q) sum_{m,q,nu} |g_mn,nu(k,q)|^2
+ *                                  [ delta(e_nk - e_mk+q + hw_nu,q) F_abs + delta(e_nk - e_mk+q - hw_nu,q) F_em ]
+ *   PAPER.md:60 (II.B)          channel selection: energy window, Gaussian delta, |g| cut-off
+ *   PAPER.md:94, 102 (II.C.2)   every channel feeds I(n,k) and I(m,k+q) with opposite signs; one owner
+ *                               per element of I, no atomics
+ *   PAPER.md:110 (II.C.2)       transport: same channel loop, the two sides are not +-equal, loop over the
+ *                               three field directions
+ *   PAPER.md:41-45 (II.A, Eq.1) rt-BTE: df/dt = I[f], one collision evaluation per (sub)step
+ * Readings of the points on which the paper is silent (F_abs/F_em, Gaussian normalisation, truncation,
+ * units, transport equation, integrator) are listed in DESIGN.md section "Readings" (R-1..R-24).
+ *
+ * Conventions
+ * -----------
+ *   units: eV, fs; I in 1/fs; hbar = 0.6582119569 eV fs.
+ *   full-grid linear index i = (i1*N2 + i2)*N3 + i3; k+q is component-wise modulo the grid;
+ *   iq = index of (k' - k) mod grid.  State index s = ik*nb + n (ik = compact index of an active k).
+ *   f, I, Gamma, tau: [ns = nk*nb] doubles.  N: [nq*nnu] doubles on the full q grid (nq = N1*N2*N3).
+ *   F, v, Fout: [3][ns] doubles (component-major).
+ *   Preconditions (not checked): hw(-q) = hw(q), N(-q) = N(q), g2 Hermitian (one value per unordered entry).
+ *
+ * Ownership / memory spaces
+ * -------------------------
+ *   ephc_problem arrays are HOST pointers, borrowed for the duration of ephc_build_channels only.
+ *   The handle owns the channel store in device memory (HBM) and a host copy of the canonical list.
+ *   Every pointer named *_dev is a caller-owned DEVICE buffer of doubles (8-byte aligned), borrowed for
+ *   the call; `stream` is a cudaStream_t passed as void* (NULL = default stream).  Device entry points only
+ *   enqueue work: they do not allocate, synchronise or touch the host.  Every pointer named *_host is a
+ *   caller-owned HOST buffer; the *_host entry points copy in, run the same kernels, copy out and
+ *   synchronise the stream before returning.
+ *
+ * Errors
+ * ------
+ *   All functions return 0 on success and a negative EPHC_E* code on failure; ephc_last_error() returns a
+ *   thread-local, human-readable message for the last failure.  There is no CPU fallback: without a CUDA
+ *   device every compute entry point fails with EPHC_ECUDA.
+ */
+#ifndef EPHC_H
+#define EPHC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EPHC_OK 0
+#define EPHC_EINVAL (-1)  /* null pointer, bad size, non-finite input, hw <= 0, index out of range, bad pair list */
+#define EPHC_ENOMEM (-2)  /* host or device allocation failed */
+#define EPHC_ECUDA (-3)   /* CUDA runtime error (includes "no device") */
+#define EPHC_ESTATE (-4)  /* call order: transport_iter before transport_setup, host-only handle, ... */
+#define EPHC_ELIMIT (-5)  /* problem exceeds a format limit (nb > 16, nnu > 64, > 2^31-1 states or pairs) */
+
+/* flags of ephc_problem.flags */
+#define EPHC_HOST_ONLY 1u /* build the store on the host only (no device needed): query/export work, compute fails */
+
+typedef struct ephc_handle ephc_handle;
+
+/* Input of channel selection.  All arrays on the host. */
+typedef struct ephc_problem {
+    int32_t grid[3];         /* N1, N2, N3 of the commensurate k/q grid */
+    int32_t nk;              /* number of active k points (>= 1) */
+    int32_t nb;              /* bands, 1..16 */
+    int32_t nnu;             /* phonon modes, 1..64 */
+    uint32_t flags;          /* EPHC_HOST_ONLY or 0 */
+    const int32_t *kfull;    /* [nk] full-grid index of each active k, strictly ascending */
+    const double *E;         /* [nk*nb] band energies, eV */
+    double emin, emax;       /* energy window, inclusive; a channel needs both end states inside */
+    const double *hw;        /* [nq*nnu] phonon energies on the full q grid, eV, > 0 */
+    double sigma;            /* Gaussian smearing (standard deviation), eV, > 0 */
+    double ncut;             /* a delta is kept iff |argument| < ncut*sigma (3.0 in all configs) */
+    double g2_cut;           /* a channel is kept iff g2 >= g2_cut */
+    int64_t npair;           /* number of candidate (k,k') pairs */
+    const int32_t *pair_ik;  /* [npair] compact index of k; pairs strictly ascending in (ik, ikq), ik <= ikq */
+    const int32_t *pair_ikq; /* [npair] compact index of k' = k+q */
+    const double *g2;        /* [npair*nnu*nb*nb] |g|^2 in eV^2, index ((p*nnu+nu)*nb+m)*nb+n,
+                                n = band at pair_ik, m = band at pair_ikq; self pairs symmetric in (m,n) */
+} ephc_problem;
+
+typedef struct ephc_counts {
+    int64_t ns;            /* states = nk*nb */
+    int64_t npair_active;  /* candidate pairs with at least one active channel (diagonal-only pairs included) */
+    int64_t nch;           /* unordered active channels N_ch (the metric's unit) */
+    int64_t nw;            /* non-zero delta weights N_w, N_ch <= N_w <= 2 N_ch */
+    int64_t ndiag;         /* q=0, n==m terms (transport only) */
+    int64_t gather_entries;   /* ordered entries of the destination-sorted (two-sided) store */
+    int64_t gather_halfpairs; /* (k <- k') half-pair rows of that store */
+    int64_t scatter_entries;  /* entries of the once-stored (one-sided) store */
+    int64_t scatter_pairs;
+    int64_t store_bytes_gather;   /* device bytes of the two-sided store (collision + transport share it) */
+    int64_t store_bytes_scatter;  /* device bytes of the one-sided store incl. its transposed index */
+    int64_t store_bytes_transport;/* device bytes of the per-entry transport weights (0 before transport_setup) */
+    int64_t alg_bytes_collision;  /* B_alg of one collision evaluation */
+    int64_t alg_bytes_transport;  /* B_alg of one transport iteration */
+    int32_t n_workunits, n_rounds, n_tasks; /* launch geometry of the gather kernels */
+    int32_t reserved;
+} ephc_counts;
+
+/* Channel selection + store construction ("performed only once on CPUs").
+ * Validates the problem (EPHC_EINVAL / EPHC_ELIMIT), builds the canonical unordered channel list
+ * [(ik<ikq) or (ik==ikq and n<m), sorted by (ik, ikq, nu, m, n)], the destination-k-segmented stores and
+ * the transposed index, and uploads them.  *out receives the handle (NULL on failure). */
+int ephc_build_channels(const ephc_problem *p, ephc_handle **out);
+
+int ephc_query(const ephc_handle *h, ephc_counts *out);
+
+/* Canonical channel list, host arrays of length nch each (any pointer may be NULL to skip it).
+ * w_abs / w_em = (2 pi / (hbar nq)) * g2 * delta_sigma(E_a - E_b +/- hw), exactly 0 when that delta is cut. */
+int ephc_export_channels(const ephc_handle *h, int32_t *ik, int32_t *ikq, int32_t *iq, int32_t *n,
+                         int32_t *m, int32_t *nu, double *w_abs, double *w_em);
+/* q=0, n==m terms: state index, iq (always the q=0 index), nu, weights; length ndiag each. */
+int ephc_export_diag(const ephc_handle *h, int32_t *s, int32_t *iq, int32_t *nu, double *w_abs, double *w_em);
+
+/* Decoded image of the two-sided (gather) store, for structural tests of the host builder; only available on
+ * handles built with EPHC_HOST_ONLY.  Arrays of length gather_entries (any may be NULL), in store order:
+ * destination state, partner state, canonical iq, mode, kind (0: F_abs, 1: F_em as seen from the destination),
+ * diagonal flag, weight.  Walks work units -> rounds -> tasks exactly as the kernels do. */
+int ephc_export_gather(const ephc_handle *h, int32_t *dest, int32_t *partner, int32_t *iq, int32_t *nu,
+                       int32_t *kind, int32_t *diag, double *w);
+
+/* Choice of collision algorithm for ephc_collision / ephc_rt_step:
+ *   0 = gather  : destination-sorted two-sided store, one kernel, every ordered term read once
+ *   1 = scatter : once-stored channels, forward segmented reduce + per-pair reverse partials gathered
+ *                 through the transposed index (PAPER.md:88-102 restructured; no global atomics) */
+int ephc_set_variant(ephc_handle *h, int variant);
+
+/* I[s] = collision integral of Eq. 2 for occupations f and phonon occupations N. */
+int ephc_collision(ephc_handle *h, const double *f_dev, const double *N_dev, double *I_dev, void *stream);
+
+/* Linearised-BTE scattering-in weights about equilibrium f0 (reading R-16):
+ * W(a<-b) = w_em (1 + N - f0_b) + w_abs (N + f0_b) per ordered term, kept in the handle;
+ * Gamma[a] = sum_b W(a<-b). */
+int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const double *N_dev, double *Gamma_dev,
+                         void *stream);
+/* One iteration Fout[al][a] = tau[a] * ( v[al][a] + sum_b W(a<-b) F[al][b] ), al = x,y,z. */
+int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
+                        double *Fout_dev, void *stream);
+
+/* nsteps classical RK4 steps of df/dt = I[f] with N fixed (reading R-18), f updated in place.
+ * sumf_dev (may be NULL): [nsteps+1], sum_s f_s before the first step and after every step.
+ * The axpy of every stage is fused into the collision kernel's epilogue. */
+int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
+                 double *sumf_dev, void *stream);
+
+/* Host-buffer variants (end-to-end path): copy in, run the same kernels, copy out, synchronise. */
+int ephc_collision_host(ephc_handle *h, const double *f_host, const double *N_host, double *I_host);
+/* tau = 1/Gamma (0 where Gamma == 0), F0 = tau*v, then niter iterations; Gamma_host may be NULL. */
+int ephc_transport_solve_host(ephc_handle *h, const double *f0_host, const double *N_host,
+                              const double *v_host, int niter, double *F_host, double *Gamma_host);
+int ephc_rt_step_host(ephc_handle *h, double *f_host, const double *N_host, double dt_fs, int nsteps,
+                      double *sumf_host);
+
+/* Number of kernel launches enqueued by this library since the handle was created (for bench.py). */
+int64_t ephc_launch_count(const ephc_handle *h);
+
+int ephc_destroy(ephc_handle *h);
+const char *ephc_last_error(void);
+const char *ephc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EPHC_H */

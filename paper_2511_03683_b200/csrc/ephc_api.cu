@@ -1,0 +1,485 @@
+// ephc_api.cu -- the C ABI declared in include/ephc.h: handle, uploads, kernel launches, error reporting.
+// Product code: shares nothing with oracle/.  No CPU fallback: compute entry points need a CUDA device.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ephc_internal.h"
+#include "ephc_kernels.cuh"
+
+using namespace ephc;
+
+static thread_local std::string g_err;
+
+static int fail(int code, const std::string &msg) {
+    g_err = msg;
+    return code;
+}
+#define CUDA_TRY(expr)                                                                            \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(EPHC_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));          \
+    } while (0)
+
+struct ephc_handle {
+    Dims d{};
+    bool host_only = false;
+    int variant = 0;
+    Canonical can;
+    GatherHost ghost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_gather)
+    std::vector<int32_t> pair_ik, pair_ikq;  // copy of the candidate pair list (export)
+    // gather store: counts
+    int64_t g_entries = 0, g_halfpairs = 0;
+    int32_t n_wu = 0, n_rounds = 0, n_tasks = 0;
+    // device image
+    uint32_t *d_code = nullptr;
+    double *d_w = nullptr;
+    int32_t *d_hp_k = nullptr, *d_hp_q = nullptr;
+    Task *d_tasks = nullptr;
+    Round *d_rounds = nullptr;
+    WorkUnit *d_wus = nullptr;
+    double *d_gW = nullptr;      // transport weights, allocated by transport_setup
+    bool transport_ready = false;
+    // scratch for rt_step / host variants (allocated lazily, freed in destroy)
+    double *d_y[2] = {nullptr, nullptr}, *d_ksum = nullptr, *d_wusum = nullptr;
+    double *d_hf = nullptr, *d_hN = nullptr, *d_hI = nullptr;  // host-variant staging: f, N, I
+    double *d_tr[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // Gamma, tau, v, F, F'
+    double *d_sumf = nullptr;
+    int64_t sumf_cap = 0;
+    int64_t launches = 0;
+    int64_t bytes_gather = 0, bytes_transport = 0;
+    bool attrs_set = false;
+};
+
+static void free_dev(ephc_handle *h) {
+    void *ptrs[] = {h->d_code, h->d_w, h->d_hp_k, h->d_hp_q, h->d_tasks, h->d_rounds, h->d_wus, h->d_gW,
+                    h->d_y[0], h->d_y[1], h->d_ksum, h->d_wusum, h->d_hf, h->d_hN, h->d_hI, h->d_tr[0],
+                    h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+}
+
+template <class T>
+static int upload(T **dst, const std::vector<T> &src, int64_t *bytes) {
+    const size_t n = src.size() * sizeof(T);
+    CUDA_TRY(cudaMalloc((void **)dst, n > 0 ? n : sizeof(T)));
+    if (n) CUDA_TRY(cudaMemcpy(*dst, src.data(), n, cudaMemcpyHostToDevice));
+    *bytes += (int64_t)n;
+    return EPHC_OK;
+}
+
+extern "C" const char *ephc_last_error(void) { return g_err.c_str(); }
+extern "C" const char *ephc_version(void) { return "ephc 0.1 (sm_100a, fp64)"; }
+
+extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
+    if (out) *out = nullptr;
+    if (!p || !out) return fail(EPHC_EINVAL, "null argument");
+    if (!p->kfull || !p->E || !p->hw || (p->npair > 0 && (!p->pair_ik || !p->pair_ikq || !p->g2)))
+        return fail(EPHC_EINVAL, "null array in ephc_problem");
+    if (p->nk < 1 || p->nb < 1 || p->nnu < 1 || p->npair < 0 || p->grid[0] < 1 || p->grid[1] < 1 || p->grid[2] < 1)
+        return fail(EPHC_EINVAL, "nk, nb, nnu, grid must be >= 1 and npair >= 0");
+    if (p->nb > 16 || p->nnu > 64) return fail(EPHC_ELIMIT, "format limit: nb <= 16, nnu <= 64");
+    const int64_t nq = (int64_t)p->grid[0] * p->grid[1] * p->grid[2];
+    const int64_t ns = (int64_t)p->nk * p->nb;
+    if (nq > 0x7fffffffLL / p->nnu || ns > 0x7fffffffLL || p->npair > 0x7fffffffLL)
+        return fail(EPHC_ELIMIT, "format limit: nq*nnu, nk*nb and npair must fit in 31 bits");
+    if (p->nk > nq) return fail(EPHC_EINVAL, "nk exceeds the number of grid points");
+
+    ephc_handle *h = new (std::nothrow) ephc_handle();
+    if (!h) return fail(EPHC_ENOMEM, "host allocation failed (handle)");
+    h->d.grid[0] = p->grid[0];
+    h->d.grid[1] = p->grid[1];
+    h->d.grid[2] = p->grid[2];
+    h->d.nk = p->nk;
+    h->d.nb = p->nb;
+    h->d.nnu = p->nnu;
+    h->d.nq = nq;
+    h->d.ns = ns;
+    h->d.C = 2.0 * kPi / (kHbar * (double)nq);  // R-8: N_q = points of the full grid
+    h->host_only = (p->flags & EPHC_HOST_ONLY) != 0;
+
+    std::string err;
+    int rc = build_canonical(p, h->d, h->can, err);
+    GatherHost g;
+    if (rc == EPHC_OK) rc = build_gather(p, h->d, h->can, g, err);
+    if (rc != EPHC_OK) {
+        delete h;
+        return fail(rc, err);
+    }
+    h->pair_ik.assign(p->pair_ik, p->pair_ik + p->npair);
+    h->pair_ikq.assign(p->pair_ikq, p->pair_ikq + p->npair);
+    h->g_entries = (int64_t)g.code.size();
+    h->g_halfpairs = (int64_t)g.hp_k.size();
+    h->n_wu = (int32_t)g.wus.size();
+    h->n_rounds = (int32_t)g.rounds.size();
+    h->n_tasks = (int32_t)g.tasks.size();
+    h->bytes_gather = 0;
+    if (!h->host_only) {
+        int dev_count = 0;
+        cudaError_t ce = cudaGetDeviceCount(&dev_count);
+        if (ce != cudaSuccess || dev_count == 0) {
+            delete h;
+            return fail(EPHC_ECUDA, "no CUDA device (pass EPHC_HOST_ONLY to build without one)");
+        }
+        int64_t b = 0;
+        rc = upload(&h->d_code, g.code, &b);
+        if (rc == EPHC_OK) rc = upload(&h->d_w, g.w, &b);
+        if (rc == EPHC_OK) rc = upload(&h->d_hp_k, g.hp_k, &b);
+        if (rc == EPHC_OK) rc = upload(&h->d_hp_q, g.hp_q, &b);
+        if (rc == EPHC_OK) rc = upload(&h->d_tasks, g.tasks, &b);
+        if (rc == EPHC_OK) rc = upload(&h->d_rounds, g.rounds, &b);
+        if (rc == EPHC_OK) rc = upload(&h->d_wus, g.wus, &b);
+        if (rc != EPHC_OK) {
+            free_dev(h);
+            delete h;
+            return rc;
+        }
+        h->bytes_gather = b;
+    } else {
+        h->ghost = g;
+        h->bytes_gather = (int64_t)(g.code.size() * 4 + g.w.size() * 8 + g.hp_k.size() * 8 +
+                                    g.tasks.size() * sizeof(Task) + g.rounds.size() * sizeof(Round) +
+                                    g.wus.size() * sizeof(WorkUnit));
+    }
+    *out = h;
+    return EPHC_OK;
+}
+
+extern "C" int ephc_destroy(ephc_handle *h) {
+    if (!h) return EPHC_OK;
+    if (!h->host_only) free_dev(h);
+    delete h;
+    return EPHC_OK;
+}
+
+extern "C" int ephc_query(const ephc_handle *h, ephc_counts *o) {
+    if (!h || !o) return fail(EPHC_EINVAL, "null argument");
+    std::memset(o, 0, sizeof(*o));
+    o->ns = h->d.ns;
+    o->npair_active = h->can.npair_active;
+    o->nch = h->can.nch;
+    o->nw = h->can.nw;
+    o->ndiag = h->can.ndiag;
+    o->gather_entries = h->g_entries;
+    o->gather_halfpairs = h->g_halfpairs;
+    o->store_bytes_gather = h->bytes_gather;
+    o->store_bytes_transport = h->bytes_transport;
+    // B_alg: every item the method must move once per evaluation.
+    //   8 N_w weights + 4 N_ch channel index + 12 N_pair (ik, ikq, iq) + 16 N_s (read f, write I) + 8 nnu N_q,active
+    int64_t nq_active = 0;
+    {
+        std::vector<uint8_t> seen((size_t)h->d.nq, 0);
+        const int64_t npair = (int64_t)h->pair_ik.size();
+        for (int64_t ip = 0; ip < npair; ++ip)
+            if (h->can.pair_ch0[ip + 1] > h->can.pair_ch0[ip] && !seen[h->can.pair_iq[ip]]) {
+                seen[h->can.pair_iq[ip]] = 1;
+                ++nq_active;
+            }
+    }
+    o->alg_bytes_collision = 8 * h->can.nw + 4 * h->can.nch + 12 * h->can.npair_active + 16 * h->d.ns +
+                             8 * (int64_t)h->d.nnu * nq_active;
+    //   transport: two weights per channel (16 N_ch), index, pairs, F and F' (3 components), v, tau
+    o->alg_bytes_transport = 16 * h->can.nch + 4 * h->can.nch + 12 * h->can.npair_active +
+                             (3 * 8 * 3 + 8) * h->d.ns;
+    o->n_workunits = h->n_wu;
+    o->n_rounds = h->n_rounds;
+    o->n_tasks = h->n_tasks;
+    return EPHC_OK;
+}
+
+extern "C" int ephc_export_channels(const ephc_handle *h, int32_t *ik, int32_t *ikq, int32_t *iq, int32_t *n,
+                                    int32_t *m, int32_t *nu, double *w_abs, double *w_em) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    const int64_t npair = (int64_t)h->pair_ik.size();
+    for (int64_t ip = 0; ip < npair; ++ip)
+        for (int64_t j = h->can.pair_ch0[ip]; j < h->can.pair_ch0[ip + 1]; ++j) {
+            const uint16_t c = h->can.ch_code[j];
+            if (ik) ik[j] = h->pair_ik[ip];
+            if (ikq) ikq[j] = h->pair_ikq[ip];
+            if (iq) iq[j] = h->can.pair_iq[ip];
+            if (n) n[j] = c & 15;
+            if (m) m[j] = (c >> 4) & 15;
+            if (nu) nu[j] = c >> 8;
+            if (w_abs) w_abs[j] = h->can.ch_wabs[j];
+            if (w_em) w_em[j] = h->can.ch_wem[j];
+        }
+    return EPHC_OK;
+}
+
+extern "C" int ephc_export_diag(const ephc_handle *h, int32_t *s, int32_t *iq, int32_t *nu, double *w_abs,
+                                double *w_em) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    for (int64_t j = 0; j < h->can.ndiag; ++j) {
+        if (s) s[j] = h->can.dg_s[j];
+        if (iq) iq[j] = h->can.iq0;
+        if (nu) nu[j] = h->can.dg_nu[j];
+        if (w_abs) w_abs[j] = h->can.dg_wabs[j];
+        if (w_em) w_em[j] = h->can.dg_wem[j];
+    }
+    return EPHC_OK;
+}
+
+extern "C" int ephc_export_gather(const ephc_handle *h, int32_t *dest, int32_t *partner, int32_t *iq, int32_t *nu,
+                                  int32_t *kind, int32_t *diag, double *w) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (!h->host_only) return fail(EPHC_ESTATE, "ephc_export_gather needs a handle built with EPHC_HOST_ONLY");
+    const GatherHost &g = h->ghost;
+    std::vector<uint8_t> seen(g.code.size(), 0);
+    for (const WorkUnit &wu : g.wus)
+        for (int32_t r = wu.r0; r < wu.r1; ++r) {
+            const Round &rd = g.rounds[r];
+            for (int32_t t = rd.t0; t < rd.t0 + rd.nt; ++t) {
+                const Task &tk = g.tasks[t];
+                if (tk.row < wu.row0 || tk.row >= wu.row0 + wu.nrows || tk.len < 1 || tk.len > kTaskLen)
+                    return fail(EPHC_ESTATE, "internal: task outside its work unit");
+                for (int64_t e = tk.e0; e < tk.e0 + tk.len; ++e) {
+                    const uint32_t c = g.code[e];
+                    const uint32_t pl = c & kPairMask;
+                    if (pl >= (uint32_t)rd.nhp || seen[e]) return fail(EPHC_ESTATE, "internal: bad pair index / entry visited twice");
+                    seen[e] = 1;
+                    if (dest) dest[e] = tk.row;
+                    if (partner) partner[e] = g.hp_k[rd.hp0 + pl] * h->d.nb + (int32_t)((c >> kBandShift) & 15);
+                    if (iq) iq[e] = g.hp_q[rd.hp0 + pl];
+                    if (nu) nu[e] = (int32_t)((c >> kModeShift) & 63);
+                    if (kind) kind[e] = (int32_t)((c >> kKindBit) & 1);
+                    if (diag) diag[e] = (int32_t)(c >> kDiagBit);
+                    if (w) w[e] = g.w[e];
+                }
+            }
+        }
+    for (uint8_t s : seen)
+        if (!s) return fail(EPHC_ESTATE, "internal: entry not covered by any task");
+    return EPHC_OK;
+}
+
+extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (variant != 0) return fail(EPHC_ESTATE, "variant 1 (scatter) is not built in this version");
+    h->variant = variant;
+    return EPHC_OK;
+}
+
+extern "C" int64_t ephc_launch_count(const ephc_handle *h) { return h ? h->launches : 0; }
+
+// ------------------------------------------------------------------------------------------------------------
+static int need_device(ephc_handle *h) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (h->host_only) return fail(EPHC_ESTATE, "handle was built with EPHC_HOST_ONLY: no device store");
+    if (!h->attrs_set) {
+        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kCollision>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)gather_smem_bytes(kCollision)));
+        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kRkStage>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)gather_smem_bytes(kRkStage)));
+        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportSetup>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)gather_smem_bytes(kTransportSetup)));
+        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)gather_smem_bytes(kTransportIter)));
+        h->attrs_set = true;
+    }
+    return EPHC_OK;
+}
+
+static GatherParams base_params(const ephc_handle *h) {
+    GatherParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.code = h->d_code;
+    P.w = h->d_w;
+    P.hp_k = h->d_hp_k;
+    P.hp_q = h->d_hp_q;
+    P.tasks = h->d_tasks;
+    P.rounds = h->d_rounds;
+    P.wus = h->d_wus;
+    P.nb = h->d.nb;
+    P.nnu = h->d.nnu;
+    P.ns = h->d.ns;
+    P.gW = h->d_gW;
+    return P;
+}
+
+template <int MODE>
+static int launch_gather(ephc_handle *h, const GatherParams &P, cudaStream_t s) {
+    if (h->n_wu > 0) {
+        gather_kernel<MODE><<<h->n_wu, kThreads, gather_smem_bytes(MODE), s>>>(P);
+        h->launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
+template <class T>
+static int ensure(T **p, size_t n) {
+    if (*p) return EPHC_OK;
+    cudaError_t e = cudaMalloc((void **)p, n > 0 ? n : 8);
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? EPHC_ENOMEM : EPHC_ECUDA,
+                                      std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    return EPHC_OK;
+}
+
+extern "C" int ephc_collision(ephc_handle *h, const double *f_dev, const double *N_dev, double *I_dev,
+                              void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f_dev || !N_dev || !I_dev) return fail(EPHC_EINVAL, "null device pointer");
+    GatherParams P = base_params(h);
+    P.f = f_dev;
+    P.N = N_dev;
+    P.out = I_dev;
+    return launch_gather<kCollision>(h, P, (cudaStream_t)stream);
+}
+
+extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const double *N_dev, double *Gamma_dev,
+                                    void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f0_dev || !N_dev || !Gamma_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (!h->d_gW) {
+        rc = ensure(&h->d_gW, (size_t)h->g_entries * 8);
+        if (rc) return rc;
+        h->bytes_transport = h->g_entries * 8;
+    }
+    GatherParams P = base_params(h);
+    P.f = f0_dev;
+    P.N = N_dev;
+    P.out = Gamma_dev;
+    rc = launch_gather<kTransportSetup>(h, P, (cudaStream_t)stream);
+    if (rc == EPHC_OK) h->transport_ready = true;
+    return rc;
+}
+
+extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
+                                   double *Fout_dev, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!F_dev || !v_dev || !tau_dev || !Fout_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (F_dev == Fout_dev) return fail(EPHC_EINVAL, "transport_iter is out of place: F_dev and Fout_dev must differ");
+    if (!h->transport_ready) return fail(EPHC_ESTATE, "call ephc_transport_setup before ephc_transport_iter");
+    GatherParams P = base_params(h);
+    P.F = F_dev;
+    P.v = v_dev;
+    P.tau = tau_dev;
+    P.out = Fout_dev;
+    return launch_gather<kTransportIter>(h, P, (cudaStream_t)stream);
+}
+
+extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
+                            double *sumf_dev, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f_dev || !N_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (nsteps < 0 || !std::isfinite(dt_fs)) return fail(EPHC_EINVAL, "nsteps >= 0 and finite dt required");
+    const size_t nb8 = (size_t)h->d.ns * 8;
+    if ((rc = ensure(&h->d_y[0], nb8)) || (rc = ensure(&h->d_y[1], nb8)) || (rc = ensure(&h->d_ksum, nb8)) ||
+        (rc = ensure(&h->d_wusum, (size_t)(h->n_wu > 0 ? h->n_wu : 1) * 8)))
+        return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (sumf_dev) {
+        sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev);
+        h->launches++;
+    }
+    GatherParams P = base_params(h);
+    P.N = N_dev;
+    P.dt = dt_fs;
+    P.f0 = f_dev;
+    P.ksum = h->d_ksum;
+    P.wu_sum = sumf_dev ? h->d_wusum : nullptr;
+    for (int it = 0; it < nsteps; ++it) {
+        // stage 1 gathers f, writes y2 -> y[0]; stage 2 gathers y[0], writes y3 -> y[1];
+        // stage 3 gathers y[1], writes y4 -> y[0]; stage 4 gathers y[0], updates f in place.
+        const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
+        double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
+        for (int st = 0; st < 4; ++st) {
+            P.stage = st + 1;
+            P.f = src[st];
+            P.ynext = dst[st];
+            rc = launch_gather<kRkStage>(h, P, s);
+            if (rc) return rc;
+        }
+        if (sumf_dev) {
+            if (h->n_wu > 0)
+                sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, h->n_wu, sumf_dev + it + 1);
+            else
+                sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev + it + 1);
+            h->launches++;
+        }
+    }
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
+// ---- host-buffer variants (end-to-end path) ----------------------------------------------------------------------
+extern "C" int ephc_collision_host(ephc_handle *h, const double *f_host, const double *N_host, double *I_host) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f_host || !N_host || !I_host) return fail(EPHC_EINVAL, "null host pointer");
+    const size_t nf = (size_t)h->d.ns * 8, nN = (size_t)h->d.nq * h->d.nnu * 8;
+    if ((rc = ensure(&h->d_hf, nf)) || (rc = ensure(&h->d_hN, nN)) || (rc = ensure(&h->d_hI, nf))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(h->d_hf, f_host, nf, cudaMemcpyHostToDevice, 0));
+    CUDA_TRY(cudaMemcpyAsync(h->d_hN, N_host, nN, cudaMemcpyHostToDevice, 0));
+    rc = ephc_collision(h, h->d_hf, h->d_hN, h->d_hI, nullptr);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(I_host, h->d_hI, nf, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return EPHC_OK;
+}
+
+extern "C" int ephc_transport_solve_host(ephc_handle *h, const double *f0_host, const double *N_host,
+                                         const double *v_host, int niter, double *F_host, double *Gamma_host) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f0_host || !N_host || !v_host || !F_host || niter < 0) return fail(EPHC_EINVAL, "bad argument");
+    const int64_t ns = h->d.ns;
+    const size_t nf = (size_t)ns * 8, nN = (size_t)h->d.nq * h->d.nnu * 8;
+    if ((rc = ensure(&h->d_hf, nf)) || (rc = ensure(&h->d_hN, nN)) || (rc = ensure(&h->d_tr[0], nf)) ||
+        (rc = ensure(&h->d_tr[1], nf)) || (rc = ensure(&h->d_tr[2], 3 * nf)) || (rc = ensure(&h->d_tr[3], 3 * nf)) ||
+        (rc = ensure(&h->d_tr[4], 3 * nf)))
+        return rc;
+    double *Gam = h->d_tr[0], *tau = h->d_tr[1], *v = h->d_tr[2], *Fa = h->d_tr[3], *Fb = h->d_tr[4];
+    CUDA_TRY(cudaMemcpyAsync(h->d_hf, f0_host, nf, cudaMemcpyHostToDevice, 0));
+    CUDA_TRY(cudaMemcpyAsync(h->d_hN, N_host, nN, cudaMemcpyHostToDevice, 0));
+    CUDA_TRY(cudaMemcpyAsync(v, v_host, 3 * nf, cudaMemcpyHostToDevice, 0));
+    rc = ephc_transport_setup(h, h->d_hf, h->d_hN, Gam, nullptr);
+    if (rc) return rc;
+    tau_f0_kernel<<<(unsigned)((ns + 255) / 256), 256>>>(Gam, v, tau, Fa, ns);
+    h->launches++;
+    for (int it = 0; it < niter; ++it) {
+        rc = ephc_transport_iter(h, Fa, v, tau, Fb, nullptr);
+        if (rc) return rc;
+        double *t = Fa;
+        Fa = Fb;
+        Fb = t;
+    }
+    CUDA_TRY(cudaMemcpyAsync(F_host, Fa, 3 * nf, cudaMemcpyDeviceToHost, 0));
+    if (Gamma_host) CUDA_TRY(cudaMemcpyAsync(Gamma_host, Gam, nf, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return EPHC_OK;
+}
+
+extern "C" int ephc_rt_step_host(ephc_handle *h, double *f_host, const double *N_host, double dt_fs, int nsteps,
+                                 double *sumf_host) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f_host || !N_host || nsteps < 0) return fail(EPHC_EINVAL, "bad argument");
+    const size_t nf = (size_t)h->d.ns * 8, nN = (size_t)h->d.nq * h->d.nnu * 8;
+    if ((rc = ensure(&h->d_hf, nf)) || (rc = ensure(&h->d_hN, nN))) return rc;
+    if (sumf_host && h->sumf_cap < nsteps + 1) {
+        if (h->d_sumf) cudaFree(h->d_sumf);
+        h->d_sumf = nullptr;
+        if ((rc = ensure(&h->d_sumf, (size_t)(nsteps + 1) * 8))) return rc;
+        h->sumf_cap = nsteps + 1;
+    }
+    CUDA_TRY(cudaMemcpyAsync(h->d_hf, f_host, nf, cudaMemcpyHostToDevice, 0));
+    CUDA_TRY(cudaMemcpyAsync(h->d_hN, N_host, nN, cudaMemcpyHostToDevice, 0));
+    rc = ephc_rt_step(h, h->d_hf, h->d_hN, dt_fs, nsteps, sumf_host ? h->d_sumf : nullptr, nullptr);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(f_host, h->d_hf, nf, cudaMemcpyDeviceToHost, 0));
+    if (sumf_host)
+        CUDA_TRY(cudaMemcpyAsync(sumf_host, h->d_sumf, (size_t)(nsteps + 1) * 8, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return EPHC_OK;
+}
