@@ -1,0 +1,362 @@
+#!/usr/bin/env python
+"""bench.py -- channel-terms/s of the e-ph collision-integral hot path on B200 (BASELINE.json metric).
+
+One "step" = one pass of the whole hot path over the Si-like transport workload
+(BASELINE.json configs[1]; configs[4] is the same channel set):
+    1 collision evaluation + 1 transport_setup + 20 transport iterations (3 Cartesian components)
+    + 1 RK4 rt-BTE step (4 collision evaluations with fused axpy) + the conservation scalar
+  = 26 channel-loop evaluations; channel-terms per step = 26 * N_ch (N_ch = unordered active channels).
+
+`value`     device-resident: inputs in HBM before the timed region, CUDA events on the launching stream.
+`e2e`       the same step through the *_host entry points of the C ABI: pinned host buffers, H2D/D2H inside.
+`roofline`  for the kernel with the largest share of the step: algorithmic bytes per launch (DESIGN.md
+            "Roofline") / mean launch duration measured here with CUDA events, vs MEASURED_PEAKS.json.
+`cpu_baseline`  the CPU oracle (oracle/, as it stands, serial) on a bounded sample of the same workload.
+
+--impl reference  times the oracle instead (rank 0 only).  N > 1: independent replicas, one per GPU, seeds
+differ per rank ("weak"); k-sharding with an all-gather of f is DESIGN.md's NEXT-1.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+N_TRANSPORT_ITERS = 20
+EVALS_PER_STEP = 1 + 1 + N_TRANSPORT_ITERS + 4
+METRIC = "collision-integral channel-terms/s (fp64)"
+UNIT = "channel-terms/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="si", help="workload: si (default, BASELINE configs[1]) | tiny | gaas | bigcell")
+    ap.add_argument("--grid", type=int, default=0, help="override the grid edge (smaller copies for quick runs)")
+    ap.add_argument("--pair-prob", type=float, default=0.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def make_workload(args, seed_offset=0):
+    from ephc_inputs import make_problem
+    kw = {}
+    if args.grid:
+        kw["grid"] = (args.grid,) * 3
+    if args.pair_prob:
+        kw["pair_prob"] = args.pair_prob
+    if seed_offset:
+        kw["seed"] = 20251103 + 100 * seed_offset + 1
+    return make_problem(args.config, **kw)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            c = [x.strip() for x in r.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------
+def oracle_step(L, p, n_iters, n_rt):
+    """The same step on the CPU oracle (bounded: n_iters transport iterations, n_rt RK4 steps)."""
+    L.collision(p.f, p.N)
+    G = L.transport_setup(p.f0, p.N)
+    tau = np.where(G > 0, 1.0 / np.where(G > 0, G, 1.0), 0.0)
+    F = tau[None, :] * p.v
+    for _ in range(n_iters):
+        F = L.transport_iter(p.f0, p.N, F, p.v, tau)
+    if n_rt:
+        L.rt_step(p.f, p.N, 1.0, n_rt)
+    return 1 + 1 + n_iters + 4 * n_rt
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    p = make_workload(args)
+    L = oracle.OracleList(p)
+    # bounded sample per step: collision + setup + 2 transport iterations + 1 RK4 step = 8 evaluations
+    n_iters, n_rt = 2, 1
+    for _ in range(max(args.warmup, 0)):
+        oracle_step(L, p, 0, 0)
+    t0 = time.perf_counter()
+    evals = 0
+    for _ in range(args.steps):
+        evals += oracle_step(L, p, n_iters, n_rt)
+    dt = time.perf_counter() - t0
+    val = L.nch * evals / dt
+    sample = (f"per step: 1 collision + 1 transport_setup + {n_iters} transport iterations + {n_rt} RK4 step "
+              f"({evals // max(args.steps, 1)} of the {EVALS_PER_STEP} evaluations of a full step), full channel set")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(args, p, L.nch),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def workload_config(args, p, nch):
+    return {"workload": f"{p.name}: {p.grid[0]}x{p.grid[1]}x{p.grid[2]} k-grid, window [{p.emin},{p.emax}] eV, "
+                        f"{p.nk} active k, {p.nb} bands, {p.nnu} modes, sigma={p.sigma} eV",
+            "n_channels": int(nch), "n_states": int(p.ns), "n_pairs_candidate": int(p.npair),
+            "step": f"1 collision + 1 transport_setup + {N_TRANSPORT_ITERS} transport_iter (3 components) + 1 RK4 "
+                    f"rt_step (4 evaluations) + sum f = {EVALS_PER_STEP} channel-loop evaluations",
+            "seed": int(p.seed)}
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2511_03683_b200 as ephc
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    p = make_workload(args, seed_offset=rank)       # replicas: an independent problem per rank
+    t0 = time.perf_counter()
+    h = ephc.build_channels(p)
+    t_build = time.perf_counter() - t0
+    q = h.query()
+    nch, ns = q["nch"], p.ns
+    dev = torch.device("cuda", local)
+
+    def d(x):
+        return torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64).reshape(-1), device=dev)
+
+    f, f0, N, v = d(p.f), d(p.f0), d(p.N), d(p.v)
+    I = torch.empty(ns, device=dev, dtype=torch.float64)
+    G = torch.empty(ns, device=dev, dtype=torch.float64)
+    tau = torch.empty(ns, device=dev, dtype=torch.float64)
+    Fa = torch.empty(3 * ns, device=dev, dtype=torch.float64)
+    Fb = torch.empty(3 * ns, device=dev, dtype=torch.float64)
+    frt = f.clone()
+    sumf = torch.zeros(2, device=dev, dtype=torch.float64)
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        """ev: list collecting (label, start_event, end_event) per phase."""
+        def mark():
+            e = torch.cuda.Event(enable_timing=True)
+            e.record(stream)
+            return e
+        e0 = mark() if ev is not None else None
+        h.collision(f, N, I, stream)
+        e1 = mark() if ev is not None else None
+        h.transport_setup(f0, N, G, stream)
+        e2 = mark() if ev is not None else None
+        h.transport_start(G, v, tau, Fa, stream)
+        e3 = mark() if ev is not None else None
+        a, b = Fa, Fb
+        for _ in range(N_TRANSPORT_ITERS):
+            h.transport_iter(a, v, tau, b, stream)
+            a, b = b, a
+        e4 = mark() if ev is not None else None
+        h.rt_step(frt, N, 1.0, 1, sumf, stream)
+        e5 = mark() if ev is not None else None
+        if ev is not None:
+            ev.append((e0, e1, e2, e3, e4, e5))
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = h.launch_count()
+    ev = []
+    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    start.record(stream)
+    for _ in range(args.steps):
+        step(ev)
+    stop.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = h.launch_count() - l0
+    ms_total = start.elapsed_time(stop)
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+        tot = torch.tensor([float(nch)], device=dev, dtype=torch.float64)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        nch_all = float(tot.item())
+    else:
+        nch_all = float(nch)
+    value = nch_all * EVALS_PER_STEP * args.steps / (ms_total * 1e-3)
+
+    # per-phase device times (this rank)
+    ph = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(5)] for e in ev]) if ev else np.zeros((1, 5))
+    ms_coll, ms_setup, ms_tau, ms_iter, ms_rt = ph.mean(axis=0)
+    peak, peak_src = peaks()
+    kern = {}
+
+    def roof(name, ms_launch, alg_bytes, share):
+        gbs = alg_bytes / (ms_launch * 1e-3) / 1e9 if ms_launch > 0 else 0.0
+        kern[name] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                      "traffic": None, "alg_bytes_per_launch": int(alg_bytes), "us_per_launch": 1e3 * ms_launch,
+                      "share_of_step": share, "channel_terms_per_s": nch / (ms_launch * 1e-3) if ms_launch > 0 else 0.0}
+
+    ms_step = ms_total / max(args.steps, 1)
+    roof("collision (gather_kernel<0>)", ms_coll, q["alg_bytes_collision"], ms_coll / ms_step)
+    roof("transport_setup (gather_kernel<2>)", ms_setup, q["alg_bytes_collision"] + 8 * q["gather_entries"], ms_setup / ms_step)
+    roof("transport_iter (gather_kernel<3>)", ms_iter / N_TRANSPORT_ITERS, q["alg_bytes_transport"], ms_iter / ms_step)
+    # an RK stage moves the collision bytes plus the fused axpy vectors (f0, ksum r/w, ynext): 32 B per state
+    roof("rk4 stage (gather_kernel<1>)", ms_rt / 4, q["alg_bytes_collision"] + 32 * ns, ms_rt / ms_step)
+    dominant = max(kern, key=lambda k: kern[k]["share_of_step"])
+    roofline = dict(kern[dominant], kernel=dominant, peak_source=peak_src)
+    traffic_path = os.path.join(ROOT, "profiles", "traffic.json")       # dram bytes per launch from the ncu capture
+    if os.path.exists(traffic_path):
+        with open(traffic_path) as fh:
+            tr = json.load(fh)
+        for k in kern:
+            kern[k]["traffic"] = tr.get(k)
+        roofline["traffic"] = tr.get(dominant)
+
+    # ---- end to end: the same step through host buffers ------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda x: torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64).reshape(-1)).pin_memory()
+        hf, hf0, hN, hv = pin(p.f), pin(p.f0), pin(p.N), pin(p.v)
+        hI, hF, hG = pin(np.zeros(ns)), pin(np.zeros(3 * ns)), pin(np.zeros(ns))
+        hfrt, hs = pin(p.f), pin(np.zeros(2))
+
+        def step_host():
+            h.collision_host(hf, hN, hI)
+            h.transport_solve_host(hf0, hN, hv, N_TRANSPORT_ITERS, hF, hG)
+            h.rt_step_host(hfrt, hN, 1.0, 1, hs)
+        h2d = 8 * (ns + p.nq * p.nnu) + 8 * (ns + p.nq * p.nnu + 3 * ns) + 8 * (ns + p.nq * p.nnu)
+        d2h = 8 * ns + 8 * (3 * ns + ns) + 8 * (ns + 2)
+        for _ in range(max(args.warmup, 0)):
+            step_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            step_host()
+        barrier()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": nch_all * EVALS_PER_STEP * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt / max(args.steps, 1)}
+
+    # ---- CPU oracle on a bounded sample (rank 0, N = 1 only) -----------------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        L = oracle.OracleList(p)
+        assert L.nch == nch, "oracle and library disagree on the channel count"
+        t0 = time.perf_counter()
+        evals = oracle_step(L, p, 4, 1)
+        dt = time.perf_counter() - t0
+        cpu = {"value": L.nch * evals / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"one pass: 1 collision + 1 transport_setup + 4 transport iterations + 1 RK4 step = {evals} of the "
+                         f"{EVALS_PER_STEP} evaluations of a step, full channel set ({dt:.1f} s, serial C, gcc -O2)",
+               "host_cores_available": os.cpu_count()}
+
+    if rank == 0:
+        cfg = workload_config(args, p, nch)
+        cfg.update({"l2": f"no flush: every evaluation streams the {q['store_bytes_gather'] / 1e6:.0f} MB store "
+                          f"(+{q['store_bytes_transport'] / 1e6:.0f} MB transport weights), larger than the 126 MB L2",
+                    "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (one problem per GPU)",
+                    "build_channels_s": t_build, "store_bytes": q["store_bytes_gather"] + q["store_bytes_transport"]})
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+               "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg, "e2e": e2e,
+               "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "kernels": kern,
+               "cpu_baseline": cpu}
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -137,6 +137,9 @@ int ephc_collision(ephc_handle *h, const double *f_dev, const double *N_dev, dou
  * Gamma[a] = sum_b W(a<-b). */
 int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const double *N_dev, double *Gamma_dev,
                          void *stream);
+/* Start of the iteration: tau[a] = 1/Gamma[a] (0 where Gamma[a] == 0) and F0[al][a] = tau[a] v[al][a]. */
+int ephc_transport_start(ephc_handle *h, const double *Gamma_dev, const double *v_dev, double *tau_dev,
+                         double *F0_dev, void *stream);
 /* One iteration Fout[al][a] = tau[a] * ( v[al][a] + sum_b W(a<-b) F[al][b] ), al = x,y,z. */
 int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
                         double *Fout_dev, void *stream);

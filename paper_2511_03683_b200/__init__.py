@@ -71,6 +71,7 @@ def _load():
         "ephc_set_variant": (i32, [vp, i32]),
         "ephc_collision": (i32, [vp, vp, vp, vp, vp]),
         "ephc_transport_setup": (i32, [vp, vp, vp, vp, vp]),
+        "ephc_transport_start": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_transport_iter": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_rt_step": (i32, [vp, vp, vp, dbl, i32, vp, vp]),
         "ephc_collision_host": (i32, [vp, vp, vp, vp]),
@@ -201,6 +202,11 @@ class Handle:
         _check(_load().ephc_transport_setup(self._h, _dev_ptr(f0, self.ns, "f0"),
                                             _dev_ptr(N, self.nq * self.nnu, "N"),
                                             _dev_ptr(Gamma, self.ns, "Gamma"), _stream_ptr(stream)))
+
+    def transport_start(self, Gamma, v, tau, F0, stream=None):
+        _check(_load().ephc_transport_start(self._h, _dev_ptr(Gamma, self.ns, "Gamma"), _dev_ptr(v, 3 * self.ns, "v"),
+                                            _dev_ptr(tau, self.ns, "tau"), _dev_ptr(F0, 3 * self.ns, "F0"),
+                                            _stream_ptr(stream)))
 
     def transport_iter(self, F, v, tau, Fout, stream=None):
         _check(_load().ephc_transport_iter(self._h, _dev_ptr(F, 3 * self.ns, "F"), _dev_ptr(v, 3 * self.ns, "v"),

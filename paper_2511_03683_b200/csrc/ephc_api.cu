@@ -352,6 +352,18 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
     return rc;
 }
 
+extern "C" int ephc_transport_start(ephc_handle *h, const double *Gamma_dev, const double *v_dev, double *tau_dev,
+                                    double *F0_dev, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!Gamma_dev || !v_dev || !tau_dev || !F0_dev) return fail(EPHC_EINVAL, "null device pointer");
+    const int64_t ns = h->d.ns;
+    tau_f0_kernel<<<(unsigned)((ns + 255) / 256), 256, 0, (cudaStream_t)stream>>>(Gamma_dev, v_dev, tau_dev, F0_dev, ns);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
 extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
                                    double *Fout_dev, void *stream) {
     int rc = need_device(h);
@@ -445,8 +457,8 @@ extern "C" int ephc_transport_solve_host(ephc_handle *h, const double *f0_host, 
     CUDA_TRY(cudaMemcpyAsync(v, v_host, 3 * nf, cudaMemcpyHostToDevice, 0));
     rc = ephc_transport_setup(h, h->d_hf, h->d_hN, Gam, nullptr);
     if (rc) return rc;
-    tau_f0_kernel<<<(unsigned)((ns + 255) / 256), 256>>>(Gam, v, tau, Fa, ns);
-    h->launches++;
+    rc = ephc_transport_start(h, Gam, v, tau, Fa, nullptr);
+    if (rc) return rc;
     for (int it = 0; it < niter; ++it) {
         rc = ephc_transport_iter(h, Fa, v, tau, Fb, nullptr);
         if (rc) return rc;

@@ -1,0 +1,205 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs.  Bar (BASELINE.json north_star): channel lists / indices bit-exact (tests/test_host_build.py),
+I, Gamma, F and f(t) within max|d| <= 1e-11 * max|.| in fp64."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2511_03683_b200 as ephc
+from ephc_inputs import make_problem, bose_einstein
+from helpers import manual_problem, exact_energy_problem
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def dev(x):
+    return torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64).reshape(-1), device="cuda")
+
+
+def _small_problems():
+    out = [make_problem("tiny", grid=(4, 4, 4), seed=5)]
+    p = make_problem("tiny", grid=(4, 4, 4), window=(0.08, 0.22), seed=99)
+    p.g2_cut = float(np.quantile(p.g2, 0.2))
+    p.hw[...] = p.hw * 0.5
+    p.N = bose_einstein(p.hw, 300.0).reshape(-1)
+    out.append(p)
+    out.append(make_problem("si", grid=(12, 12, 12), pair_prob=0.3, seed=3))
+    out.append(make_problem("gaas", grid=(24, 24, 24), pair_prob=0.5, seed=4, window=(0.0, 0.5)))
+    out.append(make_problem("bigcell", grid=(3, 3, 3), pair_prob=0.2, seed=6))
+    out.append(make_problem("tiny"))                                   # config 1 at full size (5e5 channels)
+    out.append(make_problem("rt", grid=(14, 14, 14), pair_prob=0.3, seed=8))
+    return out
+
+
+IDS = ["tiny4", "window_cut_diag", "si12", "gaas24", "bigcell3", "tiny_full", "rt14"]
+
+
+@pytest.fixture(scope="module", params=range(len(IDS)), ids=IDS)
+def case(request):
+    p = _small_problems()[request.param]
+    return p, oracle.OracleList(p), ephc.build_channels(p)
+
+
+def _relerr(a, b):
+    return np.abs(np.asarray(a) - np.asarray(b)).max() / max(np.abs(b).max(), 1e-300)
+
+
+def test_collision_matches_oracle(case):
+    p, L, h = case
+    f, N, I = dev(p.f), dev(p.N), torch.full((p.ns,), np.nan, device="cuda", dtype=torch.float64)
+    h.collision(f, N, I)
+    Io = L.collision(p.f, p.N)
+    got = I.cpu().numpy()
+    assert np.isfinite(got).all()
+    assert _relerr(got, Io) <= TOL
+    assert abs(got.sum()) <= 1e-12 * np.abs(got).sum()                   # particle number
+    out = ~((p.E.reshape(-1) >= p.emin) & (p.E.reshape(-1) <= p.emax))
+    assert np.all(got[out] == 0.0)
+    # bit-reproducible: one owner per element, fixed summation order
+    I2 = torch.empty_like(I)
+    h.collision(f, N, I2)
+    assert torch.equal(I, I2)
+    # host-buffer entry point gives the same bits
+    Ih = np.zeros(p.ns)
+    h.collision_host(p.f, p.N, Ih)
+    assert np.array_equal(Ih, got)
+    # other occupations through the same store
+    rng = np.random.default_rng(1)
+    f2, N2 = rng.uniform(0, 1, p.ns), rng.uniform(0, 3, p.nq * p.nnu)
+    h.collision(dev(f2), dev(N2), I)
+    assert _relerr(I.cpu().numpy(), L.collision(f2, N2)) <= TOL
+
+
+def test_transport_matches_oracle(case):
+    p, L, h = case
+    f0, N = dev(p.f0), dev(p.N)
+    G = torch.empty(p.ns, device="cuda", dtype=torch.float64)
+    h.transport_setup(f0, N, G)
+    Go = L.transport_setup(p.f0, p.N)
+    assert _relerr(G.cpu().numpy(), Go) <= TOL
+    tau_o = np.where(Go > 0, 1.0 / np.where(Go > 0, Go, 1.0), 0.0)
+    rng = np.random.default_rng(2)
+    F = rng.normal(size=(3, p.ns)); v = rng.normal(size=(3, p.ns))
+    Fo = L.transport_iter(p.f0, p.N, F, v, tau_o)
+    Fout = torch.empty(3 * p.ns, device="cuda", dtype=torch.float64)
+    h.transport_iter(dev(F), dev(v), dev(tau_o), Fout)
+    assert _relerr(Fout.cpu().numpy().reshape(3, -1), Fo) <= TOL
+    # 20 iterations from F0 = tau v through the host-buffer solver (config 2's schedule)
+    Fh, Gh = np.zeros((3, p.ns)), np.zeros(p.ns)
+    h.transport_solve_host(p.f0, p.N, p.v, 20, Fh, Gh)
+    Fr = tau_o[None, :] * p.v
+    for _ in range(20):
+        Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau_o)
+    assert _relerr(Gh, Go) <= TOL
+    assert _relerr(Fh, Fr) <= 1e-10                                    # 20 chained iterations
+
+
+def test_rt_step_matches_oracle(case):
+    p, L, h = case
+    nsteps = 25
+    dt = 1.0
+    f = dev(p.f)
+    sumf = torch.zeros(nsteps + 1, device="cuda", dtype=torch.float64)
+    h.rt_step(f, dev(p.N), dt, nsteps, sumf)
+    fo, so = L.rt_step(p.f, p.N, dt, nsteps)
+    got, sg = f.cpu().numpy(), sumf.cpu().numpy()
+    assert _relerr(got, fo) <= TOL
+    assert np.abs(sg - so).max() <= 1e-12 * abs(so[0])
+    assert np.abs(sg - sg[0]).max() <= 1e-12 * abs(sg[0])               # electron number conserved each step
+    assert np.abs(got - p.f).max() > 0
+    # twice the same bits; host-buffer variant too; without the conservation scalar too
+    f2 = dev(p.f)
+    h.rt_step(f2, dev(p.N), dt, nsteps, None)
+    assert torch.equal(f, f2)
+    fh, sh = p.f.copy(), np.zeros(nsteps + 1)
+    h.rt_step_host(fh, p.N, dt, nsteps, sh)
+    assert np.array_equal(fh, got) and np.array_equal(sh, sg)
+
+
+def test_pins_on_gpu():
+    # P1 worked example (tests/golden/p1_single_channel.txt) and P4 detailed balance, on the CUDA path
+    hw = 0.03
+    p = manual_problem((1, 1, 1), E=[[0.0, hw]], hw=[[hw]], pairs=[(0, 0)], g2=[[[[0.0, 1e-4], [1e-4, 0.0]]]],
+                       sigma=0.010, f=[0.5, 0.25], N=[1.0])
+    h = ephc.build_channels(p)
+    I = np.zeros(2)
+    h.collision_host(p.f, p.N, I)
+    assert I[0] == pytest.approx(-0.0047602984273419701349, rel=1e-12) and I[1] == -I[0]
+    p = exact_energy_problem()
+    h = ephc.build_channels(p)
+    I = np.zeros(p.ns)
+    h.collision_host(p.f, p.N, I)
+    ch = h.export_channels()
+    scale = (ch["w_abs"] + ch["w_em"]).max() * 50
+    assert np.abs(I).max() <= 1e-13 * scale
+    f2 = p.f.copy(); f2[::3] *= 0.5
+    h.collision_host(f2, p.N, I)
+    assert np.abs(I).max() > 1e-6 * scale
+
+
+def test_degenerate_inputs_on_gpu():
+    # no channels at all: I = 0, f unchanged, F = tau*v = 0
+    p = manual_problem((2, 1, 1), E=[[0.0], [1.0]], hw=[[0.02], [0.02]], pairs=[(0, 1)], g2=np.ones((1, 1, 1, 1)), sigma=0.01)
+    h = ephc.build_channels(p)
+    I = np.full(p.ns, 7.0)
+    h.collision_host(p.f, p.N, I)
+    assert np.all(I == 0.0)
+    f = p.f.copy(); s = np.zeros(4)
+    h.rt_step_host(f, p.N, 1.0, 3, s)
+    assert np.array_equal(f, p.f) and np.all(s == p.f.sum())
+    # diagonal-only problem: collision 0, Gamma > 0
+    p = manual_problem((1, 1, 1), E=[[0.0]], hw=[[0.02]], pairs=[(0, 0)], g2=np.ones((1, 1, 1, 1)), sigma=0.01)
+    h = ephc.build_channels(p)
+    I = np.full(1, 7.0)
+    h.collision_host(p.f, p.N, I)
+    assert I[0] == 0.0
+    F, G = np.zeros((3, 1)), np.zeros(1)
+    h.transport_solve_host(p.f, p.N, np.ones((3, 1)), 2, F, G)
+    L = oracle.OracleList(p)
+    assert G[0] == pytest.approx(L.transport_setup(p.f, p.N)[0], rel=1e-14) and G[0] > 0
+    # transport_iter before transport_setup is an error, not a silent zero
+    h2 = ephc.build_channels(p)
+    z = torch.zeros(3, device="cuda", dtype=torch.float64)
+    with pytest.raises(ephc.EphcError):
+        h2.transport_iter(z, z.clone(), torch.zeros(1, device="cuda", dtype=torch.float64), z.clone())
+
+
+def test_multi_round_segments_on_gpu(monkeypatch):
+    monkeypatch.setenv("EPHC_ROUND_PAIRS", "7")
+    monkeypatch.setenv("EPHC_WU_ENTRIES", "300")
+    for p in _small_problems()[:4]:
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p)
+        q = h.query()
+        assert q["n_rounds"] > 2 * q["n_workunits"]
+        I = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I)
+        assert _relerr(I, L.collision(p.f, p.N)) <= TOL
+        F, G = np.zeros((3, p.ns)), np.zeros(p.ns)
+        h.transport_solve_host(p.f0, p.N, p.v, 3, F, G)
+        Go = L.transport_setup(p.f0, p.N)
+        tau = np.where(Go > 0, 1.0 / np.where(Go > 0, Go, 1.0), 0.0)
+        Fr = tau[None, :] * p.v
+        for _ in range(3):
+            Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau)
+        assert _relerr(F, Fr) <= TOL
+        f = p.f.copy()
+        h.rt_step_host(f, p.N, 1.0, 5, None)
+        assert _relerr(f, L.rt_step(p.f, p.N, 1.0, 5)[0]) <= TOL
+
+
+def test_stream_argument_is_honoured():
+    p = make_problem("si", grid=(12, 12, 12), pair_prob=0.3, seed=3)
+    h = ephc.build_channels(p)
+    L = oracle.OracleList(p)
+    s = torch.cuda.Stream()
+    f, N = dev(p.f), dev(p.N)
+    I = torch.zeros(p.ns, device="cuda", dtype=torch.float64)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        h.collision(f, N, I, stream=s)
+    s.synchronize()
+    assert _relerr(I.cpu().numpy(), L.collision(p.f, p.N)) <= TOL
