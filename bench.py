@@ -47,6 +47,7 @@ def parse():
     ap.add_argument("--config", default="si", help="workload: si (default, BASELINE configs[1]) | tiny | gaas | bigcell")
     ap.add_argument("--grid", type=int, default=0, help="override the grid edge (smaller copies for quick runs)")
     ap.add_argument("--pair-prob", type=float, default=0.0)
+    ap.add_argument("--variant", type=int, default=-1, help="-1: library default (tiles when available), 0: gather, 1: tiles")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -202,6 +203,9 @@ def main():
     t0 = time.perf_counter()
     h = ephc.build_channels(p)
     t_build = time.perf_counter() - t0
+    if args.variant >= 0:
+        h.set_variant(args.variant)
+    variant = h.get_variant()
     q = h.query()
     nch, ns = q["nch"], p.ns
     dev = torch.device("cuda", local)
@@ -284,11 +288,18 @@ def main():
                       "share_of_step": share, "channel_terms_per_s": nch / (ms_launch * 1e-3) if ms_launch > 0 else 0.0}
 
     ms_step = ms_total / max(args.steps, 1)
-    roof("collision (gather_kernel<0>)", ms_coll, q["alg_bytes_collision"], ms_coll / ms_step)
-    roof("transport_setup (gather_kernel<2>)", ms_setup, q["alg_bytes_collision"] + 8 * q["gather_entries"], ms_setup / ms_step)
-    roof("transport_iter (gather_kernel<3>)", ms_iter / N_TRANSPORT_ITERS, q["alg_bytes_transport"], ms_iter / ms_step)
+    if variant == 1:
+        kn = {"c": "tile_kernel<0> + finish_kernel<0>", "s": "tile_kernel<2> + finish_kernel<2>",
+              "i": "tile_kernel<3> + finish_kernel<3>", "r": "tile_kernel<0> + finish_kernel<1>"}
+        w_setup = 16 * q["scatter_entries"]
+    else:
+        kn = {"c": "gather_kernel<0>", "s": "gather_kernel<2>", "i": "gather_kernel<3>", "r": "gather_kernel<1>"}
+        w_setup = 8 * q["gather_entries"]
+    roof(f"collision ({kn['c']})", ms_coll, q["alg_bytes_collision"], ms_coll / ms_step)
+    roof(f"transport_setup ({kn['s']})", ms_setup, q["alg_bytes_collision"] + w_setup, ms_setup / ms_step)
+    roof(f"transport_iter ({kn['i']})", ms_iter / N_TRANSPORT_ITERS, q["alg_bytes_transport"], ms_iter / ms_step)
     # an RK stage moves the collision bytes plus the fused axpy vectors (f0, ksum r/w, ynext): 32 B per state
-    roof("rk4 stage (gather_kernel<1>)", ms_rt / 4, q["alg_bytes_collision"] + 32 * ns, ms_rt / ms_step)
+    roof(f"rk4 stage ({kn['r']})", ms_rt / 4, q["alg_bytes_collision"] + 32 * ns, ms_rt / ms_step)
     dominant = max(kern, key=lambda k: kern[k]["share_of_step"])
     roofline = dict(kern[dominant], kernel=dominant, peak_source=peak_src)
     traffic_path = os.path.join(ROOT, "profiles", "traffic.json")       # dram bytes per launch from the ncu capture
@@ -344,10 +355,12 @@ def main():
 
     if rank == 0:
         cfg = workload_config(args, p, nch)
-        cfg.update({"l2": f"no flush: every evaluation streams the {q['store_bytes_gather'] / 1e6:.0f} MB store "
+        sb = q["store_bytes_scatter"] if variant == 1 else q["store_bytes_gather"]
+        cfg.update({"variant": "tiles" if variant == 1 else "gather",
+                    "l2": f"no flush: every evaluation streams the {sb / 1e6:.0f} MB store "
                           f"(+{q['store_bytes_transport'] / 1e6:.0f} MB transport weights), larger than the 126 MB L2",
                     "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (one problem per GPU)",
-                    "build_channels_s": t_build, "store_bytes": q["store_bytes_gather"] + q["store_bytes_transport"]})
+                    "build_channels_s": t_build, "store_bytes": sb + q["store_bytes_transport"]})
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg, "e2e": e2e,

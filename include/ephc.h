@@ -90,8 +90,8 @@ typedef struct ephc_counts {
     int64_t ndiag;         /* q=0, n==m terms (transport only) */
     int64_t gather_entries;   /* ordered entries of the destination-sorted (two-sided) store */
     int64_t gather_halfpairs; /* (k <- k') half-pair rows of that store */
-    int64_t scatter_entries;  /* entries of the once-stored (one-sided) store */
-    int64_t scatter_pairs;
+    int64_t scatter_entries;  /* entries of the once-stored (tile) store, = nw + diagonal weights; 0 if unavailable */
+    int64_t scatter_pairs;    /* pair records of that store */
     int64_t store_bytes_gather;   /* device bytes of the two-sided store (collision + transport share it) */
     int64_t store_bytes_scatter;  /* device bytes of the one-sided store incl. its transposed index */
     int64_t store_bytes_transport;/* device bytes of the per-entry transport weights (0 before transport_setup) */
@@ -123,11 +123,22 @@ int ephc_export_diag(const ephc_handle *h, int32_t *s, int32_t *iq, int32_t *nu,
 int ephc_export_gather(const ephc_handle *h, int32_t *dest, int32_t *partner, int32_t *iq, int32_t *nu,
                        int32_t *kind, int32_t *diag, double *w);
 
+/* Decoded image of the once-stored (tile) store, same conditions as ephc_export_gather.  Arrays of length
+ * scatter_entries in store order: state a = (n,k), state b = (m,k'), canonical iq, mode, kind (0: w_abs, 1: w_em,
+ * as seen from a), diagonal flag, weight.  Walks CTAs -> tiles -> slices -> lanes exactly as the kernels do and
+ * checks tickets, slots and coverage on the way. */
+int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
+                      int32_t *diag, double *w);
+
 /* Choice of collision algorithm for ephc_collision / ephc_rt_step:
  *   0 = gather  : destination-sorted two-sided store, one kernel, every ordered term read once
- *   1 = scatter : once-stored channels, forward segmented reduce + per-pair reverse partials gathered
- *                 through the transposed index (PAPER.md:88-102 restructured; no global atomics) */
+ *   1 = tiles   : once-stored channels grouped into (k-block, k'-block) tiles; one lane per (k,k') pair updates
+ *                 both ends of its channels in shared memory in a fixed ticket order, per-tile partial sums
+ *                 are added per state by a second kernel (PAPER.md:88-102 restructured; no atomics).
+ *                 Available for nb <= 4, nnu <= 8, nq <= 2^24; it is the default when available.
+ * ephc_transport_setup must be called again after a change of variant. */
 int ephc_set_variant(ephc_handle *h, int variant);
+int ephc_get_variant(const ephc_handle *h);
 
 /* I[s] = collision integral of Eq. 2 for occupations f and phonon occupations N. */
 int ephc_collision(ephc_handle *h, const double *f_dev, const double *N_dev, double *I_dev, void *stream);

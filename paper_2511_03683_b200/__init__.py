@@ -68,7 +68,9 @@ def _load():
         "ephc_export_channels": (i32, [vp] * 9),
         "ephc_export_diag": (i32, [vp] * 6),
         "ephc_export_gather": (i32, [vp] * 8),
+        "ephc_export_tiles": (i32, [vp] * 8),
         "ephc_set_variant": (i32, [vp, i32]),
+        "ephc_get_variant": (i32, [vp]),
         "ephc_collision": (i32, [vp, vp, vp, vp, vp]),
         "ephc_transport_setup": (i32, [vp, vp, vp, vp, vp]),
         "ephc_transport_start": (i32, [vp, vp, vp, vp, vp, vp]),
@@ -187,8 +189,22 @@ class Handle:
         keys = ("dest", "partner", "iq", "nu", "kind", "diag", "w")
         return {k: a[:ne] for k, a in zip(keys, ints + [w])}
 
+    def export_tiles(self) -> dict:
+        ne = self.query()["scatter_entries"]
+        n = max(ne, 1)
+        ints = [np.zeros(n, np.int32) for _ in range(6)]
+        w = np.zeros(n, np.float64)
+        _check(_load().ephc_export_tiles(self._h, *[a.ctypes.data for a in ints], w.ctypes.data))
+        keys = ("a", "b", "iq", "nu", "kind", "diag", "w")
+        return {k: a[:ne] for k, a in zip(keys, ints + [w])}
+
     def set_variant(self, variant: int):
         _check(_load().ephc_set_variant(self._h, int(variant)))
+
+    def get_variant(self) -> int:
+        v = int(_load().ephc_get_variant(self._h))
+        _check(min(v, 0))
+        return v
 
     def launch_count(self) -> int:
         return int(_load().ephc_launch_count(self._h))

@@ -2,8 +2,10 @@
 // Product code: shares nothing with oracle/.  No CPU fallback: compute entry points need a CUDA device.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -11,6 +13,7 @@
 
 #include "ephc_internal.h"
 #include "ephc_kernels.cuh"
+#include "ephc_tile_kernels.cuh"
 
 using namespace ephc;
 
@@ -55,12 +58,30 @@ struct ephc_handle {
     int64_t launches = 0;
     int64_t bytes_gather = 0, bytes_transport = 0;
     bool attrs_set = false;
+    // tile store (variant 1)
+    TileHost thost;  // arrays kept only for EPHC_HOST_ONLY handles (ephc_export_tiles); scalars always
+    bool tile_ok = false;
+    int64_t t_entries = 0, t_pieces = 0, t_part_rows = 0, bytes_tile = 0;
+    int32_t t_ncta = 0, t_R = 0, t_nblk = 0, t_nslot = 0, t_ntile = 0;
+    double *dt_w = nullptr, *dt_part = nullptr, *dt_Wf = nullptr, *dt_Wr = nullptr;
+    uint16_t *dt_code = nullptr;
+    uint32_t *dt_prec = nullptr;
+    TileSlice *dt_slices = nullptr;
+    TileHdr *dt_tiles = nullptr;
+    TileCta *dt_ctas = nullptr;
+    int32_t *dt_blk_row0 = nullptr, *dt_row_state = nullptr, *dt_state_row = nullptr, *dt_state_blk = nullptr,
+            *dt_blk_slot_ptr = nullptr, *dt_blk_slots = nullptr;
+    int64_t *dt_slot_off = nullptr;
+    int transport_variant = -1;
 };
 
 static void free_dev(ephc_handle *h) {
     void *ptrs[] = {h->d_code, h->d_w, h->d_hp_k, h->d_hp_q, h->d_tasks, h->d_rounds, h->d_wus, h->d_gW,
                     h->d_y[0], h->d_y[1], h->d_ksum, h->d_wusum, h->d_hf, h->d_hN, h->d_hI, h->d_tr[0],
-                    h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf};
+                    h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
+                    h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
+                    h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_slot_ptr, h->dt_blk_slots,
+                    h->dt_slot_off};
     for (void *p : ptrs)
         if (p) cudaFree(p);
 }
@@ -112,6 +133,39 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         delete h;
         return fail(rc, err);
     }
+    // tile store (variant 1): two CTAs per SM walk the tile sequence
+    int n_sm = 148;
+    if (!h->host_only) {
+        int dev = 0;
+        cudaDeviceProp prop;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&prop, dev) == cudaSuccess)
+            n_sm = prop.multiProcessorCount;
+    }
+    int ncta = 2 * n_sm;
+    if (const char *e = std::getenv("EPHC_TILE_CTAS")) ncta = std::max(1, std::atoi(e));
+    TileHost &th = h->thost;
+    rc = build_tiles(p, h->d, h->can, ncta, th, err);
+    if (rc != EPHC_OK) {
+        delete h;
+        return fail(rc, err);
+    }
+    h->tile_ok = th.supported;
+    if (th.supported) {
+        h->t_entries = (int64_t)th.w.size();
+        h->t_pieces = th.npiece;
+        h->t_part_rows = th.part_rows;
+        h->t_ncta = th.ncta;
+        h->t_R = th.R;
+        h->t_nblk = th.nblk;
+        h->t_nslot = (int32_t)th.slot_off.size();
+        h->t_ntile = (int32_t)th.tiles.size();
+        h->bytes_tile = (int64_t)(th.w.size() * 8 + th.code.size() * 2 + th.prec.size() * 4 +
+                                  th.slices.size() * sizeof(TileSlice) + th.tiles.size() * sizeof(TileHdr) +
+                                  th.ctas.size() * sizeof(TileCta) + th.slot_off.size() * 8 +
+                                  (th.blk_row0.size() + th.row_state.size() + th.state_row.size() +
+                                   th.state_blk.size() + th.blk_slot_ptr.size() + th.blk_slots.size()) * 4);
+        h->variant = 1;
+    }
     h->pair_ik.assign(p->pair_ik, p->pair_ik + p->npair);
     h->pair_ikq.assign(p->pair_ikq, p->pair_ikq + p->npair);
     h->g_entries = (int64_t)g.code.size();
@@ -135,6 +189,32 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         if (rc == EPHC_OK) rc = upload(&h->d_tasks, g.tasks, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_rounds, g.rounds, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_wus, g.wus, &b);
+        if (rc == EPHC_OK && th.supported) {
+            int64_t bt = 0;
+            rc = upload(&h->dt_w, th.w, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_code, th.code, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_prec, th.prec, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_slices, th.slices, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_tiles, th.tiles, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_ctas, th.ctas, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_blk_row0, th.blk_row0, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_row_state, th.row_state, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_state_row, th.state_row, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_state_blk, th.state_blk, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_blk_slot_ptr, th.blk_slot_ptr, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_blk_slots, th.blk_slots, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_slot_off, th.slot_off, &bt);
+            if (rc == EPHC_OK) {
+                cudaError_t ce2 = cudaMalloc((void **)&h->dt_part, (size_t)std::max<int64_t>(1, th.part_rows) * 3 * 8);
+                if (ce2 != cudaSuccess) rc = fail(EPHC_ENOMEM, "cudaMalloc (partial sums) failed");
+            }
+            // the device owns the image now; keep only the scalars
+            TileHost empty;
+            empty.supported = th.supported;
+            empty.R = th.R; empty.nblk = th.nblk; empty.nrows = th.nrows; empty.ncta = th.ncta;
+            empty.part_rows = th.part_rows; empty.npiece = th.npiece;
+            th = empty;
+        }
         if (rc != EPHC_OK) {
             free_dev(h);
             delete h;
@@ -169,6 +249,9 @@ extern "C" int ephc_query(const ephc_handle *h, ephc_counts *o) {
     o->gather_entries = h->g_entries;
     o->gather_halfpairs = h->g_halfpairs;
     o->store_bytes_gather = h->bytes_gather;
+    o->scatter_entries = h->t_entries;
+    o->scatter_pairs = h->t_pieces;
+    o->store_bytes_scatter = h->bytes_tile;
     o->store_bytes_transport = h->bytes_transport;
     // B_alg: every item the method must move once per evaluation.
     //   8 N_w weights + 4 N_ch channel index + 12 N_pair (ik, ikq, iq) + 16 N_s (read f, write I) + 8 nnu N_q,active
@@ -258,12 +341,91 @@ extern "C" int ephc_export_gather(const ephc_handle *h, int32_t *dest, int32_t *
     return EPHC_OK;
 }
 
+extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu,
+                                 int32_t *kind, int32_t *diag, double *w) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (!h->host_only) return fail(EPHC_ESTATE, "ephc_export_tiles needs a handle built with EPHC_HOST_ONLY");
+    if (!h->tile_ok) return fail(EPHC_ESTATE, "tile store not available for this problem: " + h->thost.why);
+    const TileHost &t = h->thost;
+    const int64_t npc = t.npiece;
+    std::vector<uint8_t> seen(t.w.size(), 0), tile_seen(t.tiles.size(), 0);
+    std::vector<int32_t> tick_a((size_t)t.R), tick_b((size_t)t.R);
+    for (const TileCta &cta : t.ctas)
+        for (int32_t it = cta.t0; it < cta.t1; ++it) {
+            const TileHdr &th = t.tiles[it];
+            if (tile_seen[it]++) return fail(EPHC_ESTATE, "internal: tile walked by two CTAs");
+            const bool dg = th.bi == th.bj;
+            if (th.bi > th.bj || th.a_slot < 0 || (dg != (th.b_slot < 0)))
+                return fail(EPHC_ESTATE, "internal: bad tile header");
+            auto in_list = [&](int32_t blk, int32_t slot) {
+                for (int32_t i = t.blk_slot_ptr[blk]; i < t.blk_slot_ptr[blk + 1]; ++i)
+                    if (t.blk_slots[i] == slot) return true;
+                return false;
+            };
+            if (!in_list(th.bi, th.a_slot) || (!dg && !in_list(th.bj, th.b_slot)))
+                return fail(EPHC_ESTATE, "internal: slot missing from its block list");
+            const int32_t rows_a = t.blk_row0[th.bi + 1] - t.blk_row0[th.bi];
+            const int32_t rows_b = t.blk_row0[th.bj + 1] - t.blk_row0[th.bj];
+            std::fill(tick_a.begin(), tick_a.end(), 0);
+            std::fill(tick_b.begin(), tick_b.end(), 0);
+            std::vector<int32_t> &tb = dg ? tick_a : tick_b;
+            for (int32_t sidx = th.s0; sidx < th.s0 + th.ns; ++sidx) {
+                const TileSlice &sl = t.slices[sidx];
+                if (sl.np < 1 || sl.np > 32) return fail(EPHC_ESTATE, "internal: bad slice");
+                int len[32];
+                for (int l = 0; l < sl.np; ++l) {
+                    len[l] = (int)(t.prec[npc + sl.p0 + l] >> 24);
+                    if (len[l] < 1 || (l > 0 && len[l] > len[l - 1]) || (l == 0 && len[l] != sl.maxlen))
+                        return fail(EPHC_ESTATE, "internal: lane lengths must descend from maxlen");
+                }
+                std::vector<int> colstart((size_t)sl.maxlen + 1, 0);
+                for (int i = 0; i < sl.maxlen; ++i) {
+                    int cnt = 0;
+                    for (int l = 0; l < sl.np; ++l) cnt += len[l] > i;
+                    colstart[i + 1] = colstart[i] + cnt;
+                }
+                for (int l = 0; l < sl.np; ++l) {
+                    const uint32_t r0 = t.prec[sl.p0 + l], r1 = t.prec[npc + sl.p0 + l], r2 = t.prec[2 * npc + sl.p0 + l];
+                    const int32_t ra = r0 & 0xffff, rb = r0 >> 16;
+                    const int32_t nia = ((r2 >> 12) & 3) + 1, nib = ((r2 >> 28) & 3) + 1;
+                    if (ra + nia > rows_a || rb + nib > rows_b) return fail(EPHC_ESTATE, "internal: row outside its block");
+                    if ((int32_t)(r2 & 0xfff) != tick_a[ra]++ || (int32_t)((r2 >> 16) & 0xfff) != tb[rb]++)
+                        return fail(EPHC_ESTATE, "internal: tickets out of order");
+                    for (int i = 0; i < len[l]; ++i) {
+                        const int64_t o = sl.e0 + colstart[i] + l;
+                        if (o < 0 || o >= (int64_t)seen.size() || seen[o]) return fail(EPHC_ESTATE, "internal: entry visited twice");
+                        seen[o] = 1;
+                        const uint16_t c = t.code[o];
+                        const int32_t n = c & 3, m = (c >> kTcM) & 3;
+                        if (n >= nia || m >= nib) return fail(EPHC_ESTATE, "internal: band rank outside the window");
+                        if (a) a[o] = t.row_state[t.blk_row0[th.bi] + ra + n];
+                        if (b) b[o] = t.row_state[t.blk_row0[th.bj] + rb + m];
+                        if (iq) iq[o] = (int32_t)(r1 & 0xffffff);
+                        if (nu) nu[o] = (c >> kTcNu) & 7;
+                        if (kind) kind[o] = (c >> kTcKind) & 1;
+                        if (diag) diag[o] = (c >> kTcDiag) & 1;
+                        if (w) w[o] = t.w[o];
+                    }
+                }
+            }
+        }
+    for (uint8_t s : seen)
+        if (!s) return fail(EPHC_ESTATE, "internal: entry not covered by any slice");
+    for (uint8_t s : tile_seen)
+        if (!s) return fail(EPHC_ESTATE, "internal: tile not assigned to a CTA");
+    return EPHC_OK;
+}
+
 extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
-    if (variant != 0) return fail(EPHC_ESTATE, "variant 1 (scatter) is not built in this version");
+    if (variant != 0 && variant != 1) return fail(EPHC_EINVAL, "variant must be 0 (gather) or 1 (tiles)");
+    if (variant == 1 && !h->tile_ok)
+        return fail(EPHC_ESTATE, "tile store not available for this problem: " + h->thost.why);
     h->variant = variant;
     return EPHC_OK;
 }
+
+extern "C" int ephc_get_variant(const ephc_handle *h) { return h ? h->variant : EPHC_EINVAL; }
 
 extern "C" int64_t ephc_launch_count(const ephc_handle *h) { return h ? h->launches : 0; }
 
@@ -280,8 +442,82 @@ static int need_device(ephc_handle *h) {
                                       (int)gather_smem_bytes(kTransportSetup)));
         CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)gather_smem_bytes(kTransportIter)));
+        if (h->tile_ok) {
+            const int sc = (int)tile_smem_bytes(kTCollision, h->t_R), si = (int)tile_smem_bytes(kTIter, h->t_R);
+#define EPHC_TILE_ATTR(NB_)                                                                                       \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, sc)); \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTSetup, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, sc));     \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTIter, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, si));
+            EPHC_TILE_ATTR(1)
+            EPHC_TILE_ATTR(2)
+            EPHC_TILE_ATTR(4)
+#undef EPHC_TILE_ATTR
+        }
         h->attrs_set = true;
     }
+    return EPHC_OK;
+}
+
+static TileParams tile_params(const ephc_handle *h) {
+    TileParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.w = h->dt_w;
+    P.code = h->dt_code;
+    P.prec = h->dt_prec;
+    P.npiece = h->t_pieces;
+    P.slices = h->dt_slices;
+    P.tiles = h->dt_tiles;
+    P.ctas = h->dt_ctas;
+    P.blk_row0 = h->dt_blk_row0;
+    P.row_state = h->dt_row_state;
+    P.slot_off = h->dt_slot_off;
+    P.R = h->t_R;
+    P.nnu = h->d.nnu;
+    P.ns = h->d.ns;
+    P.part = h->dt_part;
+    P.Wf = h->dt_Wf;
+    P.Wr = h->dt_Wr;
+    return P;
+}
+
+static FinishParams finish_params(const ephc_handle *h) {
+    FinishParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.state_row = h->dt_state_row;
+    P.state_blk = h->dt_state_blk;
+    P.blk_row0 = h->dt_blk_row0;
+    P.blk_slot_ptr = h->dt_blk_slot_ptr;
+    P.blk_slots = h->dt_blk_slots;
+    P.slot_off = h->dt_slot_off;
+    P.part = h->dt_part;
+    P.ns = h->d.ns;
+    return P;
+}
+
+static inline unsigned finish_grid(const ephc_handle *h) { return (unsigned)((h->d.ns + 255) / 256); }
+
+template <int MODE>
+static int launch_tile(ephc_handle *h, const TileParams &P, cudaStream_t s) {
+    if (h->t_ntile > 0) {
+        const size_t sm = tile_smem_bytes(MODE, h->t_R);
+        const int nb = h->d.nb;
+        if (nb <= 1)
+            tile_kernel<MODE, 1><<<h->t_ncta, kTileThreads, sm, s>>>(P);
+        else if (nb <= 2)
+            tile_kernel<MODE, 2><<<h->t_ncta, kTileThreads, sm, s>>>(P);
+        else
+            tile_kernel<MODE, 4><<<h->t_ncta, kTileThreads, sm, s>>>(P);
+        h->launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
+template <int FMODE>
+static int launch_finish(ephc_handle *h, const FinishParams &P, cudaStream_t s) {
+    finish_kernel<FMODE><<<finish_grid(h), 256, 0, s>>>(P);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
     return EPHC_OK;
 }
 
@@ -326,6 +562,15 @@ extern "C" int ephc_collision(ephc_handle *h, const double *f_dev, const double 
     int rc = need_device(h);
     if (rc) return rc;
     if (!f_dev || !N_dev || !I_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (h->variant == 1) {
+        TileParams T = tile_params(h);
+        T.f = f_dev;
+        T.N = N_dev;
+        if ((rc = launch_tile<kTCollision>(h, T, (cudaStream_t)stream))) return rc;
+        FinishParams Fp = finish_params(h);
+        Fp.out = I_dev;
+        return launch_finish<kFCollision>(h, Fp, (cudaStream_t)stream);
+    }
     GatherParams P = base_params(h);
     P.f = f_dev;
     P.N = N_dev;
@@ -338,17 +583,39 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
     int rc = need_device(h);
     if (rc) return rc;
     if (!f0_dev || !N_dev || !Gamma_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (h->variant == 1) {
+        if (!h->dt_Wf) {
+            if ((rc = ensure(&h->dt_Wf, (size_t)h->t_entries * 8)) || (rc = ensure(&h->dt_Wr, (size_t)h->t_entries * 8)))
+                return rc;
+            h->bytes_transport += h->t_entries * 16;
+        }
+        TileParams T = tile_params(h);
+        T.f = f0_dev;
+        T.N = N_dev;
+        if ((rc = launch_tile<kTSetup>(h, T, (cudaStream_t)stream))) return rc;
+        FinishParams Fp = finish_params(h);
+        Fp.out = Gamma_dev;
+        rc = launch_finish<kFSetup>(h, Fp, (cudaStream_t)stream);
+        if (rc == EPHC_OK) {
+            h->transport_ready = true;
+            h->transport_variant = 1;
+        }
+        return rc;
+    }
     if (!h->d_gW) {
         rc = ensure(&h->d_gW, (size_t)h->g_entries * 8);
         if (rc) return rc;
-        h->bytes_transport = h->g_entries * 8;
+        h->bytes_transport += h->g_entries * 8;
     }
     GatherParams P = base_params(h);
     P.f = f0_dev;
     P.N = N_dev;
     P.out = Gamma_dev;
     rc = launch_gather<kTransportSetup>(h, P, (cudaStream_t)stream);
-    if (rc == EPHC_OK) h->transport_ready = true;
+    if (rc == EPHC_OK) {
+        h->transport_ready = true;
+        h->transport_variant = 0;
+    }
     return rc;
 }
 
@@ -370,7 +637,18 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
     if (rc) return rc;
     if (!F_dev || !v_dev || !tau_dev || !Fout_dev) return fail(EPHC_EINVAL, "null device pointer");
     if (F_dev == Fout_dev) return fail(EPHC_EINVAL, "transport_iter is out of place: F_dev and Fout_dev must differ");
-    if (!h->transport_ready) return fail(EPHC_ESTATE, "call ephc_transport_setup before ephc_transport_iter");
+    if (!h->transport_ready || h->transport_variant != h->variant)
+        return fail(EPHC_ESTATE, "call ephc_transport_setup (with the current variant) before ephc_transport_iter");
+    if (h->variant == 1) {
+        TileParams T = tile_params(h);
+        T.F = F_dev;
+        if ((rc = launch_tile<kTIter>(h, T, (cudaStream_t)stream))) return rc;
+        FinishParams Fp = finish_params(h);
+        Fp.out = Fout_dev;
+        Fp.v = v_dev;
+        Fp.tau = tau_dev;
+        return launch_finish<kFIter>(h, Fp, (cudaStream_t)stream);
+    }
     GatherParams P = base_params(h);
     P.F = F_dev;
     P.v = v_dev;
@@ -387,7 +665,7 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
     if (nsteps < 0 || !std::isfinite(dt_fs)) return fail(EPHC_EINVAL, "nsteps >= 0 and finite dt required");
     const size_t nb8 = (size_t)h->d.ns * 8;
     if ((rc = ensure(&h->d_y[0], nb8)) || (rc = ensure(&h->d_y[1], nb8)) || (rc = ensure(&h->d_ksum, nb8)) ||
-        (rc = ensure(&h->d_wusum, (size_t)(h->n_wu > 0 ? h->n_wu : 1) * 8)))
+        (rc = ensure(&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, finish_grid(h)), 1) * 8)))
         return rc;
     cudaStream_t s = (cudaStream_t)stream;
     if (sumf_dev) {
@@ -406,6 +684,21 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
         for (int st = 0; st < 4; ++st) {
+            if (h->variant == 1) {
+                TileParams T = tile_params(h);
+                T.f = src[st];
+                T.N = N_dev;
+                if ((rc = launch_tile<kTCollision>(h, T, s))) return rc;
+                FinishParams Fp = finish_params(h);
+                Fp.stage = st + 1;
+                Fp.dt = dt_fs;
+                Fp.f0 = f_dev;
+                Fp.ynext = dst[st];
+                Fp.ksum = h->d_ksum;
+                Fp.blk_sum = sumf_dev ? h->d_wusum : nullptr;
+                if ((rc = launch_finish<kFRkStage>(h, Fp, s))) return rc;
+                continue;
+            }
             P.stage = st + 1;
             P.f = src[st];
             P.ynext = dst[st];
@@ -413,7 +706,9 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
             if (rc) return rc;
         }
         if (sumf_dev) {
-            if (h->n_wu > 0)
+            if (h->variant == 1)
+                sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);
+            else if (h->n_wu > 0)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, h->n_wu, sumf_dev + it + 1);
             else
                 sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev + it + 1);

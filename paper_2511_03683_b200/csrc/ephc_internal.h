@@ -77,4 +77,58 @@ struct Dims {
 int build_canonical(const ephc_problem *p, const Dims &d, Canonical &c, std::string &err);
 int build_gather(const ephc_problem *p, const Dims &d, const Canonical &c, GatherHost &g, std::string &err);
 
+// ---- tile store (variant 1): every channel stored once, both of its ends updated by the same thread ----------
+// (DESIGN.md "Tile store").  States inside the energy window get a compact row index; compact rows are cut into
+// blocks of <= R rows (whole k points); tile (I,J), I <= J, holds every active pair with k in block I and k' in
+// block J.  A CTA walks a contiguous run of tiles; per tile it keeps f (or F) and the accumulators of both
+// blocks in shared memory, processes the tile's pairs one lane per pair (slices of 32 pairs, sorted by length,
+// entries stored column-major per slice), and adds every pair's partial sums into the shared accumulators in a
+// fixed, host-assigned ticket order per k point (plain read-modify-write, no atomics, bit-reproducible).
+constexpr int kTileNbMax = 4;        // bands handled in registers (compact band rank < 4)
+constexpr int kTileNnuMax = 8;       // modes handled in registers
+constexpr int kTilePieceMax = 255;   // entries per pair record (longer pairs are split into pieces)
+constexpr int kTileTicketMax = 4095; // pair records per k point and tile
+// entry code (uint16): compact band rank at k | rank at k' << 2 | mode << 4 | kind << 7 | diagonal << 8
+constexpr uint32_t kTcM = 2, kTcNu = 4, kTcKind = 7, kTcDiag = 8;
+// pair record: 3 x uint32, stored as three arrays [3][npiece]
+//   [0] first compact row of k, local to block I | first compact row of k', local to block J << 16
+//   [1] canonical iq (24 bits) | number of entries (8 bits) << 24
+//   [2] ticket at k (12 bits) | (in-window bands at k) - 1 << 12 | ticket at k' << 16 | (bands at k') - 1 << 28
+struct TileSlice {   // 32 pair records, lanes sorted by descending length
+    int64_t e0;      // first entry
+    int32_t p0;      // first pair record
+    int16_t np;      // pair records (1..32)
+    int16_t maxlen;  // entries of lane 0
+};
+struct TileHdr {
+    int32_t s0, ns;          // slice range
+    int32_t bi, bj;          // blocks
+    int32_t a_slot, b_slot;  // partial-sum slots (b_slot = -1 on a diagonal tile)
+    int32_t flags;           // bit 0: first tile of an a-run (stage block I, zero its accumulators); bit 1: last
+    int32_t pad;
+};
+struct TileCta {
+    int32_t t0, t1;          // tile range
+};
+struct TileHost {
+    int32_t R = 0, nblk = 0, nrows = 0, ncta = 0;
+    std::vector<int32_t> blk_row0;    // [nblk+1] compact row range of a block
+    std::vector<int32_t> row_state;   // [nrows] state index of a compact row
+    std::vector<int32_t> state_row;   // [ns] compact row of a state, -1 outside the window
+    std::vector<int32_t> state_blk;   // [ns] block of a state's row, -1 outside the window
+    std::vector<double> w;            // entries
+    std::vector<uint16_t> code;
+    std::vector<uint32_t> prec;       // [3][npiece]
+    std::vector<TileSlice> slices;
+    std::vector<TileHdr> tiles;
+    std::vector<TileCta> ctas;
+    std::vector<int64_t> slot_off;    // [nslot] offset of a slot in rows (x components in the kernels)
+    std::vector<int32_t> blk_slot_ptr, blk_slots;  // CSR: slots that hold partial sums of a block
+    int64_t part_rows = 0;            // total rows of all slots
+    int64_t npiece = 0;               // pair records
+    bool supported = false;           // false: shape outside the register path (nb > 4, nnu > 8, ...)
+    std::string why;                  // reason when unsupported
+};
+int build_tiles(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, TileHost &t, std::string &err);
+
 }  // namespace ephc

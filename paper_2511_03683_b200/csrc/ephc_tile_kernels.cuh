@@ -1,0 +1,385 @@
+// ephc_tile_kernels.cuh -- sm_100a kernels of the tile path (variant 1): every channel is read ONCE and updates
+// both I(n,k) and I(m,k+q); no atomics on global or shared memory.
+//
+// tile_kernel<MODE, NB>: a CTA walks a contiguous run of (k-block I, k'-block J) tiles.  Per tile it keeps, in
+// shared memory, the inputs of both blocks (f, or F for transport) and one accumulator per compact row of both
+// blocks.  A warp takes slices of 32 pair records; one LANE = one (k, k') pair:
+//   prologue  the pair's f_a[0..nb), f_b[0..nb) (shared memory) and N[iq, 0..nnu) (L2) go to registers
+//   loop      the pair's entries stream from HBM, column-major per slice (coalesced, every byte used once);
+//             Eq. 2's summand is evaluated from registers and added to per-band register accumulators of both ends
+//   epilogue  the lane adds its <= nb partial sums per end into the shared accumulators of k and of k', in the
+//             ticket order the host assigned per k point: a plain load-add-store once the k point's counter
+//             shows the lane's ticket.  The order is fixed, so results are bit-reproducible.
+// At the end of a tile (or of a run of tiles with the same block I) the accumulators go to a partial-sum slot.
+// finish_kernel: one thread per state adds the slots of its block in a fixed order and applies the epilogue
+// (I, the fused RK4 stage update, Gamma, or tau (v + sum)).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "ephc_internal.h"
+
+namespace ephc {
+
+enum TileMode : int { kTCollision = 0, kTSetup = 2, kTIter = 3 };
+enum FinishMode : int { kFCollision = 0, kFRkStage = 1, kFSetup = 2, kFIter = 3 };
+
+struct TileParams {
+    // store
+    const double *w;
+    const uint16_t *code;
+    const uint32_t *prec;  // [3][npiece]
+    int64_t npiece;
+    const TileSlice *slices;
+    const TileHdr *tiles;
+    const TileCta *ctas;
+    const int32_t *blk_row0, *row_state;
+    const int64_t *slot_off;
+    int32_t R, nnu;
+    int64_t ns;
+    // inputs
+    const double *f;  // occupations (collision / RK stage input y_j / f0 of transport_setup)
+    const double *N;
+    const double *F;  // transport_iter input [3][ns]
+    // outputs
+    double *part;     // partial-sum slots, [part_rows][C]
+    double *Wf, *Wr;  // per entry: W(a<-b), W(b<-a); written by setup, read by iter
+};
+
+struct FinishParams {
+    const int32_t *state_row, *state_blk, *blk_row0, *blk_slot_ptr, *blk_slots;
+    const int64_t *slot_off;
+    const double *part;
+    int64_t ns;
+    double *out;  // I, Gamma or Fout
+    // rk stage
+    int32_t stage;
+    double dt;
+    double *f0, *ynext, *ksum, *blk_sum;
+    // transport
+    const double *v, *tau;
+};
+
+template <int NB>
+__device__ __forceinline__ double sel_nb(const double (&a)[NB], int j) {
+    if (NB == 1) return a[0];
+    if (NB == 2) return (j & 1) ? a[1] : a[0];
+    const double lo = (j & 1) ? a[1 % NB] : a[0], hi = (j & 1) ? a[3 % NB] : a[2 % NB];
+    return (j & 2) ? hi : lo;
+}
+__device__ __forceinline__ double sel8(const double (&a)[8], int j) {
+    const double x0 = (j & 1) ? a[1] : a[0], x1 = (j & 1) ? a[3] : a[2], x2 = (j & 1) ? a[5] : a[4],
+                 x3 = (j & 1) ? a[7] : a[6];
+    const double y0 = (j & 2) ? x1 : x0, y1 = (j & 2) ? x3 : x2;
+    return (j & 4) ? y1 : y0;
+}
+template <int NB>
+__device__ __forceinline__ void put_nb(double (&a)[NB], int j, double x) {
+#pragma unroll
+    for (int i = 0; i < NB; ++i) a[i] = (j == i) ? x : a[i];
+}
+
+__device__ __forceinline__ unsigned ld_cnt(const uint16_t *p) { return *(const volatile uint16_t *)p; }
+__device__ __forceinline__ void st_cnt(uint16_t *p, unsigned v) { *(volatile uint16_t *)p = (uint16_t)v; }
+
+constexpr int kTileThreads = 256;
+
+inline size_t tile_smem_bytes(int mode, int R) {
+    const int C = (mode == kTIter) ? 3 : 1;
+    const size_t rows = (size_t)R + kTileNbMax;
+    return 4 * rows * C * sizeof(double) + 2 * (((size_t)R + 7) & ~(size_t)7) * sizeof(uint16_t) + 16;
+}
+
+template <int MODE, int NB>
+__global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_kernel(const TileParams P) {
+    constexpr int C = (MODE == kTIter) ? 3 : 1;
+    extern __shared__ double smem[];
+    const int R = P.R, rows_al = R + kTileNbMax;
+    double *sIa = smem;                    // inputs of block I:  f[row] or F[row][3]
+    double *sIb = sIa + rows_al * C;       // inputs of block J
+    double *sAa = sIb + rows_al * C;       // accumulators of block I
+    double *sAb = sAa + rows_al * C;       // accumulators of block J
+    uint16_t *sCa = reinterpret_cast<uint16_t *>(sAb + rows_al * C);  // ticket counters per k point (first row)
+    uint16_t *sCb = sCa + ((R + 7) & ~7);
+    int *sNext = reinterpret_cast<int *>(sCb + ((R + 7) & ~7));
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const TileCta cta = P.ctas[blockIdx.x];
+    const int nnu = P.nnu;
+    const int64_t np_all = P.npiece;
+
+    for (int it = cta.t0; it < cta.t1; ++it) {
+        const TileHdr th = P.tiles[it];
+        const bool dg = (th.bi == th.bj);
+        const int row0a = P.blk_row0[th.bi], rows_a = P.blk_row0[th.bi + 1] - row0a;
+        const int row0b = P.blk_row0[th.bj], rows_b = P.blk_row0[th.bj + 1] - row0b;
+        // ---- stage the inputs of both blocks, clear accumulators and ticket counters ------------------------------
+        if (th.flags & 1) {
+            for (int r = tid; r < rows_a + kTileNbMax; r += kTileThreads) {
+                const int64_t s = (r < rows_a) ? P.row_state[row0a + r] : -1;
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    sIa[r * C + c] = (s < 0) ? 0.0 : (MODE == kTIter ? P.F[(int64_t)c * P.ns + s] : P.f[s]);
+                    sAa[r * C + c] = 0.0;
+                }
+            }
+        }
+        if (!dg) {
+            for (int r = tid; r < rows_b + kTileNbMax; r += kTileThreads) {
+                const int64_t s = (r < rows_b) ? P.row_state[row0b + r] : -1;
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    sIb[r * C + c] = (s < 0) ? 0.0 : (MODE == kTIter ? P.F[(int64_t)c * P.ns + s] : P.f[s]);
+                    sAb[r * C + c] = 0.0;
+                }
+            }
+        }
+        for (int r = tid; r < R; r += kTileThreads) {
+            sCa[r] = 0;
+            sCb[r] = 0;
+        }
+        if (tid == 0) *sNext = 0;
+        __syncthreads();
+        const double *inB = dg ? sIa : sIb;
+        double *accB = dg ? sAa : sAb;
+        uint16_t *cntB = dg ? sCa : sCb;
+
+        // ---- slices: one lane per pair record --------------------------------------------------------------------------
+        while (true) {
+            int g = 0;
+            if (lane == 0) g = atomicAdd(sNext, 1);  // order of execution only
+            g = __shfl_sync(0xffffffffu, g, 0);
+            if (g >= th.ns) break;
+            const int4 sl4 = __ldg(reinterpret_cast<const int4 *>(P.slices + th.s0 + g));
+            const int64_t e0 = ((int64_t)(uint32_t)sl4.x) | ((int64_t)sl4.y << 32);
+            const int p0 = sl4.z;
+            const int np = (int)(int16_t)(sl4.w & 0xffff), maxlen = (int)(int16_t)((uint32_t)sl4.w >> 16);
+            const bool live = lane < np;
+            uint32_t r0 = 0, r1 = 0, r2 = 0;
+            if (live) {
+                r0 = __ldcs(P.prec + p0 + lane);
+                r1 = __ldcs(P.prec + np_all + p0 + lane);
+                r2 = __ldcs(P.prec + 2 * np_all + p0 + lane);
+            }
+            const int ra = r0 & 0xffffu, rb = r0 >> 16;
+            const int len = (int)(r1 >> 24);
+            const double *wp = P.w + e0 + lane;
+            const uint16_t *cp = P.code + e0 + lane;
+
+            double acc_a[C][NB], acc_b[C][NB];
+#pragma unroll
+            for (int c = 0; c < C; ++c)
+#pragma unroll
+                for (int j = 0; j < NB; ++j) acc_a[c][j] = acc_b[c][j] = 0.0;
+
+            if (MODE == kTIter) {
+                // F_a[n][c], F_b[m][c] in registers
+                double Fa[3][NB], Fb[3][NB];
+#pragma unroll
+                for (int j = 0; j < NB; ++j)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        Fa[c][j] = sIa[(ra + j) * 3 + c];
+                        Fb[c][j] = inB[(rb + j) * 3 + c];
+                    }
+                const double *wfp = P.Wf + e0 + lane, *wrp = P.Wr + e0 + lane;
+                int off = 0;
+                for (int i = 0; i < maxlen; i += 2) {
+                    const bool a0 = len > i, a1 = len > i + 1;
+                    const int c0 = __popc(__ballot_sync(0xffffffffu, a0)), c1 = __popc(__ballot_sync(0xffffffffu, a1));
+                    double wf0 = 0.0, wr0 = 0.0, wf1 = 0.0, wr1 = 0.0;
+                    unsigned k0 = 0, k1 = 0;
+                    if (a0) {
+                        wf0 = __ldcs(wfp + off);
+                        wr0 = __ldcs(wrp + off);
+                        k0 = __ldcs(cp + off);
+                    }
+                    if (a1) {
+                        wf1 = __ldcs(wfp + off + c0);
+                        wr1 = __ldcs(wrp + off + c0);
+                        k1 = __ldcs(cp + off + c0);
+                    }
+                    off += c0 + c1;
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const double wf = u ? wf1 : wf0, wr = u ? wr1 : wr0;
+                        const unsigned k = u ? k1 : k0;
+                        const int n = k & 3u, m = (k >> kTcM) & 3u;
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            put_nb<NB>(acc_a[c], n, fma(wf, sel_nb<NB>(Fb[c], m), sel_nb<NB>(acc_a[c], n)));
+                            put_nb<NB>(acc_b[c], m, fma(wr, sel_nb<NB>(Fa[c], n), sel_nb<NB>(acc_b[c], m)));
+                        }
+                    }
+                }
+            } else {
+                double fa[NB], fb[NB], Nq[8];
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    fa[j] = sIa[ra + j];
+                    fb[j] = inB[rb + j];
+                }
+                {
+                    const double *Np = P.N + (int64_t)(r1 & 0xffffffu) * nnu;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) Nq[j] = (j < nnu) ? __ldg(Np + j) : 0.0;
+                }
+                int off = 0;
+                for (int i = 0; i < maxlen; i += 2) {
+                    const bool a0 = len > i, a1 = len > i + 1;
+                    const int c0 = __popc(__ballot_sync(0xffffffffu, a0)), c1 = __popc(__ballot_sync(0xffffffffu, a1));
+                    double w0 = 0.0, w1 = 0.0;
+                    unsigned k0 = 0, k1 = 0;
+                    if (a0) {
+                        w0 = __ldcs(wp + off);
+                        k0 = __ldcs(cp + off);
+                    }
+                    if (a1) {
+                        w1 = __ldcs(wp + off + c0);
+                        k1 = __ldcs(cp + off + c0);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const double wv = u ? w1 : w0;
+                        const unsigned k = u ? k1 : k0;
+                        const int n = k & 3u, m = (k >> kTcM) & 3u, nu = (k >> kTcNu) & 7u;
+                        const bool em = (k >> kTcKind) & 1u, diag = (k >> kTcDiag) & 1u;
+                        const double xa = sel_nb<NB>(fa, n), xb = sel_nb<NB>(fb, m), Nn = sel8(Nq, nu);
+                        if (MODE == kTCollision) {
+                            // Eq. 2 summand (reading R-1), rearranged:  F_abs = (fa-fb) N + fa fb - fb,
+                            //                                         F_em  = (fa-fb) N + fa - fa fb
+                            const double pr = xa * xb;
+                            const double s = em ? (xa - pr) : (pr - xb);
+                            const double T = (diag ? 0.0 : wv) * fma(xa - xb, Nn, s);
+                            put_nb<NB>(acc_a[0], n, sel_nb<NB>(acc_a[0], n) + T);
+                            put_nb<NB>(acc_b[0], m, sel_nb<NB>(acc_b[0], m) + T);
+                        } else {
+                            // reading R-16: W(a<-b) = w (1 + N - f0_b) [em] or w (N + f0_b) [abs];
+                            //               W(b<-a) = w (N + f0_a) [em] or w (1 + N - f0_a) [abs]; diagonal: forward only
+                            const double Wf = em ? wv * (1.0 + Nn - xb) : wv * (Nn + xb);
+                            const double Wr = diag ? 0.0 : (em ? wv * (Nn + xa) : wv * (1.0 + Nn - xa));
+                            const bool act = u ? a1 : a0;
+                            const int o = u ? off + c0 : off;
+                            if (act) {
+                                P.Wf[e0 + lane + o] = Wf;
+                                P.Wr[e0 + lane + o] = Wr;
+                            }
+                            put_nb<NB>(acc_a[0], n, sel_nb<NB>(acc_a[0], n) + Wf);
+                            put_nb<NB>(acc_b[0], m, sel_nb<NB>(acc_b[0], m) + Wr);
+                        }
+                    }
+                    off += c0 + c1;
+                }
+            }
+
+            // ---- epilogue: ticket-ordered read-modify-write of the shared accumulators -------------------------------
+            // Collision: I[a] -= T, I[b] += T.  Transport: both ends add their own weight sums.
+            const unsigned ta = r2 & 0xfffu, tb = (r2 >> 16) & 0xfffu;
+            const int nia = (int)((r2 >> 12) & 3u) + 1, nib = (int)((r2 >> 28) & 3u) + 1;
+            bool pa = live, pb = live;
+            while (__any_sync(0xffffffffu, pa || pb)) {
+                if (pa && ld_cnt(sCa + ra) == ta) {
+                    __threadfence_block();
+#pragma unroll
+                    for (int j = 0; j < NB; ++j)
+                        if (j < nia) {
+#pragma unroll
+                            for (int c = 0; c < C; ++c) {
+                                const double x = acc_a[c][j];
+                                sAa[(ra + j) * C + c] += (MODE == kTCollision) ? -x : x;
+                            }
+                        }
+                    __threadfence_block();
+                    st_cnt(sCa + ra, ta + 1);
+                    pa = false;
+                }
+                if (pb && !pa && ld_cnt(cntB + rb) == tb) {
+                    __threadfence_block();
+#pragma unroll
+                    for (int j = 0; j < NB; ++j)
+                        if (j < nib) {
+#pragma unroll
+                            for (int c = 0; c < C; ++c) accB[(rb + j) * C + c] += acc_b[c][j];
+                        }
+                    __threadfence_block();
+                    st_cnt(cntB + rb, tb + 1);
+                    pb = false;
+                }
+                __syncwarp();
+            }
+        }
+        __syncthreads();
+        // ---- partial sums of this tile / run go to their slots ---------------------------------------------------------
+        if (!dg) {
+            double *dst = P.part + P.slot_off[th.b_slot] * C;
+            for (int i = tid; i < rows_b * C; i += kTileThreads) dst[i] = sAb[i];
+        }
+        if (th.flags & 2) {
+            double *dst = P.part + P.slot_off[th.a_slot] * C;
+            for (int i = tid; i < rows_a * C; i += kTileThreads) dst[i] = sAa[i];
+        }
+        __syncthreads();
+    }
+}
+
+// One thread per state: sum of the block's partial-sum slots in list order, then the epilogue of the call.
+template <int FMODE>
+__global__ void __launch_bounds__(256) finish_kernel(const FinishParams P) {
+    constexpr int C = (FMODE == kFIter) ? 3 : 1;
+    const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double sum[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) sum[c] = 0.0;
+    double fsum = 0.0;
+    if (a < P.ns) {
+        const int cr = P.state_row[a];
+        if (cr >= 0) {
+            const int b = P.state_blk[a];
+            const int64_t r = cr - P.blk_row0[b];
+            for (int i = P.blk_slot_ptr[b]; i < P.blk_slot_ptr[b + 1]; ++i) {
+                const double *src = P.part + (P.slot_off[P.blk_slots[i]] + r) * C;
+#pragma unroll
+                for (int c = 0; c < C; ++c) sum[c] += src[c];
+            }
+        }
+        if (FMODE == kFCollision || FMODE == kFSetup) {
+            P.out[a] = sum[0];
+        } else if (FMODE == kFIter) {
+            const double ta = P.tau[a];
+#pragma unroll
+            for (int c = 0; c < C; ++c) P.out[(int64_t)c * P.ns + a] = ta * (P.v[(int64_t)c * P.ns + a] + sum[c]);
+        } else {  // RK4 stage (reading R-18): k_j = I[y_j]
+            const double k = sum[0];
+            const double f0 = P.f0[a];
+            if (P.stage == 1) {
+                P.ksum[a] = k;
+                P.ynext[a] = f0 + 0.5 * P.dt * k;
+            } else if (P.stage == 2) {
+                P.ksum[a] += 2.0 * k;
+                P.ynext[a] = f0 + 0.5 * P.dt * k;
+            } else if (P.stage == 3) {
+                P.ksum[a] += 2.0 * k;
+                P.ynext[a] = f0 + P.dt * k;
+            } else {
+                const double fn = f0 + P.dt / 6.0 * (P.ksum[a] + k);
+                P.f0[a] = fn;
+                fsum = fn;
+            }
+        }
+    }
+    if (FMODE == kFRkStage) {
+        if (P.stage == 4 && P.blk_sum != nullptr) {  // uniform over the grid
+            __shared__ double sRed[8];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) fsum += __shfl_xor_sync(0xffffffffu, fsum, o);
+            if ((threadIdx.x & 31) == 0) sRed[threadIdx.x >> 5] = fsum;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double s = 0.0;
+                for (int wi = 0; wi < 8; ++wi) s += sRed[wi];
+                P.blk_sum[blockIdx.x] = s;
+            }
+        }
+    }
+}
+
+}  // namespace ephc

@@ -37,10 +37,20 @@ def _small_problems():
 IDS = ["tiny4", "window_cut_diag", "si12", "gaas24", "bigcell3", "tiny_full", "rt14"]
 
 
-@pytest.fixture(scope="module", params=range(len(IDS)), ids=IDS)
+VARIANTS = {0: "gather", 1: "tiles"}
+
+
+@pytest.fixture(scope="module", params=[(i, v) for i in range(len(IDS)) for v in VARIANTS],
+                ids=[f"{n}-{VARIANTS[v]}" for n in IDS for v in VARIANTS])
 def case(request):
-    p = _small_problems()[request.param]
-    return p, oracle.OracleList(p), ephc.build_channels(p)
+    idx, variant = request.param
+    p = _small_problems()[idx]
+    h = ephc.build_channels(p)
+    if variant == 1 and h.query()["scatter_entries"] == 0 and h.query()["nw"] > 0:
+        assert h.get_variant() == 0
+        pytest.skip("tile store covers nb <= 4, nnu <= 8 (DESIGN.md): this shape runs on the gather path")
+    h.set_variant(variant)
+    return p, oracle.OracleList(p), h
 
 
 def _relerr(a, b):
@@ -173,6 +183,7 @@ def test_multi_round_segments_on_gpu(monkeypatch):
     for p in _small_problems()[:4]:
         L = oracle.OracleList(p)
         h = ephc.build_channels(p)
+        h.set_variant(0)
         q = h.query()
         assert q["n_rounds"] > 2 * q["n_workunits"]
         I = np.zeros(p.ns)
@@ -189,6 +200,37 @@ def test_multi_round_segments_on_gpu(monkeypatch):
         f = p.f.copy()
         h.rt_step_host(f, p.N, 1.0, 5, None)
         assert _relerr(f, L.rt_step(p.f, p.N, 1.0, 5)[0]) <= TOL
+
+
+@pytest.mark.parametrize("rows,ctas", [(8, 3), (16, 40), (64, 1), (2048, 7)])
+def test_tile_geometry_on_gpu(monkeypatch, rows, ctas):
+    # many small tiles, runs cut by CTA boundaries, one CTA for everything, one tile for everything
+    monkeypatch.setenv("EPHC_TILE_ROWS", str(rows))
+    monkeypatch.setenv("EPHC_TILE_CTAS", str(ctas))
+    for p in _small_problems()[:4]:
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p)
+        assert h.get_variant() == 1
+        I = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I)
+        assert _relerr(I, L.collision(p.f, p.N)) <= TOL
+        I2 = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I2)
+        assert np.array_equal(I, I2)
+        F, G = np.zeros((3, p.ns)), np.zeros(p.ns)
+        h.transport_solve_host(p.f0, p.N, p.v, 3, F, G)
+        Go = L.transport_setup(p.f0, p.N)
+        assert _relerr(G, Go) <= TOL
+        tau = np.where(Go > 0, 1.0 / np.where(Go > 0, Go, 1.0), 0.0)
+        Fr = tau[None, :] * p.v
+        for _ in range(3):
+            Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau)
+        assert _relerr(F, Fr) <= TOL
+        f = p.f.copy()
+        s = np.zeros(6)
+        h.rt_step_host(f, p.N, 1.0, 5, s)
+        fo, so = L.rt_step(p.f, p.N, 1.0, 5)
+        assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
 
 
 def test_stream_argument_is_honoured():

@@ -110,6 +110,54 @@ def test_gather_store_holds_every_ordered_term_once(prob):
     assert np.abs(G - Go).max() <= 1e-12 * Go.max()
 
 
+@pytest.mark.parametrize("rows,ctas", [(None, None), (8, 5), (16, 64), (2048, 1)])
+def test_tile_store_holds_every_channel_once(prob, rows, ctas, monkeypatch):
+    if rows is not None:
+        monkeypatch.setenv("EPHC_TILE_ROWS", str(rows))
+        monkeypatch.setenv("EPHC_TILE_CTAS", str(ctas))
+    L = oracle.OracleList(prob)
+    h = ephc.build_channels(prob, flags=ephc.HOST_ONLY)
+    q = h.query()
+    if prob.nb > 4 or prob.nnu > 8:
+        assert q["scatter_entries"] == 0 and h.get_variant() == 0     # outside the register path: gather store
+        with pytest.raises(ephc.EphcError):
+            h.set_variant(1)
+        return
+    assert h.get_variant() == 1
+    t = h.export_tiles()      # also checks tickets, slots, lane order and that every entry is covered once
+    ch, dg = L.export(), L.export_diag()
+    nw_d = int((dg["w_abs"] != 0).sum() + (dg["w_em"] != 0).sum())
+    assert q["scatter_entries"] == L.nw + nw_d
+    a = ch["ik"] * prob.nb + ch["n"]
+    b = ch["ikq"] * prob.nb + ch["m"]
+    rows_, ws = [], []
+    for wk, kd in (("w_abs", 0), ("w_em", 1)):
+        sel = ch[wk] != 0
+        rows_.append(np.stack([a[sel], b[sel], ch["iq"][sel], ch["nu"][sel], np.full(sel.sum(), kd), np.zeros(sel.sum(), int)]))
+        ws.append(ch[wk][sel])
+        seld = dg[wk] != 0
+        rows_.append(np.stack([dg["s"][seld], dg["s"][seld], dg["iq"][seld], dg["nu"][seld], np.full(seld.sum(), kd), np.ones(seld.sum(), int)]))
+        ws.append(dg[wk][seld])
+    exp = np.concatenate(rows_, axis=1).astype(np.int64)
+    expw = np.concatenate(ws)
+    got = np.stack([t[k] for k in ("a", "b", "iq", "nu", "kind", "diag")]).astype(np.int64)
+    assert exp.shape == got.shape
+    oe = np.lexsort(exp[::-1]); og = np.lexsort(got[::-1])
+    assert np.array_equal(exp[:, oe], got[:, og])
+    assert _ulp_close(t["w"][og], expw[oe], 4)
+    # the store, evaluated with numpy in Eq. 2's printed form, reproduces the oracle's collision integral
+    f, N = prob.f, prob.N
+    fa, fb, Nq = f[t["a"]], f[t["b"]], N[t["iq"].astype(np.int64) * prob.nnu + t["nu"]]
+    out_, in_ = fa * (1 - fb), fb * (1 - fa)
+    T = t["w"] * np.where(t["kind"] == 1, out_ * (Nq + 1) - in_ * Nq, out_ * Nq - in_ * (Nq + 1))
+    T = np.where(t["diag"] == 1, 0.0, T)
+    I = np.zeros(prob.ns)
+    np.add.at(I, t["a"], -T)
+    np.add.at(I, t["b"], T)
+    Io = L.collision(f, N)
+    assert np.abs(I - Io).max() <= 1e-12 * np.abs(Io).max()
+
+
 def test_launch_geometry_limits():
     # a segment with more half-pairs than one round can stage (tiny 8x8x8: 512 partners per k, 5 doubles each)
     # and a dense many-band block: both must split into rounds/tasks within the kernel's limits
