@@ -133,7 +133,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         delete h;
         return fail(rc, err);
     }
-    // tile store (variant 1): two CTAs per SM walk the tile sequence
+    // tile store (variant 1): three CTAs per SM walk the tile sequence
     int n_sm = 148;
     if (!h->host_only) {
         int dev = 0;
@@ -141,7 +141,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         if (cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&prop, dev) == cudaSuccess)
             n_sm = prop.multiProcessorCount;
     }
-    int ncta = 2 * n_sm;
+    int ncta = 3 * n_sm;
     if (const char *e = std::getenv("EPHC_TILE_CTAS")) ncta = std::max(1, std::atoi(e));
     TileHost &th = h->thost;
     rc = build_tiles(p, h->d, h->can, ncta, th, err);
@@ -443,11 +443,13 @@ static int need_device(ephc_handle *h) {
         CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)gather_smem_bytes(kTransportIter)));
         if (h->tile_ok) {
-            const int sc = (int)tile_smem_bytes(kTCollision, h->t_R), si = (int)tile_smem_bytes(kTIter, h->t_R);
 #define EPHC_TILE_ATTR(NB_)                                                                                       \
-    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, sc)); \
-    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTSetup, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, sc));     \
-    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTIter, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, si));
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
+                                  (int)tile_smem_bytes(kTCollision, h->t_R, NB_)));                                 \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTSetup, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,           \
+                                  (int)tile_smem_bytes(kTSetup, h->t_R, NB_)));                                     \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTIter, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,            \
+                                  (int)tile_smem_bytes(kTIter, h->t_R, NB_)));
             EPHC_TILE_ATTR(1)
             EPHC_TILE_ATTR(2)
             EPHC_TILE_ATTR(4)
@@ -499,14 +501,13 @@ static inline unsigned finish_grid(const ephc_handle *h) { return (unsigned)((h-
 template <int MODE>
 static int launch_tile(ephc_handle *h, const TileParams &P, cudaStream_t s) {
     if (h->t_ntile > 0) {
-        const size_t sm = tile_smem_bytes(MODE, h->t_R);
         const int nb = h->d.nb;
         if (nb <= 1)
-            tile_kernel<MODE, 1><<<h->t_ncta, kTileThreads, sm, s>>>(P);
+            tile_kernel<MODE, 1><<<h->t_ncta, kTileThreads, tile_smem_bytes(MODE, h->t_R, 1), s>>>(P);
         else if (nb <= 2)
-            tile_kernel<MODE, 2><<<h->t_ncta, kTileThreads, sm, s>>>(P);
+            tile_kernel<MODE, 2><<<h->t_ncta, kTileThreads, tile_smem_bytes(MODE, h->t_R, 2), s>>>(P);
         else
-            tile_kernel<MODE, 4><<<h->t_ncta, kTileThreads, sm, s>>>(P);
+            tile_kernel<MODE, 4><<<h->t_ncta, kTileThreads, tile_smem_bytes(MODE, h->t_R, 4), s>>>(P);
         h->launches++;
     }
     CUDA_TRY(cudaGetLastError());

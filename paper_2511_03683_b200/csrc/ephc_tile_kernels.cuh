@@ -82,16 +82,28 @@ __device__ __forceinline__ unsigned ld_cnt(const uint16_t *p) { return *(const v
 __device__ __forceinline__ void st_cnt(uint16_t *p, unsigned v) { *(volatile uint16_t *)p = (uint16_t)v; }
 
 constexpr int kTileThreads = 256;
+constexpr int kTileBatch = 4;  // entries per lane whose loads are in flight while the previous batch is evaluated
 
-inline size_t tile_smem_bytes(int mode, int R) {
+// Per-thread private rows in shared memory (row r of thread t at [r * kTileThreads + t]: conflict-free):
+//   collision / setup: 0..3 f_a[n], 4..7 f_b[m], 8..15 N[nu], 16..19 sums for k, 20..23 sums for k'
+//   transport_iter:    (c*NB + n) sums for k, (3*NB + c*NB + m) sums for k'
+// Dynamic indexing by band / mode costs one LDS here instead of a chain of selects on registers.
+constexpr int kRowBytes = kTileThreads * 8;
+inline int tile_priv_rows(int mode, int nbp) { return (mode == kTIter) ? 6 * nbp : 24; }
+
+inline size_t tile_smem_bytes(int mode, int R, int nbp) {
     const int C = (mode == kTIter) ? 3 : 1;
     const size_t rows = (size_t)R + kTileNbMax;
-    return 4 * rows * C * sizeof(double) + 2 * (((size_t)R + 7) & ~(size_t)7) * sizeof(uint16_t) + 16;
+    return 4 * rows * C * sizeof(double) + 2 * (((size_t)R + 7) & ~(size_t)7) * sizeof(uint16_t) + 16 +
+           (size_t)tile_priv_rows(mode, nbp) * kRowBytes;
 }
+
+__device__ __forceinline__ double &prow(char *tb, unsigned byte_off) { return *reinterpret_cast<double *>(tb + byte_off); }
 
 template <int MODE, int NB>
 __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_kernel(const TileParams P) {
     constexpr int C = (MODE == kTIter) ? 3 : 1;
+    constexpr int U = kTileBatch;
     extern __shared__ double smem[];
     const int R = P.R, rows_al = R + kTileNbMax;
     double *sIa = smem;                    // inputs of block I:  f[row] or F[row][3]
@@ -101,8 +113,10 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
     uint16_t *sCa = reinterpret_cast<uint16_t *>(sAb + rows_al * C);  // ticket counters per k point (first row)
     uint16_t *sCb = sCa + ((R + 7) & ~7);
     int *sNext = reinterpret_cast<int *>(sCb + ((R + 7) & ~7));
+    double *sPriv = reinterpret_cast<double *>(sNext + 4);
 
     const int tid = threadIdx.x, lane = tid & 31;
+    char *tb = reinterpret_cast<char *>(sPriv + tid);
     const TileCta cta = P.ctas[blockIdx.x];
     const int nnu = P.nnu;
     const int64_t np_all = P.npiece;
@@ -162,17 +176,38 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
             }
             const int ra = r0 & 0xffffu, rb = r0 >> 16;
             const int len = (int)(r1 >> 24);
-            const double *wp = P.w + e0 + lane;
-            const uint16_t *cp = P.code + e0 + lane;
+            const int64_t eb = e0 + lane;
 
-            double acc_a[C][NB], acc_b[C][NB];
+            // batch loader: columns i0 .. i0+U-1 of the slice (column i holds the lanes with len > i, a prefix)
+            int off = 0;
+            double wq[U], vq[U];
+            unsigned kq[U];
+            int oq[U];
+            auto load_batch = [&](int i0) {
 #pragma unroll
-            for (int c = 0; c < C; ++c)
-#pragma unroll
-                for (int j = 0; j < NB; ++j) acc_a[c][j] = acc_b[c][j] = 0.0;
+                for (int u = 0; u < U; ++u) {
+                    const bool act = len > i0 + u;
+                    const int cnt = __popc(__ballot_sync(0xffffffffu, act));
+                    wq[u] = 0.0;
+                    vq[u] = 0.0;
+                    kq[u] = 0;
+                    oq[u] = off;
+                    if (act) {
+                        kq[u] = __ldcs(P.code + eb + off);
+                        if (MODE == kTIter) {
+                            wq[u] = __ldcs(P.Wf + eb + off);
+                            vq[u] = __ldcs(P.Wr + eb + off);
+                        } else {
+                            wq[u] = __ldcs(P.w + eb + off);
+                        }
+                    }
+                    off += cnt;
+                }
+            };
+            load_batch(0);
 
+            double acc_a[C][NB], acc_b[C][NB];  // this lane's sums per end and band, filled before the epilogue
             if (MODE == kTIter) {
-                // F_a[n][c], F_b[m][c] in registers
                 double Fa[3][NB], Fb[3][NB];
 #pragma unroll
                 for (int j = 0; j < NB; ++j)
@@ -181,93 +216,107 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                         Fa[c][j] = sIa[(ra + j) * 3 + c];
                         Fb[c][j] = inB[(rb + j) * 3 + c];
                     }
-                const double *wfp = P.Wf + e0 + lane, *wrp = P.Wr + e0 + lane;
-                int off = 0;
-                for (int i = 0; i < maxlen; i += 2) {
-                    const bool a0 = len > i, a1 = len > i + 1;
-                    const int c0 = __popc(__ballot_sync(0xffffffffu, a0)), c1 = __popc(__ballot_sync(0xffffffffu, a1));
-                    double wf0 = 0.0, wr0 = 0.0, wf1 = 0.0, wr1 = 0.0;
-                    unsigned k0 = 0, k1 = 0;
-                    if (a0) {
-                        wf0 = __ldcs(wfp + off);
-                        wr0 = __ldcs(wrp + off);
-                        k0 = __ldcs(cp + off);
-                    }
-                    if (a1) {
-                        wf1 = __ldcs(wfp + off + c0);
-                        wr1 = __ldcs(wrp + off + c0);
-                        k1 = __ldcs(cp + off + c0);
-                    }
-                    off += c0 + c1;
 #pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const double wf = u ? wf1 : wf0, wr = u ? wr1 : wr0;
-                        const unsigned k = u ? k1 : k0;
-                        const int n = k & 3u, m = (k >> kTcM) & 3u;
+                for (int j = 0; j < 6 * NB; ++j) prow(tb, j * kRowBytes) = 0.0;
+                for (int i = 0; i < maxlen; i += U) {
+                    double wc[U], vc[U];
+                    unsigned kc[U];
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        wc[u] = wq[u];
+                        vc[u] = vq[u];
+                        kc[u] = kq[u];
+                    }
+                    if (i + U < maxlen) load_batch(i + U);
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        const int n = kc[u] & 3u, m = (kc[u] >> kTcM) & 3u;
+                        char *pa_ = tb + n * kRowBytes, *pb_ = tb + (3 * NB + m) * kRowBytes;
+                        double sa[3], sb[3];
 #pragma unroll
                         for (int c = 0; c < 3; ++c) {
-                            put_nb<NB>(acc_a[c], n, fma(wf, sel_nb<NB>(Fb[c], m), sel_nb<NB>(acc_a[c], n)));
-                            put_nb<NB>(acc_b[c], m, fma(wr, sel_nb<NB>(Fa[c], n), sel_nb<NB>(acc_b[c], m)));
+                            sa[c] = prow(pa_, c * NB * kRowBytes);
+                            sb[c] = prow(pb_, c * NB * kRowBytes);
+                        }
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            prow(pa_, c * NB * kRowBytes) = fma(wc[u], sel_nb<NB>(Fb[c], m), sa[c]);
+                            prow(pb_, c * NB * kRowBytes) = fma(vc[u], sel_nb<NB>(Fa[c], n), sb[c]);
                         }
                     }
                 }
-            } else {
-                double fa[NB], fb[NB], Nq[8];
 #pragma unroll
-                for (int j = 0; j < NB; ++j) {
-                    fa[j] = sIa[ra + j];
-                    fb[j] = inB[rb + j];
-                }
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        acc_a[c][j] = prow(tb, (c * NB + j) * kRowBytes);
+                        acc_b[c][j] = prow(tb, (3 * NB + c * NB + j) * kRowBytes);
+                    }
+            } else {
                 {
                     const double *Np = P.N + (int64_t)(r1 & 0xffffffu) * nnu;
+                    double Nq[8];
 #pragma unroll
                     for (int j = 0; j < 8; ++j) Nq[j] = (j < nnu) ? __ldg(Np + j) : 0.0;
-                }
-                int off = 0;
-                for (int i = 0; i < maxlen; i += 2) {
-                    const bool a0 = len > i, a1 = len > i + 1;
-                    const int c0 = __popc(__ballot_sync(0xffffffffu, a0)), c1 = __popc(__ballot_sync(0xffffffffu, a1));
-                    double w0 = 0.0, w1 = 0.0;
-                    unsigned k0 = 0, k1 = 0;
-                    if (a0) {
-                        w0 = __ldcs(wp + off);
-                        k0 = __ldcs(cp + off);
-                    }
-                    if (a1) {
-                        w1 = __ldcs(wp + off + c0);
-                        k1 = __ldcs(cp + off + c0);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        prow(tb, j * kRowBytes) = sIa[ra + j];
+                        prow(tb, (4 + j) * kRowBytes) = inB[rb + j];
                     }
 #pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const double wv = u ? w1 : w0;
-                        const unsigned k = u ? k1 : k0;
-                        const int n = k & 3u, m = (k >> kTcM) & 3u, nu = (k >> kTcNu) & 7u;
+                    for (int j = 0; j < 8; ++j) {
+                        prow(tb, (8 + j) * kRowBytes) = Nq[j];
+                        prow(tb, (16 + j) * kRowBytes) = 0.0;
+                    }
+                }
+                for (int i = 0; i < maxlen; i += U) {
+                    double wc[U];
+                    unsigned kc[U];
+                    int oc[U];
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        wc[u] = wq[u];
+                        kc[u] = kq[u];
+                        oc[u] = oq[u];
+                    }
+                    const int ibase = i;
+                    if (i + U < maxlen) load_batch(i + U);
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        const unsigned k = kc[u];
+                        char *pa_ = tb + (k & 3u) * kRowBytes;
+                        char *pb_ = tb + (4 + ((k >> kTcM) & 3u)) * kRowBytes;
+                        const double Nn = prow(tb, (8 + ((k >> kTcNu) & 7u)) * kRowBytes);
+                        const double xa = prow(pa_, 0), xb = prow(pb_, 0);
                         const bool em = (k >> kTcKind) & 1u, diag = (k >> kTcDiag) & 1u;
-                        const double xa = sel_nb<NB>(fa, n), xb = sel_nb<NB>(fb, m), Nn = sel8(Nq, nu);
                         if (MODE == kTCollision) {
                             // Eq. 2 summand (reading R-1), rearranged:  F_abs = (fa-fb) N + fa fb - fb,
                             //                                         F_em  = (fa-fb) N + fa - fa fb
                             const double pr = xa * xb;
                             const double s = em ? (xa - pr) : (pr - xb);
-                            const double T = (diag ? 0.0 : wv) * fma(xa - xb, Nn, s);
-                            put_nb<NB>(acc_a[0], n, sel_nb<NB>(acc_a[0], n) + T);
-                            put_nb<NB>(acc_b[0], m, sel_nb<NB>(acc_b[0], m) + T);
+                            const double T = (diag ? 0.0 : wc[u]) * fma(xa - xb, Nn, s);
+                            const double sa = prow(pa_, 16 * kRowBytes), sb = prow(pb_, 16 * kRowBytes);
+                            prow(pa_, 16 * kRowBytes) = sa + T;
+                            prow(pb_, 16 * kRowBytes) = sb + T;
                         } else {
                             // reading R-16: W(a<-b) = w (1 + N - f0_b) [em] or w (N + f0_b) [abs];
                             //               W(b<-a) = w (N + f0_a) [em] or w (1 + N - f0_a) [abs]; diagonal: forward only
-                            const double Wf = em ? wv * (1.0 + Nn - xb) : wv * (Nn + xb);
-                            const double Wr = diag ? 0.0 : (em ? wv * (Nn + xa) : wv * (1.0 + Nn - xa));
-                            const bool act = u ? a1 : a0;
-                            const int o = u ? off + c0 : off;
-                            if (act) {
-                                P.Wf[e0 + lane + o] = Wf;
-                                P.Wr[e0 + lane + o] = Wr;
+                            const double Wf = em ? wc[u] * (1.0 + Nn - xb) : wc[u] * (Nn + xb);
+                            const double Wr = diag ? 0.0 : (em ? wc[u] * (Nn + xa) : wc[u] * (1.0 + Nn - xa));
+                            if (len > ibase + u) {
+                                P.Wf[eb + oc[u]] = Wf;
+                                P.Wr[eb + oc[u]] = Wr;
                             }
-                            put_nb<NB>(acc_a[0], n, sel_nb<NB>(acc_a[0], n) + Wf);
-                            put_nb<NB>(acc_b[0], m, sel_nb<NB>(acc_b[0], m) + Wr);
+                            const double sa = prow(pa_, 16 * kRowBytes), sb = prow(pb_, 16 * kRowBytes);
+                            prow(pa_, 16 * kRowBytes) = sa + Wf;
+                            prow(pb_, 16 * kRowBytes) = sb + Wr;
                         }
                     }
-                    off += c0 + c1;
+                }
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    acc_a[0][j] = prow(tb, (16 + j) * kRowBytes);
+                    acc_b[0][j] = prow(tb, (20 + j) * kRowBytes);
                 }
             }
 

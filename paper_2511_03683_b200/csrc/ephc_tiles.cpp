@@ -107,7 +107,7 @@ int build_tiles(const ephc_problem *p, const Dims &d, const Canonical &c, int nc
             const double nblk_t = std::sqrt(2.0 * 8.0 * ncta);
             const int r_bal = (int)std::ceil((double)std::max(t.nrows, 1) / nblk_t);
             R = std::max(std::min(R, r_bal), 32);
-            if (const char *e = std::getenv("EPHC_TILE_ROWS")) R = std::max(nb, std::min(2048, std::atoi(e)));
+            if (const char *e = std::getenv("EPHC_TILE_ROWS")) R = std::max(nb, std::min(1536, std::atoi(e)));  // 1536: transport_iter fits 227 KB
             R = std::max(R, nb);
         }
         t.R = R;
@@ -132,15 +132,20 @@ int build_tiles(const ephc_problem *p, const Dims &d, const Canonical &c, int nc
         const int64_t ntile_all = nblk * (nblk + 1) / 2;
         auto tile_id = [&](int64_t I, int64_t J) { return I * nblk - I * (I - 1) / 2 + (J - I); };
 
-        // ---- pieces per tile (canonical order inside a tile, then stable sort by descending length) --------------
+        // ---- pieces per tile (canonical order inside a tile, then stable sort by length) ----------------------------
         std::vector<int32_t> plen((size_t)npair, 0);
 #pragma omp parallel for schedule(dynamic, 4096)
         for (int64_t ip = 0; ip < npair; ++ip) plen[ip] = pair_len(c, ip);
+        // a pair longer than piece_max entries is cut into pieces (separate pair records, consecutive tickets): the
+        // longest slice bounds the idle tail of a tile
+        int piece_max = 24;
+        if (const char *e = std::getenv("EPHC_TILE_PIECE")) piece_max = std::atoi(e);
+        piece_max = std::max(1, std::min(kTilePieceMax, piece_max));
         std::vector<int64_t> tile_p0((size_t)ntile_all + 1, 0);
         for (int64_t ip = 0; ip < npair; ++ip) {
             if (plen[ip] == 0) continue;
             const int64_t tid = tile_id(blk_of_k[p->pair_ik[ip]], blk_of_k[p->pair_ikq[ip]]);
-            tile_p0[tid + 1] += (plen[ip] + kTilePieceMax - 1) / kTilePieceMax;
+            tile_p0[tid + 1] += (plen[ip] + piece_max - 1) / piece_max;
         }
         for (int64_t i = 0; i < ntile_all; ++i) tile_p0[i + 1] += tile_p0[i];
         const int64_t npiece = tile_p0[ntile_all];
@@ -154,8 +159,8 @@ int build_tiles(const ephc_problem *p, const Dims &d, const Canonical &c, int nc
             for (int64_t ip = 0; ip < npair; ++ip) {
                 if (plen[ip] == 0) continue;
                 const int64_t tid = tile_id(blk_of_k[p->pair_ik[ip]], blk_of_k[p->pair_ikq[ip]]);
-                for (int32_t f = 0; f < plen[ip]; f += kTilePieceMax)
-                    pieces[cur[tid]++] = Piece{(int32_t)ip, f, std::min(kTilePieceMax, plen[ip] - f)};
+                for (int32_t f = 0; f < plen[ip]; f += piece_max)
+                    pieces[cur[tid]++] = Piece{(int32_t)ip, f, std::min(piece_max, plen[ip] - f)};
             }
         }
         // non-empty tiles in row-major (I, J) order
@@ -175,7 +180,11 @@ int build_tiles(const ephc_problem *p, const Dims &d, const Canonical &c, int nc
 #pragma omp parallel for schedule(dynamic, 8)
         for (int64_t it = 0; it < ntile; ++it) {
             Piece *b = pieces.data() + tile_p0[live[it]], *e = pieces.data() + tile_p0[live[it] + 1];
-            std::stable_sort(b, e, [](const Piece &x, const Piece &y) { return x.len > y.len; });
+            // slices in ASCENDING length (a slice that starts earlier also ends earlier, so a lane rarely waits for
+            // the ticket of a pair in an earlier slice); lanes of one slice in descending length (the active lanes
+            // of every column are a prefix)
+            std::stable_sort(b, e, [](const Piece &x, const Piece &y) { return x.len < y.len; });
+            for (Piece *q = b; q < e; q += 32) std::reverse(q, std::min(q + 32, e));
             int64_t ne = 0;
             for (Piece *q = b; q != e; ++q) ne += q->len;
             tile_e0[it + 1] = ne;
