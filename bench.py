@@ -47,7 +47,7 @@ def parse():
     ap.add_argument("--config", default="si", help="workload: si (default, BASELINE configs[1]) | tiny | gaas | bigcell")
     ap.add_argument("--grid", type=int, default=0, help="override the grid edge (smaller copies for quick runs)")
     ap.add_argument("--pair-prob", type=float, default=0.0)
-    ap.add_argument("--variant", type=int, default=-1, help="-1: library default (tiles when available), 0: gather, 1: tiles")
+    ap.add_argument("--variant", type=int, default=-1, help="-1: automatic (library default), 0: gather, 1: tiles")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -205,7 +205,7 @@ def main():
     t_build = time.perf_counter() - t0
     if args.variant >= 0:
         h.set_variant(args.variant)
-    variant = h.get_variant()
+    variant, tvariant = h.get_variant(), h.get_transport_variant()
     q = h.query()
     nch, ns = q["nch"], p.ns
     dev = torch.device("cuda", local)
@@ -288,13 +288,13 @@ def main():
                       "share_of_step": share, "channel_terms_per_s": nch / (ms_launch * 1e-3) if ms_launch > 0 else 0.0}
 
     ms_step = ms_total / max(args.steps, 1)
+    kn = {"c": "gather_kernel<0>", "s": "gather_kernel<2>", "i": "gather_kernel<3>", "r": "gather_kernel<1>"}
+    w_setup = 8 * q["gather_entries"]
     if variant == 1:
-        kn = {"c": "tile_kernel<0> + finish_kernel<0>", "s": "tile_kernel<2> + finish_kernel<2>",
-              "i": "tile_kernel<3> + finish_kernel<3>", "r": "tile_kernel<0> + finish_kernel<1>"}
+        kn.update({"c": "tile_kernel<0> + finish_kernel<0>", "r": "tile_kernel<0> + finish_kernel<1>"})
+    if tvariant == 1:
+        kn.update({"s": "tile_kernel<2> + finish_kernel<2>", "i": "tile_kernel<3> + finish_kernel<3>"})
         w_setup = 16 * q["scatter_entries"]
-    else:
-        kn = {"c": "gather_kernel<0>", "s": "gather_kernel<2>", "i": "gather_kernel<3>", "r": "gather_kernel<1>"}
-        w_setup = 8 * q["gather_entries"]
     roof(f"collision ({kn['c']})", ms_coll, q["alg_bytes_collision"], ms_coll / ms_step)
     roof(f"transport_setup ({kn['s']})", ms_setup, q["alg_bytes_collision"] + w_setup, ms_setup / ms_step)
     roof(f"transport_iter ({kn['i']})", ms_iter / N_TRANSPORT_ITERS, q["alg_bytes_transport"], ms_iter / ms_step)
@@ -355,8 +355,9 @@ def main():
 
     if rank == 0:
         cfg = workload_config(args, p, nch)
-        sb = q["store_bytes_scatter"] if variant == 1 else q["store_bytes_gather"]
-        cfg.update({"variant": "tiles" if variant == 1 else "gather",
+        sb = (q["store_bytes_scatter"] if 1 in (variant, tvariant) else 0) + (q["store_bytes_gather"] if 0 in (variant, tvariant) else 0)
+        names = {0: "gather", 1: "tiles"}
+        cfg.update({"variant": f"collision/rt: {names[variant]}, transport: {names[tvariant]}",
                     "l2": f"no flush: every evaluation streams the {sb / 1e6:.0f} MB store "
                           f"(+{q['store_bytes_transport'] / 1e6:.0f} MB transport weights), larger than the 126 MB L2",
                     "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (one problem per GPU)",

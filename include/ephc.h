@@ -130,15 +130,20 @@ int ephc_export_gather(const ephc_handle *h, int32_t *dest, int32_t *partner, in
 int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
                       int32_t *diag, double *w);
 
-/* Choice of collision algorithm for ephc_collision / ephc_rt_step:
+/* Choice of algorithm:
  *   0 = gather  : destination-sorted two-sided store, one kernel, every ordered term read once
- *   1 = tiles   : once-stored channels grouped into (k-block, k'-block) tiles; one lane per (k,k') pair updates
+ *   1 = tiles   : once-stored channels grouped into (k-strip, k'-range) tiles; one lane per (k,k') pair updates
  *                 both ends of its channels in shared memory in a fixed ticket order, per-tile partial sums
  *                 are added per state by a second kernel (PAPER.md:88-102 restructured; no atomics).
- *                 Available for nb <= 4, nnu <= 8, nq <= 2^24; it is the default when available.
- * ephc_transport_setup must be called again after a change of variant. */
+ *                 Available for nb <= 4, nnu <= 8, nq <= 2^24.
+ *  -1 = automatic (default): ephc_collision / ephc_rt_step use the tile store when it is available,
+ *                 ephc_transport_setup / ephc_transport_iter the gather store (the faster choice per call as
+ *                 measured on B200).
+ * ephc_transport_setup must be called again after a change of variant.  ephc_get_variant returns the variant
+ * ephc_collision will use, ephc_get_transport_variant the one the transport calls will use. */
 int ephc_set_variant(ephc_handle *h, int variant);
 int ephc_get_variant(const ephc_handle *h);
+int ephc_get_transport_variant(const ephc_handle *h);
 
 /* I[s] = collision integral of Eq. 2 for occupations f and phonon occupations N. */
 int ephc_collision(ephc_handle *h, const double *f_dev, const double *N_dev, double *I_dev, void *stream);

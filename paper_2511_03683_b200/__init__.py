@@ -71,6 +71,7 @@ def _load():
         "ephc_export_tiles": (i32, [vp] * 8),
         "ephc_set_variant": (i32, [vp, i32]),
         "ephc_get_variant": (i32, [vp]),
+        "ephc_get_transport_variant": (i32, [vp]),
         "ephc_collision": (i32, [vp, vp, vp, vp, vp]),
         "ephc_transport_setup": (i32, [vp, vp, vp, vp, vp]),
         "ephc_transport_start": (i32, [vp, vp, vp, vp, vp, vp]),
@@ -202,7 +203,14 @@ class Handle:
         _check(_load().ephc_set_variant(self._h, int(variant)))
 
     def get_variant(self) -> int:
+        """Variant ephc_collision / ephc_rt_step will use (0 gather, 1 tiles)."""
         v = int(_load().ephc_get_variant(self._h))
+        _check(min(v, 0))
+        return v
+
+    def get_transport_variant(self) -> int:
+        """Variant ephc_transport_setup / ephc_transport_iter will use."""
+        v = int(_load().ephc_get_transport_variant(self._h))
         _check(min(v, 0))
         return v
 

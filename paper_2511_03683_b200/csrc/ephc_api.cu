@@ -33,7 +33,7 @@ static int fail(int code, const std::string &msg) {
 struct ephc_handle {
     Dims d{};
     bool host_only = false;
-    int variant = 0;
+    int variant = 0;  // -1: automatic (collision / rt_step on the tile store, transport on the gather store)
     Canonical can;
     GatherHost ghost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_gather)
     std::vector<int32_t> pair_ik, pair_ikq;  // copy of the candidate pair list (export)
@@ -62,7 +62,7 @@ struct ephc_handle {
     TileHost thost;  // arrays kept only for EPHC_HOST_ONLY handles (ephc_export_tiles); scalars always
     bool tile_ok = false;
     int64_t t_entries = 0, t_pieces = 0, t_part_rows = 0, bytes_tile = 0;
-    int32_t t_ncta = 0, t_R = 0, t_nblk = 0, t_nslot = 0, t_ntile = 0;
+    int32_t t_ncta = 0, t_Ra = 0, t_Rb = 0, t_nblk = 0, t_nslot = 0, t_ntile = 0;
     double *dt_w = nullptr, *dt_part = nullptr, *dt_Wf = nullptr, *dt_Wr = nullptr;
     uint16_t *dt_code = nullptr;
     uint32_t *dt_prec = nullptr;
@@ -70,8 +70,8 @@ struct ephc_handle {
     TileHdr *dt_tiles = nullptr;
     TileCta *dt_ctas = nullptr;
     int32_t *dt_blk_row0 = nullptr, *dt_row_state = nullptr, *dt_state_row = nullptr, *dt_state_blk = nullptr,
-            *dt_blk_slot_ptr = nullptr, *dt_blk_slots = nullptr;
-    int64_t *dt_slot_off = nullptr;
+            *dt_blk_ent_ptr = nullptr;
+    int64_t *dt_slot_off = nullptr, *dt_blk_ent_off = nullptr;
     int transport_variant = -1;
 };
 
@@ -80,7 +80,7 @@ static void free_dev(ephc_handle *h) {
                     h->d_y[0], h->d_y[1], h->d_ksum, h->d_wusum, h->d_hf, h->d_hN, h->d_hI, h->d_tr[0],
                     h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
-                    h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_slot_ptr, h->dt_blk_slots,
+                    h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
                     h->dt_slot_off};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -133,7 +133,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         delete h;
         return fail(rc, err);
     }
-    // tile store (variant 1): three CTAs per SM walk the tile sequence
+    // tile store (variant 1): two CTAs per SM walk the tile sequence (transport_iter: one CTA of twice the size per SM takes two shares)
     int n_sm = 148;
     if (!h->host_only) {
         int dev = 0;
@@ -141,7 +141,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         if (cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&prop, dev) == cudaSuccess)
             n_sm = prop.multiProcessorCount;
     }
-    int ncta = 3 * n_sm;
+    int ncta = 2 * n_sm;
     if (const char *e = std::getenv("EPHC_TILE_CTAS")) ncta = std::max(1, std::atoi(e));
     TileHost &th = h->thost;
     rc = build_tiles(p, h->d, h->can, ncta, th, err);
@@ -155,7 +155,8 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         h->t_pieces = th.npiece;
         h->t_part_rows = th.part_rows;
         h->t_ncta = th.ncta;
-        h->t_R = th.R;
+        h->t_Ra = th.Ra;
+        h->t_Rb = th.Rb;
         h->t_nblk = th.nblk;
         h->t_nslot = (int32_t)th.slot_off.size();
         h->t_ntile = (int32_t)th.tiles.size();
@@ -163,8 +164,8 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
                                   th.slices.size() * sizeof(TileSlice) + th.tiles.size() * sizeof(TileHdr) +
                                   th.ctas.size() * sizeof(TileCta) + th.slot_off.size() * 8 +
                                   (th.blk_row0.size() + th.row_state.size() + th.state_row.size() +
-                                   th.state_blk.size() + th.blk_slot_ptr.size() + th.blk_slots.size()) * 4);
-        h->variant = 1;
+                                   th.state_blk.size() + th.blk_ent_ptr.size()) * 4 + th.blk_ent_off.size() * 8);
+        h->variant = -1;
     }
     h->pair_ik.assign(p->pair_ik, p->pair_ik + p->npair);
     h->pair_ikq.assign(p->pair_ikq, p->pair_ikq + p->npair);
@@ -201,8 +202,8 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             if (rc == EPHC_OK) rc = upload(&h->dt_row_state, th.row_state, &bt);
             if (rc == EPHC_OK) rc = upload(&h->dt_state_row, th.state_row, &bt);
             if (rc == EPHC_OK) rc = upload(&h->dt_state_blk, th.state_blk, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_blk_slot_ptr, th.blk_slot_ptr, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_blk_slots, th.blk_slots, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_blk_ent_ptr, th.blk_ent_ptr, &bt);
+            if (rc == EPHC_OK) rc = upload(&h->dt_blk_ent_off, th.blk_ent_off, &bt);
             if (rc == EPHC_OK) rc = upload(&h->dt_slot_off, th.slot_off, &bt);
             if (rc == EPHC_OK) {
                 cudaError_t ce2 = cudaMalloc((void **)&h->dt_part, (size_t)std::max<int64_t>(1, th.part_rows) * 3 * 8);
@@ -211,7 +212,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             // the device owns the image now; keep only the scalars
             TileHost empty;
             empty.supported = th.supported;
-            empty.R = th.R; empty.nblk = th.nblk; empty.nrows = th.nrows; empty.ncta = th.ncta;
+            empty.Ra = th.Ra; empty.Rb = th.Rb; empty.nblk = th.nblk; empty.nrows = th.nrows; empty.ncta = th.ncta;
             empty.part_rows = th.part_rows; empty.npiece = th.npiece;
             th = empty;
         }
@@ -349,24 +350,25 @@ extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, i
     const TileHost &t = h->thost;
     const int64_t npc = t.npiece;
     std::vector<uint8_t> seen(t.w.size(), 0), tile_seen(t.tiles.size(), 0);
-    std::vector<int32_t> tick_a((size_t)t.R), tick_b((size_t)t.R);
+    std::vector<int32_t> tick_a((size_t)t.Ra), tick_b((size_t)t.Rb);
+    const int64_t nslot = (int64_t)t.slot_off.size();
     for (const TileCta &cta : t.ctas)
         for (int32_t it = cta.t0; it < cta.t1; ++it) {
             const TileHdr &th = t.tiles[it];
             if (tile_seen[it]++) return fail(EPHC_ESTATE, "internal: tile walked by two CTAs");
-            const bool dg = th.bi == th.bj;
-            if (th.bi > th.bj || th.a_slot < 0 || (dg != (th.b_slot < 0)))
+            const bool dg = (th.flags & 4) != 0;
+            const bool first = (it == cta.t0) || t.tiles[it - 1].a_row0 != th.a_row0;
+            const bool last = (it + 1 == cta.t1) || t.tiles[it + 1].a_row0 != th.a_row0;
+            if (th.a_slot < 0 || th.a_slot >= nslot || (dg != (th.b_slot < 0)) || th.b_slot >= nslot ||
+                first != ((th.flags & 1) != 0) || last != ((th.flags & 2) != 0) || th.a_rows > t.Ra || th.b_rows > t.Rb ||
+                (dg && (th.b_row0 != th.a_row0 || th.b_rows != th.a_rows)) || (!dg && th.b_row0 < th.a_row0 + th.a_rows))
                 return fail(EPHC_ESTATE, "internal: bad tile header");
-            auto in_list = [&](int32_t blk, int32_t slot) {
-                for (int32_t i = t.blk_slot_ptr[blk]; i < t.blk_slot_ptr[blk + 1]; ++i)
-                    if (t.blk_slots[i] == slot) return true;
-                return false;
-            };
-            if (!in_list(th.bi, th.a_slot) || (!dg && !in_list(th.bj, th.b_slot)))
-                return fail(EPHC_ESTATE, "internal: slot missing from its block list");
-            const int32_t rows_a = t.blk_row0[th.bi + 1] - t.blk_row0[th.bi];
-            const int32_t rows_b = t.blk_row0[th.bj + 1] - t.blk_row0[th.bj];
-            std::fill(tick_a.begin(), tick_a.end(), 0);
+            if (t.slot_row0[th.a_slot] != th.a_row0 || t.slot_rows[th.a_slot] != th.a_rows ||
+                (!dg && (t.slot_row0[th.b_slot] != th.b_row0 || t.slot_rows[th.b_slot] != th.b_rows)) ||
+                (!first && th.a_slot != t.tiles[it - 1].a_slot))
+                return fail(EPHC_ESTATE, "internal: slot does not match its tile");
+            const int32_t rows_a = th.a_rows, rows_b = th.b_rows;
+            if (first) std::fill(tick_a.begin(), tick_a.end(), 0);
             std::fill(tick_b.begin(), tick_b.end(), 0);
             std::vector<int32_t> &tb = dg ? tick_a : tick_b;
             for (int32_t sidx = th.s0; sidx < th.s0 + th.ns; ++sidx) {
@@ -398,8 +400,8 @@ extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, i
                         const uint16_t c = t.code[o];
                         const int32_t n = c & 3, m = (c >> kTcM) & 3;
                         if (n >= nia || m >= nib) return fail(EPHC_ESTATE, "internal: band rank outside the window");
-                        if (a) a[o] = t.row_state[t.blk_row0[th.bi] + ra + n];
-                        if (b) b[o] = t.row_state[t.blk_row0[th.bj] + rb + m];
+                        if (a) a[o] = t.row_state[th.a_row0 + ra + n];
+                        if (b) b[o] = t.row_state[th.b_row0 + rb + m];
                         if (iq) iq[o] = (int32_t)(r1 & 0xffffff);
                         if (nu) nu[o] = (c >> kTcNu) & 7;
                         if (kind) kind[o] = (c >> kTcKind) & 1;
@@ -413,19 +415,36 @@ extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, i
         if (!s) return fail(EPHC_ESTATE, "internal: entry not covered by any slice");
     for (uint8_t s : tile_seen)
         if (!s) return fail(EPHC_ESTATE, "internal: tile not assigned to a CTA");
+    // the finish kernel reaches every row of every slot exactly once through the fine-block lists
+    {
+        std::vector<uint8_t> cover((size_t)t.part_rows, 0);
+        for (int32_t b = 0; b < t.nblk; ++b)
+            for (int32_t i = t.blk_ent_ptr[b]; i < t.blk_ent_ptr[b + 1]; ++i)
+                for (int32_t r = 0; r < t.blk_row0[b + 1] - t.blk_row0[b]; ++r) {
+                    const int64_t o = t.blk_ent_off[i] + r;
+                    if (o < 0 || o >= t.part_rows || cover[o]++) return fail(EPHC_ESTATE, "internal: slot row listed twice");
+                }
+        for (uint8_t cv : cover)
+            if (!cv) return fail(EPHC_ESTATE, "internal: slot row not listed for the finish kernel");
+    }
     return EPHC_OK;
 }
 
+// variant used by ephc_collision / ephc_rt_step, and by ephc_transport_setup / ephc_transport_iter
+static inline int coll_variant(const ephc_handle *h) { return h->variant < 0 ? (h->tile_ok ? 1 : 0) : h->variant; }
+static inline int tr_variant(const ephc_handle *h) { return h->variant < 0 ? 0 : h->variant; }
+
 extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
-    if (variant != 0 && variant != 1) return fail(EPHC_EINVAL, "variant must be 0 (gather) or 1 (tiles)");
+    if (variant < -1 || variant > 1) return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather) or 1 (tiles)");
     if (variant == 1 && !h->tile_ok)
         return fail(EPHC_ESTATE, "tile store not available for this problem: " + h->thost.why);
     h->variant = variant;
     return EPHC_OK;
 }
 
-extern "C" int ephc_get_variant(const ephc_handle *h) { return h ? h->variant : EPHC_EINVAL; }
+extern "C" int ephc_get_variant(const ephc_handle *h) { return h ? coll_variant(h) : EPHC_EINVAL; }
+extern "C" int ephc_get_transport_variant(const ephc_handle *h) { return h ? tr_variant(h) : EPHC_EINVAL; }
 
 extern "C" int64_t ephc_launch_count(const ephc_handle *h) { return h ? h->launches : 0; }
 
@@ -445,11 +464,11 @@ static int need_device(ephc_handle *h) {
         if (h->tile_ok) {
 #define EPHC_TILE_ATTR(NB_)                                                                                       \
     CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
-                                  (int)tile_smem_bytes(kTCollision, h->t_R, NB_)));                                 \
+                                  (int)tile_smem_bytes(kTCollision, h->t_Ra, h->t_Rb)));                            \
     CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTSetup, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,           \
-                                  (int)tile_smem_bytes(kTSetup, h->t_R, NB_)));                                     \
+                                  (int)tile_smem_bytes(kTSetup, h->t_Ra, h->t_Rb)));                                \
     CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTIter, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,            \
-                                  (int)tile_smem_bytes(kTIter, h->t_R, NB_)));
+                                  (int)tile_smem_bytes(kTIter, h->t_Ra, h->t_Rb)));
             EPHC_TILE_ATTR(1)
             EPHC_TILE_ATTR(2)
             EPHC_TILE_ATTR(4)
@@ -470,10 +489,12 @@ static TileParams tile_params(const ephc_handle *h) {
     P.slices = h->dt_slices;
     P.tiles = h->dt_tiles;
     P.ctas = h->dt_ctas;
-    P.blk_row0 = h->dt_blk_row0;
     P.row_state = h->dt_row_state;
     P.slot_off = h->dt_slot_off;
-    P.R = h->t_R;
+    P.Ra = h->t_Ra;
+    P.Rb = h->t_Rb;
+    P.cta_group = 1;
+    P.ncta = h->t_ncta;
     P.nnu = h->d.nnu;
     P.ns = h->d.ns;
     P.part = h->dt_part;
@@ -488,9 +509,8 @@ static FinishParams finish_params(const ephc_handle *h) {
     P.state_row = h->dt_state_row;
     P.state_blk = h->dt_state_blk;
     P.blk_row0 = h->dt_blk_row0;
-    P.blk_slot_ptr = h->dt_blk_slot_ptr;
-    P.blk_slots = h->dt_blk_slots;
-    P.slot_off = h->dt_slot_off;
+    P.blk_ent_ptr = h->dt_blk_ent_ptr;
+    P.blk_ent_off = h->dt_blk_ent_off;
     P.part = h->dt_part;
     P.ns = h->d.ns;
     return P;
@@ -499,15 +519,19 @@ static FinishParams finish_params(const ephc_handle *h) {
 static inline unsigned finish_grid(const ephc_handle *h) { return (unsigned)((h->d.ns + 255) / 256); }
 
 template <int MODE>
-static int launch_tile(ephc_handle *h, const TileParams &P, cudaStream_t s) {
+static int launch_tile(ephc_handle *h, TileParams P, cudaStream_t s) {
     if (h->t_ntile > 0) {
         const int nb = h->d.nb;
+        const size_t sm = tile_smem_bytes(MODE, h->t_Ra, h->t_Rb);
+        const int threads = (MODE == kTIter) ? kTileThreadsIter : kTileThreads;
+        P.cta_group = (MODE == kTIter) ? 2 : 1;
+        const unsigned grid = (unsigned)((h->t_ncta + P.cta_group - 1) / P.cta_group);
         if (nb <= 1)
-            tile_kernel<MODE, 1><<<h->t_ncta, kTileThreads, tile_smem_bytes(MODE, h->t_R, 1), s>>>(P);
+            tile_kernel<MODE, 1><<<grid, threads, sm, s>>>(P);
         else if (nb <= 2)
-            tile_kernel<MODE, 2><<<h->t_ncta, kTileThreads, tile_smem_bytes(MODE, h->t_R, 2), s>>>(P);
+            tile_kernel<MODE, 2><<<grid, threads, sm, s>>>(P);
         else
-            tile_kernel<MODE, 4><<<h->t_ncta, kTileThreads, tile_smem_bytes(MODE, h->t_R, 4), s>>>(P);
+            tile_kernel<MODE, 4><<<grid, threads, sm, s>>>(P);
         h->launches++;
     }
     CUDA_TRY(cudaGetLastError());
@@ -563,7 +587,7 @@ extern "C" int ephc_collision(ephc_handle *h, const double *f_dev, const double 
     int rc = need_device(h);
     if (rc) return rc;
     if (!f_dev || !N_dev || !I_dev) return fail(EPHC_EINVAL, "null device pointer");
-    if (h->variant == 1) {
+    if (coll_variant(h) == 1) {
         TileParams T = tile_params(h);
         T.f = f_dev;
         T.N = N_dev;
@@ -584,7 +608,7 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
     int rc = need_device(h);
     if (rc) return rc;
     if (!f0_dev || !N_dev || !Gamma_dev) return fail(EPHC_EINVAL, "null device pointer");
-    if (h->variant == 1) {
+    if (tr_variant(h) == 1) {
         if (!h->dt_Wf) {
             if ((rc = ensure(&h->dt_Wf, (size_t)h->t_entries * 8)) || (rc = ensure(&h->dt_Wr, (size_t)h->t_entries * 8)))
                 return rc;
@@ -638,9 +662,9 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
     if (rc) return rc;
     if (!F_dev || !v_dev || !tau_dev || !Fout_dev) return fail(EPHC_EINVAL, "null device pointer");
     if (F_dev == Fout_dev) return fail(EPHC_EINVAL, "transport_iter is out of place: F_dev and Fout_dev must differ");
-    if (!h->transport_ready || h->transport_variant != h->variant)
+    if (!h->transport_ready || h->transport_variant != tr_variant(h))
         return fail(EPHC_ESTATE, "call ephc_transport_setup (with the current variant) before ephc_transport_iter");
-    if (h->variant == 1) {
+    if (tr_variant(h) == 1) {
         TileParams T = tile_params(h);
         T.F = F_dev;
         if ((rc = launch_tile<kTIter>(h, T, (cudaStream_t)stream))) return rc;
@@ -685,7 +709,7 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
         for (int st = 0; st < 4; ++st) {
-            if (h->variant == 1) {
+            if (coll_variant(h) == 1) {
                 TileParams T = tile_params(h);
                 T.f = src[st];
                 T.N = N_dev;
@@ -707,7 +731,7 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
             if (rc) return rc;
         }
         if (sumf_dev) {
-            if (h->variant == 1)
+            if (coll_variant(h) == 1)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);
             else if (h->n_wu > 0)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, h->n_wu, sumf_dev + it + 1);

@@ -79,9 +79,10 @@ int build_gather(const ephc_problem *p, const Dims &d, const Canonical &c, Gathe
 
 // ---- tile store (variant 1): every channel stored once, both of its ends updated by the same thread ----------
 // (DESIGN.md "Tile store").  States inside the energy window get a compact row index; compact rows are cut into
-// blocks of <= R rows (whole k points); tile (I,J), I <= J, holds every active pair with k in block I and k' in
-// block J.  A CTA walks a contiguous run of tiles; per tile it keeps f (or F) and the accumulators of both
-// blocks in shared memory, processes the tile's pairs one lane per pair (slices of 32 pairs, sorted by length,
+// fine blocks (whole k points), fine blocks into strips.  A tile holds every active pair with k in strip I and
+// k' in a range of fine blocks (or in strip I itself: diagonal tile); tile boundaries are chosen so that every
+// CTA gets the same work in one to three tiles.  Per tile the CTA keeps f (or F) and the accumulators of both
+// row ranges in shared memory, processes the tile's pairs one lane per pair (slices of 32 pairs, sorted by length,
 // entries stored column-major per slice), and adds every pair's partial sums into the shared accumulators in a
 // fixed, host-assigned ticket order per k point (plain read-modify-write, no atomics, bit-reproducible).
 constexpr int kTileNbMax = 4;        // bands handled in registers (compact band rank < 4)
@@ -102,20 +103,24 @@ struct TileSlice {   // 32 pair records, lanes sorted by descending length
 };
 struct TileHdr {
     int32_t s0, ns;          // slice range
-    int32_t bi, bj;          // blocks
+    int32_t a_row0, a_rows;  // compact rows of the k side (a strip of fine blocks)
+    int32_t b_row0, b_rows;  // compact rows of the k' side (a range of fine blocks; the strip itself on a diagonal tile)
     int32_t a_slot, b_slot;  // partial-sum slots (b_slot = -1 on a diagonal tile)
-    int32_t flags;           // bit 0: first tile of an a-run (stage block I, zero its accumulators); bit 1: last
+    int32_t flags;           // bit 0: first tile of an a-run (stage the strip, zero its accumulators); bit 1: last;
+                             // bit 2: diagonal tile (k and k' in the same strip: one set of arrays)
+    int32_t p0, npc;         // first pair record and number of pair records (slice g holds records p0 + 32 g ...)
     int32_t pad;
 };
 struct TileCta {
     int32_t t0, t1;          // tile range
 };
 struct TileHost {
-    int32_t R = 0, nblk = 0, nrows = 0, ncta = 0;
-    std::vector<int32_t> blk_row0;    // [nblk+1] compact row range of a block
+    int32_t Ra = 0, Rb = 0;           // largest a_rows / b_rows of any tile (shared-memory sizing)
+    int32_t nblk = 0, nrows = 0, ncta = 0;
+    std::vector<int32_t> blk_row0;    // [nblk+1] compact row range of a FINE block (unit of tile boundaries)
     std::vector<int32_t> row_state;   // [nrows] state index of a compact row
     std::vector<int32_t> state_row;   // [ns] compact row of a state, -1 outside the window
-    std::vector<int32_t> state_blk;   // [ns] block of a state's row, -1 outside the window
+    std::vector<int32_t> state_blk;   // [ns] fine block of a state's row, -1 outside the window
     std::vector<double> w;            // entries
     std::vector<uint16_t> code;
     std::vector<uint32_t> prec;       // [3][npiece]
@@ -123,7 +128,9 @@ struct TileHost {
     std::vector<TileHdr> tiles;
     std::vector<TileCta> ctas;
     std::vector<int64_t> slot_off;    // [nslot] offset of a slot in rows (x components in the kernels)
-    std::vector<int32_t> blk_slot_ptr, blk_slots;  // CSR: slots that hold partial sums of a block
+    std::vector<int32_t> slot_row0, slot_rows;  // [nslot] compact row range a slot covers
+    std::vector<int32_t> blk_ent_ptr; // [nblk+1] CSR over fine blocks: the slots that hold partial sums of the block
+    std::vector<int64_t> blk_ent_off; // per entry: row offset in the partial-sum buffer of the block's first row
     int64_t part_rows = 0;            // total rows of all slots
     int64_t npiece = 0;               // pair records
     bool supported = false;           // false: shape outside the register path (nb > 4, nnu > 8, ...)

@@ -32,9 +32,11 @@ struct TileParams {
     const TileSlice *slices;
     const TileHdr *tiles;
     const TileCta *ctas;
-    const int32_t *blk_row0, *row_state;
+    const int32_t *row_state;
     const int64_t *slot_off;
-    int32_t R, nnu;
+    int32_t Ra, Rb, nnu;
+    int32_t cta_group;     // consecutive TileCta shares walked by one CTA (1, or 2 for the 512-thread kernels)
+    int32_t ncta;          // number of TileCta shares
     int64_t ns;
     // inputs
     const double *f;  // occupations (collision / RK stage input y_j / f0 of transport_setup)
@@ -46,8 +48,8 @@ struct TileParams {
 };
 
 struct FinishParams {
-    const int32_t *state_row, *state_blk, *blk_row0, *blk_slot_ptr, *blk_slots;
-    const int64_t *slot_off;
+    const int32_t *state_row, *state_blk, *blk_row0, *blk_ent_ptr;
+    const int64_t *blk_ent_off;
     const double *part;
     int64_t ns;
     double *out;  // I, Gamma or Fout
@@ -81,133 +83,160 @@ __device__ __forceinline__ void put_nb(double (&a)[NB], int j, double x) {
 __device__ __forceinline__ unsigned ld_cnt(const uint16_t *p) { return *(const volatile uint16_t *)p; }
 __device__ __forceinline__ void st_cnt(uint16_t *p, unsigned v) { *(volatile uint16_t *)p = (uint16_t)v; }
 
-constexpr int kTileThreads = 256;
-constexpr int kTileBatch = 4;  // entries per lane whose loads are in flight while the previous batch is evaluated
+constexpr int kTileThreads = 256;      // collision / transport_setup: two CTAs per SM
+constexpr int kTileThreadsIter = 512;  // transport_iter: one CTA per SM, accumulators in registers
+constexpr int kTileBatch = 4;          // entries per lane whose loads are in flight while the previous batch is evaluated
 
-// Per-thread private rows in shared memory (row r of thread t at [r * kTileThreads + t]: conflict-free):
-//   collision / setup: 0..3 f_a[n], 4..7 f_b[m], 8..15 N[nu], 16..19 sums for k, 20..23 sums for k'
-//   transport_iter:    (c*NB + n) sums for k, (3*NB + c*NB + m) sums for k'
+// Per-thread private rows in shared memory of the collision / setup kernels (row r of thread t at
+// [r * kTileThreads + t]: conflict-free):  0..3 f_a[n], 4..7 f_b[m], 8..15 N[nu], 16..19 sums for k, 20..23 sums for k'.
 // Dynamic indexing by band / mode costs one LDS here instead of a chain of selects on registers.
 constexpr int kRowBytes = kTileThreads * 8;
-inline int tile_priv_rows(int mode, int nbp) { return (mode == kTIter) ? 6 * nbp : 24; }
+constexpr int kPrivRows = 24;
 
-inline size_t tile_smem_bytes(int mode, int R, int nbp) {
+inline size_t tile_smem_bytes(int mode, int Ra, int Rb) {
     const int C = (mode == kTIter) ? 3 : 1;
-    const size_t rows = (size_t)R + kTileNbMax;
-    return 4 * rows * C * sizeof(double) + 2 * (((size_t)R + 7) & ~(size_t)7) * sizeof(uint16_t) + 16 +
-           (size_t)tile_priv_rows(mode, nbp) * kRowBytes;
+    const size_t rows = (size_t)Ra + (size_t)Rb + 2 * kTileNbMax;
+    const size_t cnt = (((size_t)Ra + 7) & ~(size_t)7) + (((size_t)Rb + 7) & ~(size_t)7);
+    return 2 * rows * C * sizeof(double) + cnt * sizeof(uint16_t) + 16 +
+           (mode == kTIter ? 0 : (size_t)kPrivRows * kRowBytes);
 }
 
 __device__ __forceinline__ double &prow(char *tb, unsigned byte_off) { return *reinterpret_cast<double *>(tb + byte_off); }
 
 template <int MODE, int NB>
-__global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_kernel(const TileParams P) {
+__global__ void __launch_bounds__((MODE == kTIter) ? kTileThreadsIter : kTileThreads, (MODE == kTIter) ? 1 : 2)
+tile_kernel(const TileParams P) {
     constexpr int C = (MODE == kTIter) ? 3 : 1;
-    constexpr int U = kTileBatch;
+    constexpr int U = (MODE == kTIter) ? 2 : kTileBatch;
+    constexpr int NT = (MODE == kTIter) ? kTileThreadsIter : kTileThreads;
     extern __shared__ double smem[];
-    const int R = P.R, rows_al = R + kTileNbMax;
-    double *sIa = smem;                    // inputs of block I:  f[row] or F[row][3]
-    double *sIb = sIa + rows_al * C;       // inputs of block J
-    double *sAa = sIb + rows_al * C;       // accumulators of block I
-    double *sAb = sAa + rows_al * C;       // accumulators of block J
-    uint16_t *sCa = reinterpret_cast<uint16_t *>(sAb + rows_al * C);  // ticket counters per k point (first row)
-    uint16_t *sCb = sCa + ((R + 7) & ~7);
-    int *sNext = reinterpret_cast<int *>(sCb + ((R + 7) & ~7));
+    const int ra_al = P.Ra + kTileNbMax, rb_al = P.Rb + kTileNbMax;
+    double *sIa = smem;                  // inputs of the k rows:  f[row] or F[row][3]
+    double *sIb = sIa + ra_al * C;       // inputs of the k' rows
+    double *sAa = sIb + rb_al * C;       // accumulators of the k rows
+    double *sAb = sAa + ra_al * C;       // accumulators of the k' rows
+    uint16_t *sCa = reinterpret_cast<uint16_t *>(sAb + rb_al * C);  // ticket counters per k point (first row)
+    uint16_t *sCb = sCa + ((P.Ra + 7) & ~7);
+    int *sNext = reinterpret_cast<int *>(sCb + ((P.Rb + 7) & ~7));
     double *sPriv = reinterpret_cast<double *>(sNext + 4);
 
     const int tid = threadIdx.x, lane = tid & 31;
     char *tb = reinterpret_cast<char *>(sPriv + tid);
-    const TileCta cta = P.ctas[blockIdx.x];
     const int nnu = P.nnu;
     const int64_t np_all = P.npiece;
+    const int share0 = blockIdx.x * P.cta_group, share1 = min(share0 + P.cta_group, P.ncta);
+    const int t_begin = P.ctas[share0].t0, t_end = P.ctas[share1 - 1].t1;
 
-    for (int it = cta.t0; it < cta.t1; ++it) {
+    for (int it = t_begin; it < t_end; ++it) {
         const TileHdr th = P.tiles[it];
-        const bool dg = (th.bi == th.bj);
-        const int row0a = P.blk_row0[th.bi], rows_a = P.blk_row0[th.bi + 1] - row0a;
-        const int row0b = P.blk_row0[th.bj], rows_b = P.blk_row0[th.bj + 1] - row0b;
-        // ---- stage the inputs of both blocks, clear accumulators and ticket counters ------------------------------
+        const bool dg = (th.flags & 4) != 0;
+        // ---- stage the inputs of both row ranges, clear accumulators and ticket counters ------------------------------
         if (th.flags & 1) {
-            for (int r = tid; r < rows_a + kTileNbMax; r += kTileThreads) {
-                const int64_t s = (r < rows_a) ? P.row_state[row0a + r] : -1;
+            for (int r = tid; r < th.a_rows + kTileNbMax; r += NT) {
+                const int64_t s = (r < th.a_rows) ? P.row_state[th.a_row0 + r] : -1;
 #pragma unroll
                 for (int c = 0; c < C; ++c) {
                     sIa[r * C + c] = (s < 0) ? 0.0 : (MODE == kTIter ? P.F[(int64_t)c * P.ns + s] : P.f[s]);
                     sAa[r * C + c] = 0.0;
                 }
+                if (r < th.a_rows) sCa[r] = 0;
             }
         }
         if (!dg) {
-            for (int r = tid; r < rows_b + kTileNbMax; r += kTileThreads) {
-                const int64_t s = (r < rows_b) ? P.row_state[row0b + r] : -1;
+            for (int r = tid; r < th.b_rows + kTileNbMax; r += NT) {
+                const int64_t s = (r < th.b_rows) ? P.row_state[th.b_row0 + r] : -1;
 #pragma unroll
                 for (int c = 0; c < C; ++c) {
                     sIb[r * C + c] = (s < 0) ? 0.0 : (MODE == kTIter ? P.F[(int64_t)c * P.ns + s] : P.f[s]);
                     sAb[r * C + c] = 0.0;
                 }
+                if (r < th.b_rows) sCb[r] = 0;
             }
         }
-        for (int r = tid; r < R; r += kTileThreads) {
-            sCa[r] = 0;
-            sCb[r] = 0;
-        }
-        if (tid == 0) *sNext = 0;
         __syncthreads();
         const double *inB = dg ? sIa : sIb;
         double *accB = dg ? sAa : sAb;
         uint16_t *cntB = dg ? sCa : sCb;
 
-        // ---- slices: one lane per pair record --------------------------------------------------------------------------
-        while (true) {
-            int g = 0;
-            if (lane == 0) g = atomicAdd(sNext, 1);  // order of execution only
-            g = __shfl_sync(0xffffffffu, g, 0);
-            if (g >= th.ns) break;
-            const int4 sl4 = __ldg(reinterpret_cast<const int4 *>(P.slices + th.s0 + g));
-            const int64_t e0 = ((int64_t)(uint32_t)sl4.x) | ((int64_t)sl4.y << 32);
-            const int p0 = sl4.z;
-            const int np = (int)(int16_t)(sl4.w & 0xffff), maxlen = (int)(int16_t)((uint32_t)sl4.w >> 16);
-            const bool live = lane < np;
-            uint32_t r0 = 0, r1 = 0, r2 = 0;
-            if (live) {
-                r0 = __ldcs(P.prec + p0 + lane);
-                r1 = __ldcs(P.prec + np_all + p0 + lane);
-                r2 = __ldcs(P.prec + 2 * np_all + p0 + lane);
+        // ---- slices: one lane per pair record; warp w takes slices w, w + nwarps, ... in order -----------------------
+        // Two slices ahead: header + pair records (stage A).  One slice ahead: N[iq, :] and the first batch of
+        // entries (stage B, needs A).  The dependent global loads of a slice are thus in flight while the
+        // previous slices are evaluated.
+        struct PreA {
+            int4 h;
+            uint32_t r0, r1, r2;
+        };
+        struct PreB {
+            double Nq[(MODE == kTIter) ? 1 : 8];
+            double wq[U], vq[(MODE == kTIter) ? U : 1];
+            unsigned kq[U];
+            int oq[U];
+            int off;
+        };
+        constexpr int NW = NT / 32;
+        const int warp = tid >> 5;
+        auto loadA = [&](int g, PreA &A) {
+            A.h = __ldg(reinterpret_cast<const int4 *>(P.slices + th.s0 + g));
+            const int p0 = th.p0 + 32 * g;
+            A.r0 = A.r1 = A.r2 = 0;
+            if (lane < th.npc - 32 * g) {
+                A.r0 = __ldcs(P.prec + p0 + lane);
+                A.r1 = __ldcs(P.prec + np_all + p0 + lane);
+                A.r2 = __ldcs(P.prec + 2 * np_all + p0 + lane);
             }
+        };
+        // columns i0 .. i0+U-1 of a slice (column i holds the lanes with len > i, a prefix of the lanes)
+        auto load_batch = [&](int64_t eb, int len, int i0, PreB &B) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const bool act = len > i0 + u;
+                const int cnt = __popc(__ballot_sync(0xffffffffu, act));
+                B.wq[u] = 0.0;
+                if (MODE == kTIter) B.vq[u] = 0.0;
+                B.kq[u] = 0;
+                B.oq[u] = B.off;
+                if (act) {
+                    B.kq[u] = __ldcs(P.code + eb + B.off);
+                    if (MODE == kTIter) {
+                        B.wq[u] = __ldcs(P.Wf + eb + B.off);
+                        B.vq[u] = __ldcs(P.Wr + eb + B.off);
+                    } else {
+                        B.wq[u] = __ldcs(P.w + eb + B.off);
+                    }
+                }
+                B.off += cnt;
+            }
+        };
+        auto loadB = [&](const PreA &A, PreB &B) {
+            const int64_t eb = (((int64_t)(uint32_t)A.h.x) | ((int64_t)A.h.y << 32)) + lane;
+            if (MODE != kTIter) {
+                const double *Np = P.N + (int64_t)(A.r1 & 0xffffffu) * nnu;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) B.Nq[j] = (j < nnu) ? __ldg(Np + j) : 0.0;
+            }
+            B.off = 0;
+            load_batch(eb, (int)(A.r1 >> 24), 0, B);
+        };
+        PreA A1, A2, A3;
+        PreB B1, B2;
+        if (warp < th.ns) loadA(warp, A1);
+        if (warp + NW < th.ns) loadA(warp + NW, A2);
+        if (warp < th.ns) loadB(A1, B1);
+        for (int g = warp; g < th.ns; g += NW) {
+            if (g + NW < th.ns) loadB(A2, B2);
+            if (g + 2 * NW < th.ns) loadA(g + 2 * NW, A3);
+            const int64_t e0 = ((int64_t)(uint32_t)A1.h.x) | ((int64_t)A1.h.y << 32);
+            const int np = (int)(int16_t)(A1.h.w & 0xffff), maxlen = (int)(int16_t)((uint32_t)A1.h.w >> 16);
+            const bool live = lane < np;
+            const uint32_t r0 = A1.r0, r1 = A1.r1, r2 = A1.r2;
             const int ra = r0 & 0xffffu, rb = r0 >> 16;
             const int len = (int)(r1 >> 24);
             const int64_t eb = e0 + lane;
+            PreB &Bq = B1;
 
-            // batch loader: columns i0 .. i0+U-1 of the slice (column i holds the lanes with len > i, a prefix)
-            int off = 0;
-            double wq[U], vq[U];
-            unsigned kq[U];
-            int oq[U];
-            auto load_batch = [&](int i0) {
-#pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const bool act = len > i0 + u;
-                    const int cnt = __popc(__ballot_sync(0xffffffffu, act));
-                    wq[u] = 0.0;
-                    vq[u] = 0.0;
-                    kq[u] = 0;
-                    oq[u] = off;
-                    if (act) {
-                        kq[u] = __ldcs(P.code + eb + off);
-                        if (MODE == kTIter) {
-                            wq[u] = __ldcs(P.Wf + eb + off);
-                            vq[u] = __ldcs(P.Wr + eb + off);
-                        } else {
-                            wq[u] = __ldcs(P.w + eb + off);
-                        }
-                    }
-                    off += cnt;
-                }
-            };
-            load_batch(0);
-
-            double acc_a[C][NB], acc_b[C][NB];  // this lane's sums per end and band, filled before the epilogue
+            double acc_a[C][NB], acc_b[C][NB];  // this lane's sums per end and band
             if (MODE == kTIter) {
+                // F_a[n][c], F_b[m][c] and the sums in registers (one CTA per SM: 128 registers per thread)
                 double Fa[3][NB], Fb[3][NB];
 #pragma unroll
                 for (int j = 0; j < NB; ++j)
@@ -215,49 +244,31 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                     for (int c = 0; c < 3; ++c) {
                         Fa[c][j] = sIa[(ra + j) * 3 + c];
                         Fb[c][j] = inB[(rb + j) * 3 + c];
+                        acc_a[c][j] = 0.0;
+                        acc_b[c][j] = 0.0;
                     }
-#pragma unroll
-                for (int j = 0; j < 6 * NB; ++j) prow(tb, j * kRowBytes) = 0.0;
                 for (int i = 0; i < maxlen; i += U) {
                     double wc[U], vc[U];
                     unsigned kc[U];
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
-                        wc[u] = wq[u];
-                        vc[u] = vq[u];
-                        kc[u] = kq[u];
+                        wc[u] = Bq.wq[u];
+                        vc[u] = Bq.vq[u];
+                        kc[u] = Bq.kq[u];
                     }
-                    if (i + U < maxlen) load_batch(i + U);
+                    if (i + U < maxlen) load_batch(eb, len, i + U, Bq);
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         const int n = kc[u] & 3u, m = (kc[u] >> kTcM) & 3u;
-                        char *pa_ = tb + n * kRowBytes, *pb_ = tb + (3 * NB + m) * kRowBytes;
-                        double sa[3], sb[3];
 #pragma unroll
                         for (int c = 0; c < 3; ++c) {
-                            sa[c] = prow(pa_, c * NB * kRowBytes);
-                            sb[c] = prow(pb_, c * NB * kRowBytes);
-                        }
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            prow(pa_, c * NB * kRowBytes) = fma(wc[u], sel_nb<NB>(Fb[c], m), sa[c]);
-                            prow(pb_, c * NB * kRowBytes) = fma(vc[u], sel_nb<NB>(Fa[c], n), sb[c]);
+                            put_nb<NB>(acc_a[c], n, fma(wc[u], sel_nb<NB>(Fb[c], m), sel_nb<NB>(acc_a[c], n)));
+                            put_nb<NB>(acc_b[c], m, fma(vc[u], sel_nb<NB>(Fa[c], n), sel_nb<NB>(acc_b[c], m)));
                         }
                     }
                 }
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int j = 0; j < NB; ++j) {
-                        acc_a[c][j] = prow(tb, (c * NB + j) * kRowBytes);
-                        acc_b[c][j] = prow(tb, (3 * NB + c * NB + j) * kRowBytes);
-                    }
             } else {
                 {
-                    const double *Np = P.N + (int64_t)(r1 & 0xffffffu) * nnu;
-                    double Nq[8];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) Nq[j] = (j < nnu) ? __ldg(Np + j) : 0.0;
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         prow(tb, j * kRowBytes) = sIa[ra + j];
@@ -265,7 +276,7 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                     }
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
-                        prow(tb, (8 + j) * kRowBytes) = Nq[j];
+                        prow(tb, (8 + j) * kRowBytes) = Bq.Nq[j];
                         prow(tb, (16 + j) * kRowBytes) = 0.0;
                     }
                 }
@@ -275,12 +286,12 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                     int oc[U];
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
-                        wc[u] = wq[u];
-                        kc[u] = kq[u];
-                        oc[u] = oq[u];
+                        wc[u] = Bq.wq[u];
+                        kc[u] = Bq.kq[u];
+                        oc[u] = Bq.oq[u];
                     }
                     const int ibase = i;
-                    if (i + U < maxlen) load_batch(i + U);
+                    if (i + U < maxlen) load_batch(eb, len, i + U, Bq);
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         const unsigned k = kc[u];
@@ -288,6 +299,7 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                         char *pb_ = tb + (4 + ((k >> kTcM) & 3u)) * kRowBytes;
                         const double Nn = prow(tb, (8 + ((k >> kTcNu) & 7u)) * kRowBytes);
                         const double xa = prow(pa_, 0), xb = prow(pb_, 0);
+                        const double sa = prow(pa_, 16 * kRowBytes), sb = prow(pb_, 16 * kRowBytes);
                         const bool em = (k >> kTcKind) & 1u, diag = (k >> kTcDiag) & 1u;
                         if (MODE == kTCollision) {
                             // Eq. 2 summand (reading R-1), rearranged:  F_abs = (fa-fb) N + fa fb - fb,
@@ -295,7 +307,6 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                             const double pr = xa * xb;
                             const double s = em ? (xa - pr) : (pr - xb);
                             const double T = (diag ? 0.0 : wc[u]) * fma(xa - xb, Nn, s);
-                            const double sa = prow(pa_, 16 * kRowBytes), sb = prow(pb_, 16 * kRowBytes);
                             prow(pa_, 16 * kRowBytes) = sa + T;
                             prow(pb_, 16 * kRowBytes) = sb + T;
                         } else {
@@ -307,7 +318,6 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                                 P.Wf[eb + oc[u]] = Wf;
                                 P.Wr[eb + oc[u]] = Wr;
                             }
-                            const double sa = prow(pa_, 16 * kRowBytes), sb = prow(pb_, 16 * kRowBytes);
                             prow(pa_, 16 * kRowBytes) = sa + Wf;
                             prow(pb_, 16 * kRowBytes) = sb + Wr;
                         }
@@ -322,7 +332,7 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
 
             // ---- epilogue: ticket-ordered read-modify-write of the shared accumulators -------------------------------
             // Collision: I[a] -= T, I[b] += T.  Transport: both ends add their own weight sums.
-            const unsigned ta = r2 & 0xfffu, tb = (r2 >> 16) & 0xfffu;
+            const unsigned ta = r2 & 0xfffu, tb2 = (r2 >> 16) & 0xfffu;
             const int nia = (int)((r2 >> 12) & 3u) + 1, nib = (int)((r2 >> 28) & 3u) + 1;
             bool pa = live, pb = live;
             while (__any_sync(0xffffffffu, pa || pb)) {
@@ -341,7 +351,7 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                     st_cnt(sCa + ra, ta + 1);
                     pa = false;
                 }
-                if (pb && !pa && ld_cnt(cntB + rb) == tb) {
+                if (pb && !pa && ld_cnt(cntB + rb) == tb2) {
                     __threadfence_block();
 #pragma unroll
                     for (int j = 0; j < NB; ++j)
@@ -350,21 +360,24 @@ __global__ void __launch_bounds__(kTileThreads, (MODE == kTIter) ? 2 : 3) tile_k
                             for (int c = 0; c < C; ++c) accB[(rb + j) * C + c] += acc_b[c][j];
                         }
                     __threadfence_block();
-                    st_cnt(cntB + rb, tb + 1);
+                    st_cnt(cntB + rb, tb2 + 1);
                     pb = false;
                 }
                 __syncwarp();
             }
+            A1 = A2;
+            B1 = B2;
+            A2 = A3;
         }
         __syncthreads();
         // ---- partial sums of this tile / run go to their slots ---------------------------------------------------------
         if (!dg) {
             double *dst = P.part + P.slot_off[th.b_slot] * C;
-            for (int i = tid; i < rows_b * C; i += kTileThreads) dst[i] = sAb[i];
+            for (int i = tid; i < th.b_rows * C; i += NT) dst[i] = sAb[i];
         }
         if (th.flags & 2) {
             double *dst = P.part + P.slot_off[th.a_slot] * C;
-            for (int i = tid; i < rows_a * C; i += kTileThreads) dst[i] = sAa[i];
+            for (int i = tid; i < th.a_rows * C; i += NT) dst[i] = sAa[i];
         }
         __syncthreads();
     }
@@ -384,8 +397,8 @@ __global__ void __launch_bounds__(256) finish_kernel(const FinishParams P) {
         if (cr >= 0) {
             const int b = P.state_blk[a];
             const int64_t r = cr - P.blk_row0[b];
-            for (int i = P.blk_slot_ptr[b]; i < P.blk_slot_ptr[b + 1]; ++i) {
-                const double *src = P.part + (P.slot_off[P.blk_slots[i]] + r) * C;
+            for (int i = P.blk_ent_ptr[b]; i < P.blk_ent_ptr[b + 1]; ++i) {
+                const double *src = P.part + (P.blk_ent_off[i] + r) * C;
 #pragma unroll
                 for (int c = 0; c < C; ++c) sum[c] += src[c];
             }
