@@ -14,6 +14,7 @@
 #include "ephc_internal.h"
 #include "ephc_kernels.cuh"
 #include "ephc_tile_kernels.cuh"
+#include "ephc_row_kernels.cuh"
 
 using namespace ephc;
 
@@ -73,6 +74,17 @@ struct ephc_handle {
             *dt_blk_ent_ptr = nullptr;
     int64_t *dt_slot_off = nullptr, *dt_blk_ent_off = nullptr;
     int transport_variant = -1;
+    // row store (transport_iter of the gather path)
+    bool rows_ok = false;
+    int32_t r_nstrip = 0, r_Rb = 0, r_Ra = 0;
+    int64_t bytes_rows = 0;
+    double *dr_W = nullptr;
+    uint16_t *dr_idx = nullptr;
+    uint32_t *dr_perm = nullptr;
+    RowSeg *dr_segs = nullptr;
+    RowTile *dr_tiles = nullptr;
+    RowStrip *dr_strips = nullptr;
+    int32_t *dr_row_state = nullptr, *dr_state_row = nullptr;
 };
 
 static void free_dev(ephc_handle *h) {
@@ -81,7 +93,8 @@ static void free_dev(ephc_handle *h) {
                     h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
-                    h->dt_slot_off};
+                    h->dt_slot_off, h->dr_W, h->dr_idx, h->dr_perm, h->dr_segs, h->dr_tiles, h->dr_strips,
+                    h->dr_row_state, h->dr_state_row};
     for (void *p : ptrs)
         if (p) cudaFree(p);
 }
@@ -167,6 +180,25 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
                                    th.state_blk.size() + th.blk_ent_ptr.size()) * 4 + th.blk_ent_off.size() * 8);
         h->variant = -1;
     }
+    // row store for transport_iter (one CTA of 1024 threads per SM, one strip each)
+    RowHost rh;
+    const bool want_rows = std::getenv("EPHC_NO_ROWS") == nullptr;
+    if (want_rows) {
+        int nstrip = n_sm;
+        if (const char *e = std::getenv("EPHC_ROW_STRIPS")) nstrip = std::max(1, std::atoi(e));
+        rc = build_rows(p, h->d, g, nstrip, rh, err);
+        if (rc != EPHC_OK) {
+            delete h;
+            return fail(rc, err);
+        }
+        h->rows_ok = row_smem_bytes(rh.Rb, rh.Ra) <= 200 * 1024;
+        h->r_nstrip = (int32_t)rh.strips.size();
+        h->r_Rb = rh.Rb;
+        h->r_Ra = rh.Ra;
+        h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.perm.size() * 4 + rh.segs.size() * sizeof(RowSeg) +
+                                  rh.tiles.size() * sizeof(RowTile) + rh.strips.size() * sizeof(RowStrip) +
+                                  (rh.row_state.size() + rh.state_row.size()) * 4);
+    }
     h->pair_ik.assign(p->pair_ik, p->pair_ik + p->npair);
     h->pair_ikq.assign(p->pair_ikq, p->pair_ikq + p->npair);
     h->g_entries = (int64_t)g.code.size();
@@ -190,6 +222,16 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         if (rc == EPHC_OK) rc = upload(&h->d_tasks, g.tasks, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_rounds, g.rounds, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_wus, g.wus, &b);
+        if (rc == EPHC_OK && h->rows_ok) {
+            int64_t br = 0;
+            rc = upload(&h->dr_idx, rh.idx, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_perm, rh.perm, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_segs, rh.segs, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_tiles, rh.tiles, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_strips, rh.strips, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_row_state, rh.row_state, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_state_row, rh.state_row, &br);
+        }
         if (rc == EPHC_OK && th.supported) {
             int64_t bt = 0;
             rc = upload(&h->dt_w, th.w, &bt);
@@ -249,7 +291,7 @@ extern "C" int ephc_query(const ephc_handle *h, ephc_counts *o) {
     o->ndiag = h->can.ndiag;
     o->gather_entries = h->g_entries;
     o->gather_halfpairs = h->g_halfpairs;
-    o->store_bytes_gather = h->bytes_gather;
+    o->store_bytes_gather = h->bytes_gather + h->bytes_rows;
     o->scatter_entries = h->t_entries;
     o->scatter_pairs = h->t_pieces;
     o->store_bytes_scatter = h->bytes_tile;
@@ -461,6 +503,9 @@ static int need_device(ephc_handle *h) {
                                       (int)gather_smem_bytes(kTransportSetup)));
         CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)gather_smem_bytes(kTransportIter)));
+        if (h->rows_ok)
+            CUDA_TRY(cudaFuncSetAttribute(row_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)row_smem_bytes(h->r_Rb, h->r_Ra)));
         if (h->tile_ok) {
 #define EPHC_TILE_ATTR(NB_)                                                                                       \
     CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
@@ -637,6 +682,17 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
     P.N = N_dev;
     P.out = Gamma_dev;
     rc = launch_gather<kTransportSetup>(h, P, (cudaStream_t)stream);
+    if (rc == EPHC_OK && h->rows_ok && h->g_entries > 0) {
+        // the iteration runs on the row store: same ordered terms, regrouped; bring the weights into its order
+        if (!h->dr_W) {
+            if ((rc = ensure(&h->dr_W, (size_t)h->g_entries * 8))) return rc;
+            h->bytes_transport += h->g_entries * 8;
+        }
+        row_permute_kernel<<<(unsigned)((h->g_entries + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+            h->d_gW, h->dr_perm, h->dr_W, h->g_entries);
+        h->launches++;
+        CUDA_TRY(cudaGetLastError());
+    }
     if (rc == EPHC_OK) {
         h->transport_ready = true;
         h->transport_variant = 0;
@@ -673,6 +729,30 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
         Fp.v = v_dev;
         Fp.tau = tau_dev;
         return launch_finish<kFIter>(h, Fp, (cudaStream_t)stream);
+    }
+    if (h->rows_ok) {
+        RowParams R;
+        std::memset(&R, 0, sizeof(R));
+        R.W = h->dr_W;
+        R.idx = h->dr_idx;
+        R.segs = h->dr_segs;
+        R.tiles = h->dr_tiles;
+        R.strips = h->dr_strips;
+        R.row_state = h->dr_row_state;
+        R.state_row = h->dr_state_row;
+        R.Rb = h->r_Rb;
+        R.Ra = h->r_Ra;
+        R.nstrip = h->r_nstrip;
+        R.ns = h->d.ns;
+        R.F = F_dev;
+        R.v = v_dev;
+        R.tau = tau_dev;
+        R.out = Fout_dev;
+        row_iter_kernel<<<(unsigned)std::max(h->r_nstrip, 1), kRowThreads, row_smem_bytes(h->r_Rb, h->r_Ra),
+                          (cudaStream_t)stream>>>(R);
+        h->launches++;
+        CUDA_TRY(cudaGetLastError());
+        return EPHC_OK;
     }
     GatherParams P = base_params(h);
     P.F = F_dev;

@@ -138,4 +138,37 @@ struct TileHost {
 };
 int build_tiles(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, TileHost &t, std::string &err);
 
+// ---- row store (transport_iter): destination-sorted, two-sided, tiled over the partner rows ---------------------
+// In the transport iteration the two directions of a channel carry DIFFERENT weights W(a<-b), W(b<-a)
+// (PAPER.md:110), so storing every ordered term with its destination costs no extra weight bytes.  Compact rows
+// (states inside the window) are cut into strips of equal ordered-entry count, one per CTA, which is the single
+// owner of its rows of F'.  The partner rows are cut into ranges of <= Rb rows whose F values
+// are staged in shared memory; inside a (strip, range) tile every destination row has one contiguous segment
+// of entries (weight fp64 + partner row relative to the range, uint16), segments sorted by descending length.
+struct RowSeg {        // 16 bytes: one destination row inside one tile
+    uint32_t start;    // first entry, relative to the strip's first entry
+    uint32_t len;
+    uint32_t row;      // destination row, local to the strip
+    uint32_t pad;
+};
+struct RowTile {
+    int32_t seg0, nseg;      // segment range
+    int32_t col0, ncols;     // partner rows staged for this tile (compact row range)
+};
+struct RowStrip {
+    int64_t e0;              // first entry of the strip
+    int32_t row0, nrows;     // destination rows (compact)
+    int32_t t0, t1;          // tile range
+};
+struct RowHost {
+    int32_t Rb = 0, Ra = 0, nrows = 0;
+    std::vector<int32_t> row_state, state_row;
+    std::vector<uint16_t> idx;        // per entry: partner row - col0 of its tile
+    std::vector<uint32_t> perm;       // per entry: index of the same ordered term in the gather store (weights come from there)
+    std::vector<RowSeg> segs;
+    std::vector<RowTile> tiles;
+    std::vector<RowStrip> strips;
+};
+int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int nstrip, RowHost &r, std::string &err);
+
 }  // namespace ephc

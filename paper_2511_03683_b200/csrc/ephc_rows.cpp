@@ -1,0 +1,141 @@
+// ephc_rows.cpp -- host side of the row store used by ephc_transport_iter (see ephc_internal.h "row store").
+// Built once from the two-sided gather store ("performed only once on CPUs"): the same ordered terms,
+// regrouped by (strip of destination rows, range of partner rows, destination row).
+//
+// Product code: shares nothing with oracle/.
+#include <algorithm>
+#include <cstdlib>
+#include <numeric>
+
+#include "ephc_internal.h"
+
+namespace ephc {
+
+int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int nstrip, RowHost &r, std::string &err) {
+    const int nb = d.nb;
+    const int64_t nent = (int64_t)g.code.size();
+    r = RowHost();
+    if (nent >= 0xffffffffLL) {
+        err = "row store: more than 2^32-1 ordered entries";
+        return EPHC_ELIMIT;
+    }
+    if (nstrip < 1) nstrip = 1;
+    try {
+        // compact rows: states inside the window (R-7), in state order
+        r.state_row.assign((size_t)d.ns, -1);
+        for (int64_t s = 0; s < d.ns; ++s)
+            if (p->E[s] >= p->emin && p->E[s] <= p->emax) {
+                r.state_row[s] = (int32_t)r.row_state.size();
+                r.row_state.push_back((int32_t)s);
+            }
+        r.nrows = (int32_t)r.row_state.size();
+        int Rb = 4096;
+        if (const char *e = std::getenv("EPHC_ROW_RANGE")) Rb = std::atoi(e);
+        Rb = std::max(32, std::min(4096, Rb));
+        r.Rb = Rb;
+        const int32_t nrange = std::max(1, (r.nrows + Rb - 1) / Rb);
+
+        // destination / partner row of every gather entry (walk work units -> rounds -> tasks as the kernels do)
+        std::vector<int32_t> drow((size_t)nent), prow((size_t)nent);
+        const int64_t nwu = (int64_t)g.wus.size();
+#pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t iw = 0; iw < nwu; ++iw) {
+            const WorkUnit &wu = g.wus[iw];
+            for (int32_t rr = wu.r0; rr < wu.r1; ++rr) {
+                const Round &rd = g.rounds[rr];
+                for (int32_t t = rd.t0; t < rd.t0 + rd.nt; ++t) {
+                    const Task &tk = g.tasks[t];
+                    for (int64_t e = tk.e0; e < tk.e0 + tk.len; ++e) {
+                        const uint32_t c = g.code[e];
+                        const int32_t ps = g.hp_k[rd.hp0 + (c & kPairMask)] * nb + (int32_t)((c >> kBandShift) & 15);
+                        drow[e] = r.state_row[tk.row];
+                        prow[e] = r.state_row[ps];
+                    }
+                }
+            }
+        }
+        for (int64_t e = 0; e < nent; ++e)
+            if (drow[e] < 0 || prow[e] < 0) {
+                err = "internal: ordered entry with a state outside the window";
+                return EPHC_ESTATE;
+            }
+        // entries per (row, range) and per row
+        std::vector<uint32_t> cnt((size_t)r.nrows * nrange, 0);
+        for (int64_t e = 0; e < nent; ++e) cnt[(size_t)drow[e] * nrange + prow[e] / Rb]++;
+        std::vector<int64_t> row_cnt((size_t)r.nrows + 1, 0);
+        for (int32_t i = 0; i < r.nrows; ++i) {
+            int64_t sum = 0;
+            for (int32_t c = 0; c < nrange; ++c) sum += cnt[(size_t)i * nrange + c];
+            row_cnt[i + 1] = row_cnt[i] + sum;
+        }
+        // strips of equal entry count (row granularity)
+        int Ra_cap = 2048;
+        std::vector<int32_t> strip_row0(1, 0);
+        for (int s = 1; s <= nstrip; ++s) {
+            const int64_t goal = nent * (int64_t)s / nstrip;
+            int32_t r1 = (int32_t)(std::lower_bound(row_cnt.begin(), row_cnt.end(), goal) - row_cnt.begin());
+            r1 = std::max(r1, strip_row0.back());
+            if (s == nstrip) r1 = r.nrows;
+            while (r1 - strip_row0.back() > Ra_cap) {  // an (almost) empty stretch of rows: cut it
+                strip_row0.push_back(strip_row0.back() + Ra_cap);
+            }
+            if (r1 > strip_row0.back() || s == nstrip) strip_row0.push_back(r1);
+        }
+        if (strip_row0.back() != r.nrows) strip_row0.push_back(r.nrows);
+        const int32_t ns_real = (int32_t)strip_row0.size() - 1;
+        r.strips.resize((size_t)ns_real);
+        r.Ra = 1;
+        // per strip: tiles and segments (sorted by descending length), entry offsets
+        std::vector<int64_t> seg_abs((size_t)r.nrows * nrange, 0);  // absolute first entry of (row, range)
+        int64_t e_run = 0;
+        for (int32_t s = 0; s < ns_real; ++s) {
+            RowStrip &st = r.strips[s];
+            st.row0 = strip_row0[s];
+            st.nrows = strip_row0[s + 1] - strip_row0[s];
+            st.e0 = e_run;
+            st.t0 = (int32_t)r.tiles.size();
+            r.Ra = std::max(r.Ra, st.nrows);
+            for (int32_t c = 0; c < nrange; ++c) {
+                std::vector<std::pair<uint32_t, int32_t>> rows;  // (len, row)
+                for (int32_t i = st.row0; i < st.row0 + st.nrows; ++i) {
+                    const uint32_t n = cnt[(size_t)i * nrange + c];
+                    if (n) rows.emplace_back(n, i);
+                }
+                if (rows.empty()) continue;
+                std::stable_sort(rows.begin(), rows.end(),
+                                 [](const std::pair<uint32_t, int32_t> &x, const std::pair<uint32_t, int32_t> &y) { return x.first > y.first; });
+                RowTile tl;
+                tl.seg0 = (int32_t)r.segs.size();
+                tl.nseg = (int32_t)rows.size();
+                tl.col0 = c * Rb;
+                tl.ncols = std::min(Rb, r.nrows - tl.col0);
+                for (const auto &q : rows) {
+                    if (e_run - st.e0 > 0xffffffffLL) {
+                        err = "row store: strip with more than 2^32 entries";
+                        return EPHC_ELIMIT;
+                    }
+                    r.segs.push_back(RowSeg{(uint32_t)(e_run - st.e0), q.first, (uint32_t)(q.second - st.row0), 0u});
+                    seg_abs[(size_t)q.second * nrange + c] = e_run;
+                    e_run += q.first;
+                }
+                r.tiles.push_back(tl);
+            }
+            st.t1 = (int32_t)r.tiles.size();
+        }
+        // scatter the entries (gather order inside a segment)
+        r.idx.resize((size_t)nent);
+        r.perm.resize((size_t)nent);
+        for (int64_t e = 0; e < nent; ++e) {
+            const int32_t c = prow[e] / Rb;
+            const int64_t o = seg_abs[(size_t)drow[e] * nrange + c]++;
+            r.idx[o] = (uint16_t)(prow[e] - c * Rb);
+            r.perm[o] = (uint32_t)e;
+        }
+    } catch (const std::bad_alloc &) {
+        err = "host allocation failed (row store)";
+        return EPHC_ENOMEM;
+    }
+    return EPHC_OK;
+}
+
+}  // namespace ephc
