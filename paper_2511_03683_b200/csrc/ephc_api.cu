@@ -78,7 +78,8 @@ struct ephc_handle {
     bool rows_ok = false;
     int32_t r_nstrip = 0, r_Rb = 0, r_Ra = 0;
     int64_t bytes_rows = 0;
-    double *dr_W = nullptr;
+    double *dr_W = nullptr, *dr_Fc = nullptr;
+    int32_t r_nrows = 0;
     uint16_t *dr_idx = nullptr;
     uint32_t *dr_perm = nullptr;
     RowSeg *dr_segs = nullptr;
@@ -93,7 +94,7 @@ static void free_dev(ephc_handle *h) {
                     h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
-                    h->dt_slot_off, h->dr_W, h->dr_idx, h->dr_perm, h->dr_segs, h->dr_tiles, h->dr_strips,
+                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_idx, h->dr_perm, h->dr_segs, h->dr_tiles, h->dr_strips,
                     h->dr_row_state, h->dr_state_row};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -191,10 +192,11 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             delete h;
             return fail(rc, err);
         }
-        h->rows_ok = row_smem_bytes(rh.Rb, rh.Ra) <= 200 * 1024;
+        h->rows_ok = row_smem_bytes(rh.Rb, rh.Ra) <= 220 * 1024;
         h->r_nstrip = (int32_t)rh.strips.size();
         h->r_Rb = rh.Rb;
         h->r_Ra = rh.Ra;
+        h->r_nrows = rh.nrows;
         h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.perm.size() * 4 + rh.segs.size() * sizeof(RowSeg) +
                                   rh.tiles.size() * sizeof(RowTile) + rh.strips.size() * sizeof(RowStrip) +
                                   (rh.row_state.size() + rh.state_row.size()) * 4);
@@ -231,6 +233,8 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             if (rc == EPHC_OK) rc = upload(&h->dr_strips, rh.strips, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_row_state, rh.row_state, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_state_row, rh.state_row, &br);
+            if (rc == EPHC_OK && cudaMalloc((void **)&h->dr_Fc, ((size_t)rh.nrows * 3 + 4) * 8) != cudaSuccess)
+                rc = fail(EPHC_ENOMEM, "cudaMalloc (compact F) failed");
         }
         if (rc == EPHC_OK && th.supported) {
             int64_t bt = 0;
@@ -744,7 +748,12 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
         R.Ra = h->r_Ra;
         R.nstrip = h->r_nstrip;
         R.ns = h->d.ns;
-        R.F = F_dev;
+        if (h->r_nrows > 0) {
+            row_compact_kernel<<<(unsigned)((h->r_nrows + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+                F_dev, h->dr_row_state, h->dr_Fc, h->r_nrows, h->d.ns);
+            h->launches++;
+        }
+        R.Fc = h->dr_Fc;
         R.v = v_dev;
         R.tau = tau_dev;
         R.out = Fout_dev;

@@ -1,7 +1,8 @@
 // ephc_row_kernels.cuh -- sm_100a kernels of the row store: the transport iteration
 //     F'[al][a] = tau[a] ( v[al][a] + sum_b W(a<-b) F[al][b] ),  al = x, y, z           (reading R-16)
 // One CTA = one strip of destination rows and their single owner (no atomics).  The partner rows
-// are walked in ranges; per range the CTA stages F[0..3)[partner] in shared memory ([row][3], 24 B per row), then
+// are walked in ranges; per range the CTA stages F[0..3)[partner] in shared memory ([row][3], 24 B per row; copied
+// asynchronously one range ahead from a compact copy of F), then
 // groups of 8 lanes take one destination row each: the lanes stream that row's (weight, partner) entries of this
 // range from HBM (contiguous, every byte used once), multiply by the staged F and reduce with three shuffles;
 // the group's first lane adds the three sums to the row's accumulators in shared memory (one owner per row and
@@ -16,6 +17,10 @@ namespace ephc {
 
 constexpr int kRowThreads = 1024;  // one CTA per SM: the staging traffic is (number of strips) x |F|
 constexpr int kRowGroup = 8;  // lanes per destination row
+#ifndef EPHC_ROW_BATCH
+#define EPHC_ROW_BATCH 4
+#endif
+constexpr int kRowBatch = EPHC_ROW_BATCH;
 
 struct RowParams {
     const double *W;        // per entry, row-store order
@@ -26,11 +31,33 @@ struct RowParams {
     const int32_t *row_state, *state_row;
     int32_t Rb, Ra, nstrip;
     int64_t ns;
-    const double *F, *v, *tau;
+    const double *Fc;       // F of the compact rows, [nrows][3] (row_compact_kernel), padded by 2 doubles
+    const double *v, *tau;
     double *out;
 };
 
-inline size_t row_smem_bytes(int Rb, int Ra) { return ((size_t)Rb + (size_t)Ra) * 3 * sizeof(double); }
+inline size_t row_smem_bytes(int Rb, int Ra) { return ((size_t)Rb + (size_t)Ra) * 3 * sizeof(double) + 48; }
+
+// F[3][ns] (API layout) -> Fc[nrows][3]: the rows a tile stages are then one contiguous block
+__global__ void __launch_bounds__(256) row_compact_kernel(const double *F, const int32_t *row_state, double *Fc, int nrows,
+                                                           int64_t ns) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < nrows) {
+        const int64_t s = row_state[r];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) Fc[(int64_t)r * 3 + c] = F[(int64_t)c * ns + s];
+    }
+}
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
 
 // weights of the gather store (written by its transport_setup kernel) -> row-store order
 __global__ void __launch_bounds__(256) row_permute_kernel(const double *gW, const uint32_t *perm, double *W, int64_t n) {
@@ -40,11 +67,12 @@ __global__ void __launch_bounds__(256) row_permute_kernel(const double *gW, cons
 
 __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParams P) {
     extern __shared__ double smem[];
-    double *sF = smem;               // [Rb][3]
-    double *sAcc = smem + P.Rb * 3;  // [Ra][3]
+    double *sF = smem;                       // staged partner rows [Rb][3]
+    double *sAcc = smem + (P.Rb * 3 + 2);    // [Ra][3]
+    int *sNext = reinterpret_cast<int *>(sAcc + P.Ra * 3);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int sub = lane / kRowGroup, gl = lane % kRowGroup;
-    constexpr int NW = kRowThreads / 32, GPW = 32 / kRowGroup;  // warps, row groups per warp
+    constexpr int GPW = 32 / kRowGroup;  // row groups per warp
 
     // states outside the window receive no contribution: F' = tau v (grid-stride over all states)
     for (int64_t s = (int64_t)blockIdx.x * kRowThreads + tid; s < P.ns; s += (int64_t)gridDim.x * kRowThreads)
@@ -62,13 +90,22 @@ __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParam
     for (int t = st.t0; t < st.t1; ++t) {
         const RowTile tl = P.tiles[t];
         __syncthreads();  // previous tile done with sF (and sAcc zeroed)
-        for (int i = tid; i < tl.ncols; i += kRowThreads) {
-            const int64_t s = P.row_state[tl.col0 + i];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) sF[i * 3 + c] = P.F[(int64_t)c * P.ns + s];
+        {   // stage the tile's partner rows: 16-byte copies global -> shared, no registers in between
+            const double *src = P.Fc + (int64_t)tl.col0 * 3;
+            const int n16 = (tl.ncols * 3 + 1) / 2;
+            for (int i = tid; i < n16; i += kRowThreads) cp_async16(sF + 2 * i, src + 2 * i);
+            cp_async_commit();
+            if (tid == 0) *sNext = 0;
+            cp_async_wait<0>();
         }
         __syncthreads();
-        for (int sg0 = warp * GPW; sg0 < tl.nseg; sg0 += NW * GPW) {
+        // segments are sorted by descending length; warps take four at a time from a shared counter
+        // (order of execution only: every row has one segment per tile, hence one writer)
+        while (true) {
+            int sg0 = 0;
+            if (lane == 0) sg0 = atomicAdd(sNext, GPW);
+            sg0 = __shfl_sync(0xffffffffu, sg0, 0);
+            if (sg0 >= tl.nseg) break;
             const int sg = sg0 + sub;
             uint32_t start = 0, len = 0, row = 0;
             if (sg < tl.nseg) {
@@ -80,12 +117,12 @@ __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParam
             const double *w = Wb + start;
             const uint16_t *ix = Ib + start;
             double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-            // four entries per lane in flight
-            for (uint32_t i = gl; i < len; i += 4 * kRowGroup) {
-                double wv[4];
-                unsigned jv[4];
+            // kRowBatch entries per lane in flight
+            for (uint32_t i = gl; i < len; i += kRowBatch * kRowGroup) {
+                double wv[kRowBatch];
+                unsigned jv[kRowBatch];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < kRowBatch; ++u) {
                     const uint32_t ii = i + u * kRowGroup;
                     wv[u] = 0.0;
                     jv[u] = 0;
@@ -95,7 +132,7 @@ __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParam
                     }
                 }
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < kRowBatch; ++u) {
                     const double *f = sF + jv[u] * 3;
                     a0 = fma(wv[u], f[0], a0);
                     a1 = fma(wv[u], f[1], a1);

@@ -29,9 +29,9 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
                 r.row_state.push_back((int32_t)s);
             }
         r.nrows = (int32_t)r.row_state.size();
-        int Rb = 4096;
+        int Rb = 6144;
         if (const char *e = std::getenv("EPHC_ROW_RANGE")) Rb = std::atoi(e);
-        Rb = std::max(32, std::min(4096, Rb));
+        Rb = std::max(32, std::min(8192, Rb)) & ~1;  // even: 16-byte aligned staging copies
         r.Rb = Rb;
         const int32_t nrange = std::max(1, (r.nrows + Rb - 1) / Rb);
 
