@@ -288,8 +288,12 @@ def main():
                       "share_of_step": share, "channel_terms_per_s": nch / (ms_launch * 1e-3) if ms_launch > 0 else 0.0}
 
     ms_step = ms_total / max(args.steps, 1)
-    kn = {"c": "gather_kernel<0>", "s": "gather_kernel<2>", "i": "gather_kernel<3>", "r": "gather_kernel<1>"}
-    w_setup = 8 * q["gather_entries"]
+    kn = {"c": "gather_kernel<0>", "s": "gather_kernel<2> + row_permute_kernel", "r": "gather_kernel<1>",
+          "i": "row_compact_kernel + row_iter_kernel"}
+    w_setup = 8 * q["gather_entries"] + 20 * q["gather_entries"]   # write W, then permute it into row-store order
+    if os.environ.get("EPHC_NO_ROWS"):
+        kn.update({"s": "gather_kernel<2>", "i": "gather_kernel<3>"})
+        w_setup = 8 * q["gather_entries"]
     if variant == 1:
         kn.update({"c": "tile_kernel<0> + finish_kernel<0>", "r": "tile_kernel<0> + finish_kernel<1>"})
     if tvariant == 1:
@@ -357,7 +361,8 @@ def main():
         cfg = workload_config(args, p, nch)
         sb = (q["store_bytes_scatter"] if 1 in (variant, tvariant) else 0) + (q["store_bytes_gather"] if 0 in (variant, tvariant) else 0)
         names = {0: "gather", 1: "tiles"}
-        cfg.update({"variant": f"collision/rt: {names[variant]}, transport: {names[tvariant]}",
+        tname = names[tvariant] if (tvariant == 1 or os.environ.get("EPHC_NO_ROWS")) else "rows (setup on gather)"
+        cfg.update({"variant": f"collision/rt: {names[variant]}, transport: {tname}",
                     "l2": f"no flush: every evaluation streams the {sb / 1e6:.0f} MB store "
                           f"(+{q['store_bytes_transport'] / 1e6:.0f} MB transport weights), larger than the 126 MB L2",
                     "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (one problem per GPU)",

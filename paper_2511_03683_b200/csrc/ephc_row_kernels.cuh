@@ -117,20 +117,31 @@ __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParam
             const double *w = Wb + start;
             const uint16_t *ix = Ib + start;
             double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-            // kRowBatch entries per lane in flight
+            // kRowBatch entries per lane are in flight while the previous kRowBatch are multiplied
+            double wn[kRowBatch];
+            unsigned jn[kRowBatch];
+            auto load_batch = [&](uint32_t i) {
+#pragma unroll
+                for (int u = 0; u < kRowBatch; ++u) {
+                    const uint32_t ii = i + u * kRowGroup;
+                    wn[u] = 0.0;
+                    jn[u] = 0;
+                    if (ii < len) {
+                        wn[u] = __ldcs(w + ii);
+                        jn[u] = __ldcs(ix + ii);
+                    }
+                }
+            };
+            load_batch(gl);
             for (uint32_t i = gl; i < len; i += kRowBatch * kRowGroup) {
                 double wv[kRowBatch];
                 unsigned jv[kRowBatch];
 #pragma unroll
                 for (int u = 0; u < kRowBatch; ++u) {
-                    const uint32_t ii = i + u * kRowGroup;
-                    wv[u] = 0.0;
-                    jv[u] = 0;
-                    if (ii < len) {
-                        wv[u] = __ldcs(w + ii);
-                        jv[u] = __ldcs(ix + ii);
-                    }
+                    wv[u] = wn[u];
+                    jv[u] = jn[u];
                 }
+                if (i + kRowBatch * kRowGroup < len) load_batch(i + kRowBatch * kRowGroup);
 #pragma unroll
                 for (int u = 0; u < kRowBatch; ++u) {
                     const double *f = sF + jv[u] * 3;
