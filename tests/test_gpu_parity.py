@@ -245,3 +245,47 @@ def test_stream_argument_is_honoured():
         h.collision(f, N, I, stream=s)
     s.synchronize()
     assert _relerr(I.cpu().numpy(), L.collision(p.f, p.N)) <= TOL
+
+
+def test_full_size_bench_workload_matches_oracle():
+    # BASELINE.json configs[1] / [4] at full size (1.26e7 channels), default variants = the launch configuration bench.py
+    # times: every element of I, Gamma, F' and f(t) against the list oracle, plus sampled states against the definition.
+    p = make_problem("si")
+    L = oracle.OracleList(p)
+    h = ephc.build_channels(p)
+    assert h.query()["nch"] == L.nch > 1.0e7 and h.get_variant() == 1 and h.get_transport_variant() == 0
+    f, N = dev(p.f), dev(p.N)
+    I = torch.empty(p.ns, device="cuda", dtype=torch.float64)
+    h.collision(f, N, I)
+    got = I.cpu().numpy()
+    Io = L.collision(p.f, p.N)
+    assert _relerr(got, Io) <= TOL
+    assert abs(got.sum()) <= 1e-12 * np.abs(got).sum()
+    st = np.random.default_rng(5).choice(np.flatnonzero(Io != 0.0), 24, replace=False).astype(np.int32)
+    Is = oracle.collision_sampled(p, p.f, p.N, st)
+    assert np.abs(got[st] - Is).max() <= TOL * np.abs(Io).max()
+    I2 = torch.empty_like(I)
+    h.collision(f, N, I2)
+    assert torch.equal(I, I2)
+    # transport: Gamma and two iterations from F0 = tau v
+    G = torch.empty(p.ns, device="cuda", dtype=torch.float64)
+    h.transport_setup(dev(p.f0), N, G)
+    Go = L.transport_setup(p.f0, p.N)
+    assert _relerr(G.cpu().numpy(), Go) <= TOL
+    tau_o = np.where(Go > 0, 1.0 / np.where(Go > 0, Go, 1.0), 0.0)
+    Fr = tau_o[None, :] * p.v
+    Fa, Fb = dev(Fr), torch.empty(3 * p.ns, device="cuda", dtype=torch.float64)
+    v, tau = dev(p.v), dev(tau_o)
+    for _ in range(2):
+        h.transport_iter(Fa, v, tau, Fb)
+        Fa, Fb = Fb, Fa
+        Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau_o)
+    assert _relerr(Fa.cpu().numpy().reshape(3, -1), Fr) <= TOL
+    # rt-BTE (config 5's initial condition is make_problem("rt"); same channel set): 2 RK4 steps
+    pr = make_problem("rt")
+    fr = dev(pr.f)
+    sumf = torch.zeros(3, device="cuda", dtype=torch.float64)
+    h.rt_step(fr, dev(pr.N), 1.0, 2, sumf)
+    fo, so = L.rt_step(pr.f, pr.N, 1.0, 2)
+    assert _relerr(fr.cpu().numpy(), fo) <= TOL
+    assert np.abs(sumf.cpu().numpy() - so).max() <= 1e-12 * abs(so[0])
