@@ -15,6 +15,7 @@
 #include "ephc_kernels.cuh"
 #include "ephc_tile_kernels.cuh"
 #include "ephc_row_kernels.cuh"
+#include "ephc_stream_kernels.cuh"
 
 using namespace ephc;
 
@@ -34,7 +35,7 @@ static int fail(int code, const std::string &msg) {
 struct ephc_handle {
     Dims d{};
     bool host_only = false;
-    int variant = 0;  // -1: automatic (collision / rt_step on the tile store, transport on the gather store)
+    int variant = -1;  // -1: automatic (collision / rt_step on the tile store, transport on the gather store)
     Canonical can;
     GatherHost ghost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_gather)
     std::vector<int32_t> pair_ik, pair_ikq;  // copy of the candidate pair list (export)
@@ -74,6 +75,20 @@ struct ephc_handle {
             *dt_blk_ent_ptr = nullptr;
     int64_t *dt_slot_off = nullptr, *dt_blk_ent_off = nullptr;
     int transport_variant = -1;
+    // stream store (variant 2)
+    bool stream_ok = false;
+    std::string stream_why;
+    int32_t s_ncta = 0, s_Ra = 0, s_Rb = 0, s_ntile = 0;
+    int64_t s_entries = 0, s_part_rows = 0, bytes_stream = 0;
+    double *ds_w = nullptr, *ds_part = nullptr;
+    uint32_t *ds_code = nullptr, *ds_iq = nullptr;
+    uint16_t *ds_perm = nullptr, *ds_aid = nullptr, *ds_ast = nullptr, *ds_bid = nullptr, *ds_bst = nullptr;
+    StreamChunk *ds_chunks = nullptr;
+    StreamTile *ds_tiles = nullptr;
+    TileCta *ds_ctas = nullptr;
+    int32_t *ds_row_state = nullptr, *ds_state_row = nullptr, *ds_state_blk = nullptr, *ds_blk_row0 = nullptr,
+            *ds_blk_ent_ptr = nullptr;
+    int64_t *ds_slot_off = nullptr, *ds_blk_ent_off = nullptr;
     // row store (transport_iter of the gather path)
     bool rows_ok = false;
     int32_t r_nstrip = 0, r_Rb = 0, r_Ra = 0;
@@ -95,7 +110,10 @@ static void free_dev(ephc_handle *h) {
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
                     h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_idx, h->dr_perm, h->dr_segs, h->dr_tiles, h->dr_strips,
-                    h->dr_row_state, h->dr_state_row};
+                    h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
+                    h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_ctas, h->ds_row_state,
+                    h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
+                    h->ds_blk_ent_off};
     for (void *p : ptrs)
         if (p) cudaFree(p);
 }
@@ -179,7 +197,29 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
                                   th.ctas.size() * sizeof(TileCta) + th.slot_off.size() * 8 +
                                   (th.blk_row0.size() + th.row_state.size() + th.state_row.size() +
                                    th.state_blk.size() + th.blk_ent_ptr.size()) * 4 + th.blk_ent_off.size() * 8);
-        h->variant = -1;
+    }
+    // stream store (variant 2): one CTA of 1024 threads per SM
+    StreamHost sh;
+    if (std::getenv("EPHC_NO_STREAM") == nullptr) {
+        int nshare = n_sm;
+        if (const char *e = std::getenv("EPHC_STREAM_CTAS")) nshare = std::max(1, std::atoi(e));
+        rc = build_stream(p, h->d, h->can, nshare, sh, err);
+        if (rc != EPHC_OK) {
+            delete h;
+            return fail(rc, err);
+        }
+        h->stream_ok = sh.supported && stream_smem_bytes(sh.Ra, sh.Rb) <= 220 * 1024;
+        h->stream_why = sh.why;
+        h->s_ncta = sh.ncta;
+        h->s_Ra = sh.Ra;
+        h->s_Rb = sh.Rb;
+        h->s_ntile = (int32_t)sh.tiles.size();
+        h->s_entries = (int64_t)sh.w.size();
+        h->s_part_rows = sh.part_rows;
+        h->bytes_stream = (int64_t)(sh.w.size() * 8 + sh.code.size() * 4 + sh.perm.size() * 2 +
+                                    (sh.arow_id.size() + sh.brow_id.size()) * 4 + sh.iq.size() * 4 +
+                                    sh.chunks.size() * sizeof(StreamChunk) + sh.tiles.size() * sizeof(StreamTile));
+        sh.perm.resize(sh.perm.size() + 8, 0);  // the staging copies read whole 8-byte pieces
     }
     // row store for transport_iter (one CTA of 1024 threads per SM, one strip each)
     RowHost rh;
@@ -224,6 +264,29 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         if (rc == EPHC_OK) rc = upload(&h->d_tasks, g.tasks, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_rounds, g.rounds, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_wus, g.wus, &b);
+        if (rc == EPHC_OK && h->stream_ok) {
+            int64_t bs = 0;
+            rc = upload(&h->ds_w, sh.w, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_code, sh.code, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_perm, sh.perm, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_aid, sh.arow_id, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_ast, sh.arow_start, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_bid, sh.brow_id, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_bst, sh.brow_start, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_iq, sh.iq, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_chunks, sh.chunks, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_tiles, sh.tiles, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_ctas, sh.ctas, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_row_state, sh.row_state, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_state_row, sh.state_row, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_state_blk, sh.state_blk, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_blk_row0, sh.blk_row0, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_blk_ent_ptr, sh.blk_ent_ptr, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_blk_ent_off, sh.blk_ent_off, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_slot_off, sh.slot_off, &bs);
+            if (rc == EPHC_OK && cudaMalloc((void **)&h->ds_part, (size_t)std::max<int64_t>(1, sh.part_rows) * 8) != cudaSuccess)
+                rc = fail(EPHC_ENOMEM, "cudaMalloc (stream partial sums) failed");
+        }
         if (rc == EPHC_OK && h->rows_ok) {
             int64_t br = 0;
             rc = upload(&h->dr_idx, rh.idx, &br);
@@ -298,7 +361,7 @@ extern "C" int ephc_query(const ephc_handle *h, ephc_counts *o) {
     o->store_bytes_gather = h->bytes_gather + h->bytes_rows;
     o->scatter_entries = h->t_entries;
     o->scatter_pairs = h->t_pieces;
-    o->store_bytes_scatter = h->bytes_tile;
+    o->store_bytes_scatter = h->bytes_tile + h->bytes_stream;
     o->store_bytes_transport = h->bytes_transport;
     // B_alg: every item the method must move once per evaluation.
     //   8 N_w weights + 4 N_ch channel index + 12 N_pair (ik, ikq, iq) + 16 N_s (read f, write I) + 8 nnu N_q,active
@@ -477,12 +540,17 @@ extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, i
 }
 
 // variant used by ephc_collision / ephc_rt_step, and by ephc_transport_setup / ephc_transport_iter
-static inline int coll_variant(const ephc_handle *h) { return h->variant < 0 ? (h->tile_ok ? 1 : 0) : h->variant; }
-static inline int tr_variant(const ephc_handle *h) { return h->variant < 0 ? 0 : h->variant; }
+static inline int coll_variant(const ephc_handle *h) {
+    return h->variant < 0 ? (h->stream_ok ? 2 : (h->tile_ok ? 1 : 0)) : h->variant;
+}
+static inline int tr_variant(const ephc_handle *h) { return (h->variant < 0 || h->variant == 2) ? 0 : h->variant; }
 
 extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
-    if (variant < -1 || variant > 1) return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather) or 1 (tiles)");
+    if (variant < -1 || variant > 2)
+        return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather), 1 (tiles) or 2 (stream)");
+    if (variant == 2 && !h->stream_ok)
+        return fail(EPHC_ESTATE, "stream store not available for this problem: " + h->stream_why);
     if (variant == 1 && !h->tile_ok)
         return fail(EPHC_ESTATE, "tile store not available for this problem: " + h->thost.why);
     h->variant = variant;
@@ -507,6 +575,9 @@ static int need_device(ephc_handle *h) {
                                       (int)gather_smem_bytes(kTransportSetup)));
         CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)gather_smem_bytes(kTransportIter)));
+        if (h->stream_ok)
+            CUDA_TRY(cudaFuncSetAttribute(stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)stream_smem_bytes(h->s_Ra, h->s_Rb)));
         if (h->rows_ok)
             CUDA_TRY(cudaFuncSetAttribute(row_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)row_smem_bytes(h->r_Rb, h->r_Ra)));
@@ -631,11 +702,62 @@ static int ensure(T **p, size_t n) {
     return EPHC_OK;
 }
 
+static int launch_stream(ephc_handle *h, const double *f, const double *N, cudaStream_t s) {
+    if (h->s_ntile > 0) {
+        StreamParams P;
+        std::memset(&P, 0, sizeof(P));
+        P.w = h->ds_w;
+        P.code = h->ds_code;
+        P.perm = h->ds_perm;
+        P.arow_id = h->ds_aid;
+        P.arow_start = h->ds_ast;
+        P.brow_id = h->ds_bid;
+        P.brow_start = h->ds_bst;
+        P.iq = h->ds_iq;
+        P.chunks = h->ds_chunks;
+        P.tiles = h->ds_tiles;
+        P.ctas = h->ds_ctas;
+        P.row_state = h->ds_row_state;
+        P.slot_off = h->ds_slot_off;
+        P.Ra = h->s_Ra;
+        P.Rb = h->s_Rb;
+        P.nnu = h->d.nnu;
+        P.ncta = h->s_ncta;
+        P.ns = h->d.ns;
+        P.f = f;
+        P.N = N;
+        P.part = h->ds_part;
+        stream_kernel<<<(unsigned)h->s_ncta, kStreamThreads, stream_smem_bytes(h->s_Ra, h->s_Rb), s>>>(P);
+        h->launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
+static FinishParams finish_params_stream(const ephc_handle *h) {
+    FinishParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.state_row = h->ds_state_row;
+    P.state_blk = h->ds_state_blk;
+    P.blk_row0 = h->ds_blk_row0;
+    P.blk_ent_ptr = h->ds_blk_ent_ptr;
+    P.blk_ent_off = h->ds_blk_ent_off;
+    P.part = h->ds_part;
+    P.ns = h->d.ns;
+    return P;
+}
+
 extern "C" int ephc_collision(ephc_handle *h, const double *f_dev, const double *N_dev, double *I_dev,
                               void *stream) {
     int rc = need_device(h);
     if (rc) return rc;
     if (!f_dev || !N_dev || !I_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (coll_variant(h) == 2) {
+        if ((rc = launch_stream(h, f_dev, N_dev, (cudaStream_t)stream))) return rc;
+        FinishParams Fp = finish_params_stream(h);
+        Fp.out = I_dev;
+        return launch_finish<kFCollision>(h, Fp, (cudaStream_t)stream);
+    }
     if (coll_variant(h) == 1) {
         TileParams T = tile_params(h);
         T.f = f_dev;
@@ -798,6 +920,18 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
         for (int st = 0; st < 4; ++st) {
+            if (coll_variant(h) == 2) {
+                if ((rc = launch_stream(h, src[st], N_dev, s))) return rc;
+                FinishParams Fp = finish_params_stream(h);
+                Fp.stage = st + 1;
+                Fp.dt = dt_fs;
+                Fp.f0 = f_dev;
+                Fp.ynext = dst[st];
+                Fp.ksum = h->d_ksum;
+                Fp.blk_sum = sumf_dev ? h->d_wusum : nullptr;
+                if ((rc = launch_finish<kFRkStage>(h, Fp, s))) return rc;
+                continue;
+            }
             if (coll_variant(h) == 1) {
                 TileParams T = tile_params(h);
                 T.f = src[st];
@@ -820,7 +954,7 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
             if (rc) return rc;
         }
         if (sumf_dev) {
-            if (coll_variant(h) == 1)
+            if (coll_variant(h) >= 1)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);
             else if (h->n_wu > 0)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, h->n_wu, sumf_dev + it + 1);

@@ -171,4 +171,51 @@ struct RowHost {
 };
 int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int nstrip, RowHost &r, std::string &err);
 
+// ---- stream store (variant 2, collision / RK stages): one LANE per ENTRY ------------------------------------------
+// Same tiles and partial-sum slots as the tile store (strip of k rows x range of k' rows, both staged in shared
+// memory), but inside a tile the entries are sorted by their k-side row and cut into chunks of <= 4096 entries.
+// A chunk is evaluated by all threads of the CTA, one entry per lane and step, fully coalesced; the per-entry terms
+// T stay in shared memory and are then summed per k row (contiguous runs) and per k' row (through a chunk-local
+// permutation) by one thread per row: one owner per row and chunk, no atomics, fixed order.
+//   entry: w fp64 + code uint32 = k row - chunk.a0 (8 bit) | k' row - tile.b_row0 (11 bit) << 8 |
+//                                 N slot = pair_in_chunk * nnu + mode (12 bit) << 19 | kind << 31
+constexpr int kStreamChunk = 4096;
+constexpr int kStreamRbMax = 2048;
+struct StreamChunk {          // 48 bytes
+    int64_t e0;               // first entry (also first perm element)
+    int32_t ne;               // entries
+    int32_t a0;               // k row (local to the tile) that a_loc counts from
+    int32_t ar0, nar;         // k-row tasks:  arow_id / arow_start [ar0 .. ar0+nar], start relative to the chunk
+    int32_t br0, nbr;         // k'-row tasks
+    int32_t q0, nq;           // pairs: iq[q0 .. q0+nq)
+    int32_t pad0, pad1;       // pad0: first element of the chunk's permutation / 4 (starts are multiples of 4)
+};
+struct StreamTile {
+    int32_t c0, nc;           // chunk range
+    int32_t a_row0, a_rows, b_row0, b_rows;
+    int32_t a_slot, b_slot;
+    int32_t flags;            // as TileHdr
+    int32_t pad;
+};
+struct StreamHost {
+    int32_t Ra = 0, Rb = 0, nblk = 0, nrows = 0, ncta = 0, rf = 0;
+    std::vector<int32_t> blk_row0, row_state, state_row, state_blk;
+    std::vector<double> w;
+    std::vector<uint32_t> code;
+    std::vector<uint16_t> perm;                 // per chunk (padded to a multiple of 4): chunk-local entry index, sorted by k' row
+    std::vector<uint16_t> arow_id, arow_start;  // per k-row task (+1 sentinel per chunk in arow_start)
+    std::vector<uint16_t> brow_id, brow_start;
+    std::vector<uint32_t> iq;                   // per (chunk, pair)
+    std::vector<StreamChunk> chunks;
+    std::vector<StreamTile> tiles;
+    std::vector<TileCta> ctas;
+    std::vector<int64_t> slot_off;
+    std::vector<int32_t> slot_row0, slot_rows, blk_ent_ptr;
+    std::vector<int64_t> blk_ent_off;
+    int64_t part_rows = 0;
+    bool supported = false;
+    std::string why;
+};
+int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, StreamHost &t, std::string &err);
+
 }  // namespace ephc

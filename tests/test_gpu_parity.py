@@ -37,7 +37,7 @@ def _small_problems():
 IDS = ["tiny4", "window_cut_diag", "si12", "gaas24", "bigcell3", "tiny_full", "rt14"]
 
 
-VARIANTS = {0: "gather", 1: "tiles"}
+VARIANTS = {0: "gather", 1: "tiles", 2: "stream"}
 
 
 @pytest.fixture(scope="module", params=[(i, v) for i in range(len(IDS)) for v in VARIANTS],
@@ -47,8 +47,8 @@ def case(request):
     p = _small_problems()[idx]
     h = ephc.build_channels(p)
     if variant == 1 and h.query()["scatter_entries"] == 0 and h.query()["nw"] > 0:
-        assert h.get_variant() == 0
-        pytest.skip("tile store covers nb <= 4, nnu <= 8 (DESIGN.md): this shape runs on the gather path")
+        assert h.get_variant() in (0, 2)
+        pytest.skip("tile store covers nb <= 4, nnu <= 8 (DESIGN.md): this shape runs on the stream / gather stores")
     h.set_variant(variant)
     return p, oracle.OracleList(p), h
 
@@ -210,7 +210,7 @@ def test_tile_geometry_on_gpu(monkeypatch, rows, ctas):
     for p in _small_problems()[:4]:
         L = oracle.OracleList(p)
         h = ephc.build_channels(p)
-        assert h.get_variant() == 1
+        h.set_variant(1)
         I = np.zeros(p.ns)
         h.collision_host(p.f, p.N, I)
         assert _relerr(I, L.collision(p.f, p.N)) <= TOL
@@ -226,6 +226,30 @@ def test_tile_geometry_on_gpu(monkeypatch, rows, ctas):
         for _ in range(3):
             Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau)
         assert _relerr(F, Fr) <= TOL
+        f = p.f.copy()
+        s = np.zeros(6)
+        h.rt_step_host(f, p.N, 1.0, 5, s)
+        fo, so = L.rt_step(p.f, p.N, 1.0, 5)
+        assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
+
+
+@pytest.mark.parametrize("rows,fine,ctas", [(16, 4, 3), (64, 8, 40), (2048, 128, 1), (256, 16, 7)])
+def test_stream_geometry_on_gpu(monkeypatch, rows, fine, ctas):
+    # many small tiles and chunks, runs cut by share boundaries, one CTA for everything
+    monkeypatch.setenv("EPHC_STREAM_ROWS", str(rows))
+    monkeypatch.setenv("EPHC_STREAM_ROWS_B", str(rows))
+    monkeypatch.setenv("EPHC_STREAM_FINE", str(fine))
+    monkeypatch.setenv("EPHC_STREAM_CTAS", str(ctas))
+    for p in _small_problems()[:5]:
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p)
+        assert h.get_variant() == 2
+        I = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I)
+        assert _relerr(I, L.collision(p.f, p.N)) <= TOL
+        I2 = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I2)
+        assert np.array_equal(I, I2)
         f = p.f.copy()
         s = np.zeros(6)
         h.rt_step_host(f, p.N, 1.0, 5, s)
@@ -253,7 +277,7 @@ def test_full_size_bench_workload_matches_oracle():
     p = make_problem("si")
     L = oracle.OracleList(p)
     h = ephc.build_channels(p)
-    assert h.query()["nch"] == L.nch > 1.0e7 and h.get_variant() == 1 and h.get_transport_variant() == 0
+    assert h.query()["nch"] == L.nch > 1.0e7 and h.get_variant() == 2 and h.get_transport_variant() == 0
     f, N = dev(p.f), dev(p.N)
     I = torch.empty(p.ns, device="cuda", dtype=torch.float64)
     h.collision(f, N, I)
