@@ -47,7 +47,7 @@ def parse():
     ap.add_argument("--config", default="si", help="workload: si (default, BASELINE configs[1]) | tiny | gaas | bigcell")
     ap.add_argument("--grid", type=int, default=0, help="override the grid edge (smaller copies for quick runs)")
     ap.add_argument("--pair-prob", type=float, default=0.0)
-    ap.add_argument("--variant", type=int, default=-1, help="-1: automatic (library default), 0: gather, 1: tiles")
+    ap.add_argument("--variant", type=int, default=-1, help="-1: automatic (library default), 0: gather, 1: tiles, 2: stream")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -296,6 +296,8 @@ def main():
         w_setup = 8 * q["gather_entries"]
     if variant == 1:
         kn.update({"c": "tile_kernel<0> + finish_kernel<0>", "r": "tile_kernel<0> + finish_kernel<1>"})
+    if variant == 2:
+        kn.update({"c": "stream_kernel + finish_kernel<0>", "r": "stream_kernel + finish_kernel<1>"})
     if tvariant == 1:
         kn.update({"s": "tile_kernel<2> + finish_kernel<2>", "i": "tile_kernel<3> + finish_kernel<3>"})
         w_setup = 16 * q["scatter_entries"]
@@ -359,8 +361,8 @@ def main():
 
     if rank == 0:
         cfg = workload_config(args, p, nch)
-        sb = (q["store_bytes_scatter"] if 1 in (variant, tvariant) else 0) + (q["store_bytes_gather"] if 0 in (variant, tvariant) else 0)
-        names = {0: "gather", 1: "tiles"}
+        sb = (q["store_bytes_scatter"] if (variant in (1, 2) or tvariant == 1) else 0) + (q["store_bytes_gather"] if 0 in (variant, tvariant) else 0)
+        names = {0: "gather", 1: "tiles", 2: "stream"}
         tname = names[tvariant] if (tvariant == 1 or os.environ.get("EPHC_NO_ROWS")) else "rows (setup on gather)"
         cfg.update({"variant": f"collision/rt: {names[variant]}, transport: {tname}",
                     "l2": f"no flush: every evaluation streams the {sb / 1e6:.0f} MB store "

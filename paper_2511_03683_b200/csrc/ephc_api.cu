@@ -198,10 +198,10 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
                                   (th.blk_row0.size() + th.row_state.size() + th.state_row.size() +
                                    th.state_blk.size() + th.blk_ent_ptr.size()) * 4 + th.blk_ent_off.size() * 8);
     }
-    // stream store (variant 2): one CTA of 1024 threads per SM
+    // stream store (variant 2): two CTAs of 512 threads per SM
     StreamHost sh;
     if (std::getenv("EPHC_NO_STREAM") == nullptr) {
-        int nshare = n_sm;
+        int nshare = 2 * n_sm;
         if (const char *e = std::getenv("EPHC_STREAM_CTAS")) nshare = std::max(1, std::atoi(e));
         rc = build_stream(p, h->d, h->can, nshare, sh, err);
         if (rc != EPHC_OK) {

@@ -173,14 +173,15 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
 
 // ---- stream store (variant 2, collision / RK stages): one LANE per ENTRY ------------------------------------------
 // Same tiles and partial-sum slots as the tile store (strip of k rows x range of k' rows, both staged in shared
-// memory), but inside a tile the entries are sorted by their k-side row and cut into chunks of <= 4096 entries.
+// memory), but inside a tile the entries are sorted by their k-side row and cut into chunks of <= 2048 entries.
 // A chunk is evaluated by all threads of the CTA, one entry per lane and step, fully coalesced; the per-entry terms
 // T stay in shared memory and are then summed per k row (contiguous runs) and per k' row (through a chunk-local
 // permutation) by one thread per row: one owner per row and chunk, no atomics, fixed order.
 //   entry: w fp64 + code uint32 = k row - chunk.a0 (8 bit) | k' row - tile.b_row0 (11 bit) << 8 |
 //                                 N slot = pair_in_chunk * nnu + mode (12 bit) << 19 | kind << 31
-constexpr int kStreamChunk = 4096;
-constexpr int kStreamRbMax = 2048;
+constexpr int kStreamChunk = 2048;     // entries per chunk
+constexpr int kStreamNSlots = 2048;    // N values staged per chunk
+constexpr int kStreamRbMax = 2048;    // 11-bit k' row in the entry code
 struct StreamChunk {          // 48 bytes
     int64_t e0;               // first entry (also first perm element)
     int32_t ne;               // entries

@@ -41,7 +41,7 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
             }
         t.nrows = (int32_t)t.row_state.size();
         // fine blocks of Rf rows, strips of Ra rows (multiples of Rf), k' ranges of <= Rb rows
-        int Rf = 128, Ra = 1536, Rb = 2048;
+        int Rf = 128, Ra = 1024, Rb = 1536;
         if (const char *e = std::getenv("EPHC_STREAM_FINE")) Rf = std::atoi(e);
         if (const char *e = std::getenv("EPHC_STREAM_ROWS")) Ra = std::atoi(e);
         if (const char *e = std::getenv("EPHC_STREAM_ROWS_B")) Rb = std::atoi(e);
@@ -69,17 +69,25 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
             return (j < (I + 1) * bps) ? atom0[I] : atom0[I] + 1 + (j - (I + 1) * bps);
         };
         // entries and work per atom
-        std::vector<int64_t> atom_ne((size_t)natom + 1, 0);
+        // work of an atom: its entries plus a per-pair cost (N[iq,:] staging, chunks cut by the slot limit)
+        int pair_cost = 4;  // measured on B200 (Si workload): 0 -> 155 us, 4 -> 141 us, 8 -> 146 us
+        if (const char *e = std::getenv("EPHC_STREAM_PAIR_COST")) pair_cost = std::max(0, std::atoi(e));
+        std::vector<int64_t> atom_ne((size_t)natom + 1, 0), atom_wk((size_t)natom + 1, 0);
         for (int64_t ip = 0; ip < npair; ++ip) {
             const int64_t sa = (int64_t)p->pair_ik[ip] * nb, sb = (int64_t)p->pair_ikq[ip] * nb;
             for (int64_t j = c.pair_ch0[ip]; j < c.pair_ch0[ip + 1]; ++j) {
                 const int n = c.ch_code[j] & 15, m = (c.ch_code[j] >> 4) & 15;
                 const int64_t at = atom_of(t.state_row[sa + n], t.state_row[sb + m]);
-                atom_ne[at + 1] += (c.ch_wabs[j] != 0.0) + (c.ch_wem[j] != 0.0);
+                const int ne = (c.ch_wabs[j] != 0.0) + (c.ch_wem[j] != 0.0);
+                atom_ne[at + 1] += ne;
+                atom_wk[at + 1] += ne + (j == c.pair_ch0[ip] ? pair_cost : 0);
             }
         }
-        for (int64_t i = 0; i < natom; ++i) atom_ne[i + 1] += atom_ne[i];
-        const int64_t nent = atom_ne[natom];
+        for (int64_t i = 0; i < natom; ++i) {
+            atom_ne[i + 1] += atom_ne[i];
+            atom_wk[i + 1] += atom_wk[i];
+        }
+        const int64_t nent = atom_ne[natom], nwork = atom_wk[natom];
         // contiguous shares of equal work; tiles = consecutive atoms of one strip inside a share, <= Rb rows
         t.ncta = ncta;
         t.ctas.assign((size_t)ncta, TileCta{0, 0});
@@ -88,10 +96,10 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
         {
             int64_t at = 0;
             for (int cta = 0; cta < ncta; ++cta) {
-                const int64_t goal = nent * (int64_t)(cta + 1) / ncta;
+                const int64_t goal = nwork * (int64_t)(cta + 1) / ncta;
                 t.ctas[cta].t0 = (int32_t)tile_at0.size();
                 const int64_t first = at;
-                while (at < natom && (cta == ncta - 1 || (atom_ne[at] + atom_ne[at + 1]) / 2 <= goal)) ++at;
+                while (at < natom && (cta == ncta - 1 || (atom_wk[at] + atom_wk[at + 1]) / 2 <= goal)) ++at;
                 int64_t a0 = first;
                 while (a0 < at) {
                     if (atom_ne[a0 + 1] == atom_ne[a0]) {
@@ -162,7 +170,7 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
             std::vector<uint16_t> perm, aid, ast, bid, bst;
         };
         std::vector<TileOut> outs((size_t)ntile);
-        const int pair_cap = std::max(1, 4096 / nnu);
+        const int pair_cap = std::max(1, kStreamNSlots / nnu);
 #pragma omp parallel
         {
             std::vector<int32_t> slot_of((size_t)npair, -1);
@@ -328,6 +336,26 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
             nar += ch.nar;
             nbr += ch.nbr;
             nq += ch.nq;
+        }
+        {
+            double mn[4] = {1e30, 1e30, 1e30, 1e30}, mx[4] = {0, 0, 0, 0};
+            for (const TileCta &ct : t.ctas) {
+                double v[4] = {0, 0, 0, 0};
+                for (int32_t it = ct.t0; it < ct.t1; ++it) {
+                    v[3] += 1;
+                    for (int32_t ci = t.tiles[it].c0; ci < t.tiles[it].c0 + t.tiles[it].nc; ++ci) {
+                        v[0] += t.chunks[ci].ne;
+                        v[1] += 1;
+                        v[2] += t.chunks[ci].nq;
+                    }
+                }
+                for (int j = 0; j < 4; ++j) {
+                    mn[j] = std::min(mn[j], v[j]);
+                    mx[j] = std::max(mx[j], v[j]);
+                }
+            }
+            std::fprintf(stderr, "stream shares: entries %.0f..%.0f, chunks %.0f..%.0f, pairs %.0f..%.0f, tiles %.0f..%.0f\n", mn[0], mx[0],
+                         mn[1], mx[1], mn[2], mx[2], mn[3], mx[3]);
         }
         const double n = (double)std::max<size_t>(t.chunks.size(), 1);
         std::fprintf(stderr, "stream store: %zu tiles, %zu chunks, per chunk: %.0f entries, %.0f k rows, %.0f k' rows, %.0f pairs; Ra %d Rb %d\n",

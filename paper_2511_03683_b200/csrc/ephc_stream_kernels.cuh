@@ -3,9 +3,9 @@
 // channels of a state", here both inside one kernel and with the per-channel terms kept in shared memory instead of
 // the paper's sc_col array in global memory).
 //
-// A CTA of 1024 threads walks its share of tiles (strip of k rows x range of k' rows; f of both ranges and one
+// A CTA of 512 threads (two per SM) walks its share of tiles (strip of k rows x range of k' rows; f of both ranges and one
 // accumulator per row of both ranges in shared memory).  A tile's entries are sorted by k row and cut into chunks of
-// <= 4096.  Per chunk:
+// <= 2048.  Per chunk:
 //   phase 1  every thread evaluates Eq. 2's summand T of its <= 4 entries (weights and codes stream from HBM fully
 //            coalesced, loaded one chunk ahead; N[iq,nu] of the chunk's pairs was copied to shared memory one chunk
 //            ahead with cp.async) and stores T to shared memory;
@@ -21,9 +21,10 @@
 
 namespace ephc {
 
-constexpr int kStreamThreads = 1024;
+constexpr int kStreamThreads = 512;   // two CTAs per SM: the barrier waits of one overlap with the work of the other
 constexpr int kStreamEpt = kStreamChunk / kStreamThreads;  // entries per thread and chunk
-constexpr int kStreamNSlots = 4096;                         // N values staged per chunk (12-bit slot)
+constexpr int kBT = (kStreamRbMax + kStreamThreads - 1) / kStreamThreads;  // k' row tasks per thread and chunk
+static_assert(2 * 256 <= kStreamThreads, "two lanes per k row, <= 256 k rows per chunk");
 
 struct StreamParams {
     const double *w;
@@ -51,7 +52,7 @@ __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gmem_src) 
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gmem_src));
 }
 
-__global__ void __launch_bounds__(kStreamThreads, 1) stream_kernel(const StreamParams P) {
+__global__ void __launch_bounds__(kStreamThreads, 2) stream_kernel(const StreamParams P) {
     extern __shared__ double smem[];
     double *sIa = smem;                      // f of the k rows
     double *sIb = sIa + P.Ra + 2;            // f of the k' rows
@@ -124,15 +125,19 @@ __global__ void __launch_bounds__(kStreamThreads, 1) stream_kernel(const StreamP
             const uint16_t *cP = sPerm + buf * kStreamChunk;
             if (ci + 1 < th.nc) chn = P.chunks[th.c0 + ci + 1];
             // row tasks of this chunk (<= 256 k rows, <= 2048 k' rows): headers to registers before they are needed
-            int ta_row = 0, ta_s0 = 0, ta_s1 = 0, tb_row[2], tb_s0[2], tb_s1[2];
-            if (tid < ch.nar) {
-                ta_row = __ldg(P.arow_id + ch.ar0 + tid);
-                ta_s0 = __ldg(P.arow_start + ch.ar0 + tid);
-                ta_s1 = __ldg(P.arow_start + ch.ar0 + tid + 1);
+            // k rows: two lanes per row from the low warps; k' rows: one thread per row from the high warps downwards
+            int ta_row = 0, ta_s0 = 0, ta_s1 = 0, tb_row[kBT], tb_s0[kBT], tb_s1[kBT];
+            const int arow = tid >> 1, apart = tid & 1;
+            if (arow < ch.nar) {
+                ta_row = __ldg(P.arow_id + ch.ar0 + arow);
+                const int s0 = __ldg(P.arow_start + ch.ar0 + arow), s1 = __ldg(P.arow_start + ch.ar0 + arow + 1);
+                const int q = (s1 - s0 + 1) >> 1;
+                ta_s0 = min(s0 + apart * q, s1);
+                ta_s1 = min(ta_s0 + q, s1);
             }
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const int id = tid + u * kStreamThreads;
+            for (int u = 0; u < kBT; ++u) {
+                const int id = (kStreamThreads - 1 - tid) + u * kStreamThreads;
                 tb_row[u] = tb_s0[u] = tb_s1[u] = 0;
                 if (id < ch.nbr) {
                     tb_row[u] = __ldg(P.brow_id + ch.br0 + id);
@@ -158,18 +163,24 @@ __global__ void __launch_bounds__(kStreamThreads, 1) stream_kernel(const StreamP
             }
             __syncthreads();
             // ---- phase 2: one thread per row of the chunk ----------------------------------------------------------------
-            if (tid < ch.nar) {
+            if (tid < 2 * ((ch.nar + 15) & ~15)) {  // whole warps: the shuffle below needs all their lanes
                 double sum = 0.0;
                 for (int i = ta_s0; i < ta_s1; ++i) sum += sT[i];
-                sAa[ta_row] -= sum;
+                sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+                if (apart == 0 && arow < ch.nar) sAa[ta_row] -= sum;
             }
             if (dg) __syncthreads();  // the same row can be a k row and a k' row of a diagonal tile
 #pragma unroll
-            for (int u = 0; u < 2; ++u)
-                if (tid + u * kStreamThreads < ch.nbr) {
-                    double sum = 0.0;
-                    for (int i = tb_s0[u]; i < tb_s1[u]; ++i) sum += sT[cP[i]];
-                    accB[tb_row[u]] += sum;
+            for (int u = 0; u < kBT; ++u)
+                if ((kStreamThreads - 1 - tid) + u * kStreamThreads < ch.nbr) {
+                    double s0 = 0.0, s1 = 0.0;
+                    int i = tb_s0[u];
+                    for (; i + 1 < tb_s1[u]; i += 2) {
+                        s0 += sT[cP[i]];
+                        s1 += sT[cP[i + 1]];
+                    }
+                    if (i < tb_s1[u]) s0 += sT[cP[i]];
+                    accB[tb_row[u]] += s0 + s1;
                 }
             ch = chn;
         }
