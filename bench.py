@@ -166,6 +166,18 @@ def run_reference(args):
     }))
 
 
+def reduce_over_ranks(dist, dev, ms_total, nch):
+    """Replicas: the job's time is the MAX over ranks, its work the SUM of the ranks' channels."""
+    if dist is None:
+        return float(ms_total), float(nch)
+    import torch
+    t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    tot = torch.tensor([float(nch)], device=dev, dtype=torch.float64)
+    dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(tot.item())
+
+
 def workload_config(args, p, nch):
     return {"workload": f"{p.name}: {p.grid[0]}x{p.grid[1]}x{p.grid[2]} k-grid, window [{p.emin},{p.emax}] eV, "
                         f"{p.nk} active k, {p.nb} bands, {p.nnu} modes, sigma={p.sigma} eV",
@@ -263,16 +275,7 @@ def main():
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     launches = h.launch_count() - l0
-    ms_total = start.elapsed_time(stop)
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-        tot = torch.tensor([float(nch)], device=dev, dtype=torch.float64)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        nch_all = float(tot.item())
-    else:
-        nch_all = float(nch)
+    ms_total, nch_all = reduce_over_ranks(dist, dev, start.elapsed_time(stop), nch)
     value = nch_all * EVALS_PER_STEP * args.steps / (ms_total * 1e-3)
 
     # per-phase device times (this rank)
