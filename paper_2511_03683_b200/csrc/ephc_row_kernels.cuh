@@ -100,40 +100,48 @@ __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParam
         }
         __syncthreads();
         // segments are sorted by descending length; warps take four at a time from a shared counter
-        // (order of execution only: every row has one segment per tile, hence one writer)
-        while (true) {
-            int sg0 = 0;
-            if (lane == 0) sg0 = atomicAdd(sNext, GPW);
-            sg0 = __shfl_sync(0xffffffffu, sg0, 0);
-            if (sg0 >= tl.nseg) break;
-            const int sg = sg0 + sub;
-            uint32_t start = 0, len = 0, row = 0;
-            if (sg < tl.nseg) {
-                const uint4 q = __ldg(reinterpret_cast<const uint4 *>(P.segs + tl.seg0 + sg));
+        // (order of execution only: every row has one segment per tile, hence one writer).  The header of the next
+        // group of segments is fetched while the current one is processed, and its first batch of entries is loaded
+        // during the last batch of the current one, so that no load latency is exposed between segments.
+        auto fetch = [&](int &sg0, uint32_t &start, uint32_t &len, uint32_t &row) {
+            int g = 0;
+            if (lane == 0) g = atomicAdd(sNext, GPW);
+            sg0 = __shfl_sync(0xffffffffu, g, 0);
+            start = len = row = 0;
+            if (sg0 + sub < tl.nseg) {
+                const uint4 q = __ldg(reinterpret_cast<const uint4 *>(P.segs + tl.seg0 + sg0 + sub));
                 start = q.x;
                 len = q.y;
                 row = q.z;
             }
-            const double *w = Wb + start;
-            const uint16_t *ix = Ib + start;
-            double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-            // kRowBatch entries per lane are in flight while the previous kRowBatch are multiplied
-            double wn[kRowBatch];
-            unsigned jn[kRowBatch];
-            auto load_batch = [&](uint32_t i) {
+        };
+        double wn[kRowBatch];
+        unsigned jn[kRowBatch];
+        auto load_batch = [&](uint32_t start, uint32_t len, uint32_t i) {
 #pragma unroll
-                for (int u = 0; u < kRowBatch; ++u) {
-                    const uint32_t ii = i + u * kRowGroup;
-                    wn[u] = 0.0;
-                    jn[u] = 0;
-                    if (ii < len) {
-                        wn[u] = __ldcs(w + ii);
-                        jn[u] = __ldcs(ix + ii);
-                    }
+            for (int u = 0; u < kRowBatch; ++u) {
+                const uint32_t ii = i + u * kRowGroup;
+                wn[u] = 0.0;
+                jn[u] = 0;
+                if (ii < len) {
+                    wn[u] = __ldcs(Wb + start + ii);
+                    jn[u] = __ldcs(Ib + start + ii);
                 }
-            };
-            load_batch(gl);
-            for (uint32_t i = gl; i < len; i += kRowBatch * kRowGroup) {
+            }
+        };
+        int sg0, sgN;
+        uint32_t start, len, row, startN, lenN, rowN;
+        fetch(sg0, start, len, row);
+        if (sg0 < tl.nseg) load_batch(start, len, gl);
+        while (sg0 < tl.nseg) {
+            fetch(sgN, startN, lenN, rowN);
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+            const uint32_t step = kRowBatch * kRowGroup;
+            // all lanes of the warp run the same number of trips (the longest segment of the four)
+            uint32_t lmax = len;
+            lmax = max(lmax, __shfl_xor_sync(0xffffffffu, lmax, 8));
+            lmax = max(lmax, __shfl_xor_sync(0xffffffffu, lmax, 16));
+            for (uint32_t ib = 0; ib < lmax; ib += step) {
                 double wv[kRowBatch];
                 unsigned jv[kRowBatch];
 #pragma unroll
@@ -141,7 +149,10 @@ __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParam
                     wv[u] = wn[u];
                     jv[u] = jn[u];
                 }
-                if (i + kRowBatch * kRowGroup < len) load_batch(i + kRowBatch * kRowGroup);
+                if (ib + step < lmax)
+                    load_batch(start, len, ib + step + gl);
+                else if (sgN < tl.nseg)
+                    load_batch(startN, lenN, gl);
 #pragma unroll
                 for (int u = 0; u < kRowBatch; ++u) {
                     const double *f = sF + jv[u] * 3;
@@ -156,11 +167,15 @@ __global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParam
                 a1 += __shfl_xor_sync(0xffffffffu, a1, o);
                 a2 += __shfl_xor_sync(0xffffffffu, a2, o);
             }
-            if (gl == 0 && sg < tl.nseg) {  // the only writer of this row in this tile
+            if (gl == 0 && sg0 + sub < tl.nseg) {  // the only writer of this row in this tile
                 sAcc[row * 3 + 0] += a0;
                 sAcc[row * 3 + 1] += a1;
                 sAcc[row * 3 + 2] += a2;
             }
+            sg0 = sgN;
+            start = startN;
+            len = lenN;
+            row = rowN;
         }
     }
     __syncthreads();
