@@ -85,7 +85,8 @@ struct ephc_handle {
     uint16_t *ds_perm = nullptr, *ds_aid = nullptr, *ds_ast = nullptr, *ds_bid = nullptr, *ds_bst = nullptr;
     StreamChunk *ds_chunks = nullptr;
     StreamTile *ds_tiles = nullptr;
-    TileCta *ds_ctas = nullptr;
+    int32_t *ds_order = nullptr;
+    int *ds_counter = nullptr;
     int32_t *ds_row_state = nullptr, *ds_state_row = nullptr, *ds_state_blk = nullptr, *ds_blk_row0 = nullptr,
             *ds_blk_ent_ptr = nullptr;
     int64_t *ds_slot_off = nullptr, *ds_blk_ent_off = nullptr;
@@ -111,7 +112,7 @@ static void free_dev(ephc_handle *h) {
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
                     h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_idx, h->dr_perm, h->dr_segs, h->dr_tiles, h->dr_strips,
                     h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
-                    h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_ctas, h->ds_row_state,
+                    h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_order, h->ds_counter, h->ds_row_state,
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
                     h->ds_blk_ent_off};
     for (void *p : ptrs)
@@ -276,7 +277,10 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             if (rc == EPHC_OK) rc = upload(&h->ds_iq, sh.iq, &bs);
             if (rc == EPHC_OK) rc = upload(&h->ds_chunks, sh.chunks, &bs);
             if (rc == EPHC_OK) rc = upload(&h->ds_tiles, sh.tiles, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_ctas, sh.ctas, &bs);
+            if (rc == EPHC_OK) rc = upload(&h->ds_order, sh.order, &bs);
+            if (rc == EPHC_OK && (cudaMalloc((void **)&h->ds_counter, 64) != cudaSuccess ||
+                                  cudaMemset(h->ds_counter, 0, 64) != cudaSuccess))
+                rc = fail(EPHC_ENOMEM, "cudaMalloc (tile counter) failed");
             if (rc == EPHC_OK) rc = upload(&h->ds_row_state, sh.row_state, &bs);
             if (rc == EPHC_OK) rc = upload(&h->ds_state_row, sh.state_row, &bs);
             if (rc == EPHC_OK) rc = upload(&h->ds_state_blk, sh.state_blk, &bs);
@@ -716,7 +720,9 @@ static int launch_stream(ephc_handle *h, const double *f, const double *N, cudaS
         P.iq = h->ds_iq;
         P.chunks = h->ds_chunks;
         P.tiles = h->ds_tiles;
-        P.ctas = h->ds_ctas;
+        P.order = h->ds_order;
+        P.counter = h->ds_counter;
+        P.ntile = h->s_ntile;
         P.row_state = h->ds_row_state;
         P.slot_off = h->ds_slot_off;
         P.Ra = h->s_Ra;
@@ -744,6 +750,7 @@ static FinishParams finish_params_stream(const ephc_handle *h) {
     P.blk_ent_off = h->ds_blk_ent_off;
     P.part = h->ds_part;
     P.ns = h->d.ns;
+    P.reset = h->ds_counter;
     return P;
 }
 

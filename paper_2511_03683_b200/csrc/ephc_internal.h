@@ -209,7 +209,8 @@ struct StreamHost {
     std::vector<uint32_t> iq;                   // per (chunk, pair)
     std::vector<StreamChunk> chunks;
     std::vector<StreamTile> tiles;
-    std::vector<TileCta> ctas;
+    std::vector<int32_t> order;                 // tiles by descending work: the order in which CTAs take them
+    std::vector<TileCta> ctas;                  // shares used to cut the tiles (host only)
     std::vector<int64_t> slot_off;
     std::vector<int32_t> slot_row0, slot_rows, blk_ent_ptr;
     std::vector<int64_t> blk_ent_off;

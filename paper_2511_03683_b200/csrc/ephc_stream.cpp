@@ -89,17 +89,22 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
         }
         const int64_t nent = atom_ne[natom], nwork = atom_wk[natom];
         // contiguous shares of equal work; tiles = consecutive atoms of one strip inside a share, <= Rb rows
+        // Tiles are cut so that a CTA gets about `tiles_per_cta` of them; the kernel hands them out dynamically,
+        // largest first (t.order), so every tile is self-contained (own partial-sum slots for both row ranges).
+        int tiles_per_cta = 3;
+        if (const char *e = std::getenv("EPHC_STREAM_TILES_PER_CTA")) tiles_per_cta = std::max(1, std::atoi(e));
         t.ncta = ncta;
-        t.ctas.assign((size_t)ncta, TileCta{0, 0});
+        const int nshare = ncta * tiles_per_cta;
+        t.ctas.assign((size_t)nshare, TileCta{0, 0});
         std::vector<int64_t> tile_at0, tile_at1;
         std::vector<int32_t> tile_strip;
         {
             int64_t at = 0;
-            for (int cta = 0; cta < ncta; ++cta) {
-                const int64_t goal = nwork * (int64_t)(cta + 1) / ncta;
+            for (int cta = 0; cta < nshare; ++cta) {
+                const int64_t goal = nwork * (int64_t)(cta + 1) / nshare;
                 t.ctas[cta].t0 = (int32_t)tile_at0.size();
                 const int64_t first = at;
-                while (at < natom && (cta == ncta - 1 || (atom_wk[at] + atom_wk[at + 1]) / 2 <= goal)) ++at;
+                while (at < natom && (cta == nshare - 1 || (atom_wk[at] + atom_wk[at + 1]) / 2 <= goal)) ++at;
                 int64_t a0 = first;
                 while (a0 < at) {
                     if (atom_ne[a0 + 1] == atom_ne[a0]) {
@@ -292,12 +297,12 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
             o = TileOut();
         }
         // a-runs, partial-sum slots and the per-fine-block lists (as in the tile store)
-        for (int cta = 0; cta < ncta; ++cta)
-            for (int32_t it = t.ctas[cta].t0; it < t.ctas[cta].t1; ++it) {
-                const bool first = (it == t.ctas[cta].t0) || (tile_strip[it - 1] != tile_strip[it]);
-                const bool last = (it + 1 == t.ctas[cta].t1) || (tile_strip[it + 1] != tile_strip[it]);
-                t.tiles[it].flags |= (first ? 1 : 0) | (last ? 2 : 0);
-            }
+        for (int64_t it = 0; it < ntile; ++it) t.tiles[it].flags |= 3;  // every tile stages and flushes both row ranges
+        t.order.resize((size_t)ntile);
+        for (int64_t it = 0; it < ntile; ++it) t.order[it] = (int32_t)it;
+        std::stable_sort(t.order.begin(), t.order.end(), [&](int32_t x, int32_t y) {
+            return atom_wk[tile_at1[x]] - atom_wk[tile_at0[x]] > atom_wk[tile_at1[y]] - atom_wk[tile_at0[y]];
+        });
         int64_t rows = 0;
         auto new_slot = [&](int32_t row0, int32_t nrows) {
             const int32_t sl = (int32_t)t.slot_off.size();

@@ -3,7 +3,7 @@
 // channels of a state", here both inside one kernel and with the per-channel terms kept in shared memory instead of
 // the paper's sc_col array in global memory).
 //
-// A CTA of 512 threads (two per SM) walks its share of tiles (strip of k rows x range of k' rows; f of both ranges and one
+// A CTA of 512 threads (two per SM) takes tiles from a global counter, largest first (strip of k rows x range of k' rows; f of both ranges and one
 // accumulator per row of both ranges in shared memory).  A tile's entries are sorted by k row and cut into chunks of
 // <= 2048.  Per chunk:
 //   phase 1  every thread evaluates Eq. 2's summand T of its <= 4 entries (weights and codes stream from HBM fully
@@ -23,7 +23,6 @@ namespace ephc {
 
 constexpr int kStreamThreads = 512;   // two CTAs per SM: the barrier waits of one overlap with the work of the other
 constexpr int kStreamEpt = kStreamChunk / kStreamThreads;  // entries per thread and chunk
-constexpr int kBT = (kStreamRbMax + kStreamThreads - 1) / kStreamThreads;  // k' row tasks per thread and chunk
 static_assert(2 * 256 <= kStreamThreads, "two lanes per k row, <= 256 k rows per chunk");
 
 struct StreamParams {
@@ -33,7 +32,9 @@ struct StreamParams {
     const uint32_t *iq;
     const StreamChunk *chunks;
     const StreamTile *tiles;
-    const TileCta *ctas;
+    const int32_t *order;   // tiles by descending work
+    int *counter;           // next position in `order` (reset by finish_kernel)
+    int32_t ntile;
     const int32_t *row_state;
     const int64_t *slot_off;
     int32_t Ra, Rb, nnu, ncta;
@@ -64,13 +65,16 @@ __global__ void __launch_bounds__(kStreamThreads, 2) stream_kernel(const StreamP
     const int tid = threadIdx.x;
     const int nnu = P.nnu;
     const bool n16 = (nnu % 2 == 0) && ((reinterpret_cast<uintptr_t>(P.N) & 15) == 0);
-    if ((int)blockIdx.x >= P.ncta) return;
-    const TileCta cta = P.ctas[blockIdx.x];
+    __shared__ int sTileNo;
 
-    for (int it = cta.t0; it < cta.t1; ++it) {
-        const StreamTile th = P.tiles[it];
+    while (true) {
+        __syncthreads();  // previous tile: partial sums written, accumulators and sTileNo free
+        if (tid == 0) sTileNo = atomicAdd(P.counter, 1);  // order of execution only: every tile owns its slots
+        __syncthreads();
+        const int tno = sTileNo;
+        if (tno >= P.ntile) break;
+        const StreamTile th = P.tiles[P.order[tno]];
         const bool dg = (th.flags & 4) != 0;
-        __syncthreads();  // previous tile: partial sums written, accumulators free
         if (th.flags & 1)
             for (int r = tid; r < th.a_rows; r += kStreamThreads) {
                 sIa[r] = P.f[P.row_state[th.a_row0 + r]];
@@ -126,7 +130,7 @@ __global__ void __launch_bounds__(kStreamThreads, 2) stream_kernel(const StreamP
             if (ci + 1 < th.nc) chn = P.chunks[th.c0 + ci + 1];
             // row tasks of this chunk (<= 256 k rows, <= 2048 k' rows): headers to registers before they are needed
             // k rows: two lanes per row from the low warps; k' rows: one thread per row from the high warps downwards
-            int ta_row = 0, ta_s0 = 0, ta_s1 = 0, tb_row[kBT], tb_s0[kBT], tb_s1[kBT];
+            int ta_row = 0, ta_s0 = 0, ta_s1 = 0, tb_row = 0, tb_s0 = 0, tb_s1 = 0;
             const int arow = tid >> 1, apart = tid & 1;
             if (arow < ch.nar) {
                 ta_row = __ldg(P.arow_id + ch.ar0 + arow);
@@ -135,15 +139,11 @@ __global__ void __launch_bounds__(kStreamThreads, 2) stream_kernel(const StreamP
                 ta_s0 = min(s0 + apart * q, s1);
                 ta_s1 = min(ta_s0 + q, s1);
             }
-#pragma unroll
-            for (int u = 0; u < kBT; ++u) {
-                const int id = (kStreamThreads - 1 - tid) + u * kStreamThreads;
-                tb_row[u] = tb_s0[u] = tb_s1[u] = 0;
-                if (id < ch.nbr) {
-                    tb_row[u] = __ldg(P.brow_id + ch.br0 + id);
-                    tb_s0[u] = __ldg(P.brow_start + ch.br0 + id);
-                    tb_s1[u] = __ldg(P.brow_start + ch.br0 + id + 1);
-                }
+            const int brow = kStreamThreads - 1 - tid;  // first k' row task of this thread; further ones (rare) below
+            if (brow < ch.nbr) {
+                tb_row = __ldg(P.brow_id + ch.br0 + brow);
+                tb_s0 = __ldg(P.brow_start + ch.br0 + brow);
+                tb_s1 = __ldg(P.brow_start + ch.br0 + brow + 1);
             }
             cp_async_wait<0>();
             __syncthreads();  // staged f / N / perm visible; phase 2 of the previous chunk is done with sT
@@ -170,18 +170,21 @@ __global__ void __launch_bounds__(kStreamThreads, 2) stream_kernel(const StreamP
                 if (apart == 0 && arow < ch.nar) sAa[ta_row] -= sum;
             }
             if (dg) __syncthreads();  // the same row can be a k row and a k' row of a diagonal tile
-#pragma unroll
-            for (int u = 0; u < kBT; ++u)
-                if ((kStreamThreads - 1 - tid) + u * kStreamThreads < ch.nbr) {
-                    double s0 = 0.0, s1 = 0.0;
-                    int i = tb_s0[u];
-                    for (; i + 1 < tb_s1[u]; i += 2) {
-                        s0 += sT[cP[i]];
-                        s1 += sT[cP[i + 1]];
-                    }
-                    if (i < tb_s1[u]) s0 += sT[cP[i]];
-                    accB[tb_row[u]] += s0 + s1;
+            for (int id = brow; id < ch.nbr; id += kStreamThreads) {
+                if (id != brow) {  // more than kStreamThreads k' rows in the chunk: headers were not prefetched
+                    tb_row = __ldg(P.brow_id + ch.br0 + id);
+                    tb_s0 = __ldg(P.brow_start + ch.br0 + id);
+                    tb_s1 = __ldg(P.brow_start + ch.br0 + id + 1);
                 }
+                double s0 = 0.0, s1 = 0.0;
+                int i = tb_s0;
+                for (; i + 1 < tb_s1; i += 2) {
+                    s0 += sT[cP[i]];
+                    s1 += sT[cP[i + 1]];
+                }
+                if (i < tb_s1) s0 += sT[cP[i]];
+                accB[tb_row] += s0 + s1;
+            }
             ch = chn;
         }
         __syncthreads();

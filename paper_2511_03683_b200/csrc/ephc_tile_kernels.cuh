@@ -59,6 +59,7 @@ struct FinishParams {
     double *f0, *ynext, *ksum, *blk_sum;
     // transport
     const double *v, *tau;
+    int *reset;  // tile counter of the stream kernel, set back to 0 for the next evaluation (may be null)
 };
 
 template <int NB>
@@ -388,6 +389,7 @@ template <int FMODE>
 __global__ void __launch_bounds__(256) finish_kernel(const FinishParams P) {
     constexpr int C = (FMODE == kFIter) ? 3 : 1;
     const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a == 0 && P.reset != nullptr) *P.reset = 0;
     double sum[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) sum[c] = 0.0;
