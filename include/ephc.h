@@ -136,9 +136,13 @@ int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq,
  *                 both ends of its channels in shared memory in a fixed ticket order, per-tile partial sums
  *                 are added per state by a second kernel (PAPER.md:88-102 restructured; no atomics).
  *                 Available for nb <= 4, nnu <= 8, nq <= 2^24.
- *  -1 = automatic (default): ephc_collision / ephc_rt_step use the tile store when it is available,
- *                 ephc_transport_setup / ephc_transport_iter the gather store (the faster choice per call as
- *                 measured on B200).
+ *   2 = stream  : once-stored channels in the same tiles, one lane per ENTRY; the per-entry terms stay in shared
+ *                 memory and are summed per k row and per k' row of a chunk by one thread each (no atomics).
+ *                 Collision / rt only (transport calls then use the gather + row stores); any nb, nnu.
+ *  -1 = automatic (default): ephc_collision / ephc_rt_step use the gather store while it fits the L2 cache
+ *                 (<= 96 MB) and the stream store beyond that; ephc_transport_setup runs on the gather store and
+ *                 ephc_transport_iter on the row store built from it (the faster choice per call as measured on
+ *                 B200).
  * ephc_transport_setup must be called again after a change of variant.  ephc_get_variant returns the variant
  * ephc_collision will use, ephc_get_transport_variant the one the transport calls will use. */
 int ephc_set_variant(ephc_handle *h, int variant);

@@ -544,8 +544,13 @@ extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, i
 }
 
 // variant used by ephc_collision / ephc_rt_step, and by ephc_transport_setup / ephc_transport_iter
+// Automatic choice for collision / RK stages: the two-sided gather store while it stays resident in the 126 MB L2
+// (measured on B200: 5e5 channels 13 us vs 1170 us, 2.1e6 channels 34 us vs 87 us on the stream store), the once-stored
+// stream store beyond that (1.26e7 channels: 124 us vs 224 us).
 static inline int coll_variant(const ephc_handle *h) {
-    return h->variant < 0 ? (h->stream_ok ? 2 : (h->tile_ok ? 1 : 0)) : h->variant;
+    if (h->variant >= 0) return h->variant;
+    if (h->g_entries * 12 <= (int64_t)96 << 20) return 0;
+    return h->stream_ok ? 2 : (h->tile_ok ? 1 : 0);
 }
 static inline int tr_variant(const ephc_handle *h) { return (h->variant < 0 || h->variant == 2) ? 0 : h->variant; }
 

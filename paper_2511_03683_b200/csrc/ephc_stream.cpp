@@ -50,6 +50,11 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
             Rf = std::min(Rf, std::max(1, (int)want));
         }
         Rf = std::max(1, Rf);
+        if (!std::getenv("EPHC_STREAM_ROWS")) {
+            // small problems: enough strips for a few tiles per CTA (about nstrip^2 / 2 x fine blocks per strip tiles)
+            const int ra_small = (int)((double)std::max(t.nrows, 1) / std::sqrt(2.0 * ncta * 3.0)) * 8;
+            Ra = std::min(Ra, std::max(Rf, ra_small));
+        }
         Ra = std::max(Rf, std::min(2048, Ra) / Rf * Rf);
         Rb = std::max(Rf, std::min(kStreamRbMax, Rb) / Rf * Rf);
         t.rf = Rf;
