@@ -130,6 +130,14 @@ int ephc_export_gather(const ephc_handle *h, int32_t *dest, int32_t *partner, in
 int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
                       int32_t *diag, double *w);
 
+/* Decoded image of the stream store (variant 2), same conditions as ephc_export_gather.  Arrays of length
+ * ephc_stream_entries(h) (= nw: the q = 0, n = m terms are not stored) in store order: state a = (n,k), state b =
+ * (m,k'), canonical iq, mode, kind (0: w_abs, 1: w_em), weight.  Walks tiles (in hand-out order) -> chunks and checks
+ * the chunk limits, the k-row and k'-row tasks, the chunk-local permutations, slots and coverage on the way. */
+int ephc_export_stream(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
+                       double *w);
+int64_t ephc_stream_entries(const ephc_handle *h);
+
 /* Choice of algorithm:
  *   0 = gather  : destination-sorted two-sided store, one kernel, every ordered term read once
  *   1 = tiles   : once-stored channels grouped into (k-strip, k'-range) tiles; one lane per (k,k') pair updates

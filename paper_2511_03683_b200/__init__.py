@@ -69,6 +69,8 @@ def _load():
         "ephc_export_diag": (i32, [vp] * 6),
         "ephc_export_gather": (i32, [vp] * 8),
         "ephc_export_tiles": (i32, [vp] * 8),
+        "ephc_export_stream": (i32, [vp] * 7),
+        "ephc_stream_entries": (i64, [vp]),
         "ephc_set_variant": (i32, [vp, i32]),
         "ephc_get_variant": (i32, [vp]),
         "ephc_get_transport_variant": (i32, [vp]),
@@ -197,6 +199,15 @@ class Handle:
         w = np.zeros(n, np.float64)
         _check(_load().ephc_export_tiles(self._h, *[a.ctypes.data for a in ints], w.ctypes.data))
         keys = ("a", "b", "iq", "nu", "kind", "diag", "w")
+        return {k: a[:ne] for k, a in zip(keys, ints + [w])}
+
+    def export_stream(self) -> dict:
+        ne = int(_load().ephc_stream_entries(self._h))
+        n = max(ne, 1)
+        ints = [np.zeros(n, np.int32) for _ in range(5)]
+        w = np.zeros(n, np.float64)
+        _check(_load().ephc_export_stream(self._h, *[a.ctypes.data for a in ints], w.ctypes.data))
+        keys = ("a", "b", "iq", "nu", "kind", "w")
         return {k: a[:ne] for k, a in zip(keys, ints + [w])}
 
     def set_variant(self, variant: int):

@@ -78,6 +78,7 @@ struct ephc_handle {
     // stream store (variant 2)
     bool stream_ok = false;
     std::string stream_why;
+    StreamHost shost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_stream)
     int32_t s_ncta = 0, s_Ra = 0, s_Rb = 0, s_ntile = 0;
     int64_t s_entries = 0, s_part_rows = 0, bytes_stream = 0;
     double *ds_w = nullptr, *ds_part = nullptr;
@@ -221,6 +222,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
                                     (sh.arow_id.size() + sh.brow_id.size()) * 4 + sh.iq.size() * 4 +
                                     sh.chunks.size() * sizeof(StreamChunk) + sh.tiles.size() * sizeof(StreamTile));
         sh.perm.resize(sh.perm.size() + 8, 0);  // the staging copies read whole 8-byte pieces
+        if (h->host_only) h->shost = sh;
     }
     // row store for transport_iter (one CTA of 1024 threads per SM, one strip each)
     RowHost rh;
@@ -553,6 +555,94 @@ static inline int coll_variant(const ephc_handle *h) {
     return h->stream_ok ? 2 : (h->tile_ok ? 1 : 0);
 }
 static inline int tr_variant(const ephc_handle *h) { return (h->variant < 0 || h->variant == 2) ? 0 : h->variant; }
+
+extern "C" int ephc_export_stream(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu,
+                                  int32_t *kind, double *w) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (!h->host_only) return fail(EPHC_ESTATE, "ephc_export_stream needs a handle built with EPHC_HOST_ONLY");
+    if (!h->stream_ok) return fail(EPHC_ESTATE, "stream store not available for this problem: " + h->stream_why);
+    const StreamHost &t = h->shost;
+    const int nnu = h->d.nnu;
+    const int64_t nent = (int64_t)t.w.size();
+    std::vector<uint8_t> seen((size_t)nent, 0), tile_seen(t.tiles.size(), 0);
+    if (t.order.size() != t.tiles.size()) return fail(EPHC_ESTATE, "internal: tile order does not list every tile");
+    std::vector<uint8_t> used;
+    for (int32_t it : t.order) {
+        if (it < 0 || it >= (int32_t)t.tiles.size() || tile_seen[it]++) return fail(EPHC_ESTATE, "internal: bad tile order");
+        const StreamTile &th = t.tiles[it];
+        const bool dg = (th.flags & 4) != 0;
+        if ((th.flags & 3) != 3 || th.a_slot < 0 || (dg != (th.b_slot < 0)) || th.a_rows > t.Ra || th.b_rows > t.Rb ||
+            th.b_rows > kStreamRbMax || (dg && (th.b_row0 != th.a_row0 || th.b_rows != th.a_rows)) ||
+            (!dg && th.b_row0 < th.a_row0 + th.a_rows) || t.slot_row0[th.a_slot] != th.a_row0 ||
+            t.slot_rows[th.a_slot] != th.a_rows ||
+            (!dg && (t.slot_row0[th.b_slot] != th.b_row0 || t.slot_rows[th.b_slot] != th.b_rows)))
+            return fail(EPHC_ESTATE, "internal: bad stream tile");
+        for (int32_t ci = th.c0; ci < th.c0 + th.nc; ++ci) {
+            const StreamChunk &ch = t.chunks[ci];
+            if (ch.ne < 1 || ch.ne > kStreamChunk || ch.nq * nnu > kStreamNSlots || ch.nar < 1 || ch.nar > 256 ||
+                ch.nbr < 1 || ch.e0 < 0 || ch.e0 + ch.ne > nent)
+                return fail(EPHC_ESTATE, "internal: chunk outside its limits");
+            // k-row tasks: contiguous runs that cover the chunk; every entry of a run has the run's row
+            if (t.arow_start[ch.ar0] != 0 || t.arow_start[ch.ar0 + ch.nar] != ch.ne)
+                return fail(EPHC_ESTATE, "internal: k-row tasks do not cover the chunk");
+            for (int32_t r = 0; r < ch.nar; ++r) {
+                const int s0 = t.arow_start[ch.ar0 + r], s1 = t.arow_start[ch.ar0 + r + 1];
+                if (s0 >= s1 || (r > 0 && t.arow_id[ch.ar0 + r] <= t.arow_id[ch.ar0 + r - 1]))
+                    return fail(EPHC_ESTATE, "internal: k-row tasks out of order");
+                for (int i = s0; i < s1; ++i)
+                    if ((int32_t)(t.code[ch.e0 + i] & 255u) + ch.a0 != (int32_t)t.arow_id[ch.ar0 + r])
+                        return fail(EPHC_ESTATE, "internal: entry outside its k-row task");
+            }
+            // k'-row tasks through the permutation
+            const uint16_t *pm = t.perm.data() + 4 * (int64_t)ch.pad0;
+            used.assign((size_t)ch.ne, 0);
+            if (t.brow_start[ch.br0] != 0 || t.brow_start[ch.br0 + ch.nbr] != ch.ne)
+                return fail(EPHC_ESTATE, "internal: k'-row tasks do not cover the chunk");
+            for (int32_t r = 0; r < ch.nbr; ++r) {
+                const int s0 = t.brow_start[ch.br0 + r], s1 = t.brow_start[ch.br0 + r + 1];
+                if (s0 >= s1 || (r > 0 && t.brow_id[ch.br0 + r] <= t.brow_id[ch.br0 + r - 1]))
+                    return fail(EPHC_ESTATE, "internal: k'-row tasks out of order");
+                for (int i = s0; i < s1; ++i) {
+                    const int e = pm[i];
+                    if (e >= ch.ne || used[e]++) return fail(EPHC_ESTATE, "internal: not a permutation");
+                    if ((int32_t)((t.code[ch.e0 + e] >> 8) & 2047u) != (int32_t)t.brow_id[ch.br0 + r])
+                        return fail(EPHC_ESTATE, "internal: entry outside its k'-row task");
+                }
+            }
+            for (int32_t i = 0; i < ch.ne; ++i) {
+                const int64_t o = ch.e0 + i;
+                if (seen[o]++) return fail(EPHC_ESTATE, "internal: entry in two chunks");
+                const uint32_t c = t.code[o];
+                const int32_t ar = th.a_row0 + ch.a0 + (int32_t)(c & 255u), br = th.b_row0 + (int32_t)((c >> 8) & 2047u);
+                const int32_t slot = (int32_t)((c >> 19) & 4095u);
+                if (ar >= th.a_row0 + th.a_rows || br >= th.b_row0 + th.b_rows || slot / nnu >= ch.nq)
+                    return fail(EPHC_ESTATE, "internal: entry code out of range");
+                if (a) a[o] = t.row_state[ar];
+                if (b) b[o] = t.row_state[br];
+                if (iq) iq[o] = (int32_t)t.iq[ch.q0 + slot / nnu];
+                if (nu) nu[o] = slot % nnu;
+                if (kind) kind[o] = (int32_t)(c >> 31);
+                if (w) w[o] = t.w[o];
+            }
+        }
+    }
+    for (uint8_t sflag : seen)
+        if (!sflag) return fail(EPHC_ESTATE, "internal: entry not covered by any chunk");
+    {
+        std::vector<uint8_t> cover((size_t)t.part_rows, 0);
+        for (int32_t bl = 0; bl < t.nblk; ++bl)
+            for (int32_t i = t.blk_ent_ptr[bl]; i < t.blk_ent_ptr[bl + 1]; ++i)
+                for (int32_t r = 0; r < t.blk_row0[bl + 1] - t.blk_row0[bl]; ++r) {
+                    const int64_t o = t.blk_ent_off[i] + r;
+                    if (o < 0 || o >= t.part_rows || cover[o]++) return fail(EPHC_ESTATE, "internal: slot row listed twice");
+                }
+        for (uint8_t cv : cover)
+            if (!cv) return fail(EPHC_ESTATE, "internal: slot row not listed for the finish kernel");
+    }
+    return EPHC_OK;
+}
+
+extern "C" int64_t ephc_stream_entries(const ephc_handle *h) { return h ? h->s_entries : 0; }
 
 extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");

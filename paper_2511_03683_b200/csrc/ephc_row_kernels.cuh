@@ -15,7 +15,10 @@
 
 namespace ephc {
 
-constexpr int kRowThreads = 1024;  // one CTA per SM: the staging traffic is (number of strips) x |F|
+#ifndef EPHC_ROW_THREADS
+#define EPHC_ROW_THREADS 1024
+#endif
+constexpr int kRowThreads = EPHC_ROW_THREADS;  // 1024: one CTA per SM (the staging traffic is (number of strips) x |F|)
 constexpr int kRowGroup = 8;  // lanes per destination row
 #ifndef EPHC_ROW_BATCH
 #define EPHC_ROW_BATCH 4
@@ -65,7 +68,7 @@ __global__ void __launch_bounds__(256) row_permute_kernel(const double *gW, cons
     if (i < n) W[i] = __ldg(gW + __ldcs(perm + i));
 }
 
-__global__ void __launch_bounds__(kRowThreads, 1) row_iter_kernel(const RowParams P) {
+__global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kernel(const RowParams P) {
     extern __shared__ double smem[];
     double *sF = smem;                       // staged partner rows [Rb][3]
     double *sAcc = smem + (P.Rb * 3 + 2);    // [Ra][3]
