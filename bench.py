@@ -311,10 +311,11 @@ def main():
     roof(f"rk4 stage ({kn['r']})", ms_rt / 4, q["alg_bytes_collision"] + 32 * ns, ms_rt / ms_step)
     dominant = max(kern, key=lambda k: kern[k]["share_of_step"])
     roofline = dict(kern[dominant], kernel=dominant, peak_source=peak_src)
-    traffic_path = os.path.join(ROOT, "profiles", "traffic.json")       # dram bytes per launch from the ncu capture
+    traffic_path = os.path.join(ROOT, "profiles", "traffic.csv")        # dram bytes per launch from the ncu captures
     if os.path.exists(traffic_path):
-        with open(traffic_path) as fh:
-            tr = json.load(fh)
+        import csv
+        with open(traffic_path, newline="") as fh:
+            tr = {row["call"]: int(row["dram_bytes_per_launch"]) for row in csv.DictReader(fh)}
         for k in kern:
             kern[k]["traffic"] = tr.get(k)
         roofline["traffic"] = tr.get(dominant)
