@@ -138,6 +138,15 @@ int ephc_export_stream(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq
                        double *w);
 int64_t ephc_stream_entries(const ephc_handle *h);
 
+/* Decoded image of the resident-tile store (variant 3), same conditions as ephc_export_gather.  Arrays of length
+ * ephc_res_entries(h) (= nw) in store order (runs in hand-out order -> tiles -> entry positions): state a = (n,k),
+ * state b = (m,k'), canonical iq, mode, kind (0: w_abs, stored as the directed entry b -> a; 1: w_em, stored as
+ * a -> b), weight.  Walks the tile images exactly as the kernel does (column tables, pieces, gather lists of both
+ * rounds) and checks that every term T reaches both of its rows exactly once. */
+int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
+                    double *w);
+int64_t ephc_res_entries(const ephc_handle *h);
+
 /* Choice of algorithm:
  *   0 = gather  : destination-sorted two-sided store, one kernel, every ordered term read once
  *   1 = tiles   : once-stored channels grouped into (k-strip, k'-range) tiles; one lane per (k,k') pair updates
@@ -147,8 +156,12 @@ int64_t ephc_stream_entries(const ephc_handle *h);
  *   2 = stream  : once-stored channels in the same tiles, one lane per ENTRY; the per-entry terms stay in shared
  *                 memory and are summed per k row and per k' row of a chunk by one thread each (no atomics).
  *                 Collision / rt only (transport calls then use the gather + row stores); any nb, nnu.
+ *   3 = resident tiles: once-stored DIRECTED entries (an absorption weight is the reversed emission entry, so no
+ *                 per-entry kind), tiles whose whole image is bulk-copied (TMA) into shared memory and processed in
+ *                 place: one lane per out row piece writes the terms over the weights, one lane per row gathers them.
+ *                 Collision / rt only (transport calls then use the gather + row stores); any nb, nnu.
  *  -1 = automatic (default): ephc_collision / ephc_rt_step use the gather store while it fits the L2 cache
- *                 (<= 96 MB) and the stream store beyond that; ephc_transport_setup runs on the gather store and
+ *                 (<= 96 MB) and the resident-tile store beyond that; ephc_transport_setup runs on the gather store and
  *                 ephc_transport_iter on the row store built from it (the faster choice per call as measured on
  *                 B200).
  * ephc_transport_setup must be called again after a change of variant.  ephc_get_variant returns the variant

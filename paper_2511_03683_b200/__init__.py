@@ -71,6 +71,8 @@ def _load():
         "ephc_export_tiles": (i32, [vp] * 8),
         "ephc_export_stream": (i32, [vp] * 7),
         "ephc_stream_entries": (i64, [vp]),
+        "ephc_export_res": (i32, [vp] * 7),
+        "ephc_res_entries": (i64, [vp]),
         "ephc_set_variant": (i32, [vp, i32]),
         "ephc_get_variant": (i32, [vp]),
         "ephc_get_transport_variant": (i32, [vp]),
@@ -210,11 +212,20 @@ class Handle:
         keys = ("a", "b", "iq", "nu", "kind", "w")
         return {k: a[:ne] for k, a in zip(keys, ints + [w])}
 
+    def export_res(self) -> dict:
+        ne = int(_load().ephc_res_entries(self._h))
+        n = max(ne, 1)
+        ints = [np.zeros(n, np.int32) for _ in range(5)]
+        w = np.zeros(n, np.float64)
+        _check(_load().ephc_export_res(self._h, *[a.ctypes.data for a in ints], w.ctypes.data))
+        keys = ("a", "b", "iq", "nu", "kind", "w")
+        return {k: a[:ne] for k, a in zip(keys, ints + [w])}
+
     def set_variant(self, variant: int):
         _check(_load().ephc_set_variant(self._h, int(variant)))
 
     def get_variant(self) -> int:
-        """Variant ephc_collision / ephc_rt_step will use (0 gather, 1 tiles)."""
+        """Variant ephc_collision / ephc_rt_step will use (0 gather, 1 tiles, 2 stream, 3 resident tiles)."""
         v = int(_load().ephc_get_variant(self._h))
         _check(min(v, 0))
         return v

@@ -16,6 +16,7 @@
 #include "ephc_tile_kernels.cuh"
 #include "ephc_row_kernels.cuh"
 #include "ephc_stream_kernels.cuh"
+#include "ephc_res_kernels.cuh"
 
 using namespace ephc;
 
@@ -91,6 +92,22 @@ struct ephc_handle {
     int32_t *ds_row_state = nullptr, *ds_state_row = nullptr, *ds_state_blk = nullptr, *ds_blk_row0 = nullptr,
             *ds_blk_ent_ptr = nullptr;
     int64_t *ds_slot_off = nullptr, *ds_blk_ent_off = nullptr;
+    // resident-tile store (variant 3)
+    bool res_ok = false;
+    std::string res_why;
+    ResHost rhost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_res)
+    int32_t x_nrun = 0, x_Rcap = 0, x_ntile = 0, x_ncta = 0;
+    int64_t x_entries = 0, x_part_rows = 0, x_smem_tile = 0, bytes_res = 0;
+    unsigned char *dx_blob = nullptr;
+    uint32_t *dx_iqn = nullptr;
+    ResTile *dx_tiles = nullptr;
+    ResRun *dx_runs = nullptr;
+    int32_t *dx_order = nullptr;
+    int *dx_counter = nullptr;
+    double *dx_part = nullptr;
+    int32_t *dx_row_state = nullptr, *dx_state_row = nullptr, *dx_state_blk = nullptr, *dx_blk_row0 = nullptr,
+            *dx_blk_ent_ptr = nullptr;
+    int64_t *dx_slot_off = nullptr, *dx_blk_ent_off = nullptr;
     // row store (transport_iter of the gather path)
     bool rows_ok = false;
     int32_t r_nstrip = 0, r_Rb = 0, r_Ra = 0;
@@ -115,7 +132,9 @@ static void free_dev(ephc_handle *h) {
                     h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
                     h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_order, h->ds_counter, h->ds_row_state,
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
-                    h->ds_blk_ent_off};
+                    h->ds_blk_ent_off, h->dx_blob, h->dx_iqn, h->dx_tiles, h->dx_runs, h->dx_order, h->dx_counter, h->dx_part,
+                    h->dx_row_state, h->dx_state_row, h->dx_state_blk, h->dx_blk_row0, h->dx_blk_ent_ptr, h->dx_slot_off,
+                    h->dx_blk_ent_off};
     for (void *p : ptrs)
         if (p) cudaFree(p);
 }
@@ -224,6 +243,31 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         sh.perm.resize(sh.perm.size() + 8, 0);  // the staging copies read whole 8-byte pieces
         if (h->host_only) h->shost = sh;
     }
+    // resident-tile store (variant 3): two CTAs per SM, each with one tile image in shared memory
+    ResHost xh;
+    if (std::getenv("EPHC_NO_RES") == nullptr) {
+        int nshare = 2 * n_sm;
+        if (const char *e = std::getenv("EPHC_RES_CTAS")) nshare = std::max(1, std::atoi(e));
+        int64_t cap = kResSmemCap;
+        if (const char *e = std::getenv("EPHC_RES_SMEM")) cap = std::max(8192, std::atoi(e));
+        rc = build_res(p, h->d, h->can, nshare, cap, xh, err);
+        if (rc != EPHC_OK) {
+            delete h;
+            return fail(rc, err);
+        }
+        h->res_ok = xh.supported && res_smem_bytes(xh.Rcap, xh.smem_tile) <= 225 * 1024;
+        h->res_why = xh.why;
+        h->x_ncta = nshare;
+        h->x_nrun = (int32_t)xh.runs.size();
+        h->x_ntile = (int32_t)xh.tiles.size();
+        h->x_Rcap = xh.Rcap;
+        h->x_entries = xh.nent;
+        h->x_part_rows = xh.part_rows;
+        h->x_smem_tile = xh.smem_tile;
+        h->bytes_res = (int64_t)(xh.blob.size() + xh.iqn.size() * 4 + xh.tiles.size() * sizeof(ResTile) +
+                                 xh.runs.size() * (sizeof(ResRun) + 4));
+        if (h->host_only) h->rhost = xh;
+    }
     // row store for transport_iter (one CTA of 1024 threads per SM, one strip each)
     RowHost rh;
     const bool want_rows = std::getenv("EPHC_NO_ROWS") == nullptr;
@@ -292,6 +336,27 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             if (rc == EPHC_OK) rc = upload(&h->ds_slot_off, sh.slot_off, &bs);
             if (rc == EPHC_OK && cudaMalloc((void **)&h->ds_part, (size_t)std::max<int64_t>(1, sh.part_rows) * 8) != cudaSuccess)
                 rc = fail(EPHC_ENOMEM, "cudaMalloc (stream partial sums) failed");
+        }
+        if (rc == EPHC_OK && h->res_ok) {
+            int64_t bx = 0;
+            rc = upload(&h->dx_blob, xh.blob, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_iqn, xh.iqn, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_tiles, xh.tiles, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_runs, xh.runs, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_order, xh.order, &bx);
+            if (rc == EPHC_OK && (cudaMalloc((void **)&h->dx_counter, 64) != cudaSuccess ||
+                                  cudaMemset(h->dx_counter, 0, 64) != cudaSuccess))
+                rc = fail(EPHC_ENOMEM, "cudaMalloc (run counter) failed");
+            if (rc == EPHC_OK) rc = upload(&h->dx_row_state, xh.row_state, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_state_row, xh.state_row, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_state_blk, xh.state_blk, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_blk_row0, xh.blk_row0, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_blk_ent_ptr, xh.blk_ent_ptr, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_blk_ent_off, xh.blk_ent_off, &bx);
+            if (rc == EPHC_OK) rc = upload(&h->dx_slot_off, xh.slot_off, &bx);
+            if (rc == EPHC_OK && cudaMalloc((void **)&h->dx_part, (size_t)std::max<int64_t>(1, xh.part_rows) * 8) != cudaSuccess)
+                rc = fail(EPHC_ENOMEM, "cudaMalloc (resident-tile partial sums) failed");
+            xh = ResHost();
         }
         if (rc == EPHC_OK && h->rows_ok) {
             int64_t br = 0;
@@ -367,7 +432,7 @@ extern "C" int ephc_query(const ephc_handle *h, ephc_counts *o) {
     o->store_bytes_gather = h->bytes_gather + h->bytes_rows;
     o->scatter_entries = h->t_entries;
     o->scatter_pairs = h->t_pieces;
-    o->store_bytes_scatter = h->bytes_tile + h->bytes_stream;
+    o->store_bytes_scatter = h->bytes_tile + h->bytes_stream + h->bytes_res;
     o->store_bytes_transport = h->bytes_transport;
     // B_alg: every item the method must move once per evaluation.
     //   8 N_w weights + 4 N_ch channel index + 12 N_pair (ik, ikq, iq) + 16 N_s (read f, write I) + 8 nnu N_q,active
@@ -552,9 +617,9 @@ extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, i
 static inline int coll_variant(const ephc_handle *h) {
     if (h->variant >= 0) return h->variant;
     if (h->g_entries * 12 <= (int64_t)96 << 20) return 0;
-    return h->stream_ok ? 2 : (h->tile_ok ? 1 : 0);
+    return h->res_ok ? 3 : (h->stream_ok ? 2 : (h->tile_ok ? 1 : 0));
 }
-static inline int tr_variant(const ephc_handle *h) { return (h->variant < 0 || h->variant == 2) ? 0 : h->variant; }
+static inline int tr_variant(const ephc_handle *h) { return (h->variant < 0 || h->variant >= 2) ? 0 : h->variant; }
 
 extern "C" int ephc_export_stream(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu,
                                   int32_t *kind, double *w) {
@@ -644,10 +709,139 @@ extern "C" int ephc_export_stream(const ephc_handle *h, int32_t *a, int32_t *b, 
 
 extern "C" int64_t ephc_stream_entries(const ephc_handle *h) { return h ? h->s_entries : 0; }
 
+extern "C" int64_t ephc_res_entries(const ephc_handle *h) { return (h && h->res_ok) ? h->x_entries : 0; }
+
+extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
+                               double *w) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (!h->host_only) return fail(EPHC_ESTATE, "ephc_export_res needs a handle built with EPHC_HOST_ONLY");
+    if (!h->res_ok) return fail(EPHC_ESTATE, "resident-tile store not available for this problem: " + h->res_why);
+    const ResHost &t = h->rhost;
+    const int nnu = h->d.nnu;
+    std::vector<uint8_t> run_seen(t.runs.size(), 0), tile_seen(t.tiles.size(), 0);
+    if (t.order.size() != t.runs.size()) return fail(EPHC_ESTATE, "internal: run order does not list every run");
+    int64_t o = 0;
+    std::vector<int32_t> owner, used;
+    for (int32_t ir : t.order) {
+        if (ir < 0 || ir >= (int32_t)t.runs.size() || run_seen[ir]++) return fail(EPHC_ESTATE, "internal: bad run order");
+        const ResRun &run = t.runs[ir];
+        if (run.nt < 1 || run.a_rows < 1 || run.a_row0 % t.Ra != 0 || run.a_slot < 0 ||
+            t.slot_row0[run.a_slot] != run.a_row0 || t.slot_rows[run.a_slot] != run.a_rows)
+            return fail(EPHC_ESTATE, "internal: bad run");
+        for (int32_t it = run.t0; it < run.t0 + run.nt; ++it) {
+            if (it < 0 || it >= (int32_t)t.tiles.size() || tile_seen[it]++) return fail(EPHC_ESTATE, "internal: tile in two runs");
+            const ResTile &D = t.tiles[it];
+            const ResLayout L = res_layout(D.ne, D.npiece, D.ntask1, D.ntask2, D.nc1 + D.nc2 + D.nc3, D.ngl1 + D.ngl2);
+            const int32_t R = run.a_rows + D.b_rows;
+            const int64_t smem = (int64_t)L.bytes + 8 * (int64_t)(D.npiece + D.npart) + 16 + 8 * (int64_t)D.nq * nnu;
+            if (D.ne < 1 || L.bytes != D.blob_bytes || D.blob_off % 128 != 0 || D.blob_off + D.blob_bytes > (int64_t)t.blob.size() ||
+                smem > t.smem_tile || R > t.Rcap || R > kResRowMax || D.nq * nnu > kResSlotMax ||
+                D.ne + D.npiece + D.npart > kResXMax || D.ngl1 != D.ne + D.npiece || D.ngl2 != D.npart ||
+                (D.b_rows > 0) != (D.b_slot >= 0) || (D.b_rows > 0 && D.b_row0 < run.a_row0 + run.a_rows) ||
+                (D.b_slot >= 0 && (t.slot_row0[D.b_slot] != D.b_row0 || t.slot_rows[D.b_slot] != D.b_rows)) ||
+                D.q0 < 0 || D.q0 + D.nq > (int64_t)t.iqn.size())
+                return fail(EPHC_ESTATE, "internal: bad resident tile");
+            const unsigned char *B = t.blob.data() + D.blob_off;
+            const uint32_t *code = reinterpret_cast<const uint32_t *>(B + L.code);
+            const uint16_t *perm = reinterpret_cast<const uint16_t *>(B + L.perm);
+            const uint16_t *prow = reinterpret_cast<const uint16_t *>(B + L.prow);
+            const uint16_t *d1 = reinterpret_cast<const uint16_t *>(B + L.d1);
+            const uint16_t *d2 = reinterpret_cast<const uint16_t *>(B + L.d2);
+            const uint32_t *cols = reinterpret_cast<const uint32_t *>(B + L.cols);
+            const double *wv = reinterpret_cast<const double *>(B + L.w);
+            auto row_of = [&](int32_t loc) { return loc < run.a_rows ? run.a_row0 + loc : D.b_row0 + (loc - run.a_rows); };
+            // phase 1 exactly as the kernel walks it: owner[x] = local row that must receive X[x]
+            const int32_t nx = D.ne + D.npiece + D.npart;
+            owner.assign((size_t)nx, -1);
+            used.assign((size_t)nx, 0);
+            for (int32_t p = 0; p < D.npiece; ++p) {
+                if (prow[p] >= R) return fail(EPHC_ESTATE, "internal: piece row out of range");
+                owner[D.ne + p] = prow[p];
+                int32_t len = 0;
+                for (int32_t j = 0; j < D.nc1; ++j) {
+                    const int32_t cnt = (int32_t)(cols[j] & 0xffffu), base = (int32_t)(cols[j] >> 16);
+                    if (p >= cnt) break;
+                    ++len;
+                    const int32_t e = base + p;
+                    if (e < 0 || e >= D.ne || owner[e] >= 0) return fail(EPHC_ESTATE, "internal: entry visited twice");
+                    const uint32_t cd = code[e];
+                    const int32_t in_loc = (int32_t)((cd & 0xffffu) >> 3), slot = (int32_t)(cd >> 19);
+                    if ((cd & 7u) || in_loc >= R || slot / nnu >= D.nq) return fail(EPHC_ESTATE, "internal: entry code out of range");
+                    owner[e] = in_loc;
+                    const int32_t ro = row_of(prow[p]), ri = row_of(in_loc);
+                    if (ro == ri) return fail(EPHC_ESTATE, "internal: entry with equal ends");
+                    const int64_t x = o + e;
+                    if (a) a[x] = t.row_state[std::min(ro, ri)];
+                    if (b) b[x] = t.row_state[std::max(ro, ri)];
+                    if (iq) iq[x] = (int32_t)(t.iqn[D.q0 + slot / nnu] / (uint32_t)nnu);
+                    if (nu) nu[x] = slot % nnu;
+                    if (kind) kind[x] = ro < ri ? 1 : 0;  // out = a: emission weight; out = b: absorption weight
+                    if (w) w[x] = wv[e];
+                }
+                if (len < 1) return fail(EPHC_ESTATE, "internal: empty piece");
+            }
+            for (int32_t e = 0; e < D.ne; ++e)
+                if (owner[e] < 0) return fail(EPHC_ESTATE, "internal: entry not covered by any piece");
+            // phase 2: every X value is added exactly once, to its owner row (directly or through one partial sum)
+            std::vector<uint8_t> row_final((size_t)R, 0);
+            for (int32_t tk = 0; tk < D.ntask1; ++tk) {
+                const int32_t dst = d1[tk];
+                const bool partial = (dst & 0x8000) != 0;
+                int32_t row = partial ? -1 : dst, len = 0;
+                if (partial && (dst & 0x7fff) >= D.npart) return fail(EPHC_ESTATE, "internal: partial index out of range");
+                if (!partial && (dst >= R || row_final[dst]++)) return fail(EPHC_ESTATE, "internal: two final tasks for a row");
+                for (int32_t j = 0; j < D.nc2; ++j) {
+                    const int32_t cnt = (int32_t)(cols[D.nc1 + j] & 0xffffu), base = (int32_t)(cols[D.nc1 + j] >> 16);
+                    if (tk >= cnt) break;
+                    ++len;
+                    const int32_t x = perm[base + tk];
+                    if (base + tk >= D.ngl1 || x >= D.ne + D.npiece || used[x]++) return fail(EPHC_ESTATE, "internal: gather list");
+                    if (row < 0) row = owner[x];
+                    if (owner[x] != row) return fail(EPHC_ESTATE, "internal: gather task mixes rows");
+                }
+                if (len < 1) return fail(EPHC_ESTATE, "internal: empty gather task");
+                if (partial) owner[D.ne + D.npiece + (dst & 0x7fff)] = row;
+            }
+            for (int32_t tk = 0; tk < D.ntask2; ++tk) {
+                const int32_t row = d2[tk];
+                if (row >= R || row_final[row]++) return fail(EPHC_ESTATE, "internal: two final tasks for a row");
+                for (int32_t j = 0; j < D.nc3; ++j) {
+                    const int32_t cnt = (int32_t)(cols[D.nc1 + D.nc2 + j] & 0xffffu), base = (int32_t)(cols[D.nc1 + D.nc2 + j] >> 16);
+                    if (tk >= cnt) break;
+                    const int32_t x = perm[D.ngl1 + base + tk];
+                    if (base + tk >= D.ngl2 || x < D.ne + D.npiece || x >= nx || used[x]++ || owner[x] != row)
+                        return fail(EPHC_ESTATE, "internal: round-2 gather list");
+                }
+            }
+            for (int32_t x = 0; x < nx; ++x)
+                if (used[x] != 1) return fail(EPHC_ESTATE, "internal: X value not gathered exactly once");
+            o += D.ne;
+        }
+    }
+    if (o != t.nent) return fail(EPHC_ESTATE, "internal: resident-tile store does not hold every weight");
+    for (uint8_t s : tile_seen)
+        if (!s) return fail(EPHC_ESTATE, "internal: tile not in any run");
+    {
+        std::vector<uint8_t> cover((size_t)t.part_rows, 0);
+        for (int32_t bl = 0; bl < t.nblk; ++bl)
+            for (int32_t i = t.blk_ent_ptr[bl]; i < t.blk_ent_ptr[bl + 1]; ++i)
+                for (int32_t r = 0; r < t.blk_row0[bl + 1] - t.blk_row0[bl]; ++r) {
+                    const int64_t q = t.blk_ent_off[i] + r;
+                    if (q < 0 || q >= t.part_rows || cover[q]++) return fail(EPHC_ESTATE, "internal: slot row listed twice");
+                }
+        for (uint8_t cv : cover)
+            if (!cv) return fail(EPHC_ESTATE, "internal: slot row not listed for the finish kernel");
+    }
+    return EPHC_OK;
+}
+
+
 extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
-    if (variant < -1 || variant > 2)
-        return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather), 1 (tiles) or 2 (stream)");
+    if (variant < -1 || variant > 3)
+        return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather), 1 (tiles), 2 (stream) or 3 (resident tiles)");
+    if (variant == 3 && !h->res_ok)
+        return fail(EPHC_ESTATE, "resident-tile store not available for this problem: " + h->res_why);
     if (variant == 2 && !h->stream_ok)
         return fail(EPHC_ESTATE, "stream store not available for this problem: " + h->stream_why);
     if (variant == 1 && !h->tile_ok)
@@ -677,6 +871,9 @@ static int need_device(ephc_handle *h) {
         if (h->stream_ok)
             CUDA_TRY(cudaFuncSetAttribute(stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)stream_smem_bytes(h->s_Ra, h->s_Rb)));
+        if (h->res_ok)
+            CUDA_TRY(cudaFuncSetAttribute(res_kernel<kResThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)res_smem_bytes(h->x_Rcap, h->x_smem_tile)));
         if (h->rows_ok)
             CUDA_TRY(cudaFuncSetAttribute(row_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)row_smem_bytes(h->r_Rb, h->r_Ra)));
@@ -835,6 +1032,49 @@ static int launch_stream(ephc_handle *h, const double *f, const double *N, cudaS
     return EPHC_OK;
 }
 
+static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStream_t s) {
+    if (h->x_nrun > 0) {
+        ResParams P;
+        std::memset(&P, 0, sizeof(P));
+        P.blob = h->dx_blob;
+        P.iqn = h->dx_iqn;
+        P.tiles = h->dx_tiles;
+        P.runs = h->dx_runs;
+        P.order = h->dx_order;
+        P.counter = h->dx_counter;
+        P.nrun = h->x_nrun;
+        P.row_state = h->dx_row_state;
+        P.slot_off = h->dx_slot_off;
+        P.Rcap = h->x_Rcap;
+        P.nnu = h->d.nnu;
+        P.gran16 = (h->d.nnu % 2 == 0) && ((reinterpret_cast<uintptr_t>(N) & 15) == 0);
+        P.gran = P.gran16 ? h->d.nnu / 2 : h->d.nnu;
+        P.gran_magic = P.gran > 1 ? (uint32_t)((0x100000000ULL + (uint64_t)P.gran - 1) / (uint64_t)P.gran) : 0u;
+        P.f = f;
+        P.N = N;
+        P.part = h->dx_part;
+        const int grid = std::min(h->x_nrun, h->x_ncta);
+        res_kernel<kResThreads><<<(unsigned)grid, kResThreads, res_smem_bytes(h->x_Rcap, h->x_smem_tile), s>>>(P);
+        h->launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
+static FinishParams finish_params_res(const ephc_handle *h) {
+    FinishParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.state_row = h->dx_state_row;
+    P.state_blk = h->dx_state_blk;
+    P.blk_row0 = h->dx_blk_row0;
+    P.blk_ent_ptr = h->dx_blk_ent_ptr;
+    P.blk_ent_off = h->dx_blk_ent_off;
+    P.part = h->dx_part;
+    P.ns = h->d.ns;
+    P.reset = h->dx_counter;
+    return P;
+}
+
 static FinishParams finish_params_stream(const ephc_handle *h) {
     FinishParams P;
     std::memset(&P, 0, sizeof(P));
@@ -854,6 +1094,12 @@ extern "C" int ephc_collision(ephc_handle *h, const double *f_dev, const double 
     int rc = need_device(h);
     if (rc) return rc;
     if (!f_dev || !N_dev || !I_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (coll_variant(h) == 3) {
+        if ((rc = launch_res(h, f_dev, N_dev, (cudaStream_t)stream))) return rc;
+        FinishParams Fp = finish_params_res(h);
+        Fp.out = I_dev;
+        return launch_finish<kFCollision>(h, Fp, (cudaStream_t)stream);
+    }
     if (coll_variant(h) == 2) {
         if ((rc = launch_stream(h, f_dev, N_dev, (cudaStream_t)stream))) return rc;
         FinishParams Fp = finish_params_stream(h);
@@ -1022,9 +1268,10 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
         for (int st = 0; st < 4; ++st) {
-            if (coll_variant(h) == 2) {
-                if ((rc = launch_stream(h, src[st], N_dev, s))) return rc;
-                FinishParams Fp = finish_params_stream(h);
+            if (coll_variant(h) >= 2) {
+                const bool res = coll_variant(h) == 3;
+                if ((rc = res ? launch_res(h, src[st], N_dev, s) : launch_stream(h, src[st], N_dev, s))) return rc;
+                FinishParams Fp = res ? finish_params_res(h) : finish_params_stream(h);
                 Fp.stage = st + 1;
                 Fp.dt = dt_fs;
                 Fp.f0 = f_dev;

@@ -220,4 +220,86 @@ struct StreamHost {
 };
 int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, StreamHost &t, std::string &err);
 
+// ---- resident-tile store (variant 3, collision / RK stages) -----------------------------------------------------
+// Every weight is stored ONCE as a directed "emission-form" entry (out -> in):
+//     T = w [ (f_out - f_in) N + f_out (1 - f_in) ],   I[out] -= T,   I[in] += T
+// A channel's emission weight gives out = (n,k), in = (m,k+q); its absorption weight gives the reversed entry,
+// because F_abs(a,b) = -F_em(b,a) (reading R-1), so no per-entry kind is needed.
+// Compact rows are cut into strips of Ra rows; a tile holds the entries between one strip (A rows) and a narrow range
+// of rows after it (B rows), or inside the strip (diagonal tile), sized so that its whole image fits in shared memory:
+// the image is one contiguous, 16-byte aligned blob that a CTA fetches with bulk copies (TMA) and then works on in
+// place.  Consecutive tiles of a strip form a run: one CTA keeps the strip's f values and accumulators in shared
+// memory for the whole run.
+//   phase 1 (paper step 2): one LANE per out-row PIECE (<= Lp entries of one out row); pieces sorted by descending
+//            length, entries stored column-major over ALL pieces of the tile (entry j of piece p at col[j].base + p,
+//            no padding); the lane keeps f_out and -sum(T) in registers and overwrites w by T in shared memory.
+//   phase 2 (paper step 3): one lane per gather task: it adds the X values (T of the row's in-entries, the negated
+//            sums of its out pieces) listed for one row; rows with more than Lg inputs go through partial tasks and
+//            a second round.  One owner per row, fixed order, no atomics.
+struct ResTile {           // 80 bytes (device directory)
+    int64_t blob_off;      // byte offset of the image in the blob array (multiple of 128)
+    int32_t blob_bytes;    // multiple of 16
+    int32_t ne;            // entries
+    int32_t npiece;        // out-row pieces
+    int32_t npart;         // round-1 partial tasks (rows with more than Lg inputs)
+    int32_t ntask1, ntask2;// gather tasks of round 1 (final + partial) and round 2 (final)
+    int32_t nc1, nc2, nc3; // columns (= longest list) of pieces, round-1 tasks, round-2 tasks
+    int32_t ngl1, ngl2;    // gather-list elements of round 1 / round 2
+    int32_t q0, nq;        // pairs: iqn[q0 .. q0+nq) = iq * nnu of the tile's pairs
+    int32_t b_row0, b_rows;// B rows (b_rows = 0 on a diagonal tile)
+    int32_t b_slot;        // partial-sum slot of the B rows (-1 on a diagonal tile)
+    int32_t pad[2];
+};
+struct ResRun {            // 32 bytes: consecutive tiles of one strip, handed to one CTA
+    int32_t t0, nt;
+    int32_t a_row0, a_rows, a_slot;
+    int32_t pad[3];
+};
+// byte offsets of the sections of a tile image (each 16-byte aligned); w comes last so that the X tail (piece sums,
+// partial sums) can follow it in shared memory
+struct ResLayout {
+    int32_t code, perm, prow, d1, d2, cols, w, bytes;
+};
+#ifdef __CUDACC__
+#define EPHC_HD __host__ __device__ __forceinline__
+#else
+#define EPHC_HD inline
+#endif
+EPHC_HD int32_t res_al16(int32_t x) { return (x + 15) & ~15; }
+EPHC_HD ResLayout res_layout(int32_t ne, int32_t npiece, int32_t ntask1, int32_t ntask2, int32_t ncols, int32_t ngl) {
+    ResLayout L;
+    L.code = 0;
+    L.perm = res_al16(4 * ne);
+    L.prow = L.perm + res_al16(2 * ngl);
+    L.d1 = L.prow + res_al16(2 * npiece);
+    L.d2 = L.d1 + res_al16(2 * ntask1);
+    L.cols = L.d2 + res_al16(2 * ntask2);
+    L.w = L.cols + res_al16(4 * ncols);
+    L.bytes = L.w + res_al16(8 * ne);
+    return L;
+}
+constexpr int kResSlotMax = 8192;     // N slots (pair * nnu + mode) per tile: slot * 8 fits the 16-bit field of the code
+constexpr int kResRowMax = 8192;      // rows (A + B) per tile: row * 8 fits the 16-bit field of the code
+constexpr int kResThreads = 384;      // threads per CTA of res_kernel (two CTAs per SM)
+constexpr int64_t kResSmemCap = 112 * 1024;  // dynamic shared memory per CTA: two CTAs fit in the 227 KB of an SM
+constexpr int kResXMax = 65535;       // X positions (entries + pieces + partials) per tile: uint16 gather lists
+struct ResHost {
+    int32_t Ra = 0, Rcap = 0, rf = 0, nblk = 0, nrows = 0, nnu = 0;
+    int64_t smem_tile = 0;            // largest (blob + X tail + N rows) of any tile, bytes
+    std::vector<int32_t> blk_row0, row_state, state_row, state_blk;
+    std::vector<unsigned char> blob;  // all tile images
+    std::vector<uint32_t> iqn;        // per (tile, pair): iq * nnu
+    std::vector<ResTile> tiles;
+    std::vector<ResRun> runs;
+    std::vector<int32_t> order;       // runs by descending work
+    std::vector<int64_t> slot_off;
+    std::vector<int32_t> slot_row0, slot_rows, blk_ent_ptr;
+    std::vector<int64_t> blk_ent_off;
+    int64_t part_rows = 0, nent = 0;
+    bool supported = false;
+    std::string why;
+};
+int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, int64_t smem_cap, ResHost &t,
+              std::string &err);
+
 }  // namespace ephc

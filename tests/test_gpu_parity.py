@@ -37,7 +37,7 @@ def _small_problems():
 IDS = ["tiny4", "window_cut_diag", "si12", "gaas24", "bigcell3", "tiny_full", "rt14"]
 
 
-VARIANTS = {0: "gather", 1: "tiles", 2: "stream"}
+VARIANTS = {0: "gather", 1: "tiles", 2: "stream", 3: "res"}
 
 
 @pytest.fixture(scope="module", params=[(i, v) for i in range(len(IDS)) for v in VARIANTS],
@@ -258,6 +258,36 @@ def test_stream_geometry_on_gpu(monkeypatch, rows, fine, ctas):
         assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
 
 
+@pytest.mark.parametrize("rows,fine,smem,lp,lg,ctas", [(16, 4, 12000, 3, 2, 3), (64, 8, 20000, 2, 3, 40), (2048, 128, None, None, None, 1),
+                                                       (32, 32, 9000, 16, 4, 7)])
+def test_res_geometry_on_gpu(monkeypatch, rows, fine, smem, lp, lg, ctas):
+    # resident-tile store: many tiny tiles, tiles split by the shared-memory budget, out rows cut into pieces, rows that
+    # need the second gather round, runs longer than one tile, one CTA for everything
+    monkeypatch.setenv("EPHC_RES_ROWS", str(rows))
+    monkeypatch.setenv("EPHC_RES_ROWS_B", str(rows))
+    monkeypatch.setenv("EPHC_RES_FINE", str(fine))
+    monkeypatch.setenv("EPHC_RES_CTAS", str(ctas))
+    for k, v in (("EPHC_RES_SMEM", smem), ("EPHC_RES_LP", lp), ("EPHC_RES_LG", lg)):
+        if v is not None:
+            monkeypatch.setenv(k, str(v))
+    for p in _small_problems()[:5]:
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p)
+        assert h.get_variant() == 0          # small problem: the automatic choice is the L2-resident gather store
+        h.set_variant(3)
+        I = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I)
+        assert _relerr(I, L.collision(p.f, p.N)) <= TOL
+        I2 = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I2)
+        assert np.array_equal(I, I2)
+        f = p.f.copy()
+        s = np.zeros(6)
+        h.rt_step_host(f, p.N, 1.0, 5, s)
+        fo, so = L.rt_step(p.f, p.N, 1.0, 5)
+        assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
+
+
 def test_stream_argument_is_honoured():
     p = make_problem("si", grid=(12, 12, 12), pair_prob=0.3, seed=3)
     h = ephc.build_channels(p)
@@ -278,7 +308,7 @@ def test_full_size_bench_workload_matches_oracle():
     p = make_problem("si")
     L = oracle.OracleList(p)
     h = ephc.build_channels(p)
-    assert h.query()["nch"] == L.nch > 1.0e7 and h.get_variant() == 2 and h.get_transport_variant() == 0
+    assert h.query()["nch"] == L.nch > 1.0e7 and h.get_variant() == 3 and h.get_transport_variant() == 0
     f, N = dev(p.f), dev(p.N)
     I = torch.empty(p.ns, device="cuda", dtype=torch.float64)
     h.collision(f, N, I)

@@ -197,6 +197,49 @@ def test_stream_store_holds_every_channel_once(prob, rows, fine, ctas, monkeypat
     assert np.abs(I - Io).max() <= 1e-12 * np.abs(Io).max()
 
 
+@pytest.mark.parametrize("rows,fine,smem,lp,lg", [(None, None, None, None, None), (16, 4, 12000, 3, 2), (64, 8, 20000, 2, 3),
+                                                  (2048, 128, None, None, None), (32, 32, 9000, 16, 4)])
+def test_res_store_holds_every_weight_once(prob, rows, fine, smem, lp, lg, monkeypatch):
+    # resident-tile store (variant 3): default geometry, and forced geometries with many tiny tiles, tiles split by
+    # the shared-memory budget, out rows cut into pieces and rows whose inputs need the second gather round
+    if rows is not None:
+        monkeypatch.setenv("EPHC_RES_ROWS", str(rows))
+        monkeypatch.setenv("EPHC_RES_ROWS_B", str(rows))
+        monkeypatch.setenv("EPHC_RES_FINE", str(fine))
+    for k, v in (("EPHC_RES_SMEM", smem), ("EPHC_RES_LP", lp), ("EPHC_RES_LG", lg)):
+        if v is not None:
+            monkeypatch.setenv(k, str(v))
+    L = oracle.OracleList(prob)
+    h = ephc.build_channels(prob, flags=ephc.HOST_ONLY)
+    t = h.export_res()        # also checks the tile images: column tables, pieces, gather lists, slots, coverage
+    ch = L.export()
+    assert len(t["w"]) == L.nw
+    a = ch["ik"] * prob.nb + ch["n"]
+    b = ch["ikq"] * prob.nb + ch["m"]
+    rows_, ws = [], []
+    for wk, kd in (("w_abs", 0), ("w_em", 1)):
+        sel = ch[wk] != 0
+        rows_.append(np.stack([a[sel], b[sel], ch["iq"][sel], ch["nu"][sel], np.full(sel.sum(), kd)]))
+        ws.append(ch[wk][sel])
+    exp = np.concatenate(rows_, axis=1).astype(np.int64)
+    expw = np.concatenate(ws)
+    got = np.stack([t[k] for k in ("a", "b", "iq", "nu", "kind")]).astype(np.int64)
+    assert exp.shape == got.shape
+    oe = np.lexsort(exp[::-1]); og = np.lexsort(got[::-1])
+    assert np.array_equal(exp[:, oe], got[:, og])
+    assert _ulp_close(t["w"][og], expw[oe], 4)
+    # evaluated with numpy in Eq. 2's printed form, the store reproduces the oracle's collision integral
+    f, N = prob.f, prob.N
+    fa, fb, Nq = f[t["a"]], f[t["b"]], N[t["iq"].astype(np.int64) * prob.nnu + t["nu"]]
+    out_, in_ = fa * (1 - fb), fb * (1 - fa)
+    T = t["w"] * np.where(t["kind"] == 1, out_ * (Nq + 1) - in_ * Nq, out_ * Nq - in_ * (Nq + 1))
+    I = np.zeros(prob.ns)
+    np.add.at(I, t["a"], -T)
+    np.add.at(I, t["b"], T)
+    Io = L.collision(f, N)
+    assert np.abs(I - Io).max() <= 1e-12 * np.abs(Io).max()
+
+
 def test_launch_geometry_limits():
     # a segment with more half-pairs than one round can stage (tiny 8x8x8: 512 partners per k, 5 doubles each)
     # and a dense many-band block: both must split into rounds/tasks within the kernel's limits
