@@ -96,15 +96,13 @@ struct ephc_handle {
     bool res_ok = false;
     std::string res_why;
     ResHost rhost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_res)
-    int32_t x_nrun = 0, x_Rcap = 0, x_ntile = 0, x_ncta = 0;
+    int32_t x_Ra = 0, x_Rcap = 0, x_RbMax = 0, x_ntile = 0, x_ncta = 0, x_nrows = 0;
     int64_t x_entries = 0, x_part_rows = 0, x_smem_tile = 0, bytes_res = 0;
     unsigned char *dx_blob = nullptr;
     uint32_t *dx_iqn = nullptr;
     ResTile *dx_tiles = nullptr;
-    ResRun *dx_runs = nullptr;
-    int32_t *dx_order = nullptr;
-    int *dx_counter = nullptr;
-    double *dx_part = nullptr;
+    int32_t *dx_cta_ptr = nullptr;
+    double *dx_part = nullptr, *dx_fc = nullptr;
     int32_t *dx_row_state = nullptr, *dx_state_row = nullptr, *dx_state_blk = nullptr, *dx_blk_row0 = nullptr,
             *dx_blk_ent_ptr = nullptr;
     int64_t *dx_slot_off = nullptr, *dx_blk_ent_off = nullptr;
@@ -132,7 +130,7 @@ static void free_dev(ephc_handle *h) {
                     h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
                     h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_order, h->ds_counter, h->ds_row_state,
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
-                    h->ds_blk_ent_off, h->dx_blob, h->dx_iqn, h->dx_tiles, h->dx_runs, h->dx_order, h->dx_counter, h->dx_part,
+                    h->ds_blk_ent_off, h->dx_blob, h->dx_iqn, h->dx_tiles, h->dx_cta_ptr, h->dx_fc, h->dx_part,
                     h->dx_row_state, h->dx_state_row, h->dx_state_blk, h->dx_blk_row0, h->dx_blk_ent_ptr, h->dx_slot_off,
                     h->dx_blk_ent_off};
     for (void *p : ptrs)
@@ -243,10 +241,10 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         sh.perm.resize(sh.perm.size() + 8, 0);  // the staging copies read whole 8-byte pieces
         if (h->host_only) h->shost = sh;
     }
-    // resident-tile store (variant 3): two CTAs per SM, each with one tile image in shared memory
+    // resident-tile store (variant 3): one persistent CTA per SM with two tile buffers in shared memory
     ResHost xh;
     if (std::getenv("EPHC_NO_RES") == nullptr) {
-        int nshare = 2 * n_sm;
+        int nshare = kResCtasPerSm * n_sm;
         if (const char *e = std::getenv("EPHC_RES_CTAS")) nshare = std::max(1, std::atoi(e));
         int64_t cap = kResSmemCap;
         if (const char *e = std::getenv("EPHC_RES_SMEM")) cap = std::max(8192, std::atoi(e));
@@ -255,17 +253,19 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             delete h;
             return fail(rc, err);
         }
-        h->res_ok = xh.supported && res_smem_bytes(xh.Rcap, xh.smem_tile) <= 225 * 1024;
-        h->res_why = xh.why;
-        h->x_ncta = nshare;
-        h->x_nrun = (int32_t)xh.runs.size();
+        h->res_ok = xh.supported && res_smem_total(xh.Ra, xh.Rcap, xh.RbMax, xh.smem_tile) <= kResSmemCap;
+        h->res_why = xh.supported ? "shared-memory budget exceeded" : xh.why;
+        h->x_ncta = xh.ncta;
         h->x_ntile = (int32_t)xh.tiles.size();
+        h->x_Ra = xh.Ra;
         h->x_Rcap = xh.Rcap;
+        h->x_RbMax = xh.RbMax;
+        h->x_nrows = xh.nrows;
         h->x_entries = xh.nent;
         h->x_part_rows = xh.part_rows;
         h->x_smem_tile = xh.smem_tile;
         h->bytes_res = (int64_t)(xh.blob.size() + xh.iqn.size() * 4 + xh.tiles.size() * sizeof(ResTile) +
-                                 xh.runs.size() * (sizeof(ResRun) + 4));
+                                 xh.cta_ptr.size() * 4);
         if (h->host_only) h->rhost = xh;
     }
     // row store for transport_iter (one CTA of 1024 threads per SM, one strip each)
@@ -342,11 +342,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             rc = upload(&h->dx_blob, xh.blob, &bx);
             if (rc == EPHC_OK) rc = upload(&h->dx_iqn, xh.iqn, &bx);
             if (rc == EPHC_OK) rc = upload(&h->dx_tiles, xh.tiles, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_runs, xh.runs, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_order, xh.order, &bx);
-            if (rc == EPHC_OK && (cudaMalloc((void **)&h->dx_counter, 64) != cudaSuccess ||
-                                  cudaMemset(h->dx_counter, 0, 64) != cudaSuccess))
-                rc = fail(EPHC_ENOMEM, "cudaMalloc (run counter) failed");
+            if (rc == EPHC_OK) rc = upload(&h->dx_cta_ptr, xh.cta_ptr, &bx);
             if (rc == EPHC_OK) rc = upload(&h->dx_row_state, xh.row_state, &bx);
             if (rc == EPHC_OK) rc = upload(&h->dx_state_row, xh.state_row, &bx);
             if (rc == EPHC_OK) rc = upload(&h->dx_state_blk, xh.state_blk, &bx);
@@ -356,6 +352,9 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             if (rc == EPHC_OK) rc = upload(&h->dx_slot_off, xh.slot_off, &bx);
             if (rc == EPHC_OK && cudaMalloc((void **)&h->dx_part, (size_t)std::max<int64_t>(1, xh.part_rows) * 8) != cudaSuccess)
                 rc = fail(EPHC_ENOMEM, "cudaMalloc (resident-tile partial sums) failed");
+            if (rc == EPHC_OK && (cudaMalloc((void **)&h->dx_fc, ((size_t)xh.nrows + 4) * 8) != cudaSuccess ||
+                                  cudaMemset(h->dx_fc, 0, ((size_t)xh.nrows + 4) * 8) != cudaSuccess))
+                rc = fail(EPHC_ENOMEM, "cudaMalloc (compact f) failed");
             xh = ResHost();
         }
         if (rc == EPHC_OK && h->rows_ok) {
@@ -718,57 +717,75 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
     if (!h->res_ok) return fail(EPHC_ESTATE, "resident-tile store not available for this problem: " + h->res_why);
     const ResHost &t = h->rhost;
     const int nnu = h->d.nnu;
-    std::vector<uint8_t> run_seen(t.runs.size(), 0), tile_seen(t.tiles.size(), 0);
-    if (t.order.size() != t.runs.size()) return fail(EPHC_ESTATE, "internal: run order does not list every run");
+    if ((int32_t)t.cta_ptr.size() != t.ncta + 1 || t.cta_ptr[0] != 0 || t.cta_ptr[t.ncta] != (int32_t)t.tiles.size())
+        return fail(EPHC_ESTATE, "internal: schedule does not list every tile");
+    if (res_smem_total(t.Ra, t.Rcap, t.RbMax, t.smem_tile) > kResSmemCap || t.Ra % 2 || t.Rcap % 2 || t.RbMax % 2)
+        return fail(EPHC_ESTATE, "internal: shared-memory plan");
     int64_t o = 0;
     std::vector<int32_t> owner, used;
-    for (int32_t ir : t.order) {
-        if (ir < 0 || ir >= (int32_t)t.runs.size() || run_seen[ir]++) return fail(EPHC_ESTATE, "internal: bad run order");
-        const ResRun &run = t.runs[ir];
-        if (run.nt < 1 || run.a_rows < 1 || run.a_row0 % t.Ra != 0 || run.a_slot < 0 ||
-            t.slot_row0[run.a_slot] != run.a_row0 || t.slot_rows[run.a_slot] != run.a_rows)
-            return fail(EPHC_ESTATE, "internal: bad run");
-        for (int32_t it = run.t0; it < run.t0 + run.nt; ++it) {
-            if (it < 0 || it >= (int32_t)t.tiles.size() || tile_seen[it]++) return fail(EPHC_ESTATE, "internal: tile in two runs");
+    size_t irun = 0;
+    for (int32_t cta = 0; cta < t.ncta; ++cta) {
+        for (int32_t it = t.cta_ptr[cta]; it < t.cta_ptr[cta + 1]; ++it) {
             const ResTile &D = t.tiles[it];
-            const ResLayout L = res_layout(D.ne, D.npiece, D.ntask1, D.ntask2, D.nc1 + D.nc2 + D.nc3, D.ngl1 + D.ngl2);
+            // runs: consecutive tiles of one strip on one CTA, first / last flags, one slot for the strip
+            if (D.flags & 1) {
+                if (irun >= t.runs.size() || t.runs[irun].t0 != it || t.runs[irun].cta != cta) return fail(EPHC_ESTATE, "internal: run table");
+            } else if (irun >= t.runs.size() || it <= t.runs[irun].t0 || it >= t.runs[irun].t0 + t.runs[irun].nt) {
+                return fail(EPHC_ESTATE, "internal: tile outside its run");
+            }
+            const ResRun &run = t.runs[irun];
+            if (((D.flags & 2) != 0) != (it == run.t0 + run.nt - 1) || run.a_row0 % t.Ra != 0 || run.a_rows < 1 || run.a_rows > t.Ra ||
+                D.a_row0 != run.a_row0 || D.a_rows != run.a_rows || D.a_slot != run.a_slot || run.a_slot < 0 ||
+                t.slot_row0[run.a_slot] != run.a_row0 || t.slot_rows[run.a_slot] != run.a_rows ||
+                (it + 1 < t.cta_ptr[cta + 1] ? D.nq_next != t.tiles[it + 1].nq : D.nq_next != 0))
+                return fail(EPHC_ESTATE, "internal: bad run / tile header");
+            if (D.flags & 2) ++irun;
+            ResTile Dl = D;
+            res_set_layout(Dl, t.nl, nnu);
             const int32_t R = run.a_rows + D.b_rows;
-            const int64_t smem = (int64_t)L.bytes + 8 * (int64_t)(D.npiece + D.npart) + 16 + 8 * (int64_t)D.nq * nnu;
-            if (D.ne < 1 || L.bytes != D.blob_bytes || D.blob_off % 128 != 0 || D.blob_off + D.blob_bytes > (int64_t)t.blob.size() ||
-                smem > t.smem_tile || R > t.Rcap || R > kResRowMax || D.nq * nnu > kResSlotMax ||
-                D.ne + D.npiece + D.npart > kResXMax || D.ngl1 != D.ne + D.npiece || D.ngl2 != D.npart ||
-                (D.b_rows > 0) != (D.b_slot >= 0) || (D.b_rows > 0 && D.b_row0 < run.a_row0 + run.a_rows) ||
+            if (D.ne < 1 || std::memcmp(&Dl, &D, sizeof(D)) != 0 || (int64_t)D.a_off != t.slot_off[D.a_slot] ||
+                (D.b_slot >= 0 && (int64_t)D.b_off != t.slot_off[D.b_slot]) || D.blob_off % 128 != 0 || D.blob_off + D.blob_bytes > (int64_t)t.blob.size() ||
+                res_tile_smem(D, nnu) > t.smem_tile || R > t.Rcap || D.b_rows > t.RbMax || R > kResRowMax || D.nq * nnu > kResSlotMax ||
+                D.ne + D.npiece + D.npart > kResXMax || D.ngl1 > D.ne + D.npiece || D.ngl2 != D.npart ||
+                (D.b_rows > 0) != (D.b_slot >= 0) || (D.b_rows > 0 && (D.b_row0 < run.a_row0 + run.a_rows || D.b_row0 % 2 || run.a_rows % 2)) ||
                 (D.b_slot >= 0 && (t.slot_row0[D.b_slot] != D.b_row0 || t.slot_rows[D.b_slot] != D.b_rows)) ||
                 D.q0 < 0 || D.q0 + D.nq > (int64_t)t.iqn.size())
                 return fail(EPHC_ESTATE, "internal: bad resident tile");
+            if (D.nq_next > 0 && std::memcmp(t.blob.data() + D.blob_off + D.o_nxt, t.iqn.data() + t.tiles[it + 1].q0, (size_t)D.nq_next * 4) != 0)
+                return fail(EPHC_ESTATE, "internal: the image does not carry the next tile's iq list");
             const unsigned char *B = t.blob.data() + D.blob_off;
-            const uint32_t *code = reinterpret_cast<const uint32_t *>(B + L.code);
-            const uint16_t *perm = reinterpret_cast<const uint16_t *>(B + L.perm);
-            const uint16_t *prow = reinterpret_cast<const uint16_t *>(B + L.prow);
-            const uint16_t *d1 = reinterpret_cast<const uint16_t *>(B + L.d1);
-            const uint16_t *d2 = reinterpret_cast<const uint16_t *>(B + L.d2);
-            const uint32_t *cols = reinterpret_cast<const uint32_t *>(B + L.cols);
-            const double *wv = reinterpret_cast<const double *>(B + L.w);
+            const uint32_t *code = reinterpret_cast<const uint32_t *>(B);
+            const uint16_t *perm = reinterpret_cast<const uint16_t *>(B + D.o_perm);
+            const uint16_t *prow = reinterpret_cast<const uint16_t *>(B + D.o_prow);
+            const uint16_t *pf = reinterpret_cast<const uint16_t *>(B + D.o_pf);
+            const uint16_t *tf = reinterpret_cast<const uint16_t *>(B + D.o_tf);
+            const uint16_t *d1 = reinterpret_cast<const uint16_t *>(B + D.o_d1);
+            const uint16_t *d2 = reinterpret_cast<const uint16_t *>(B + D.o_d2);
+            const uint32_t *cols = reinterpret_cast<const uint32_t *>(B + D.o_cols);
+            const double *wv = reinterpret_cast<const double *>(B + D.o_w);
             auto row_of = [&](int32_t loc) { return loc < run.a_rows ? run.a_row0 + loc : D.b_row0 + (loc - run.a_rows); };
             // phase 1 exactly as the kernel walks it: owner[x] = local row that must receive X[x]
             const int32_t nx = D.ne + D.npiece + D.npart;
             owner.assign((size_t)nx, -1);
             used.assign((size_t)nx, 0);
-            for (int32_t p = 0; p < D.npiece; ++p) {
-                if (prow[p] >= R) return fail(EPHC_ESTATE, "internal: piece row out of range");
-                owner[D.ne + p] = prow[p];
-                int32_t len = 0;
+            int32_t pieces_seen = 0;
+            for (int32_t l = 0; l < t.nl; ++l) {
+                int32_t piece = pf[l], combo_in = -1;
+                bool open = false;
                 for (int32_t j = 0; j < D.nc1; ++j) {
                     const int32_t cnt = (int32_t)(cols[j] & 0xffffu), base = (int32_t)(cols[j] >> 16);
-                    if (p >= cnt) break;
-                    ++len;
-                    const int32_t e = base + p;
-                    if (e < 0 || e >= D.ne || owner[e] >= 0) return fail(EPHC_ESTATE, "internal: entry visited twice");
+                    if (l >= cnt) break;
+                    const int32_t e = base + l;
+                    if (piece >= D.npiece || prow[piece] >= R || e < 0 || e >= D.ne || owner[e] != -1)
+                        return fail(EPHC_ESTATE, "internal: entry visited twice / piece out of range");
                     const uint32_t cd = code[e];
                     const int32_t in_loc = (int32_t)((cd & 0xffffu) >> 3), slot = (int32_t)(cd >> 19);
-                    if ((cd & 7u) || in_loc >= R || slot / nnu >= D.nq) return fail(EPHC_ESTATE, "internal: entry code out of range");
-                    owner[e] = in_loc;
-                    const int32_t ro = row_of(prow[p]), ri = row_of(in_loc);
+                    if ((cd & 4u) || (cd & 3u) == 3u || in_loc >= R || slot / nnu >= D.nq)
+                        return fail(EPHC_ESTATE, "internal: entry code out of range");
+                    if (combo_in >= 0 && combo_in != in_loc) return fail(EPHC_ESTATE, "internal: a combo mixes in rows");
+                    combo_in = (cd & 2u) ? in_loc : -1;
+                    owner[e] = (cd & 2u) ? -2 : in_loc;  // -2: its term is part of the combo that ends later in this lane
+                    const int32_t ro = row_of(prow[piece]), ri = row_of(in_loc);
                     if (ro == ri) return fail(EPHC_ESTATE, "internal: entry with equal ends");
                     const int64_t x = o + e;
                     if (a) a[x] = t.row_state[std::min(ro, ri)];
@@ -777,30 +794,46 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
                     if (nu) nu[x] = slot % nnu;
                     if (kind) kind[x] = ro < ri ? 1 : 0;  // out = a: emission weight; out = b: absorption weight
                     if (w) w[x] = wv[e];
+                    open = true;
+                    if (cd & 1u) {
+                        if (owner[D.ne + piece] >= 0) return fail(EPHC_ESTATE, "internal: piece closed twice");
+                        owner[D.ne + piece] = prow[piece];
+                        ++piece;
+                        ++pieces_seen;
+                        open = false;
+                    }
                 }
-                if (len < 1) return fail(EPHC_ESTATE, "internal: empty piece");
+                if (open) return fail(EPHC_ESTATE, "internal: a lane ends inside a piece");
             }
+            if (pieces_seen != D.npiece) return fail(EPHC_ESTATE, "internal: piece count");
             for (int32_t e = 0; e < D.ne; ++e)
-                if (owner[e] < 0) return fail(EPHC_ESTATE, "internal: entry not covered by any piece");
+                if (owner[e] == -1) return fail(EPHC_ESTATE, "internal: entry not covered by any lane");
             // phase 2: every X value is added exactly once, to its owner row (directly or through one partial sum)
-            std::vector<uint8_t> row_final((size_t)R, 0);
-            for (int32_t tk = 0; tk < D.ntask1; ++tk) {
-                const int32_t dst = d1[tk];
-                const bool partial = (dst & 0x8000) != 0;
-                int32_t row = partial ? -1 : dst, len = 0;
-                if (partial && (dst & 0x7fff) >= D.npart) return fail(EPHC_ESTATE, "internal: partial index out of range");
-                if (!partial && (dst >= R || row_final[dst]++)) return fail(EPHC_ESTATE, "internal: two final tasks for a row");
+            std::vector<uint8_t> row_final((size_t)R, 0), task_seen((size_t)D.ntask1, 0);
+            for (int32_t l = 0; l < t.nl; ++l) {
+                int32_t task = tf[l], row = -1;
                 for (int32_t j = 0; j < D.nc2; ++j) {
                     const int32_t cnt = (int32_t)(cols[D.nc1 + j] & 0xffffu), base = (int32_t)(cols[D.nc1 + j] >> 16);
-                    if (tk >= cnt) break;
-                    ++len;
-                    const int32_t x = perm[base + tk];
-                    if (base + tk >= D.ngl1 || x >= D.ne + D.npiece || used[x]++) return fail(EPHC_ESTATE, "internal: gather list");
+                    if (l >= cnt) break;
+                    const uint32_t wd = perm[base + l];
+                    const int32_t x = (int32_t)(wd & 0x7fffu);
+                    if (base + l >= D.ngl1 || x >= D.ne + D.npiece || owner[x] < 0 || used[x]++) return fail(EPHC_ESTATE, "internal: gather list");
                     if (row < 0) row = owner[x];
                     if (owner[x] != row) return fail(EPHC_ESTATE, "internal: gather task mixes rows");
+                    if (wd & 0x8000u) {
+                        if (task >= D.ntask1 || task_seen[task]++) return fail(EPHC_ESTATE, "internal: task index");
+                        const int32_t dst = d1[task++];
+                        if (dst & 0x8000) {
+                            if ((dst & 0x7fff) >= D.npart || owner[D.ne + D.npiece + (dst & 0x7fff)] >= 0)
+                                return fail(EPHC_ESTATE, "internal: partial index out of range");
+                            owner[D.ne + D.npiece + (dst & 0x7fff)] = row;
+                        } else if (dst != row || row_final[dst]++) {
+                            return fail(EPHC_ESTATE, "internal: final task of a row");
+                        }
+                        row = -1;
+                    }
                 }
-                if (len < 1) return fail(EPHC_ESTATE, "internal: empty gather task");
-                if (partial) owner[D.ne + D.npiece + (dst & 0x7fff)] = row;
+                if (row >= 0) return fail(EPHC_ESTATE, "internal: a lane ends inside a gather task");
             }
             for (int32_t tk = 0; tk < D.ntask2; ++tk) {
                 const int32_t row = d2[tk];
@@ -814,13 +847,11 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
                 }
             }
             for (int32_t x = 0; x < nx; ++x)
-                if (used[x] != 1) return fail(EPHC_ESTATE, "internal: X value not gathered exactly once");
+                if (used[x] != (owner[x] == -2 ? 0 : 1)) return fail(EPHC_ESTATE, "internal: X value not gathered exactly once");
             o += D.ne;
         }
     }
-    if (o != t.nent) return fail(EPHC_ESTATE, "internal: resident-tile store does not hold every weight");
-    for (uint8_t s : tile_seen)
-        if (!s) return fail(EPHC_ESTATE, "internal: tile not in any run");
+    if (o != t.nent || irun != t.runs.size()) return fail(EPHC_ESTATE, "internal: resident-tile store does not hold every weight");
     {
         std::vector<uint8_t> cover((size_t)t.part_rows, 0);
         for (int32_t bl = 0; bl < t.nblk; ++bl)
@@ -872,8 +903,8 @@ static int need_device(ephc_handle *h) {
             CUDA_TRY(cudaFuncSetAttribute(stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)stream_smem_bytes(h->s_Ra, h->s_Rb)));
         if (h->res_ok)
-            CUDA_TRY(cudaFuncSetAttribute(res_kernel<kResThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)res_smem_bytes(h->x_Rcap, h->x_smem_tile)));
+            CUDA_TRY(cudaFuncSetAttribute(res_kernel<kResLanes>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)kResSmemCap));
         if (h->rows_ok)
             CUDA_TRY(cudaFuncSetAttribute(row_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)row_smem_bytes(h->r_Rb, h->r_Ra)));
@@ -1033,29 +1064,59 @@ static int launch_stream(ephc_handle *h, const double *f, const double *N, cudaS
 }
 
 static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStream_t s) {
-    if (h->x_nrun > 0) {
+    if (h->x_ntile > 0) {
+        res_compact_kernel<<<(unsigned)((h->x_nrows + 255) / 256), 256, 0, s>>>(f, h->dx_row_state, h->dx_fc, h->x_nrows);
+        h->launches++;
         ResParams P;
         std::memset(&P, 0, sizeof(P));
         P.blob = h->dx_blob;
         P.iqn = h->dx_iqn;
         P.tiles = h->dx_tiles;
-        P.runs = h->dx_runs;
-        P.order = h->dx_order;
-        P.counter = h->dx_counter;
-        P.nrun = h->x_nrun;
-        P.row_state = h->dx_row_state;
+        P.cta_ptr = h->dx_cta_ptr;
         P.slot_off = h->dx_slot_off;
+        P.Ra = h->x_Ra;
         P.Rcap = h->x_Rcap;
+        P.RbMax = h->x_RbMax;
         P.nnu = h->d.nnu;
+        P.buf_bytes = (uint32_t)res_buf_bytes(h->x_Rcap, h->x_RbMax, h->x_smem_tile);
+        P.fixed_bytes = (uint32_t)res_fixed_bytes(h->x_Ra);
         P.gran16 = (h->d.nnu % 2 == 0) && ((reinterpret_cast<uintptr_t>(N) & 15) == 0);
         P.gran = P.gran16 ? h->d.nnu / 2 : h->d.nnu;
         P.gran_magic = P.gran > 1 ? (uint32_t)((0x100000000ULL + (uint64_t)P.gran - 1) / (uint64_t)P.gran) : 0u;
-        P.f = f;
+        P.fc = h->dx_fc;
         P.N = N;
         P.part = h->dx_part;
-        const int grid = std::min(h->x_nrun, h->x_ncta);
-        res_kernel<kResThreads><<<(unsigned)grid, kResThreads, res_smem_bytes(h->x_Rcap, h->x_smem_tile), s>>>(P);
+#ifdef EPHC_RES_TIMING
+        static long long *dbg = nullptr;
+        const size_t ndbg = (size_t)h->x_ncta * (kResLanes / 32) * 8;
+        if (!dbg) cudaMalloc((void **)&dbg, ndbg * 8);
+        cudaMemset(dbg, 0, ndbg * 8);
+        P.dbg = dbg;
+#endif
+        res_kernel<kResLanes><<<(unsigned)h->x_ncta, kResLanes + 32,
+                                  (size_t)res_smem_total(h->x_Ra, h->x_Rcap, h->x_RbMax, h->x_smem_tile), s>>>(P);
         h->launches++;
+#ifdef EPHC_RES_TIMING
+        if (std::getenv("EPHC_RES_TIMING_PRINT")) {
+            std::vector<long long> hd(ndbg);
+            cudaMemcpy(hd.data(), dbg, ndbg * 8, cudaMemcpyDeviceToHost);
+            const char *nm[8] = {"loop", "wait full", "phase 1", "barrier", "phase 2 r1", "round 2", "barrier", "copy-out"};
+            const int nw = kResLanes / 32;
+            for (int k = 0; k < 8; ++k) {
+                double mean = 0, w0 = 0, wl = 0, mx = 0;
+                for (int c = 0; c < h->x_ncta; ++c)
+                    for (int w = 0; w < nw; ++w) {
+                        const double v = (double)hd[((size_t)c * nw + w) * 8 + k];
+                        mean += v;
+                        mx = std::max(mx, v);
+                        if (w == 0) w0 += v;
+                        if (w == nw - 1) wl += v;
+                    }
+                std::fprintf(stderr, "res timing %-14s mean %9.0f  warp0 %9.0f  last warp %9.0f  max %9.0f cycles per CTA\n", nm[k],
+                             mean / (h->x_ncta * nw), w0 / h->x_ncta, wl / h->x_ncta, mx);
+            }
+        }
+#endif
     }
     CUDA_TRY(cudaGetLastError());
     return EPHC_OK;
@@ -1071,7 +1132,6 @@ static FinishParams finish_params_res(const ephc_handle *h) {
     P.blk_ent_off = h->dx_blk_ent_off;
     P.part = h->dx_part;
     P.ns = h->d.ns;
-    P.reset = h->dx_counter;
     return P;
 }
 

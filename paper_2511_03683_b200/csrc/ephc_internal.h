@@ -226,72 +226,83 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
 // A channel's emission weight gives out = (n,k), in = (m,k+q); its absorption weight gives the reversed entry,
 // because F_abs(a,b) = -F_em(b,a) (reading R-1), so no per-entry kind is needed.
 // Compact rows are cut into strips of Ra rows; a tile holds the entries between one strip (A rows) and a narrow range
-// of rows after it (B rows), or inside the strip (diagonal tile), sized so that its whole image fits in shared memory:
-// the image is one contiguous, 16-byte aligned blob that a CTA fetches with bulk copies (TMA) and then works on in
-// place.  Consecutive tiles of a strip form a run: one CTA keeps the strip's f values and accumulators in shared
-// memory for the whole run.
-//   phase 1 (paper step 2): one LANE per out-row PIECE (<= Lp entries of one out row); pieces sorted by descending
-//            length, entries stored column-major over ALL pieces of the tile (entry j of piece p at col[j].base + p,
-//            no padding); the lane keeps f_out and -sum(T) in registers and overwrites w by T in shared memory.
-//   phase 2 (paper step 3): one lane per gather task: it adds the X values (T of the row's in-entries, the negated
-//            sums of its out pieces) listed for one row; rows with more than Lg inputs go through partial tasks and
-//            a second round.  One owner per row, fixed order, no atomics.
-struct ResTile {           // 80 bytes (device directory)
+// of rows after it (B rows), or inside the strip (diagonal tile), sized so that TWO tile images fit in shared memory:
+// an image is one contiguous, 16-byte aligned blob that the CTA fetches with bulk copies (TMA) one tile ahead and
+// then works on in place.  Consecutive tiles of a strip form a run: the strip's accumulators stay in shared memory
+// for the whole run.  The tiles in strip-major order are cut into one contiguous share of equal work per CTA and are
+// stored in that order.  The image is laid out for a CTA of NL = kResLanes threads:
+//   phase 1 (paper step 2): the out rows of the tile are cut into pieces of at most ceil(E / NL) entries and the
+//            pieces are packed into NL lanes of (almost) equal load, longest piece first; a lane walks its pieces one
+//            after the other, keeps f_out and -sum(T) in registers and overwrites w by T in shared memory; entry j of
+//            lane l sits at col1[j].base + l (lanes sorted by descending load: column-major, no padding); bit 0 of an
+//            entry code marks the last entry of a piece, whose sum then goes to X[ne + piece].
+//   phase 2 (paper step 3): per row one gather task = the X positions of its in-entries (T) and of its out pieces
+//            (negated sums), the last one with bit 15 set; the tasks are packed into NL lanes in the same way (word j
+//            of lane l at col2[j].base + l); a lane's tasks are numbered consecutively from tf[l] and d1[task] is the
+//            destination (a row, or 0x8000 | index of a partial sum).  Rows with more
+//            inputs than a lane's share are cut into partial tasks whose sums a second, small round adds (one lane
+//            per row, column tables col3).  One owner per row and round, fixed order, no atomics.
+struct ResTile {           // 144 bytes (device directory)
     int64_t blob_off;      // byte offset of the image in the blob array (multiple of 128)
     int32_t blob_bytes;    // multiple of 16
     int32_t ne;            // entries
     int32_t npiece;        // out-row pieces
-    int32_t npart;         // round-1 partial tasks (rows with more than Lg inputs)
-    int32_t ntask1, ntask2;// gather tasks of round 1 (final + partial) and round 2 (final)
-    int32_t nc1, nc2, nc3; // columns (= longest list) of pieces, round-1 tasks, round-2 tasks
-    int32_t ngl1, ngl2;    // gather-list elements of round 1 / round 2
+    int32_t npart;         // round-1 partial tasks
+    int32_t ntask1, ntask2;// round-1 tasks (final + partial), round-2 tasks (rows whose inputs were cut)
+    int32_t nc1, nc2, nc3; // columns of phase 1, of round 1 (both padded to multiples of 4 with empty columns), of round 2
+    int32_t ngl1, ngl2;    // stream words of round 1 (positions + destinations), gather-list elements of round 2
     int32_t q0, nq;        // pairs: iqn[q0 .. q0+nq) = iq * nnu of the tile's pairs
+    int32_t nq_next;       // pairs of the next tile of the same CTA: their iq * nnu ride in this image (section nxt)
     int32_t b_row0, b_rows;// B rows (b_rows = 0 on a diagonal tile)
     int32_t b_slot;        // partial-sum slot of the B rows (-1 on a diagonal tile)
-    int32_t pad[2];
+    int32_t a_row0, a_rows, a_slot;  // the run's strip and its partial-sum slot
+    int32_t flags;         // bit 0: first tile of its run, bit 1: last tile of its run
+    // byte offsets of the sections inside the image (= inside the tile buffer), each 16-byte aligned; w comes last so
+    // that the X tail (piece sums, partial sums) and then the N rows can follow it in shared memory
+    uint32_t o_perm, o_prow, o_pf, o_tf, o_d1, o_d2, o_cols, o_nxt, o_w, o_sn;
+    uint32_t a_off, b_off; // first element of the A / B slot in the partial-sum buffer
+    int32_t pad;
 };
-struct ResRun {            // 32 bytes: consecutive tiles of one strip, handed to one CTA
+static_assert(sizeof(ResTile) == 144, "ResTile is copied word by word");
+constexpr int kResTileWords = sizeof(ResTile) / 4;
+struct ResRun {            // host only: consecutive tiles of one strip (indices into the scheduled tile sequence)
     int32_t t0, nt;
     int32_t a_row0, a_rows, a_slot;
-    int32_t pad[3];
+    int32_t cta;
 };
-// byte offsets of the sections of a tile image (each 16-byte aligned); w comes last so that the X tail (piece sums,
-// partial sums) can follow it in shared memory
-struct ResLayout {
-    int32_t code, perm, prow, d1, d2, cols, w, bytes;
-};
-#ifdef __CUDACC__
-#define EPHC_HD __host__ __device__ __forceinline__
-#else
-#define EPHC_HD inline
-#endif
-EPHC_HD int32_t res_al16(int32_t x) { return (x + 15) & ~15; }
-EPHC_HD ResLayout res_layout(int32_t ne, int32_t npiece, int32_t ntask1, int32_t ntask2, int32_t ncols, int32_t ngl) {
-    ResLayout L;
-    L.code = 0;
-    L.perm = res_al16(4 * ne);
-    L.prow = L.perm + res_al16(2 * ngl);
-    L.d1 = L.prow + res_al16(2 * npiece);
-    L.d2 = L.d1 + res_al16(2 * ntask1);
-    L.cols = L.d2 + res_al16(2 * ntask2);
-    L.w = L.cols + res_al16(4 * ncols);
-    L.bytes = L.w + res_al16(8 * ne);
-    return L;
+inline int32_t res_al16(int32_t x) { return (x + 15) & ~15; }
+// fills the section offsets and blob_bytes of D from its counts (code section first, at offset 0)
+inline void res_set_layout(ResTile &D, int nl, int nnu) {
+    (void)nnu;
+    D.o_perm = (uint32_t)res_al16(4 * D.ne);
+    D.o_prow = D.o_perm + (uint32_t)res_al16(2 * (D.ngl1 + D.ngl2));
+    D.o_pf = D.o_prow + (uint32_t)res_al16(2 * (D.npiece + 4));
+    D.o_tf = D.o_pf + (uint32_t)res_al16(2 * nl);
+    D.o_d1 = D.o_tf + (uint32_t)res_al16(2 * nl);
+    D.o_d2 = D.o_d1 + (uint32_t)res_al16(2 * D.ntask1);
+    D.o_cols = D.o_d2 + (uint32_t)res_al16(2 * D.ntask2);
+    D.o_nxt = D.o_cols + (uint32_t)res_al16(4 * (D.nc1 + D.nc2 + D.nc3));
+    D.o_w = D.o_nxt + (uint32_t)res_al16(4 * D.nq_next);
+    D.blob_bytes = (int32_t)D.o_w + res_al16(8 * D.ne);
+    D.o_sn = (uint32_t)res_al16((int32_t)D.o_w + 8 * (D.ne + D.npiece + D.npart));
 }
+// shared memory a tile needs behind the f / accumulator arrays: image, X tail, N rows of its pairs
+inline int64_t res_tile_smem(const ResTile &D, int nnu) { return (int64_t)D.o_sn + 8 * (int64_t)D.nq * nnu; }
 constexpr int kResSlotMax = 8192;     // N slots (pair * nnu + mode) per tile: slot * 8 fits the 16-bit field of the code
 constexpr int kResRowMax = 8192;      // rows (A + B) per tile: row * 8 fits the 16-bit field of the code
-constexpr int kResThreads = 384;      // threads per CTA of res_kernel (two CTAs per SM)
-constexpr int64_t kResSmemCap = 112 * 1024;  // dynamic shared memory per CTA: two CTAs fit in the 227 KB of an SM
-constexpr int kResXMax = 65535;       // X positions (entries + pieces + partials) per tile: uint16 gather lists
+constexpr int kResLanes = 256;        // threads of a persistent CTA of res_kernel = lanes of a tile image
+constexpr int kResCtasPerSm = 2;      // the phases of the two CTAs of an SM interleave
+constexpr int64_t kResSmemCap = 112 * 1024;  // dynamic shared memory per CTA (227 KB per SM incl. static and 1 KB per CTA)
+constexpr int kResXMax = 32767;       // X positions (entries + pieces + partials) per tile: 15 bits of a stream word
 struct ResHost {
-    int32_t Ra = 0, Rcap = 0, rf = 0, nblk = 0, nrows = 0, nnu = 0;
-    int64_t smem_tile = 0;            // largest (blob + X tail + N rows) of any tile, bytes
+    int32_t Ra = 0, RbMax = 0, Rcap = 0, rf = 0, nblk = 0, nrows = 0, nnu = 0, ncta = 0, nl = 0;
+    int64_t smem_tile = 0;            // largest res_tile_smem of any tile
     std::vector<int32_t> blk_row0, row_state, state_row, state_blk;
-    std::vector<unsigned char> blob;  // all tile images
+    std::vector<unsigned char> blob;  // all tile images, in schedule order
     std::vector<uint32_t> iqn;        // per (tile, pair): iq * nnu
-    std::vector<ResTile> tiles;
+    std::vector<ResTile> tiles;       // in schedule order: the tiles of CTA c are tiles[cta_ptr[c] .. cta_ptr[c+1])
+    std::vector<int32_t> cta_ptr;
     std::vector<ResRun> runs;
-    std::vector<int32_t> order;       // runs by descending work
     std::vector<int64_t> slot_off;
     std::vector<int32_t> slot_row0, slot_rows, blk_ent_ptr;
     std::vector<int64_t> blk_ent_off;
@@ -299,6 +310,15 @@ struct ResHost {
     bool supported = false;
     std::string why;
 };
+// bytes of res_kernel's dynamic shared memory: strip accumulators, three directory entries, two tile buffers
+// (f of the A and B rows, accumulators of the B rows, image + X tail + N rows)
+inline int64_t res_buf_bytes(int Rcap, int RbMax, int64_t smem_tile) {
+    return ((int64_t)8 * Rcap + (int64_t)8 * RbMax + smem_tile + 127) & ~(int64_t)127;
+}
+inline int64_t res_fixed_bytes(int Ra) { return ((int64_t)8 * Ra + 3 * (int64_t)sizeof(ResTile) + 127) & ~(int64_t)127; }
+inline int64_t res_smem_total(int Ra, int Rcap, int RbMax, int64_t smem_tile) {
+    return res_fixed_bytes(Ra) + 2 * res_buf_bytes(Rcap, RbMax, smem_tile);
+}
 int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, int64_t smem_cap, ResHost &t,
               std::string &err);
 

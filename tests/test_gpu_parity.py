@@ -258,8 +258,8 @@ def test_stream_geometry_on_gpu(monkeypatch, rows, fine, ctas):
         assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
 
 
-@pytest.mark.parametrize("rows,fine,smem,lp,lg,ctas", [(16, 4, 12000, 3, 2, 3), (64, 8, 20000, 2, 3, 40), (2048, 128, None, None, None, 1),
-                                                       (32, 32, 9000, 16, 4, 7)])
+@pytest.mark.parametrize("rows,fine,smem,lp,lg,ctas", [(16, 4, 16000, 3, 2, 3), (64, 8, 24000, 2, 3, 40), (512, 128, None, None, None, 1),
+                                                       (32, 32, 20000, 16, 4, 7)])
 def test_res_geometry_on_gpu(monkeypatch, rows, fine, smem, lp, lg, ctas):
     # resident-tile store: many tiny tiles, tiles split by the shared-memory budget, out rows cut into pieces, rows that
     # need the second gather round, runs longer than one tile, one CTA for everything

@@ -197,8 +197,8 @@ def test_stream_store_holds_every_channel_once(prob, rows, fine, ctas, monkeypat
     assert np.abs(I - Io).max() <= 1e-12 * np.abs(Io).max()
 
 
-@pytest.mark.parametrize("rows,fine,smem,lp,lg", [(None, None, None, None, None), (16, 4, 12000, 3, 2), (64, 8, 20000, 2, 3),
-                                                  (2048, 128, None, None, None), (32, 32, 9000, 16, 4)])
+@pytest.mark.parametrize("rows,fine,smem,lp,lg", [(None, None, None, None, None), (16, 4, 16000, 3, 2), (64, 8, 24000, 2, 3),
+                                                  (512, 128, None, None, None), (32, 32, 20000, 16, 4)])
 def test_res_store_holds_every_weight_once(prob, rows, fine, smem, lp, lg, monkeypatch):
     # resident-tile store (variant 3): default geometry, and forced geometries with many tiny tiles, tiles split by
     # the shared-memory budget, out rows cut into pieces and rows whose inputs need the second gather round
