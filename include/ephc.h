@@ -30,7 +30,11 @@
  *   The handle owns the channel store in device memory (HBM) and a host copy of the canonical list.
  *   Every pointer named *_dev is a caller-owned DEVICE buffer of doubles (8-byte aligned), borrowed for
  *   the call; `stream` is a cudaStream_t passed as void* (NULL = default stream).  Device entry points only
- *   enqueue work: they do not allocate, synchronise or touch the host.  Every pointer named *_host is a
+ *   enqueue work: they do not allocate, synchronise or touch the host (all scratch -- transport weights, RK4
+ *   stages, partial sums -- is allocated by ephc_build_channels / ephc_set_variant).  A handle lives on the device
+ *   that was current at ephc_build_channels; every call makes that device current.  A handle owns ONE set of
+ *   scratch buffers and hand-out counters: only one call per handle may be in flight, i.e. all calls on a handle
+ *   must be issued to the same stream (or be ordered by the caller); use one handle per stream otherwise.  Every pointer named *_host is a
  *   caller-owned HOST buffer; the *_host entry points copy in, run the same kernels, copy out and
  *   synchronise the stream before returning.
  *
@@ -147,6 +151,13 @@ int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, i
                     double *w);
 int64_t ephc_res_entries(const ephc_handle *h);
 
+/* Decoded image of the row store (the destination-sorted store ephc_transport_iter runs on), same conditions as
+ * ephc_export_gather.  Arrays of length gather_entries in store order (strips -> partner-range tiles -> segments):
+ * destination state, partner state, position of the same ordered term in the gather store (whose weights
+ * ephc_transport_setup brings into this order).  Checks that the strips partition the destination rows, that a row has
+ * one segment per tile with segments in descending length, and that the positions are a permutation. */
+int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *partner, int64_t *gather_pos);
+
 /* Choice of algorithm:
  *   0 = gather  : destination-sorted two-sided store, one kernel, every ordered term read once
  *   1 = tiles   : once-stored channels grouped into (k-strip, k'-range) tiles; one lane per (k,k') pair updates
@@ -164,6 +175,8 @@ int64_t ephc_res_entries(const ephc_handle *h);
  *                 (<= 96 MB) and the resident-tile store beyond that; ephc_transport_setup runs on the gather store and
  *                 ephc_transport_iter on the row store built from it (the faster choice per call as measured on
  *                 B200).
+ * A store that the automatic choice does not use is built and uploaded by the first ephc_set_variant that asks for
+ * it (that call allocates and copies; ephc_build_channels builds only what the automatic choice needs).
  * ephc_transport_setup must be called again after a change of variant.  ephc_get_variant returns the variant
  * ephc_collision will use, ephc_get_transport_variant the one the transport calls will use. */
 int ephc_set_variant(ephc_handle *h, int variant);

@@ -72,6 +72,7 @@ def _load():
         "ephc_export_stream": (i32, [vp] * 7),
         "ephc_stream_entries": (i64, [vp]),
         "ephc_export_res": (i32, [vp] * 7),
+        "ephc_export_rows": (i32, [vp] * 4),
         "ephc_res_entries": (i64, [vp]),
         "ephc_set_variant": (i32, [vp, i32]),
         "ephc_get_variant": (i32, [vp]),
@@ -220,6 +221,13 @@ class Handle:
         _check(_load().ephc_export_res(self._h, *[a.ctypes.data for a in ints], w.ctypes.data))
         keys = ("a", "b", "iq", "nu", "kind", "w")
         return {k: a[:ne] for k, a in zip(keys, ints + [w])}
+
+    def export_rows(self) -> dict:
+        ne = self.query()["gather_entries"]
+        n = max(ne, 1)
+        dest, partner, pos = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int64)
+        _check(_load().ephc_export_rows(self._h, dest.ctypes.data, partner.ctypes.data, pos.ctypes.data))
+        return {"dest": dest[:ne], "partner": partner[:ne], "gather_pos": pos[:ne]}
 
     def set_variant(self, variant: int):
         _check(_load().ephc_set_variant(self._h, int(variant)))

@@ -36,6 +36,11 @@ static int fail(int code, const std::string &msg) {
 struct ephc_handle {
     Dims d{};
     bool host_only = false;
+    int device = 0, n_sm = 148;          // device the store lives on (current at ephc_build_channels)
+    std::vector<double> E;               // copy of the band energies and window: the optional stores are built from them
+    double emin = 0.0, emax = 0.0;
+    bool tile_built = false, stream_built = false, res_built = false;
+    RowHost rowhost;                     // kept only for EPHC_HOST_ONLY handles (ephc_export_rows)
     int variant = -1;  // -1: automatic (collision / rt_step on the tile store, transport on the gather store)
     Canonical can;
     GatherHost ghost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_gather)
@@ -149,6 +154,200 @@ static int upload(T **dst, const std::vector<T> &src, int64_t *bytes) {
 extern "C" const char *ephc_last_error(void) { return g_err.c_str(); }
 extern "C" const char *ephc_version(void) { return "ephc 0.1 (sm_100a, fp64)"; }
 
+// ---- the optional stores: each is built (and uploaded) once, at ephc_build_channels when the automatic choice needs
+// it, otherwise by ephc_set_variant; EPHC_HOST_ONLY handles build all of them for the export calls -----------------------
+static ephc_problem problem_view(const ephc_handle *h) {  // what the store builders read of the problem
+    ephc_problem q;
+    std::memset(&q, 0, sizeof(q));
+    q.nk = h->d.nk;
+    q.nb = h->d.nb;
+    q.nnu = h->d.nnu;
+    q.E = h->E.data();
+    q.emin = h->emin;
+    q.emax = h->emax;
+    q.npair = (int64_t)h->pair_ik.size();
+    q.pair_ik = h->pair_ik.data();
+    q.pair_ikq = h->pair_ikq.data();
+    return q;
+}
+
+static int make_tile_store(ephc_handle *h) {
+    if (h->tile_built) return EPHC_OK;
+    const ephc_problem q = problem_view(h);
+    std::string err;
+    int ncta = 2 * h->n_sm;  // two CTAs per SM walk the tile sequence
+    if (const char *e = std::getenv("EPHC_TILE_CTAS")) ncta = std::max(1, std::atoi(e));
+    TileHost &th = h->thost;
+    int rc = build_tiles(&q, h->d, h->can, ncta, th, err);
+    if (rc != EPHC_OK) return fail(rc, err);
+    h->tile_built = true;
+    h->tile_ok = th.supported && tile_smem_bytes(kTIter, th.Ra, th.Rb) <= 220 * 1024 &&
+                 tile_smem_bytes(kTCollision, th.Ra, th.Rb) <= 220 * 1024;
+    if (th.supported && !h->tile_ok) {
+        th.supported = false;
+        th.why = "tile store: shared-memory budget exceeded";
+    }
+    if (!th.supported) return EPHC_OK;
+    h->t_entries = (int64_t)th.w.size();
+    h->t_pieces = th.npiece;
+    h->t_part_rows = th.part_rows;
+    h->t_ncta = th.ncta;
+    h->t_Ra = th.Ra;
+    h->t_Rb = th.Rb;
+    h->t_nblk = th.nblk;
+    h->t_nslot = (int32_t)th.slot_off.size();
+    h->t_ntile = (int32_t)th.tiles.size();
+    h->bytes_tile = (int64_t)(th.w.size() * 8 + th.code.size() * 2 + th.prec.size() * 4 +
+                              th.slices.size() * sizeof(TileSlice) + th.tiles.size() * sizeof(TileHdr) +
+                              th.ctas.size() * sizeof(TileCta) + th.slot_off.size() * 8 +
+                              (th.blk_row0.size() + th.row_state.size() + th.state_row.size() +
+                               th.state_blk.size() + th.blk_ent_ptr.size()) * 4 + th.blk_ent_off.size() * 8);
+    if (h->host_only) return EPHC_OK;
+    int64_t bt = 0;
+    rc = upload(&h->dt_w, th.w, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_code, th.code, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_prec, th.prec, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_slices, th.slices, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_tiles, th.tiles, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_ctas, th.ctas, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_blk_row0, th.blk_row0, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_row_state, th.row_state, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_state_row, th.state_row, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_state_blk, th.state_blk, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_blk_ent_ptr, th.blk_ent_ptr, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_blk_ent_off, th.blk_ent_off, &bt);
+    if (rc == EPHC_OK) rc = upload(&h->dt_slot_off, th.slot_off, &bt);
+    if (rc == EPHC_OK && cudaMalloc((void **)&h->dt_part, (size_t)std::max<int64_t>(1, th.part_rows) * 3 * 8) != cudaSuccess)
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (partial sums) failed");
+    // transport weights of this store (two per entry), so that ephc_transport_setup never allocates
+    if (rc == EPHC_OK && (cudaMalloc((void **)&h->dt_Wf, (size_t)std::max<int64_t>(1, h->t_entries) * 8) != cudaSuccess ||
+                          cudaMalloc((void **)&h->dt_Wr, (size_t)std::max<int64_t>(1, h->t_entries) * 8) != cudaSuccess))
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (tile transport weights) failed");
+    if (rc == EPHC_OK) h->bytes_transport += h->t_entries * 16;
+    // the device owns the image now; keep only the scalars
+    TileHost empty;
+    empty.supported = th.supported;
+    empty.Ra = th.Ra; empty.Rb = th.Rb; empty.nblk = th.nblk; empty.nrows = th.nrows; empty.ncta = th.ncta;
+    empty.part_rows = th.part_rows; empty.npiece = th.npiece;
+    th = empty;
+    if (rc != EPHC_OK) h->tile_ok = false;
+    return rc;
+}
+
+static int make_stream_store(ephc_handle *h) {
+    if (h->stream_built) return EPHC_OK;
+    const ephc_problem q = problem_view(h);
+    std::string err;
+    StreamHost sh;
+    int nshare = 2 * h->n_sm;  // two CTAs of 512 threads per SM
+    if (const char *e = std::getenv("EPHC_STREAM_CTAS")) nshare = std::max(1, std::atoi(e));
+    int rc = build_stream(&q, h->d, h->can, nshare, sh, err);
+    if (rc != EPHC_OK) return fail(rc, err);
+    h->stream_built = true;
+    h->stream_ok = sh.supported && stream_smem_bytes(sh.Ra, sh.Rb) <= 220 * 1024;
+    h->stream_why = sh.supported ? "shared-memory budget exceeded" : sh.why;
+    h->s_ncta = sh.ncta;
+    h->s_Ra = sh.Ra;
+    h->s_Rb = sh.Rb;
+    h->s_ntile = (int32_t)sh.tiles.size();
+    h->s_entries = (int64_t)sh.w.size();
+    h->s_part_rows = sh.part_rows;
+    h->bytes_stream = (int64_t)(sh.w.size() * 8 + sh.code.size() * 4 + sh.perm.size() * 2 +
+                                (sh.arow_id.size() + sh.brow_id.size()) * 4 + sh.iq.size() * 4 +
+                                sh.chunks.size() * sizeof(StreamChunk) + sh.tiles.size() * sizeof(StreamTile));
+    sh.perm.resize(sh.perm.size() + 8, 0);  // the staging copies read whole 8-byte pieces
+    if (h->host_only) {
+        h->shost = std::move(sh);
+        return EPHC_OK;
+    }
+    if (!h->stream_ok) return EPHC_OK;
+    int64_t bs = 0;
+    rc = upload(&h->ds_w, sh.w, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_code, sh.code, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_perm, sh.perm, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_aid, sh.arow_id, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_ast, sh.arow_start, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_bid, sh.brow_id, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_bst, sh.brow_start, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_iq, sh.iq, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_chunks, sh.chunks, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_tiles, sh.tiles, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_order, sh.order, &bs);
+    if (rc == EPHC_OK && (cudaMalloc((void **)&h->ds_counter, 64) != cudaSuccess || cudaMemset(h->ds_counter, 0, 64) != cudaSuccess))
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (tile counter) failed");
+    if (rc == EPHC_OK) rc = upload(&h->ds_row_state, sh.row_state, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_state_row, sh.state_row, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_state_blk, sh.state_blk, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_blk_row0, sh.blk_row0, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_blk_ent_ptr, sh.blk_ent_ptr, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_blk_ent_off, sh.blk_ent_off, &bs);
+    if (rc == EPHC_OK) rc = upload(&h->ds_slot_off, sh.slot_off, &bs);
+    if (rc == EPHC_OK && cudaMalloc((void **)&h->ds_part, (size_t)std::max<int64_t>(1, sh.part_rows) * 8) != cudaSuccess)
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (stream partial sums) failed");
+    if (rc != EPHC_OK) h->stream_ok = false;
+    return rc;
+}
+
+static int make_res_store(ephc_handle *h) {
+    if (h->res_built) return EPHC_OK;
+    const ephc_problem q = problem_view(h);
+    std::string err;
+    ResHost xh;
+    int nshare = kResCtasPerSm * h->n_sm;
+    if (const char *e = std::getenv("EPHC_RES_CTAS")) nshare = std::max(1, std::atoi(e));
+    int64_t cap = kResSmemCap;
+    if (const char *e = std::getenv("EPHC_RES_SMEM")) cap = std::max(8192, std::atoi(e));
+    int rc = build_res(&q, h->d, h->can, nshare, cap, xh, err);
+    if (rc != EPHC_OK) return fail(rc, err);
+    h->res_built = true;
+    h->res_ok = xh.supported && res_smem_total(xh.Ra, xh.Rcap, xh.RbMax, xh.smem_tile) <= kResSmemCap;
+    h->res_why = xh.supported ? "shared-memory budget exceeded" : xh.why;
+    h->x_ncta = xh.ncta;
+    h->x_ntile = (int32_t)xh.tiles.size();
+    h->x_Ra = xh.Ra;
+    h->x_Rcap = xh.Rcap;
+    h->x_RbMax = xh.RbMax;
+    h->x_nrows = xh.nrows;
+    h->x_entries = xh.nent;
+    h->x_part_rows = xh.part_rows;
+    h->x_smem_tile = xh.smem_tile;
+    h->bytes_res = (int64_t)(xh.blob.size() + xh.iqn.size() * 4 + xh.tiles.size() * sizeof(ResTile) + xh.cta_ptr.size() * 4);
+    if (h->host_only) {
+        h->rhost = std::move(xh);
+        return EPHC_OK;
+    }
+    if (!h->res_ok) return EPHC_OK;
+    int64_t bx = 0;
+    rc = upload(&h->dx_blob, xh.blob, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_iqn, xh.iqn, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_tiles, xh.tiles, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_cta_ptr, xh.cta_ptr, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_row_state, xh.row_state, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_state_row, xh.state_row, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_state_blk, xh.state_blk, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_blk_row0, xh.blk_row0, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_blk_ent_ptr, xh.blk_ent_ptr, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_blk_ent_off, xh.blk_ent_off, &bx);
+    if (rc == EPHC_OK) rc = upload(&h->dx_slot_off, xh.slot_off, &bx);
+    if (rc == EPHC_OK && cudaMalloc((void **)&h->dx_part, (size_t)std::max<int64_t>(1, xh.part_rows) * 8) != cudaSuccess)
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (resident-tile partial sums) failed");
+    if (rc == EPHC_OK && (cudaMalloc((void **)&h->dx_fc, ((size_t)xh.nrows + 4) * 8) != cudaSuccess ||
+                          cudaMemset(h->dx_fc, 0, ((size_t)xh.nrows + 4) * 8) != cudaSuccess))
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (compact f) failed");
+    if (rc != EPHC_OK) h->res_ok = false;
+    return rc;
+}
+
+// Automatic choice for collision / RK stages (measured on B200): the two-sided gather store while
+// it stays resident in the 126 MB L2; beyond that the resident-tile store when a (k,k') pair carries many channels
+// (large cells: 4.99e7 channels, nb = 16, nnu = 36: 343 us vs 597 us on the stream store) and the stream store
+// otherwise (1.26e7 channels, nb = 4: 126 us vs 134 us; 1.94e8 channels, nb = 1: 2.44 ms vs 4.2 ms).
+static int auto_coll_variant(const ephc_handle *h) {
+    if (h->g_entries * 12 <= (int64_t)96 << 20) return 0;
+    const double per_pair = (double)h->can.nw / (double)std::max<int64_t>(1, h->can.npair_active);
+    return per_pair >= 64.0 ? 3 : 2;
+}
+
 extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
     if (out) *out = nullptr;
     if (!p || !out) return fail(EPHC_EINVAL, "null argument");
@@ -175,6 +374,17 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
     h->d.ns = ns;
     h->d.C = 2.0 * kPi / (kHbar * (double)nq);  // R-8: N_q = points of the full grid
     h->host_only = (p->flags & EPHC_HOST_ONLY) != 0;
+    if (!h->host_only) {
+        // the handle belongs to the device that is current now; every later call makes it current again
+        int dev_count = 0;
+        cudaDeviceProp prop;
+        if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0 || cudaGetDevice(&h->device) != cudaSuccess ||
+            cudaGetDeviceProperties(&prop, h->device) != cudaSuccess) {
+            delete h;
+            return fail(EPHC_ECUDA, "no CUDA device (pass EPHC_HOST_ONLY to build without one)");
+        }
+        h->n_sm = prop.multiProcessorCount;
+    }
 
     std::string err;
     int rc = build_canonical(p, h->d, h->can, err);
@@ -184,95 +394,25 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         delete h;
         return fail(rc, err);
     }
-    // tile store (variant 1): two CTAs per SM walk the tile sequence (transport_iter: one CTA of twice the size per SM takes two shares)
-    int n_sm = 148;
-    if (!h->host_only) {
-        int dev = 0;
-        cudaDeviceProp prop;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&prop, dev) == cudaSuccess)
-            n_sm = prop.multiProcessorCount;
-    }
-    int ncta = 2 * n_sm;
-    if (const char *e = std::getenv("EPHC_TILE_CTAS")) ncta = std::max(1, std::atoi(e));
-    TileHost &th = h->thost;
-    rc = build_tiles(p, h->d, h->can, ncta, th, err);
-    if (rc != EPHC_OK) {
+    try {
+        h->E.assign(p->E, p->E + ns);
+        h->pair_ik.assign(p->pair_ik, p->pair_ik + p->npair);
+        h->pair_ikq.assign(p->pair_ikq, p->pair_ikq + p->npair);
+    } catch (const std::bad_alloc &) {
         delete h;
-        return fail(rc, err);
+        return fail(EPHC_ENOMEM, "host allocation failed (handle)");
     }
-    h->tile_ok = th.supported;
-    if (th.supported) {
-        h->t_entries = (int64_t)th.w.size();
-        h->t_pieces = th.npiece;
-        h->t_part_rows = th.part_rows;
-        h->t_ncta = th.ncta;
-        h->t_Ra = th.Ra;
-        h->t_Rb = th.Rb;
-        h->t_nblk = th.nblk;
-        h->t_nslot = (int32_t)th.slot_off.size();
-        h->t_ntile = (int32_t)th.tiles.size();
-        h->bytes_tile = (int64_t)(th.w.size() * 8 + th.code.size() * 2 + th.prec.size() * 4 +
-                                  th.slices.size() * sizeof(TileSlice) + th.tiles.size() * sizeof(TileHdr) +
-                                  th.ctas.size() * sizeof(TileCta) + th.slot_off.size() * 8 +
-                                  (th.blk_row0.size() + th.row_state.size() + th.state_row.size() +
-                                   th.state_blk.size() + th.blk_ent_ptr.size()) * 4 + th.blk_ent_off.size() * 8);
-    }
-    // stream store (variant 2): two CTAs of 512 threads per SM
-    StreamHost sh;
-    if (std::getenv("EPHC_NO_STREAM") == nullptr) {
-        int nshare = 2 * n_sm;
-        if (const char *e = std::getenv("EPHC_STREAM_CTAS")) nshare = std::max(1, std::atoi(e));
-        rc = build_stream(p, h->d, h->can, nshare, sh, err);
-        if (rc != EPHC_OK) {
-            delete h;
-            return fail(rc, err);
-        }
-        h->stream_ok = sh.supported && stream_smem_bytes(sh.Ra, sh.Rb) <= 220 * 1024;
-        h->stream_why = sh.why;
-        h->s_ncta = sh.ncta;
-        h->s_Ra = sh.Ra;
-        h->s_Rb = sh.Rb;
-        h->s_ntile = (int32_t)sh.tiles.size();
-        h->s_entries = (int64_t)sh.w.size();
-        h->s_part_rows = sh.part_rows;
-        h->bytes_stream = (int64_t)(sh.w.size() * 8 + sh.code.size() * 4 + sh.perm.size() * 2 +
-                                    (sh.arow_id.size() + sh.brow_id.size()) * 4 + sh.iq.size() * 4 +
-                                    sh.chunks.size() * sizeof(StreamChunk) + sh.tiles.size() * sizeof(StreamTile));
-        sh.perm.resize(sh.perm.size() + 8, 0);  // the staging copies read whole 8-byte pieces
-        if (h->host_only) h->shost = sh;
-    }
-    // resident-tile store (variant 3): one persistent CTA per SM with two tile buffers in shared memory
-    ResHost xh;
-    if (std::getenv("EPHC_NO_RES") == nullptr) {
-        int nshare = kResCtasPerSm * n_sm;
-        if (const char *e = std::getenv("EPHC_RES_CTAS")) nshare = std::max(1, std::atoi(e));
-        int64_t cap = kResSmemCap;
-        if (const char *e = std::getenv("EPHC_RES_SMEM")) cap = std::max(8192, std::atoi(e));
-        rc = build_res(p, h->d, h->can, nshare, cap, xh, err);
-        if (rc != EPHC_OK) {
-            delete h;
-            return fail(rc, err);
-        }
-        h->res_ok = xh.supported && res_smem_total(xh.Ra, xh.Rcap, xh.RbMax, xh.smem_tile) <= kResSmemCap;
-        h->res_why = xh.supported ? "shared-memory budget exceeded" : xh.why;
-        h->x_ncta = xh.ncta;
-        h->x_ntile = (int32_t)xh.tiles.size();
-        h->x_Ra = xh.Ra;
-        h->x_Rcap = xh.Rcap;
-        h->x_RbMax = xh.RbMax;
-        h->x_nrows = xh.nrows;
-        h->x_entries = xh.nent;
-        h->x_part_rows = xh.part_rows;
-        h->x_smem_tile = xh.smem_tile;
-        h->bytes_res = (int64_t)(xh.blob.size() + xh.iqn.size() * 4 + xh.tiles.size() * sizeof(ResTile) +
-                                 xh.cta_ptr.size() * 4);
-        if (h->host_only) h->rhost = xh;
-    }
-    // row store for transport_iter (one CTA of 1024 threads per SM, one strip each)
+    h->emin = p->emin;
+    h->emax = p->emax;
+    h->g_entries = (int64_t)g.code.size();
+    h->g_halfpairs = (int64_t)g.hp_k.size();
+    h->n_wu = (int32_t)g.wus.size();
+    h->n_rounds = (int32_t)g.rounds.size();
+    h->n_tasks = (int32_t)g.tasks.size();
+    // row store for transport_iter (one CTA of 1024 threads per SM, one strip each), derived from the gather store
     RowHost rh;
-    const bool want_rows = std::getenv("EPHC_NO_ROWS") == nullptr;
-    if (want_rows) {
-        int nstrip = n_sm;
+    if (std::getenv("EPHC_NO_ROWS") == nullptr) {
+        int nstrip = h->n_sm;
         if (const char *e = std::getenv("EPHC_ROW_STRIPS")) nstrip = std::max(1, std::atoi(e));
         rc = build_rows(p, h->d, g, nstrip, rh, err);
         if (rc != EPHC_OK) {
@@ -287,22 +427,10 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.perm.size() * 4 + rh.segs.size() * sizeof(RowSeg) +
                                   rh.tiles.size() * sizeof(RowTile) + rh.strips.size() * sizeof(RowStrip) +
                                   (rh.row_state.size() + rh.state_row.size()) * 4);
+        if (h->host_only) h->rowhost = rh;
     }
-    h->pair_ik.assign(p->pair_ik, p->pair_ik + p->npair);
-    h->pair_ikq.assign(p->pair_ikq, p->pair_ikq + p->npair);
-    h->g_entries = (int64_t)g.code.size();
-    h->g_halfpairs = (int64_t)g.hp_k.size();
-    h->n_wu = (int32_t)g.wus.size();
-    h->n_rounds = (int32_t)g.rounds.size();
-    h->n_tasks = (int32_t)g.tasks.size();
     h->bytes_gather = 0;
     if (!h->host_only) {
-        int dev_count = 0;
-        cudaError_t ce = cudaGetDeviceCount(&dev_count);
-        if (ce != cudaSuccess || dev_count == 0) {
-            delete h;
-            return fail(EPHC_ECUDA, "no CUDA device (pass EPHC_HOST_ONLY to build without one)");
-        }
         int64_t b = 0;
         rc = upload(&h->d_code, g.code, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_w, g.w, &b);
@@ -311,52 +439,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
         if (rc == EPHC_OK) rc = upload(&h->d_tasks, g.tasks, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_rounds, g.rounds, &b);
         if (rc == EPHC_OK) rc = upload(&h->d_wus, g.wus, &b);
-        if (rc == EPHC_OK && h->stream_ok) {
-            int64_t bs = 0;
-            rc = upload(&h->ds_w, sh.w, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_code, sh.code, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_perm, sh.perm, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_aid, sh.arow_id, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_ast, sh.arow_start, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_bid, sh.brow_id, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_bst, sh.brow_start, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_iq, sh.iq, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_chunks, sh.chunks, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_tiles, sh.tiles, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_order, sh.order, &bs);
-            if (rc == EPHC_OK && (cudaMalloc((void **)&h->ds_counter, 64) != cudaSuccess ||
-                                  cudaMemset(h->ds_counter, 0, 64) != cudaSuccess))
-                rc = fail(EPHC_ENOMEM, "cudaMalloc (tile counter) failed");
-            if (rc == EPHC_OK) rc = upload(&h->ds_row_state, sh.row_state, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_state_row, sh.state_row, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_state_blk, sh.state_blk, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_blk_row0, sh.blk_row0, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_blk_ent_ptr, sh.blk_ent_ptr, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_blk_ent_off, sh.blk_ent_off, &bs);
-            if (rc == EPHC_OK) rc = upload(&h->ds_slot_off, sh.slot_off, &bs);
-            if (rc == EPHC_OK && cudaMalloc((void **)&h->ds_part, (size_t)std::max<int64_t>(1, sh.part_rows) * 8) != cudaSuccess)
-                rc = fail(EPHC_ENOMEM, "cudaMalloc (stream partial sums) failed");
-        }
-        if (rc == EPHC_OK && h->res_ok) {
-            int64_t bx = 0;
-            rc = upload(&h->dx_blob, xh.blob, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_iqn, xh.iqn, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_tiles, xh.tiles, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_cta_ptr, xh.cta_ptr, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_row_state, xh.row_state, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_state_row, xh.state_row, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_state_blk, xh.state_blk, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_blk_row0, xh.blk_row0, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_blk_ent_ptr, xh.blk_ent_ptr, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_blk_ent_off, xh.blk_ent_off, &bx);
-            if (rc == EPHC_OK) rc = upload(&h->dx_slot_off, xh.slot_off, &bx);
-            if (rc == EPHC_OK && cudaMalloc((void **)&h->dx_part, (size_t)std::max<int64_t>(1, xh.part_rows) * 8) != cudaSuccess)
-                rc = fail(EPHC_ENOMEM, "cudaMalloc (resident-tile partial sums) failed");
-            if (rc == EPHC_OK && (cudaMalloc((void **)&h->dx_fc, ((size_t)xh.nrows + 4) * 8) != cudaSuccess ||
-                                  cudaMemset(h->dx_fc, 0, ((size_t)xh.nrows + 4) * 8) != cudaSuccess))
-                rc = fail(EPHC_ENOMEM, "cudaMalloc (compact f) failed");
-            xh = ResHost();
-        }
+        h->bytes_gather = b;
         if (rc == EPHC_OK && h->rows_ok) {
             int64_t br = 0;
             rc = upload(&h->dr_idx, rh.idx, &br);
@@ -369,43 +452,35 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
             if (rc == EPHC_OK && cudaMalloc((void **)&h->dr_Fc, ((size_t)rh.nrows * 3 + 4) * 8) != cudaSuccess)
                 rc = fail(EPHC_ENOMEM, "cudaMalloc (compact F) failed");
         }
-        if (rc == EPHC_OK && th.supported) {
-            int64_t bt = 0;
-            rc = upload(&h->dt_w, th.w, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_code, th.code, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_prec, th.prec, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_slices, th.slices, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_tiles, th.tiles, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_ctas, th.ctas, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_blk_row0, th.blk_row0, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_row_state, th.row_state, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_state_row, th.state_row, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_state_blk, th.state_blk, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_blk_ent_ptr, th.blk_ent_ptr, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_blk_ent_off, th.blk_ent_off, &bt);
-            if (rc == EPHC_OK) rc = upload(&h->dt_slot_off, th.slot_off, &bt);
-            if (rc == EPHC_OK) {
-                cudaError_t ce2 = cudaMalloc((void **)&h->dt_part, (size_t)std::max<int64_t>(1, th.part_rows) * 3 * 8);
-                if (ce2 != cudaSuccess) rc = fail(EPHC_ENOMEM, "cudaMalloc (partial sums) failed");
-            }
-            // the device owns the image now; keep only the scalars
-            TileHost empty;
-            empty.supported = th.supported;
-            empty.Ra = th.Ra; empty.Rb = th.Rb; empty.nblk = th.nblk; empty.nrows = th.nrows; empty.ncta = th.ncta;
-            empty.part_rows = th.part_rows; empty.npiece = th.npiece;
-            th = empty;
-        }
-        if (rc != EPHC_OK) {
-            free_dev(h);
-            delete h;
-            return rc;
-        }
-        h->bytes_gather = b;
+        // everything the device entry points write besides the caller's buffers is allocated here, so that they only
+        // enqueue work ("allocated once"): transport weights in gather and row order, RK4 scratch, sums
+        const size_t nb8 = (size_t)ns * 8, ne8 = (size_t)std::max<int64_t>(1, h->g_entries) * 8;
+        if (rc == EPHC_OK &&
+            (cudaMalloc((void **)&h->d_gW, ne8) != cudaSuccess || (h->rows_ok && cudaMalloc((void **)&h->dr_W, ne8) != cudaSuccess) ||
+             cudaMalloc((void **)&h->d_y[0], nb8) != cudaSuccess || cudaMalloc((void **)&h->d_y[1], nb8) != cudaSuccess ||
+             cudaMalloc((void **)&h->d_ksum, nb8) != cudaSuccess ||
+             cudaMalloc((void **)&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, (ns + 255) / 256), 1) * 8) != cudaSuccess))
+            rc = fail(EPHC_ENOMEM, "cudaMalloc (transport weights / RK4 scratch) failed");
+        if (rc == EPHC_OK) h->bytes_transport += h->g_entries * 8 * (h->rows_ok ? 2 : 1);
     } else {
-        h->ghost = g;
         h->bytes_gather = (int64_t)(g.code.size() * 4 + g.w.size() * 8 + g.hp_k.size() * 8 +
                                     g.tasks.size() * sizeof(Task) + g.rounds.size() * sizeof(Round) +
                                     g.wus.size() * sizeof(WorkUnit));
+        h->ghost = std::move(g);
+    }
+    // the once-stored store of the automatic choice (the others are built when ephc_set_variant asks for them);
+    // host-only handles build all of them for the export calls
+    if (rc == EPHC_OK) {
+        const int av = auto_coll_variant(h);
+        if (h->host_only || av == 3) rc = make_res_store(h);
+        if (rc == EPHC_OK && (h->host_only || av == 2 || (av == 3 && !h->res_ok))) rc = make_stream_store(h);
+        if (rc == EPHC_OK && (h->host_only || (av >= 2 && !h->res_ok && !h->stream_ok))) rc = make_tile_store(h);
+    }
+    if (rc != EPHC_OK) {
+        const std::string msg = g_err;
+        if (!h->host_only) free_dev(h);
+        delete h;
+        return fail(rc, msg.empty() ? err : msg);
     }
     *out = h;
     return EPHC_OK;
@@ -609,14 +684,13 @@ extern "C" int ephc_export_tiles(const ephc_handle *h, int32_t *a, int32_t *b, i
     return EPHC_OK;
 }
 
-// variant used by ephc_collision / ephc_rt_step, and by ephc_transport_setup / ephc_transport_iter
-// Automatic choice for collision / RK stages: the two-sided gather store while it stays resident in the 126 MB L2
-// (measured on B200: 5e5 channels 13 us vs 1170 us, 2.1e6 channels 34 us vs 87 us on the stream store), the once-stored
-// stream store beyond that (1.26e7 channels: 124 us vs 224 us).
+// variant used by ephc_collision / ephc_rt_step (see auto_coll_variant), and by ephc_transport_setup / ephc_transport_iter
 static inline int coll_variant(const ephc_handle *h) {
     if (h->variant >= 0) return h->variant;
-    if (h->g_entries * 12 <= (int64_t)96 << 20) return 0;
-    return h->res_ok ? 3 : (h->stream_ok ? 2 : (h->tile_ok ? 1 : 0));
+    const int av = auto_coll_variant(h);
+    if (av == 0) return 0;
+    if (av == 3 && h->res_ok) return 3;
+    return h->stream_ok ? 2 : (h->res_ok ? 3 : (h->tile_ok ? 1 : 0));
 }
 static inline int tr_variant(const ephc_handle *h) { return (h->variant < 0 || h->variant >= 2) ? 0 : h->variant; }
 
@@ -707,6 +781,56 @@ extern "C" int ephc_export_stream(const ephc_handle *h, int32_t *a, int32_t *b, 
 }
 
 extern "C" int64_t ephc_stream_entries(const ephc_handle *h) { return h ? h->s_entries : 0; }
+
+extern "C" int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *partner, int64_t *gather_pos) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (!h->host_only) return fail(EPHC_ESTATE, "ephc_export_rows needs a handle built with EPHC_HOST_ONLY");
+    if (!h->rows_ok) return fail(EPHC_ESTATE, "row store not available (EPHC_NO_ROWS or shared-memory budget)");
+    const RowHost &r = h->rowhost;
+    const int64_t nent = (int64_t)r.idx.size();
+    if (nent != h->g_entries || (int64_t)r.perm.size() != nent) return fail(EPHC_ESTATE, "internal: row store size");
+    std::vector<uint8_t> seen((size_t)nent, 0), pos_seen((size_t)nent, 0);
+    std::vector<int32_t> row_tiles;
+    int32_t next_row = 0, next_tile = 0;
+    for (size_t is = 0; is < r.strips.size(); ++is) {
+        const RowStrip &st = r.strips[is];
+        // strips partition the destination rows in order; their tiles are consecutive
+        if (st.row0 != next_row || st.nrows < 0 || st.nrows > r.Ra || st.t0 != next_tile || st.t1 < st.t0)
+            return fail(EPHC_ESTATE, "internal: row strips do not partition the rows");
+        next_row = st.row0 + st.nrows;
+        next_tile = st.t1;
+        int32_t last_col0 = -1;
+        for (int32_t it = st.t0; it < st.t1; ++it) {
+            const RowTile &tl = r.tiles[it];
+            if (tl.nseg < 1 || tl.col0 % r.Rb != 0 || tl.col0 <= last_col0 || tl.ncols < 1 || tl.ncols > r.Rb ||
+                tl.col0 + tl.ncols > r.nrows)
+                return fail(EPHC_ESTATE, "internal: bad row tile");
+            last_col0 = tl.col0;
+            row_tiles.assign((size_t)std::max(st.nrows, 1), 0);
+            uint32_t last_len = 0xffffffffu;
+            for (int32_t ig = tl.seg0; ig < tl.seg0 + tl.nseg; ++ig) {
+                const RowSeg &sg = r.segs[ig];
+                // one segment per destination row and tile, longest first
+                if (sg.len < 1 || sg.len > last_len || (int32_t)sg.row >= st.nrows || row_tiles[sg.row]++)
+                    return fail(EPHC_ESTATE, "internal: row segments must descend in length, one per row and tile");
+                last_len = sg.len;
+                for (uint32_t k = 0; k < sg.len; ++k) {
+                    const int64_t o = st.e0 + sg.start + k;
+                    if (o < 0 || o >= nent || seen[o]++) return fail(EPHC_ESTATE, "internal: row entry visited twice");
+                    const int64_t gp = r.perm[o];
+                    if (gp >= nent || pos_seen[gp]++ || r.idx[o] >= tl.ncols) return fail(EPHC_ESTATE, "internal: row entry out of range");
+                    if (dest) dest[o] = r.row_state[st.row0 + (int32_t)sg.row];
+                    if (partner) partner[o] = r.row_state[tl.col0 + r.idx[o]];
+                    if (gather_pos) gather_pos[o] = gp;
+                }
+            }
+        }
+    }
+    if (next_row != r.nrows || next_tile != (int32_t)r.tiles.size()) return fail(EPHC_ESTATE, "internal: rows or tiles left over");
+    for (uint8_t v : seen)
+        if (!v) return fail(EPHC_ESTATE, "internal: row entry not covered by any segment");
+    return EPHC_OK;
+}
 
 extern "C" int64_t ephc_res_entries(const ephc_handle *h) { return (h && h->res_ok) ? h->x_entries : 0; }
 
@@ -871,6 +995,13 @@ extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
     if (variant < -1 || variant > 3)
         return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather), 1 (tiles), 2 (stream) or 3 (resident tiles)");
+    // a store that the automatic choice did not need is built (and uploaded) now: this call may allocate and copy
+    if (!h->host_only && variant >= 1) CUDA_TRY(cudaSetDevice(h->device));
+    int rc = EPHC_OK;
+    if (variant == 3) rc = make_res_store(h);
+    if (variant == 2) rc = make_stream_store(h);
+    if (variant == 1) rc = make_tile_store(h);
+    if (rc != EPHC_OK) return rc;
     if (variant == 3 && !h->res_ok)
         return fail(EPHC_ESTATE, "resident-tile store not available for this problem: " + h->res_why);
     if (variant == 2 && !h->stream_ok)
@@ -887,43 +1018,41 @@ extern "C" int ephc_get_transport_variant(const ephc_handle *h) { return h ? tr_
 extern "C" int64_t ephc_launch_count(const ephc_handle *h) { return h ? h->launches : 0; }
 
 // ------------------------------------------------------------------------------------------------------------
+// The dynamic shared-memory limit belongs to the kernel, not to a handle: it is raised once per device to a size that
+// covers every geometry the builders can produce (they keep each kernel's request below these caps).
+static int set_kernel_attributes(int device) {
+    static bool done[64] = {false};
+    if (device >= 0 && device < 64 && done[device]) return EPHC_OK;
+    const int big = 220 * 1024;
+    CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kCollision>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)gather_smem_bytes(kCollision)));
+    CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kRkStage>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)gather_smem_bytes(kRkStage)));
+    CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportSetup>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)gather_smem_bytes(kTransportSetup)));
+    CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)gather_smem_bytes(kTransportIter)));
+    CUDA_TRY(cudaFuncSetAttribute(stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<kResLanes>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResSmemCap));
+    CUDA_TRY(cudaFuncSetAttribute(row_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+#define EPHC_TILE_ATTR(NB_)                                                                                          \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)); \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTSetup, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));     \
+    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTIter, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    EPHC_TILE_ATTR(1)
+    EPHC_TILE_ATTR(2)
+    EPHC_TILE_ATTR(4)
+#undef EPHC_TILE_ATTR
+    if (device >= 0 && device < 64) done[device] = true;
+    return EPHC_OK;
+}
+
 static int need_device(ephc_handle *h) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
     if (h->host_only) return fail(EPHC_ESTATE, "handle was built with EPHC_HOST_ONLY: no device store");
-    if (!h->attrs_set) {
-        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kCollision>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)gather_smem_bytes(kCollision)));
-        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kRkStage>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)gather_smem_bytes(kRkStage)));
-        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportSetup>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)gather_smem_bytes(kTransportSetup)));
-        CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)gather_smem_bytes(kTransportIter)));
-        if (h->stream_ok)
-            CUDA_TRY(cudaFuncSetAttribute(stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)stream_smem_bytes(h->s_Ra, h->s_Rb)));
-        if (h->res_ok)
-            CUDA_TRY(cudaFuncSetAttribute(res_kernel<kResLanes>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)kResSmemCap));
-        if (h->rows_ok)
-            CUDA_TRY(cudaFuncSetAttribute(row_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)row_smem_bytes(h->r_Rb, h->r_Ra)));
-        if (h->tile_ok) {
-#define EPHC_TILE_ATTR(NB_)                                                                                       \
-    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
-                                  (int)tile_smem_bytes(kTCollision, h->t_Ra, h->t_Rb)));                            \
-    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTSetup, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,           \
-                                  (int)tile_smem_bytes(kTSetup, h->t_Ra, h->t_Rb)));                                \
-    CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTIter, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,            \
-                                  (int)tile_smem_bytes(kTIter, h->t_Ra, h->t_Rb)));
-            EPHC_TILE_ATTR(1)
-            EPHC_TILE_ATTR(2)
-            EPHC_TILE_ATTR(4)
-#undef EPHC_TILE_ATTR
-        }
-        h->attrs_set = true;
-    }
-    return EPHC_OK;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != h->device) CUDA_TRY(cudaSetDevice(h->device));
+    return set_kernel_attributes(h->device);
 }
 
 static TileParams tile_params(const ephc_handle *h) {
@@ -1188,11 +1317,6 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
     if (rc) return rc;
     if (!f0_dev || !N_dev || !Gamma_dev) return fail(EPHC_EINVAL, "null device pointer");
     if (tr_variant(h) == 1) {
-        if (!h->dt_Wf) {
-            if ((rc = ensure(&h->dt_Wf, (size_t)h->t_entries * 8)) || (rc = ensure(&h->dt_Wr, (size_t)h->t_entries * 8)))
-                return rc;
-            h->bytes_transport += h->t_entries * 16;
-        }
         TileParams T = tile_params(h);
         T.f = f0_dev;
         T.N = N_dev;
@@ -1206,11 +1330,6 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
         }
         return rc;
     }
-    if (!h->d_gW) {
-        rc = ensure(&h->d_gW, (size_t)h->g_entries * 8);
-        if (rc) return rc;
-        h->bytes_transport += h->g_entries * 8;
-    }
     GatherParams P = base_params(h);
     P.f = f0_dev;
     P.N = N_dev;
@@ -1218,10 +1337,6 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
     rc = launch_gather<kTransportSetup>(h, P, (cudaStream_t)stream);
     if (rc == EPHC_OK && h->rows_ok && h->g_entries > 0) {
         // the iteration runs on the row store: same ordered terms, regrouped; bring the weights into its order
-        if (!h->dr_W) {
-            if ((rc = ensure(&h->dr_W, (size_t)h->g_entries * 8))) return rc;
-            h->bytes_transport += h->g_entries * 8;
-        }
         row_permute_kernel<<<(unsigned)((h->g_entries + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
             h->d_gW, h->dr_perm, h->dr_W, h->g_entries);
         h->launches++;
@@ -1307,10 +1422,6 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
     if (rc) return rc;
     if (!f_dev || !N_dev) return fail(EPHC_EINVAL, "null device pointer");
     if (nsteps < 0 || !std::isfinite(dt_fs)) return fail(EPHC_EINVAL, "nsteps >= 0 and finite dt required");
-    const size_t nb8 = (size_t)h->d.ns * 8;
-    if ((rc = ensure(&h->d_y[0], nb8)) || (rc = ensure(&h->d_y[1], nb8)) || (rc = ensure(&h->d_ksum, nb8)) ||
-        (rc = ensure(&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, finish_grid(h)), 1) * 8)))
-        return rc;
     cudaStream_t s = (cudaStream_t)stream;
     if (sumf_dev) {
         sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev);

@@ -240,6 +240,24 @@ def test_res_store_holds_every_weight_once(prob, rows, fine, smem, lp, lg, monke
     assert np.abs(I - Io).max() <= 1e-12 * np.abs(Io).max()
 
 
+@pytest.mark.parametrize("rng_rows,strips", [(None, None), (32, 1), (64, 3), (32, 40)])
+def test_row_store_is_a_regrouping_of_the_gather_store(prob, rng_rows, strips, monkeypatch):
+    # the store transport_iter runs on: same ordered terms as the gather store (dest, partner), every gather position
+    # exactly once; strips / tiles / segments checked in C (ephc_export_rows)
+    if rng_rows is not None:
+        monkeypatch.setenv("EPHC_ROW_RANGE", str(rng_rows))
+        monkeypatch.setenv("EPHC_ROW_STRIPS", str(strips))
+    h = ephc.build_channels(prob, flags=ephc.HOST_ONLY)
+    g, r = h.export_gather(), h.export_rows()
+    assert len(r["dest"]) == len(g["dest"]) > 0
+    assert np.array_equal(np.sort(r["gather_pos"]), np.arange(len(g["dest"])))
+    assert np.array_equal(g["dest"][r["gather_pos"]], r["dest"])
+    assert np.array_equal(g["partner"][r["gather_pos"]], r["partner"])
+    # destination-sorted at strip granularity: the destinations of the store are non-decreasing across strips
+    inside = (prob.E.reshape(-1) >= prob.emin) & (prob.E.reshape(-1) <= prob.emax)
+    assert inside[r["dest"]].all() and inside[r["partner"]].all()
+
+
 def test_launch_geometry_limits():
     # a segment with more half-pairs than one round can stage (tiny 8x8x8: 512 partners per k, 5 doubles each)
     # and a dense many-band block: both must split into rounds/tasks within the kernel's limits

@@ -64,6 +64,27 @@ def test_sampled_definition_equals_list(small_win, tiny):
         assert np.abs(Is - IB[st]).max() <= 1e-13 * np.abs(IB).max()
 
 
+def test_threaded_collision_equals_serial(tiny, small_win):
+    # orc_collision_omp (the paper's Baseline-CPU shape: OpenMP over the list, atomic updates) is only
+    # used to time the oracle on all host cores; it is pinned to the serial loop, which P0-P5 pin: same terms,
+    # any order, so the two agree within 1e-13 of the sum of |T| that reaches a state
+    rng = np.random.default_rng(17)
+    for p, L in (tiny, small_win):
+        for f, N in ((p.f, p.N), (rng.uniform(0, 1, p.ns), rng.uniform(0, 3, p.nq * p.nnu))):
+            I1, I2 = L.collision(f, N), L.collision(f, N, omp=True)
+            ch = L.export()
+            fa, fb = f[ch["ik"] * p.nb + ch["n"]], f[ch["ikq"] * p.nb + ch["m"]]
+            Nq = N[ch["iq"].astype(np.int64) * p.nnu + ch["nu"]]
+            out_, in_ = fa * (1 - fb), fb * (1 - fa)
+            absT = np.abs(ch["w_abs"] * (out_ * Nq - in_ * (Nq + 1))) + np.abs(ch["w_em"] * (out_ * (Nq + 1) - in_ * Nq))
+            bound = np.zeros(p.ns)
+            np.add.at(bound, ch["ik"] * p.nb + ch["n"], absT)
+            np.add.at(bound, ch["ikq"] * p.nb + ch["m"], absT)
+            assert np.abs(I1).max() > 0
+            assert np.all(np.abs(I1 - I2) <= 1e-13 * bound + 1e-300)
+            assert abs(I2.sum()) <= 1e-13 * absT.sum()
+
+
 def test_canonical_list_structure(tiny):
     p, L = tiny
     ch = L.export()
