@@ -1,17 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- channel-terms/s of the e-ph collision-integral hot path on B200 (BASELINE.json metric).
 
-One "step" = one pass of the whole hot path over the Si-like transport workload
-(BASELINE.json configs[1]; configs[4] is the same channel set):
+One "step" = one pass of the whole hot path over one workload.  The headline line is
+quoted on the largest single-GPU config (gaas, BASELINE.json configs[2], 1.9e8 channels); the Si-like transport
+config (configs[1]; configs[4] is the same channel set), the large-cell config and the tiny config are timed in
+shorter runs and reported under `per_config`:
     1 collision evaluation + 1 transport_setup + 20 transport iterations (3 Cartesian components)
     + 1 RK4 rt-BTE step (4 collision evaluations with fused axpy) + the conservation scalar
   = 26 channel-loop evaluations; channel-terms per step = 26 * N_ch (N_ch = unordered active channels).
 
 `value`     device-resident: inputs in HBM before the timed region, CUDA events on the launching stream.
 `e2e`       the same step through the *_host entry points of the C ABI: pinned host buffers, H2D/D2H inside.
-`roofline`  for the kernel with the largest share of the step: algorithmic bytes per launch (DESIGN.md
-            "Roofline") / mean launch duration measured here with CUDA events, vs MEASURED_PEAKS.json.
-`cpu_baseline`  the CPU oracle (oracle/, as it stands, serial) on a bounded sample of the same workload.
+`roofline`  for the COLLISION call (the kernel north_star's target names): algorithmic bytes per launch (DESIGN.md
+            "Roofline") / mean launch duration measured here with CUDA events, vs MEASURED_PEAKS.json; `kernels`
+            holds the same figures for every call; `collision_channel_terms_per_s` is the collision call alone.
+`cpu_baseline`  the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload: serial, and
+            (`all_cores`) the paper's Baseline-CPU shape, OpenMP over the channel list with atomic updates.
 
 --impl reference  times the oracle instead (rank 0 only).  N > 1: independent replicas, one per GPU, seeds
 differ per rank ("weak"); k-sharding with an all-gather of f is DESIGN.md's NEXT-1.
@@ -44,12 +48,15 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="si", help="workload: si (default, BASELINE configs[1]) | tiny | gaas | bigcell")
+    ap.add_argument("--config", default="gaas",
+                    help="workload: gaas (default: the largest single-GPU config, BASELINE configs[2]) | si | bigcell | tiny")
     ap.add_argument("--grid", type=int, default=0, help="override the grid edge (smaller copies for quick runs)")
     ap.add_argument("--pair-prob", type=float, default=0.0)
-    ap.add_argument("--variant", type=int, default=-1, help="-1: automatic (library default), 0: gather, 1: tiles, 2: stream")
+    ap.add_argument("--variant", type=int, default=-1,
+                    help="-1: automatic (library default), 0: gather, 1: tiles, 2: stream, 3: resident tiles")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other configs")
     return ap.parse_args()
 
 
@@ -144,18 +151,20 @@ def run_reference(args):
     import oracle
     p = make_workload(args)
     L = oracle.OracleList(p)
-    # bounded sample per step: collision + setup + 2 transport iterations + 1 RK4 step = 8 evaluations
-    n_iters, n_rt = 2, 1
+    # bounded sample per step, sized so that the run ends within minutes: collision + setup + n_iters transport
+    # iterations + n_rt RK4 steps; the rate is per evaluation, so the sample stands for the whole step
+    n_iters, n_rt = (2, 1) if L.nch < 5e7 else (1, 0)
     for _ in range(max(args.warmup, 0)):
-        oracle_step(L, p, 0, 0)
+        oracle_step(L, p, 0, 0) if L.nch < 5e7 else L.collision(p.f, p.N)
     t0 = time.perf_counter()
     evals = 0
     for _ in range(args.steps):
         evals += oracle_step(L, p, n_iters, n_rt)
     dt = time.perf_counter() - t0
     val = L.nch * evals / dt
-    sample = (f"per step: 1 collision + 1 transport_setup + {n_iters} transport iterations + {n_rt} RK4 step "
-              f"({evals // max(args.steps, 1)} of the {EVALS_PER_STEP} evaluations of a full step), full channel set")
+    sample = (f"per step: 1 collision + 1 transport_setup + {n_iters} transport iterations + {n_rt} RK4 steps "
+              f"({evals // max(args.steps, 1)} of the {EVALS_PER_STEP} evaluations of a full step; the rate per evaluation is "
+              f"extrapolated to the step), full channel set, serial C")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
@@ -187,31 +196,21 @@ def workload_config(args, p, nch):
             "seed": int(p.seed)}
 
 
-def main():
-    args = parse()
-    if args.impl == "reference":
-        return run_reference(args)
-
-    import torch
-    import paper_2511_03683_b200 as ephc
-
+def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, with_e2e, with_cpu, sampler=None, with_paper=True):
+    """Builds one workload and times `steps` steps of the whole hot path on it.  Returns a dict of results."""
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    p = make_workload(args, seed_offset=rank)       # replicas: an independent problem per rank
+    a2 = argparse.Namespace(**vars(args))
+    a2.config = config_name
+    t0 = time.perf_counter()
+    p = make_workload(a2, seed_offset=rank)       # replicas: an independent problem per rank
+    t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
     h = ephc.build_channels(p)
     t_build = time.perf_counter() - t0
@@ -220,7 +219,6 @@ def main():
     variant, tvariant = h.get_variant(), h.get_transport_variant()
     q = h.query()
     nch, ns = q["nch"], p.ns
-    dev = torch.device("cuda", local)
 
     def d(x):
         return torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64).reshape(-1), device=dev)
@@ -236,7 +234,7 @@ def main():
     stream = torch.cuda.current_stream()
 
     def step(ev=None):
-        """ev: list collecting (label, start_event, end_event) per phase."""
+        """ev: list collecting the events that bracket the phases."""
         def mark():
             e = torch.cuda.Event(enable_timing=True)
             e.record(stream)
@@ -258,71 +256,80 @@ def main():
         if ev is not None:
             ev.append((e0, e1, e2, e3, e4, e5))
 
-    for _ in range(max(args.warmup, 0)):
+    for _ in range(max(warmup, 0)):
         step()
     barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
+    if sampler is not None:
         sampler.start()
     l0 = h.launch_count()
     ev = []
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     start.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step(ev)
     stop.record(stream)
     barrier()
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop() if sampler is not None else None
     launches = h.launch_count() - l0
     ms_total, nch_all = reduce_over_ranks(dist, dev, start.elapsed_time(stop), nch)
-    value = nch_all * EVALS_PER_STEP * args.steps / (ms_total * 1e-3)
+    value = nch_all * EVALS_PER_STEP * steps / (ms_total * 1e-3)
 
     # per-phase device times (this rank)
     ph = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(5)] for e in ev]) if ev else np.zeros((1, 5))
     ms_coll, ms_setup, ms_tau, ms_iter, ms_rt = ph.mean(axis=0)
     peak, peak_src = peaks()
     kern = {}
+    traffic = load_traffic(p.name)
 
-    def roof(name, ms_launch, alg_bytes, share):
+    def roof(call, kernels, ms_launch, alg_bytes, share):
         gbs = alg_bytes / (ms_launch * 1e-3) / 1e9 if ms_launch > 0 else 0.0
-        kern[name] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
-                      "traffic": None, "alg_bytes_per_launch": int(alg_bytes), "us_per_launch": 1e3 * ms_launch,
-                      "share_of_step": share, "channel_terms_per_s": nch / (ms_launch * 1e-3) if ms_launch > 0 else 0.0}
+        tr = traffic.get(call)
+        kern[f"{call} ({kernels})"] = {
+            "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+            "traffic": tr["bytes"] if tr else None, "traffic_source": tr["source"] if tr else None,
+            "alg_bytes_per_launch": int(alg_bytes), "us_per_launch": 1e3 * ms_launch, "share_of_step": share,
+            "channel_terms_per_s": nch / (ms_launch * 1e-3) if ms_launch > 0 else 0.0}
 
-    ms_step = ms_total / max(args.steps, 1)
-    kn = {"c": "gather_kernel<0>", "s": "gather_kernel<2> + row_permute_kernel", "r": "gather_kernel<1>",
-          "i": "row_compact_kernel + row_iter_kernel"}
-    w_setup = 8 * q["gather_entries"] + 20 * q["gather_entries"]   # write W, then permute it into row-store order
+    ms_step = ms_total / max(steps, 1)
+    cname = {0: "gather_kernel<0>", 1: "tile_kernel<0> + finish_kernel<0>", 2: "stream_kernel + finish_kernel<0>",
+             3: "res_compact_kernel + res_kernel + finish_kernel<0>"}[variant]
+    rname = {0: "gather_kernel<1>", 1: "tile_kernel<0> + finish_kernel<1>", 2: "stream_kernel + finish_kernel<1>",
+             3: "res_compact_kernel + res_kernel + finish_kernel<1>"}[variant]
+    sname, iname = "gather_kernel<2> + row_permute_kernel", "row_compact_kernel + row_iter_kernel"
     if os.environ.get("EPHC_NO_ROWS"):
-        kn.update({"s": "gather_kernel<2>", "i": "gather_kernel<3>"})
-        w_setup = 8 * q["gather_entries"]
-    if variant == 1:
-        kn.update({"c": "tile_kernel<0> + finish_kernel<0>", "r": "tile_kernel<0> + finish_kernel<1>"})
-    if variant == 2:
-        kn.update({"c": "stream_kernel + finish_kernel<0>", "r": "stream_kernel + finish_kernel<1>"})
+        sname, iname = "gather_kernel<2>", "gather_kernel<3>"
     if tvariant == 1:
-        kn.update({"s": "tile_kernel<2> + finish_kernel<2>", "i": "tile_kernel<3> + finish_kernel<3>"})
-        w_setup = 16 * q["scatter_entries"]
-    roof(f"collision ({kn['c']})", ms_coll, q["alg_bytes_collision"], ms_coll / ms_step)
-    roof(f"transport_setup ({kn['s']})", ms_setup, q["alg_bytes_collision"] + w_setup, ms_setup / ms_step)
-    roof(f"transport_iter ({kn['i']})", ms_iter / N_TRANSPORT_ITERS, q["alg_bytes_transport"], ms_iter / ms_step)
+        sname, iname = "tile_kernel<2> + finish_kernel<2>", "tile_kernel<3> + finish_kernel<3>"
+    roof("collision", cname, ms_coll, q["alg_bytes_collision"], ms_coll / ms_step)
+    # the collision bytes plus the 16 bytes of weights per channel that the setup produces
+    roof("transport_setup", sname, ms_setup, q["alg_bytes_collision"] + 16 * nch, ms_setup / ms_step)
+    roof("transport_iter", iname, ms_iter / N_TRANSPORT_ITERS, q["alg_bytes_transport"], ms_iter / ms_step)
     # an RK stage moves the collision bytes plus the fused axpy vectors (f0, ksum r/w, ynext): 32 B per state
-    roof(f"rk4 stage ({kn['r']})", ms_rt / 4, q["alg_bytes_collision"] + 32 * ns, ms_rt / ms_step)
-    dominant = max(kern, key=lambda k: kern[k]["share_of_step"])
-    roofline = dict(kern[dominant], kernel=dominant, peak_source=peak_src)
-    traffic_path = os.path.join(ROOT, "profiles", "traffic.csv")        # dram bytes per launch from the ncu captures
-    if os.path.exists(traffic_path):
-        import csv
-        with open(traffic_path, newline="") as fh:
-            tr = {row["call"]: int(row["dram_bytes_per_launch"]) for row in csv.DictReader(fh)}
-        for k in kern:
-            kern[k]["traffic"] = tr.get(k)
-        roofline["traffic"] = tr.get(dominant)
+    roof("rk4 stage", rname, ms_rt / 4, q["alg_bytes_collision"] + 32 * ns, ms_rt / ms_step)
+    coll_key = next(k for k in kern if k.startswith("collision"))
+    roofline = dict(kern[coll_key], kernel=coll_key, peak_source=peak_src)
+    # A/B on the same GPU: the paper's own layout and two-step algorithm as variant 4
+    if with_paper:
+        h.set_variant(4)
+        for _ in range(3):
+            h.collision(f, N, I, stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(10):
+            h.collision(f, N, I, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms_paper = e0.elapsed_time(e1) / 10
+        roof("paper-layout collision", "paper_step2_kernel + paper_step3_kernel", ms_paper, q["alg_bytes_collision"], 0.0)
+        kern[next(k for k in kern if k.startswith("paper-layout"))]["note"] = (
+            "not part of the step: PAPER.md:84-102 as two plain kernels on the same problem, for comparison; its own layout moves "
+            "about %.0f B per channel" % ((24 * q["nw"] + 8 * q["nw"] * 2 + 8 * q["nw"] * 2) / max(nch, 1)))
+        h.set_variant(args.variant)
 
     # ---- end to end: the same step through host buffers ------------------------------------------------
     e2e = None
-    if not args.no_e2e:
+    if with_e2e:
         pin = lambda x: torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64).reshape(-1)).pin_memory()
         hf, hf0, hN, hv = pin(p.f), pin(p.f0), pin(p.N), pin(p.v)
         hI, hF, hG = pin(np.zeros(ns)), pin(np.zeros(3 * ns)), pin(np.zeros(ns))
@@ -334,11 +341,11 @@ def main():
             h.rt_step_host(hfrt, hN, 1.0, 1, hs)
         h2d = 8 * (ns + p.nq * p.nnu) + 8 * (ns + p.nq * p.nnu + 3 * ns) + 8 * (ns + p.nq * p.nnu)
         d2h = 8 * ns + 8 * (3 * ns + ns) + 8 * (ns + 2)
-        for _ in range(max(args.warmup, 0)):
+        for _ in range(max(warmup, 0)):
             step_host()
         barrier()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(steps):
             step_host()
         barrier()
         dt = time.perf_counter() - t0
@@ -346,38 +353,106 @@ def main():
             t = torch.tensor([dt], device=dev, dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
-        e2e = {"value": nch_all * EVALS_PER_STEP * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt / max(args.steps, 1)}
+        e2e = {"value": nch_all * EVALS_PER_STEP * steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt / max(steps, 1)}
 
-    # ---- CPU oracle on a bounded sample (rank 0, N = 1 only) -----------------------------------------------
+    # ---- CPU oracle on a bounded sample (rank 0, N = 1 only): serial, and the paper's Baseline-CPU shape on all cores --
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if with_cpu:
         import oracle
         L = oracle.OracleList(p)
         assert L.nch == nch, "oracle and library disagree on the channel count"
+        n_it = 4 if nch < 5e7 else 1
         t0 = time.perf_counter()
-        evals = oracle_step(L, p, 4, 1)
+        evals = oracle_step(L, p, n_it, 1)
         dt = time.perf_counter() - t0
+        ncore = oracle.threads()
+        L.collision(p.f, p.N, omp=True)
+        t1 = time.perf_counter()
+        nomp = 3
+        for _ in range(nomp):
+            L.collision(p.f, p.N, omp=True)
+        dto = time.perf_counter() - t1
         cpu = {"value": L.nch * evals / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"one pass: 1 collision + 1 transport_setup + 4 transport iterations + 1 RK4 step = {evals} of the "
+               "sample": f"one pass: 1 collision + 1 transport_setup + {n_it} transport iterations + 1 RK4 step = {evals} of the "
                          f"{EVALS_PER_STEP} evaluations of a step, full channel set ({dt:.1f} s, serial C, gcc -O2)",
+               "all_cores": {"value": L.nch * nomp / dto, "unit": UNIT, "cores": int(ncore), "kind": "oracle",
+                             "sample": f"{nomp} collision evaluations, OpenMP over the channel list with atomic updates "
+                                       f"(the paper's Baseline-CPU shape, PAPER.md:74), {dto:.1f} s"},
                "host_cores_available": os.cpu_count()}
+        del L
 
+    cfg = workload_config(a2, p, nch)
+    sb = {0: q["store_bytes_gather"], 1: q["store_bytes_scatter"], 2: q["store_bytes_scatter"], 3: q["store_bytes_scatter"]}[variant]
+    if variant != 0 and tvariant == 0:
+        sb += q["store_bytes_gather"]
+    names = {0: "gather", 1: "tiles", 2: "stream", 3: "resident tiles"}
+    tname = names[tvariant] if (tvariant == 1 or os.environ.get("EPHC_NO_ROWS")) else "rows (setup on gather)"
+    coll_mb = (q["store_bytes_scatter"] if variant else q["store_bytes_gather"]) / 1e6
+    l2 = ("no flush: every collision evaluation streams its %.0f MB store, larger than the 126 MB L2" % coll_mb
+          if coll_mb > 126 else "no flush: the %.0f MB collision store FITS the 126 MB L2 (L2-resident after warm-up; the roofline fraction is not an HBM figure)" % coll_mb)
+    cfg.update({"variant": f"collision/rt: {names[variant]}, transport: {tname}", "l2": l2,
+                "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (one problem per GPU, no data-path collective)",
+                "generate_s": t_gen, "build_channels_s": t_build, "store_bytes": sb + q["store_bytes_transport"],
+                "store_bytes_per_channel": (sb + q["store_bytes_transport"]) / max(nch, 1)})
+    h.close()
+    return {"value": value, "ms_per_step": ms_step, "config": cfg, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline, "kernels": kern, "cpu_baseline": cpu,
+            "collision_channel_terms_per_s": nch_all / (ms_coll * 1e-3) if ms_coll > 0 else 0.0}
+
+
+def load_traffic(config_name):
+    """DRAM bytes per launch from the committed `ncu --set full` captures (cold caches: ncu flushes them per kernel)."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    out = {}
+    if os.path.exists(path):
+        import csv
+        with open(path, newline="") as fh:
+            for row in csv.DictReader(fh):
+                if row.get("config") == config_name:
+                    out[row["call"]] = {"bytes": int(row["dram_bytes_per_launch"]),
+                                        "source": f"ncu --set full, cold caches, build {row.get('build', '?')} ({row.get('capture', '')})"}
+    return out
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2511_03683_b200 as ephc
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    main_res = measure(args, ephc, torch, args.config, args.steps, args.warmup, rank, local, dist,
+                       with_e2e=not args.no_e2e, with_cpu=(rank == 0 and world == 1 and not args.no_cpu_baseline), sampler=sampler)
+    # the other BASELINE.json configs, shorter runs, device-resident only (parity is the tests' job)
+    per_config = {}
+    if world == 1 and not args.no_per_config and not args.grid:
+        for name in ("si", "bigcell", "tiny"):
+            if name == args.config:
+                continue
+            r = measure(args, ephc, torch, name, max(3, args.steps // 2), 3, rank, local, None, with_e2e=False, with_cpu=False)
+            per_config[name] = {k: r[k] for k in ("value", "ms_per_step", "collision_channel_terms_per_s", "config", "kernels")}
+            per_config[name]["unit"] = UNIT
     if rank == 0:
-        cfg = workload_config(args, p, nch)
-        sb = (q["store_bytes_scatter"] if (variant in (1, 2) or tvariant == 1) else 0) + (q["store_bytes_gather"] if 0 in (variant, tvariant) else 0)
-        names = {0: "gather", 1: "tiles", 2: "stream"}
-        tname = names[tvariant] if (tvariant == 1 or os.environ.get("EPHC_NO_ROWS")) else "rows (setup on gather)"
-        cfg.update({"variant": f"collision/rt: {names[variant]}, transport: {tname}",
-                    "l2": f"no flush: every evaluation streams the {sb / 1e6:.0f} MB store "
-                          f"(+{q['store_bytes_transport'] / 1e6:.0f} MB transport weights), larger than the 126 MB L2",
-                    "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (one problem per GPU)",
-                    "build_channels_s": t_build, "store_bytes": sb + q["store_bytes_transport"]})
-        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-               "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-               "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg, "e2e": e2e,
-               "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "kernels": kern,
-               "cpu_baseline": cpu}
+        out = {"metric": METRIC, "value": main_res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": main_res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+               "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": main_res["config"], "e2e": main_res["e2e"],
+               "gpu_launches": main_res["gpu_launches"], "clocks": main_res["clocks"], "roofline": main_res["roofline"],
+               "collision_channel_terms_per_s": main_res["collision_channel_terms_per_s"],
+               "kernels": main_res["kernels"], "cpu_baseline": main_res["cpu_baseline"], "per_config": per_config}
         print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

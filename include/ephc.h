@@ -103,6 +103,7 @@ typedef struct ephc_counts {
     int64_t alg_bytes_transport;  /* B_alg of one transport iteration */
     int32_t n_workunits, n_rounds, n_tasks; /* launch geometry of the gather kernels */
     int32_t reserved;
+    int64_t store_bytes_paper;    /* device bytes of the paper-layout variant incl. sc_col (0 until ephc_set_variant(h, 4)) */
 } ephc_counts;
 
 /* Channel selection + store construction ("performed only once on CPUs").
@@ -171,6 +172,10 @@ int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *partner, int6
  *                 per-entry kind), tiles whose whole image is bulk-copied (TMA) into shared memory and processed in
  *                 place: one lane per out row piece writes the terms over the weights, one lane per row gathers them.
  *                 Collision / rt only (transport calls then use the gather + row stores); any nb, nnu.
+ *   4 = paper layout: the data structure and the two GPU steps of PAPER.md:84-102 as two plain kernels (scatter /
+ *                 scatter_channels rows, step 2 writes the per-channel scratch sc_col to HBM, step 3 sums it per
+ *                 target through stargets_sources / targets).  ephc_collision only, for the A/B comparison with the
+ *                 library's own stores on the same GPU; never chosen automatically.
  *  -1 = automatic (default): ephc_collision / ephc_rt_step use the gather store while it fits the L2 cache
  *                 (<= 96 MB) and the resident-tile store beyond that; ephc_transport_setup runs on the gather store and
  *                 ephc_transport_iter on the row store built from it (the faster choice per call as measured on

@@ -42,7 +42,8 @@ class Counts(C.Structure):
         "ns", "npair_active", "nch", "nw", "ndiag", "gather_entries", "gather_halfpairs", "scatter_entries",
         "scatter_pairs", "store_bytes_gather", "store_bytes_scatter", "store_bytes_transport",
         "alg_bytes_collision", "alg_bytes_transport")] + [
-        ("n_workunits", C.c_int32), ("n_rounds", C.c_int32), ("n_tasks", C.c_int32), ("reserved", C.c_int32)]
+        ("n_workunits", C.c_int32), ("n_rounds", C.c_int32), ("n_tasks", C.c_int32), ("reserved", C.c_int32),
+        ("store_bytes_paper", C.c_int64)]
 
     def asdict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_ if n != "reserved"}

@@ -17,6 +17,7 @@
 #include "ephc_row_kernels.cuh"
 #include "ephc_stream_kernels.cuh"
 #include "ephc_res_kernels.cuh"
+#include "ephc_paper_kernels.cuh"
 
 using namespace ephc;
 
@@ -111,6 +112,14 @@ struct ephc_handle {
     int32_t *dx_row_state = nullptr, *dx_state_row = nullptr, *dx_state_blk = nullptr, *dx_blk_row0 = nullptr,
             *dx_blk_ent_ptr = nullptr;
     int64_t *dx_slot_off = nullptr, *dx_blk_ent_off = nullptr;
+    // the paper's own layout (variant 4, A/B comparison only)
+    bool paper_built = false, paper_ok = false;
+    int64_t p_rows = 0, p_targets = 0, bytes_paper = 0;
+    PaperChannel *dp_ch = nullptr;
+    int32_t *dp_ik = nullptr, *dp_ikq = nullptr, *dp_iq = nullptr;
+    uint32_t *dp_src = nullptr;
+    PaperTarget *dp_targets = nullptr;
+    double *dp_sc_col = nullptr;
     // row store (transport_iter of the gather path)
     bool rows_ok = false;
     int32_t r_nstrip = 0, r_Rb = 0, r_Ra = 0;
@@ -137,7 +146,7 @@ static void free_dev(ephc_handle *h) {
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
                     h->ds_blk_ent_off, h->dx_blob, h->dx_iqn, h->dx_tiles, h->dx_cta_ptr, h->dx_fc, h->dx_part,
                     h->dx_row_state, h->dx_state_row, h->dx_state_blk, h->dx_blk_row0, h->dx_blk_ent_ptr, h->dx_slot_off,
-                    h->dx_blk_ent_off};
+                    h->dx_blk_ent_off, h->dp_ch, h->dp_ik, h->dp_ikq, h->dp_iq, h->dp_src, h->dp_targets, h->dp_sc_col};
     for (void *p : ptrs)
         if (p) cudaFree(p);
 }
@@ -338,6 +347,71 @@ static int make_res_store(ephc_handle *h) {
     return rc;
 }
 
+// The paper's layout: scatter, scatter_channels, stargets_sources, targets, built on the CPU once.
+static int make_paper_store(ephc_handle *h) {
+    if (h->paper_built) return EPHC_OK;
+    if (h->host_only) return fail(EPHC_ESTATE, "the paper-layout variant needs a device handle");
+    const Canonical &c = h->can;
+    const int64_t npair = (int64_t)h->pair_ik.size();
+    const int nb = h->d.nb;
+    if (c.nw >= 0x7fffffffLL) return fail(EPHC_ELIMIT, "paper layout: more than 2^31 channel weights");
+    std::vector<PaperChannel> ch;
+    std::vector<int32_t> ik, ikq, iq;
+    std::vector<PaperTarget> targets;
+    std::vector<uint32_t> src;
+    try {
+        ch.reserve((size_t)c.nw);
+        std::vector<int64_t> cnt((size_t)h->d.ns + 1, 0);
+        for (int64_t ip = 0; ip < npair; ++ip) {
+            if (c.pair_ch0[ip + 1] == c.pair_ch0[ip]) continue;
+            const uint32_t row = (uint32_t)ik.size();
+            ik.push_back(h->pair_ik[ip]);
+            ikq.push_back(h->pair_ikq[ip]);
+            iq.push_back(c.pair_iq[ip]);
+            for (int64_t j = c.pair_ch0[ip]; j < c.pair_ch0[ip + 1]; ++j) {
+                const uint32_t code = c.ch_code[j];  // n | m << 4 | nu << 8
+                const int64_t a = (int64_t)h->pair_ik[ip] * nb + (code & 15), b = (int64_t)h->pair_ikq[ip] * nb + ((code >> 4) & 15);
+                for (int kind = 0; kind < 2; ++kind) {
+                    const double w = kind ? c.ch_wem[j] : c.ch_wabs[j];
+                    if (w == 0.0) continue;
+                    ch.push_back(PaperChannel{w, code | ((uint32_t)kind << 14), row});
+                    cnt[a + 1]++;
+                    cnt[b + 1]++;
+                }
+            }
+        }
+        // target layer: two rows per channel, sorted by target; one target per state that is touched
+        for (int64_t s = 0; s < h->d.ns; ++s) cnt[s + 1] += cnt[s];
+        src.resize((size_t)cnt[h->d.ns]);
+        std::vector<int64_t> cur(cnt.begin(), cnt.end() - 1);
+        for (int64_t r = 0; r < (int64_t)ch.size(); ++r) {
+            const uint32_t code = ch[r].bnds_idx;
+            const int64_t a = (int64_t)ik[ch[r].kq_idx] * nb + (code & 15), b = (int64_t)ikq[ch[r].kq_idx] * nb + ((code >> 4) & 15);
+            src[cur[a]++] = (uint32_t)r << 1;
+            src[cur[b]++] = ((uint32_t)r << 1) | 1u;
+        }
+        for (int64_t s = 0; s < h->d.ns; ++s)
+            if (cnt[s + 1] > cnt[s]) targets.push_back(PaperTarget{cnt[s], (int32_t)(cnt[s + 1] - cnt[s]), (int32_t)s});
+    } catch (const std::bad_alloc &) {
+        return fail(EPHC_ENOMEM, "host allocation failed (paper layout)");
+    }
+    h->paper_built = true;
+    h->p_rows = (int64_t)ch.size();
+    h->p_targets = (int64_t)targets.size();
+    int64_t b = 0;
+    int rc = upload(&h->dp_ch, ch, &b);
+    if (rc == EPHC_OK) rc = upload(&h->dp_ik, ik, &b);
+    if (rc == EPHC_OK) rc = upload(&h->dp_ikq, ikq, &b);
+    if (rc == EPHC_OK) rc = upload(&h->dp_iq, iq, &b);
+    if (rc == EPHC_OK) rc = upload(&h->dp_src, src, &b);
+    if (rc == EPHC_OK) rc = upload(&h->dp_targets, targets, &b);
+    if (rc == EPHC_OK && cudaMalloc((void **)&h->dp_sc_col, (size_t)std::max<int64_t>(1, h->p_rows) * 8) != cudaSuccess)
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (sc_col) failed");
+    h->bytes_paper = b + h->p_rows * 8;
+    h->paper_ok = rc == EPHC_OK;
+    return rc;
+}
+
 // Automatic choice for collision / RK stages (measured on B200): the two-sided gather store while
 // it stays resident in the 126 MB L2; beyond that the resident-tile store when a (k,k') pair carries many channels
 // (large cells: 4.99e7 channels, nb = 16, nnu = 36: 343 us vs 597 us on the stream store) and the stream store
@@ -507,6 +581,7 @@ extern "C" int ephc_query(const ephc_handle *h, ephc_counts *o) {
     o->scatter_entries = h->t_entries;
     o->scatter_pairs = h->t_pieces;
     o->store_bytes_scatter = h->bytes_tile + h->bytes_stream + h->bytes_res;
+    o->store_bytes_paper = h->bytes_paper;
     o->store_bytes_transport = h->bytes_transport;
     // B_alg: every item the method must move once per evaluation.
     //   8 N_w weights + 4 N_ch channel index + 12 N_pair (ik, ikq, iq) + 16 N_s (read f, write I) + 8 nnu N_q,active
@@ -693,6 +768,12 @@ static inline int coll_variant(const ephc_handle *h) {
     return h->stream_ok ? 2 : (h->res_ok ? 3 : (h->tile_ok ? 1 : 0));
 }
 static inline int tr_variant(const ephc_handle *h) { return (h->variant < 0 || h->variant >= 2) ? 0 : h->variant; }
+// RK stages of the paper-layout variant run on the library's own choice (variant 4 covers ephc_collision only)
+static inline int rt_variant(const ephc_handle *h) {
+    if (h->variant != 4) return coll_variant(h);
+    const int av = auto_coll_variant(h);
+    return (av == 3 && h->res_ok) ? 3 : ((av >= 2 && h->stream_ok) ? 2 : 0);
+}
 
 extern "C" int ephc_export_stream(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu,
                                   int32_t *kind, double *w) {
@@ -993,14 +1074,15 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
 
 extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
-    if (variant < -1 || variant > 3)
-        return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather), 1 (tiles), 2 (stream) or 3 (resident tiles)");
+    if (variant < -1 || variant > 4)
+        return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather), 1 (tiles), 2 (stream), 3 (resident tiles) or 4 (paper layout)");
     // a store that the automatic choice did not need is built (and uploaded) now: this call may allocate and copy
     if (!h->host_only && variant >= 1) CUDA_TRY(cudaSetDevice(h->device));
     int rc = EPHC_OK;
     if (variant == 3) rc = make_res_store(h);
     if (variant == 2) rc = make_stream_store(h);
     if (variant == 1) rc = make_tile_store(h);
+    if (variant == 4) rc = make_paper_store(h);
     if (rc != EPHC_OK) return rc;
     if (variant == 3 && !h->res_ok)
         return fail(EPHC_ESTATE, "resident-tile store not available for this problem: " + h->res_why);
@@ -1283,6 +1365,19 @@ extern "C" int ephc_collision(ephc_handle *h, const double *f_dev, const double 
     int rc = need_device(h);
     if (rc) return rc;
     if (!f_dev || !N_dev || !I_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (coll_variant(h) == 4) {  // the paper's two steps; states without a target get I = 0
+        cudaStream_t s = (cudaStream_t)stream;
+        CUDA_TRY(cudaMemsetAsync(I_dev, 0, (size_t)h->d.ns * 8, s));
+        if (h->p_rows > 0) {
+            paper_step2_kernel<<<(unsigned)((h->p_rows + 255) / 256), 256, 0, s>>>(h->dp_ch, h->dp_ik, h->dp_ikq, h->dp_iq, f_dev, N_dev,
+                                                                                   h->dp_sc_col, h->p_rows, h->d.nb, h->d.nnu);
+            paper_step3_kernel<<<(unsigned)((h->p_targets + 255) / 256), 256, 0, s>>>(h->dp_targets, h->dp_src, h->dp_sc_col, I_dev,
+                                                                                      h->p_targets);
+            h->launches += 2;
+        }
+        CUDA_TRY(cudaGetLastError());
+        return EPHC_OK;
+    }
     if (coll_variant(h) == 3) {
         if ((rc = launch_res(h, f_dev, N_dev, (cudaStream_t)stream))) return rc;
         FinishParams Fp = finish_params_res(h);
@@ -1439,8 +1534,8 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
         for (int st = 0; st < 4; ++st) {
-            if (coll_variant(h) >= 2) {
-                const bool res = coll_variant(h) == 3;
+            if (rt_variant(h) >= 2) {
+                const bool res = rt_variant(h) == 3;
                 if ((rc = res ? launch_res(h, src[st], N_dev, s) : launch_stream(h, src[st], N_dev, s))) return rc;
                 FinishParams Fp = res ? finish_params_res(h) : finish_params_stream(h);
                 Fp.stage = st + 1;
@@ -1452,7 +1547,7 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
                 if ((rc = launch_finish<kFRkStage>(h, Fp, s))) return rc;
                 continue;
             }
-            if (coll_variant(h) == 1) {
+            if (rt_variant(h) == 1) {
                 TileParams T = tile_params(h);
                 T.f = src[st];
                 T.N = N_dev;
@@ -1474,7 +1569,7 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
             if (rc) return rc;
         }
         if (sumf_dev) {
-            if (coll_variant(h) >= 1)
+            if (rt_variant(h) >= 1)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);
             else if (h->n_wu > 0)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, h->n_wu, sumf_dev + it + 1);

@@ -37,7 +37,7 @@ def _small_problems():
 IDS = ["tiny4", "window_cut_diag", "si12", "gaas24", "bigcell3", "tiny_full", "rt14"]
 
 
-VARIANTS = {0: "gather", 1: "tiles", 2: "stream", 3: "res"}
+VARIANTS = {0: "gather", 1: "tiles", 2: "stream", 3: "res", 4: "paper"}
 
 
 @pytest.fixture(scope="module", params=[(i, v) for i in range(len(IDS)) for v in VARIANTS],
