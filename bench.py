@@ -17,8 +17,9 @@ shorter runs and reported under `per_config`:
 `cpu_baseline`  the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload: serial, and
             (`all_cores`) the paper's Baseline-CPU shape, OpenMP over the channel list with atomic updates.
 
---impl reference  times the oracle instead (rank 0 only).  N > 1: independent replicas, one per GPU, seeds
-differ per rank ("weak"); k-sharding with an all-gather of f is DESIGN.md's NEXT-1.
+--impl reference  times the oracle instead (rank 0 only).  N > 1: ONE problem, k-sharded over the ranks with an
+all-gather of the owned slices after every evaluation ("strong"); --replicas runs one
+independent problem per GPU instead ("weak", no collective).
 """
 from __future__ import annotations
 
@@ -57,6 +58,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other configs")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N > 1: independent replicas (weak scaling, no collective) instead of the k-sharded problem")
     return ap.parse_args()
 
 
@@ -401,6 +404,95 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
             "collision_channel_terms_per_s": nch_all / (ms_coll * 1e-3) if ms_coll > 0 else 0.0}
 
 
+def measure_sharded(args, ephc, torch, rank, local, dist):
+    """N > 1: ONE problem, k-sharded over the ranks: every rank owns a range
+    of destination k points, computes its states and exchanges the owned slices with an NCCL all-gather after every
+    evaluation (collision, Gamma, every transport iteration, every RK stage).  Strong scaling: the total work is fixed."""
+    from paper_2511_03683_b200.sharded import ShardedSolver
+    world = dist.get_world_size()
+    dev = torch.device("cuda", local)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    t0 = time.perf_counter()
+    p = make_workload(args)                       # the same problem on every rank
+    t_gen = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    S = ShardedSolver(p, dist, dev)
+    t_build = time.perf_counter() - t0
+    q = S.h.query()
+    nch, ns = q["nch"], p.ns
+
+    def d(x):
+        return torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64).reshape(-1), device=dev)
+
+    pin = lambda x: torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64).reshape(-1)).pin_memory()
+    hf, hf0, hN, hv = pin(p.f), pin(p.f0), pin(p.N), pin(p.v)
+    f, f0, N, v = d(p.f), d(p.f0), d(p.N), d(p.v)
+    I, G, tau = (torch.empty(ns, device=dev, dtype=torch.float64) for _ in range(3))
+    Fa, Fb = (torch.empty(3 * ns, device=dev, dtype=torch.float64) for _ in range(2))
+    frt = f.clone()
+    hI, hF, hfrt = pin(np.zeros(ns)), pin(np.zeros(3 * ns)), pin(np.zeros(ns))
+    stream = torch.cuda.current_stream()
+
+    def step(host=False):
+        if host:
+            f.copy_(hf, non_blocking=True); f0.copy_(hf0, non_blocking=True)
+            N.copy_(hN, non_blocking=True); v.copy_(hv, non_blocking=True); frt.copy_(hf, non_blocking=True)
+        S.collision(f, N, I, stream)
+        F = S.transport_solve(f0, N, v, N_TRANSPORT_ITERS, G, tau, Fa, Fb, stream)
+        S.rt_step(frt, N, 1.0, 1, stream)
+        if host:
+            hI.copy_(I, non_blocking=True); hF.copy_(F, non_blocking=True); hfrt.copy_(frt, non_blocking=True)
+            torch.cuda.synchronize()
+
+    def timed(host):
+        for _ in range(max(args.warmup, 0)):
+            step(host)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = S.h.launch_count()
+        e0.record(stream)
+        for _ in range(args.steps):
+            step(host)
+        e1.record(stream)
+        barrier()
+        t = torch.tensor([e0.elapsed_time(e1)], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item()), S.h.launch_count() - l0
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    ms_total, launches = timed(False)
+    clocks = sampler.stop() if sampler else None
+    ms_e2e, _ = timed(True) if not args.no_e2e else (None, 0)
+    lo, hi = S.h.owned_states()
+    own = [None] * world
+    dist.all_gather_object(own, [lo, hi, int(S.h.query()["gather_entries"])])
+    if rank != 0:
+        return None
+    exchanges = 1 + 1 + N_TRANSPORT_ITERS * 3 + 4
+    cfg = workload_config(args, p, nch)
+    cfg.update({"variant": "collision/rt: gather (destination-sorted, two-sided), transport: rows (setup on gather)",
+                "parallelism": f"k-sharded over {world} GPUs: contiguous ranges of destination k balanced by half-pair count; "
+                               f"{exchanges} all-gathers of the owned slices per step (NCCL), <= {8 * ns} bytes each",
+                "owned_states_and_ordered_entries_per_rank": own, "generate_s": t_gen, "build_channels_s": t_build,
+                "l2": "no flush: every rank streams its share of the two-sided store in every evaluation"})
+    val = nch * EVALS_PER_STEP * args.steps / (ms_total * 1e-3)
+    e2e = None
+    if ms_e2e is not None:
+        e2e = {"value": nch * EVALS_PER_STEP * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(8 * (3 * ns + p.nq * p.nnu + 3 * ns)), "d2h_bytes_per_step": int(8 * 5 * ns),
+               "ms_per_step": ms_e2e / max(args.steps, 1)}
+    return {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / max(args.steps, 1), "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": cfg, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": None, "cpu_baseline": None}
+
+
 def load_traffic(config_name):
     """DRAM bytes per launch from the committed `ncu --set full` captures (cold caches: ncu flushes them per kernel)."""
     path = os.path.join(ROOT, "profiles", "traffic.csv")
@@ -434,6 +526,12 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
+    if world > 1 and not args.replicas:
+        out = measure_sharded(args, ephc, torch, rank, local, dist)
+        if rank == 0:
+            print(json.dumps(out))
+        dist.destroy_process_group()
+        return
     sampler = ClockSampler(local) if rank == 0 else None
     main_res = measure(args, ephc, torch, args.config, args.steps, args.warmup, rank, local, dist,
                        with_e2e=not args.no_e2e, with_cpu=(rank == 0 and world == 1 and not args.no_cpu_baseline), sampler=sampler)

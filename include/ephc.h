@@ -112,6 +112,17 @@ typedef struct ephc_counts {
  * the transposed index, and uploads them.  *out receives the handle (NULL on failure). */
 int ephc_build_channels(const ephc_problem *p, ephc_handle **out);
 
+/* k-sharded evaluation ("k points are evenly distributed over different MPI processes"):
+ * the handle owns the DESTINATION k points k_lo <= ik < k_hi (compact indices) and stores every ordered term whose
+ * destination it owns, in the destination-sorted two-sided store (variant 0) and the row store derived from it.
+ * ephc_collision, ephc_transport_setup and ephc_transport_iter then compute the owned states only (the others receive
+ * 0, resp. tau*v); they read f / F of ALL states, so the caller exchanges the owned slices between the ranks after
+ * every evaluation (one all-gather of <= ns doubles).  Time stepping goes through ephc_rt_stage with an exchange of
+ * y after each stage; ephc_rt_step is refused.  The ranges of all ranks must partition [0, nk). */
+int ephc_build_channels_range(const ephc_problem *p, int32_t k_lo, int32_t k_hi, ephc_handle **out);
+/* owned states [s_lo, s_hi) = [k_lo*nb, k_hi*nb); all states for a handle of ephc_build_channels */
+int ephc_owned_states(const ephc_handle *h, int64_t *s_lo, int64_t *s_hi);
+
 int ephc_query(const ephc_handle *h, ephc_counts *out);
 
 /* Canonical channel list, host arrays of length nch each (any pointer may be NULL to skip it).
@@ -208,6 +219,13 @@ int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev
  * The axpy of every stage is fused into the collision kernel's epilogue. */
 int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
                  double *sumf_dev, void *stream);
+
+/* One stage of the same RK4 step, for callers that exchange data between the stages (k-sharded handles):
+ *   stage 1..3: y_out = f + a dt I[y_in] (a = 1/2, 1/2, 1), the handle accumulates b I[y_in];
+ *   stage 4:    f += dt/6 (accumulated + I[y_in]) in place (y_out may be NULL).
+ * y_in of stage 1 is f itself; only the handle's own states of y_out / f are meaningful on a k-sharded handle. */
+int ephc_rt_stage(ephc_handle *h, double *f_dev, const double *y_in_dev, const double *N_dev, double dt_fs, int stage,
+                  double *y_out_dev, void *stream);
 
 /* Host-buffer variants (end-to-end path): copy in, run the same kernels, copy out, synchronise. */
 int ephc_collision_host(ephc_handle *h, const double *f_host, const double *N_host, double *I_host);

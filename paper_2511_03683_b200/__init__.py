@@ -65,6 +65,9 @@ def _load():
     vp, i64, dbl, i32 = C.c_void_p, C.c_int64, C.c_double, C.c_int
     sig = {
         "ephc_build_channels": (i32, [C.POINTER(_Problem), C.POINTER(vp)]),
+        "ephc_build_channels_range": (i32, [C.POINTER(_Problem), i32, i32, C.POINTER(vp)]),
+        "ephc_owned_states": (i32, [vp, C.POINTER(i64), C.POINTER(i64)]),
+        "ephc_rt_stage": (i32, [vp, vp, vp, vp, dbl, i32, vp, vp]),
         "ephc_query": (i32, [vp, C.POINTER(Counts)]),
         "ephc_export_channels": (i32, [vp] * 9),
         "ephc_export_diag": (i32, [vp] * 6),
@@ -268,6 +271,16 @@ class Handle:
                                            _dev_ptr(tau, self.ns, "tau"), _dev_ptr(Fout, 3 * self.ns, "Fout"),
                                            _stream_ptr(stream)))
 
+    def owned_states(self):
+        lo, hi = C.c_int64(), C.c_int64()
+        _check(_load().ephc_owned_states(self._h, C.byref(lo), C.byref(hi)))
+        return int(lo.value), int(hi.value)
+
+    def rt_stage(self, f, y_in, N, dt_fs: float, stage: int, y_out=None, stream=None):
+        _check(_load().ephc_rt_stage(self._h, _dev_ptr(f, self.ns, "f"), _dev_ptr(y_in, self.ns, "y_in"),
+                                     _dev_ptr(N, self.nq * self.nnu, "N"), float(dt_fs), int(stage),
+                                     _dev_ptr(y_out, self.ns, "y_out"), _stream_ptr(stream)))
+
     def rt_step(self, f, N, dt_fs: float, nsteps: int, sumf=None, stream=None):
         _check(_load().ephc_rt_step(self._h, _dev_ptr(f, self.ns, "f"), _dev_ptr(N, self.nq * self.nnu, "N"),
                                     float(dt_fs), int(nsteps), _dev_ptr(sumf, nsteps + 1, "sumf"),
@@ -295,8 +308,9 @@ class Handle:
         _check(_load().ephc_rt_step_host(self._h, pf, pN, float(dt_fs), int(nsteps), ps))
 
 
-def build_channels(prob, flags: int = 0) -> Handle:
-    """ephc_build_channels on an object with the fields of ephc_problem (e.g. ephc_inputs.Problem)."""
+def build_channels(prob, flags: int = 0, k_range=None) -> Handle:
+    """ephc_build_channels (or, with k_range = (k_lo, k_hi), ephc_build_channels_range) on an object with the fields of
+    ephc_problem (e.g. ephc_inputs.Problem)."""
     lib = _load()
     keep = dict(
         kfull=np.ascontiguousarray(prob.kfull, dtype=np.int32),
@@ -321,5 +335,8 @@ def build_channels(prob, flags: int = 0) -> Handle:
     for k, a in keep.items():
         setattr(p, k, a.ctypes.data if a.size else None)
     out = C.c_void_p()
-    _check(lib.ephc_build_channels(C.byref(p), C.byref(out)))
+    if k_range is None:
+        _check(lib.ephc_build_channels(C.byref(p), C.byref(out)))
+    else:
+        _check(lib.ephc_build_channels_range(C.byref(p), int(k_range[0]), int(k_range[1]), C.byref(out)))
     return Handle(out.value, nk, nb, nnu, nq)

@@ -41,6 +41,7 @@ struct ephc_handle {
     std::vector<double> E;               // copy of the band energies and window: the optional stores are built from them
     double emin = 0.0, emax = 0.0;
     bool tile_built = false, stream_built = false, res_built = false;
+    bool ranged = false;                 // built by ephc_build_channels_range: owns the destination k in [d.k_lo, d.k_hi)
     RowHost rowhost;                     // kept only for EPHC_HOST_ONLY handles (ephc_export_rows)
     int variant = -1;  // -1: automatic (collision / rt_step on the tile store, transport on the gather store)
     Canonical can;
@@ -417,12 +418,35 @@ static int make_paper_store(ephc_handle *h) {
 // (large cells: 4.99e7 channels, nb = 16, nnu = 36: 343 us vs 597 us on the stream store) and the stream store
 // otherwise (1.26e7 channels, nb = 4: 126 us vs 134 us; 1.94e8 channels, nb = 1: 2.44 ms vs 4.2 ms).
 static int auto_coll_variant(const ephc_handle *h) {
+    if (h->ranged) return 0;  // a k-sharded handle owns destinations: the two-sided, destination-sorted store
     if (h->g_entries * 12 <= (int64_t)96 << 20) return 0;
     const double per_pair = (double)h->can.nw / (double)std::max<int64_t>(1, h->can.npair_active);
     return per_pair >= 64.0 ? 3 : 2;
 }
 
+static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ranged, ephc_handle **out);
+
 extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
+    if (out) *out = nullptr;
+    if (!p || !out) return fail(EPHC_EINVAL, "null argument");
+    return build_impl(p, 0, p->nk, false, out);
+}
+
+extern "C" int ephc_build_channels_range(const ephc_problem *p, int32_t k_lo, int32_t k_hi, ephc_handle **out) {
+    if (out) *out = nullptr;
+    if (!p || !out) return fail(EPHC_EINVAL, "null argument");
+    if (k_lo < 0 || k_hi < k_lo || k_hi > p->nk) return fail(EPHC_EINVAL, "need 0 <= k_lo <= k_hi <= nk");
+    return build_impl(p, k_lo, k_hi, true, out);
+}
+
+extern "C" int ephc_owned_states(const ephc_handle *h, int64_t *s_lo, int64_t *s_hi) {
+    if (!h || !s_lo || !s_hi) return fail(EPHC_EINVAL, "null argument");
+    *s_lo = (int64_t)h->d.k_lo * h->d.nb;
+    *s_hi = (int64_t)h->d.k_hi * h->d.nb;
+    return EPHC_OK;
+}
+
+static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ranged, ephc_handle **out) {
     if (out) *out = nullptr;
     if (!p || !out) return fail(EPHC_EINVAL, "null argument");
     if (!p->kfull || !p->E || !p->hw || (p->npair > 0 && (!p->pair_ik || !p->pair_ikq || !p->g2)))
@@ -447,6 +471,9 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
     h->d.nq = nq;
     h->d.ns = ns;
     h->d.C = 2.0 * kPi / (kHbar * (double)nq);  // R-8: N_q = points of the full grid
+    h->d.k_lo = k_lo;
+    h->d.k_hi = k_hi;
+    h->ranged = ranged;
     h->host_only = (p->flags & EPHC_HOST_ONLY) != 0;
     if (!h->host_only) {
         // the handle belongs to the device that is current now; every later call makes it current again
@@ -544,7 +571,7 @@ extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
     }
     // the once-stored store of the automatic choice (the others are built when ephc_set_variant asks for them);
     // host-only handles build all of them for the export calls
-    if (rc == EPHC_OK) {
+    if (rc == EPHC_OK && !h->ranged) {
         const int av = auto_coll_variant(h);
         if (h->host_only || av == 3) rc = make_res_store(h);
         if (rc == EPHC_OK && (h->host_only || av == 2 || (av == 3 && !h->res_ok))) rc = make_stream_store(h);
@@ -1076,6 +1103,8 @@ extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (!h) return fail(EPHC_EINVAL, "null handle");
     if (variant < -1 || variant > 4)
         return fail(EPHC_EINVAL, "variant must be -1 (automatic), 0 (gather), 1 (tiles), 2 (stream), 3 (resident tiles) or 4 (paper layout)");
+    if (h->ranged && variant > 0)
+        return fail(EPHC_ESTATE, "a k-sharded handle runs on the destination-sorted stores only (variant 0)");
     // a store that the automatic choice did not need is built (and uploaded) now: this call may allocate and copy
     if (!h->host_only && variant >= 1) CUDA_TRY(cudaSetDevice(h->device));
     int rc = EPHC_OK;
@@ -1511,63 +1540,74 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
     return launch_gather<kTransportIter>(h, P, (cudaStream_t)stream);
 }
 
-extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
-                            double *sumf_dev, void *stream) {
-    int rc = need_device(h);
-    if (rc) return rc;
-    if (!f_dev || !N_dev) return fail(EPHC_EINVAL, "null device pointer");
-    if (nsteps < 0 || !std::isfinite(dt_fs)) return fail(EPHC_EINVAL, "nsteps >= 0 and finite dt required");
-    cudaStream_t s = (cudaStream_t)stream;
-    if (sumf_dev) {
-        sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev);
-        h->launches++;
+// One RK4 stage (reading R-18): k = I[y_in]; stage 1..3: y_out = f + a dt k and ksum accumulates b k; stage 4:
+// f += dt/6 (ksum + k) in place.  The axpy is the epilogue of the collision pass.
+static int rk_stage(ephc_handle *h, double *f_dev, const double *y_in, const double *N_dev, double dt_fs, int st, double *y_out,
+                    bool want_sum, cudaStream_t s) {
+    int rc;
+    const int v = rt_variant(h);
+    if (v >= 1) {
+        FinishParams Fp;
+        if (v >= 2) {
+            if ((rc = (v == 3) ? launch_res(h, y_in, N_dev, s) : launch_stream(h, y_in, N_dev, s))) return rc;
+            Fp = (v == 3) ? finish_params_res(h) : finish_params_stream(h);
+        } else {
+            TileParams T = tile_params(h);
+            T.f = y_in;
+            T.N = N_dev;
+            if ((rc = launch_tile<kTCollision>(h, T, s))) return rc;
+            Fp = finish_params(h);
+        }
+        Fp.stage = st;
+        Fp.dt = dt_fs;
+        Fp.f0 = f_dev;
+        Fp.ynext = y_out;
+        Fp.ksum = h->d_ksum;
+        Fp.blk_sum = want_sum ? h->d_wusum : nullptr;
+        return launch_finish<kFRkStage>(h, Fp, s);
     }
     GatherParams P = base_params(h);
     P.N = N_dev;
     P.dt = dt_fs;
     P.f0 = f_dev;
     P.ksum = h->d_ksum;
-    P.wu_sum = sumf_dev ? h->d_wusum : nullptr;
+    P.wu_sum = want_sum ? h->d_wusum : nullptr;
+    P.stage = st;
+    P.f = y_in;
+    P.ynext = y_out;
+    return launch_gather<kRkStage>(h, P, s);
+}
+
+extern "C" int ephc_rt_stage(ephc_handle *h, double *f_dev, const double *y_in_dev, const double *N_dev, double dt_fs, int stage,
+                             double *y_out_dev, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f_dev || !y_in_dev || !N_dev || stage < 1 || stage > 4 || (stage < 4 && !y_out_dev) || !std::isfinite(dt_fs))
+        return fail(EPHC_EINVAL, "bad argument (stage 1..4, y_out needed for stages 1..3)");
+    if (y_out_dev == y_in_dev || y_out_dev == f_dev) return fail(EPHC_EINVAL, "y_out must differ from y_in and f");
+    return rk_stage(h, f_dev, y_in_dev, N_dev, dt_fs, stage, y_out_dev, false, (cudaStream_t)stream);
+}
+
+extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
+                            double *sumf_dev, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f_dev || !N_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (nsteps < 0 || !std::isfinite(dt_fs)) return fail(EPHC_EINVAL, "nsteps >= 0 and finite dt required");
+    if (h->ranged)
+        return fail(EPHC_ESTATE, "a k-sharded handle owns part of the states: use ephc_rt_stage and exchange y between the stages");
+    cudaStream_t s = (cudaStream_t)stream;
+    if (sumf_dev) {
+        sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev);
+        h->launches++;
+    }
     for (int it = 0; it < nsteps; ++it) {
         // stage 1 gathers f, writes y2 -> y[0]; stage 2 gathers y[0], writes y3 -> y[1];
         // stage 3 gathers y[1], writes y4 -> y[0]; stage 4 gathers y[0], updates f in place.
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
-        for (int st = 0; st < 4; ++st) {
-            if (rt_variant(h) >= 2) {
-                const bool res = rt_variant(h) == 3;
-                if ((rc = res ? launch_res(h, src[st], N_dev, s) : launch_stream(h, src[st], N_dev, s))) return rc;
-                FinishParams Fp = res ? finish_params_res(h) : finish_params_stream(h);
-                Fp.stage = st + 1;
-                Fp.dt = dt_fs;
-                Fp.f0 = f_dev;
-                Fp.ynext = dst[st];
-                Fp.ksum = h->d_ksum;
-                Fp.blk_sum = sumf_dev ? h->d_wusum : nullptr;
-                if ((rc = launch_finish<kFRkStage>(h, Fp, s))) return rc;
-                continue;
-            }
-            if (rt_variant(h) == 1) {
-                TileParams T = tile_params(h);
-                T.f = src[st];
-                T.N = N_dev;
-                if ((rc = launch_tile<kTCollision>(h, T, s))) return rc;
-                FinishParams Fp = finish_params(h);
-                Fp.stage = st + 1;
-                Fp.dt = dt_fs;
-                Fp.f0 = f_dev;
-                Fp.ynext = dst[st];
-                Fp.ksum = h->d_ksum;
-                Fp.blk_sum = sumf_dev ? h->d_wusum : nullptr;
-                if ((rc = launch_finish<kFRkStage>(h, Fp, s))) return rc;
-                continue;
-            }
-            P.stage = st + 1;
-            P.f = src[st];
-            P.ynext = dst[st];
-            rc = launch_gather<kRkStage>(h, P, s);
-            if (rc) return rc;
-        }
+        for (int st = 0; st < 4; ++st)
+            if ((rc = rk_stage(h, f_dev, src[st], N_dev, dt_fs, st + 1, dst[st], sumf_dev != nullptr, s))) return rc;
         if (sumf_dev) {
             if (rt_variant(h) >= 1)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);

@@ -241,11 +241,14 @@ int build_gather(const ephc_problem *p, const Dims &d, const Canonical &c, Gathe
     auto active = [&](int64_t ip) {
         return (c.pair_ch0[ip + 1] > c.pair_ch0[ip]) || (c.pair_dg0[ip + 1] > c.pair_dg0[ip]);
     };
+    // k-sharded handles keep only the half-pairs whose DESTINATION k they own (k points are distributed
+    // over the processes); every ordered term then lives on exactly one rank
+    auto owned = [&](int32_t k) { return k >= d.k_lo && k < d.k_hi; };
     for (int64_t ip = 0; ip < npair; ++ip) {
         if (!active(ip)) continue;
         const int32_t ik = p->pair_ik[ip], ikq = p->pair_ikq[ip];
-        seg_hp0[ik + 1]++;
-        if (ikq != ik) {
+        if (owned(ik)) seg_hp0[ik + 1]++;
+        if (ikq != ik && owned(ikq)) {
             seg_hp0[ikq + 1]++;
             n_mirror[ikq]++;
         }
@@ -274,11 +277,14 @@ int build_gather(const ephc_problem *p, const Dims &d, const Canonical &c, Gathe
         for (int64_t ip = 0; ip < npair; ++ip) {
             if (!active(ip)) continue;
             const int32_t ik = p->pair_ik[ip], ikq = p->pair_ikq[ip];
-            int64_t o = cur_f[ik]++;
-            hps[o] = HalfPair{ip, ik == ikq ? 2 : 0};
-            g.hp_k[o] = ikq;
-            g.hp_q[o] = c.pair_iq[ip];
-            if (ikq != ik) {
+            int64_t o = 0;
+            if (owned(ik)) {
+                o = cur_f[ik]++;
+                hps[o] = HalfPair{ip, ik == ikq ? 2 : 0};
+                g.hp_k[o] = ikq;
+                g.hp_q[o] = c.pair_iq[ip];
+            }
+            if (ikq != ik && owned(ikq)) {
                 o = cur_m[ikq]++;
                 hps[o] = HalfPair{ip, 1};
                 g.hp_k[o] = ik;

@@ -71,6 +71,7 @@ struct Dims {
     int32_t nk, nb, nnu;
     int64_t nq, ns;
     double C;
+    int32_t k_lo = 0, k_hi = 0;  // destination k points this handle owns (k-sharded evaluation); [0, nk) = all
 };
 
 // host builder (ephc_build.cu)

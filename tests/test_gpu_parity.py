@@ -343,6 +343,62 @@ def test_handles_of_different_geometry_do_not_disturb_each_other():
     run(big, Lb, hb)
 
 
+def test_k_sharded_handles_on_one_gpu():
+    # k-sharded evaluation (ephc_build_channels_range): three ranged handles on one device stand for three ranks; their
+    # owned pieces, exchanged by hand, reproduce the oracle's collision integral, Gamma, transport iterations and RK4
+    from paper_2511_03683_b200.sharded import balanced_k_ranges
+    for p in (_small_problems()[2], _small_problems()[1]):
+        L = oracle.OracleList(p)
+        ranges = balanced_k_ranges(p, 3)
+        hs = [ephc.build_channels(p, k_range=r) for r in ranges]
+        own = [h.owned_states() for h in hs]
+        assert own[0][0] == 0 and own[-1][1] == p.ns and all(own[i][1] == own[i + 1][0] for i in range(2))
+        with pytest.raises(ephc.EphcError):
+            hs[0].set_variant(2)
+        f, N = dev(p.f), dev(p.N)
+
+        def owned_pieces(fn, ncomp=1):
+            full = torch.zeros(ncomp * p.ns, device="cuda", dtype=torch.float64)
+            for h, (lo, hi) in zip(hs, own):
+                out = torch.full((ncomp * p.ns,), float("nan"), device="cuda", dtype=torch.float64)
+                fn(h, out)
+                for c in range(ncomp):
+                    full[c * p.ns + lo:c * p.ns + hi] = out[c * p.ns + lo:c * p.ns + hi]
+            return full
+
+        I = owned_pieces(lambda h, out: h.collision(f, N, out))
+        assert _relerr(I.cpu().numpy(), L.collision(p.f, p.N)) <= TOL
+        G = owned_pieces(lambda h, out: h.transport_setup(dev(p.f0), N, out))
+        Go = L.transport_setup(p.f0, p.N)
+        assert _relerr(G.cpu().numpy(), Go) <= TOL
+        tau_o = np.where(Go > 0, 1.0 / np.where(Go > 0, Go, 1.0), 0.0)
+        Fr = tau_o[None, :] * p.v
+        F, v, tau = dev(Fr), dev(p.v), dev(tau_o)
+        for _ in range(3):
+            F = owned_pieces(lambda h, out: h.transport_iter(F, v, tau, out), 3)
+            Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau_o)
+        assert _relerr(F.cpu().numpy().reshape(3, -1), Fr) <= TOL
+        # RK4 through ephc_rt_stage with the exchange after every stage
+        fs = [dev(p.f) for _ in hs]
+        with pytest.raises(ephc.EphcError):
+            hs[0].rt_step(fs[0], N, 1.0, 1, None)
+        for _ in range(3):
+            y = fs[0].clone()
+            for stage in (1, 2, 3, 4):
+                if stage < 4:
+                    y_new = owned_pieces(lambda h, out: h.rt_stage(fs[hs.index(h)], y, N, 1.0, stage, out))
+                    y = y_new
+                else:
+                    for h, fr in zip(hs, fs):
+                        h.rt_stage(fr, y, N, 1.0, 4, None)
+                    fnew = torch.zeros(p.ns, device="cuda", dtype=torch.float64)
+                    for fr, (lo, hi) in zip(fs, own):
+                        fnew[lo:hi] = fr[lo:hi]
+                    for fr in fs:
+                        fr.copy_(fnew)
+        assert _relerr(fs[0].cpu().numpy(), L.rt_step(p.f, p.N, 1.0, 3)[0]) <= TOL
+
+
 def test_stream_argument_is_honoured():
     p = make_problem("si", grid=(12, 12, 12), pair_prob=0.3, seed=3)
     h = ephc.build_channels(p)
