@@ -58,6 +58,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other configs")
+    ap.add_argument("--sharded", action="store_true", help="use the k-sharded driver even with one rank")
     ap.add_argument("--replicas", action="store_true",
                     help="N > 1: independent replicas (weak scaling, no collective) instead of the k-sharded problem")
     return ap.parse_args()
@@ -526,7 +527,12 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    if world > 1 and not args.replicas:
+    if args.sharded and world == 1:            # the sharded driver with a single rank (checks the code path on one GPU)
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29533")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
+    if (world > 1 and not args.replicas) or args.sharded:
         out = measure_sharded(args, ephc, torch, rank, local, dist)
         if rank == 0:
             print(json.dumps(out))
