@@ -56,6 +56,10 @@ def _load():
     lib.orc_rt_step.restype = C.c_int
     lib.orc_rt_step.argtypes = [C.c_void_p, _f64p, _f64p, C.c_double, C.c_int, _f64p]
     lib.orc_collision_sampled.argtypes = prob_args + [_f64p, _f64p, C.c_int, _i32p, _f64p]
+    lib.orc_drift.restype = C.c_int
+    lib.orc_drift.argtypes = [_i32p, C.c_int, C.c_int, _i32p, _f64p, _f64p, _f64p]
+    lib.orc_rt_step_field.restype = C.c_int
+    lib.orc_rt_step_field.argtypes = [C.c_void_p, _i32p, _f64p, _f64p, _f64p, C.c_double, C.c_int, _f64p]
     _lib = lib
     return lib
 
@@ -135,6 +139,41 @@ class OracleList:
         if rc != 0:
             raise MemoryError("orc_rt_step failed")
         return f, sumf
+
+
+def drift(prob, f, field):
+    """Drift term of Eq. 1, D = -(1/hbar) F . grad_k f (reading R-25), for every state slot."""
+    out = np.zeros(prob.nk * prob.nb)
+    rc = _load().orc_drift(np.asarray(prob.grid, dtype=np.int32), prob.nk, prob.nb,
+                           np.ascontiguousarray(prob.kfull, dtype=np.int32), _f(f), _f(field), out)
+    if rc != 0:
+        raise MemoryError("orc_drift failed")
+    return out
+
+
+def rt_step_field(L, prob, f, N, field, dt, nsteps):
+    """RK4 on df/dt = D[f] + I[f] (Eq. 1 as printed)."""
+    f = _f(f).copy()
+    sumf = np.zeros(nsteps + 1)
+    rc = _load().orc_rt_step_field(L._h, np.ascontiguousarray(prob.kfull, dtype=np.int32), f, _f(N), _f(field),
+                                   float(dt), int(nsteps), sumf)
+    if rc != 0:
+        raise MemoryError("orc_rt_step_field failed")
+    return f, sumf
+
+
+def transport_moments(f0, v, F):
+    """Post-processing of the transport solution (reading R-26): S[al][be] = sum_s f0_s (1 - f0_s) v[al][s] F[be][s]
+    (-df0/dE = f0 (1 - f0) / k_B T for a Fermi-Dirac f0) and n = sum_s f0_s.  The conductivity is
+    sigma = e^2 / (Omega N_k k_B T) * S and the mobility e S / (k_B T n); the constants are the caller's."""
+    f0 = _f(f0)
+    ns = f0.size
+    v, F = _f(v).reshape(3, ns), _f(F).reshape(3, ns)
+    S = np.zeros((3, 3))
+    for a in range(3):
+        for b in range(3):
+            S[a, b] = np.sum(f0 * (1.0 - f0) * v[a] * F[b])
+    return S, float(np.sum(f0))
 
 
 def threads() -> int:

@@ -310,6 +310,68 @@ int orc_rt_step(const orc_list *L, double *f, const double *N, double dt, int ns
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Drift term of Eq. 1: D[f](n,k) = -(1/hbar) F . grad_k f.   The paper gives no discretisation (its
+ * Methods section is missing); reading R-25 of DESIGN.md: k in reduced coordinates x_i = c_i / N_i of the grid,
+ *     (grad f)_i ~ N_i/2 * [ f(n, k+e_i) - f(n, k-e_i) ]      (central difference, k +- e_i modulo the grid),
+ * a neighbour that is not an active k point counts as f = 0, F given by its three components along the reduced axes
+ * in eV, so that D is in 1/fs.  Every state slot of an active k point gets a value.
+ * ------------------------------------------------------------------------------------------- */
+int orc_drift(const int *grid, int nk, int nb, const int32_t *kfull, const double *f, const double *Ffield, double *out) {
+    int64_t nq = (int64_t)grid[0] * grid[1] * grid[2];
+    int32_t *compact = malloc(sizeof(int32_t) * (size_t)nq);
+    if (!compact) return -1;
+    for (int64_t i = 0; i < nq; ++i) compact[i] = -1;
+    for (int k = 0; k < nk; ++k) compact[kfull[k]] = k;
+    for (int k = 0; k < nk; ++k) {
+        int c[3] = {kfull[k] / (grid[1] * grid[2]), (kfull[k] / grid[2]) % grid[1], kfull[k] % grid[2]};
+        for (int n = 0; n < nb; ++n) {
+            double acc = 0.0;
+            for (int i = 0; i < 3; ++i) {
+                int cp[3] = {c[0], c[1], c[2]}, cm[3] = {c[0], c[1], c[2]};
+                cp[i] = (c[i] + 1) % grid[i];
+                cm[i] = (c[i] - 1 + grid[i]) % grid[i];
+                int32_t kp = compact[((int64_t)cp[0] * grid[1] + cp[1]) * grid[2] + cp[2]];
+                int32_t km = compact[((int64_t)cm[0] * grid[1] + cm[1]) * grid[2] + cm[2]];
+                double fp = kp >= 0 ? f[(int64_t)kp * nb + n] : 0.0;
+                double fm = km >= 0 ? f[(int64_t)km * nb + n] : 0.0;
+                acc += Ffield[i] * (0.5 * grid[i]) * (fp - fm);
+            }
+            out[(int64_t)k * nb + n] = -acc / ORC_HBAR;
+        }
+    }
+    free(compact);
+    return 0;
+}
+
+/* rt-BTE with the drift term: classical RK4 on df/dt = D[f] + I[f] (Eq. 1 as printed), N fixed. */
+int orc_rt_step_field(const orc_list *L, const int32_t *kfull, double *f, const double *N, const double *Ffield,
+                      double dt, int nsteps, double *sumf) {
+    int64_t ns = (int64_t)L->nk * L->nb;
+    double *k[4], *y = malloc(8 * (size_t)ns), *d = malloc(8 * (size_t)ns);
+    for (int j = 0; j < 4; ++j) k[j] = malloc(8 * (size_t)ns);
+    if (!k[0] || !k[1] || !k[2] || !k[3] || !y || !d) return -1;
+    const double a[3] = {0.5, 0.5, 1.0};
+    if (sumf) sumf[0] = orc_sum(f, ns);
+    for (int it = 0; it < nsteps; ++it) {
+        for (int j = 0; j < 4; ++j) {
+            const double *src = f;
+            if (j > 0) {
+                for (int64_t s = 0; s < ns; ++s) y[s] = f[s] + a[j - 1] * dt * k[j - 1][s];
+                src = y;
+            }
+            orc_collision(L, src, N, k[j]);
+            if (orc_drift(L->grid, L->nk, L->nb, kfull, src, Ffield, d)) return -1;
+            for (int64_t s = 0; s < ns; ++s) k[j][s] += d[s];
+        }
+        for (int64_t s = 0; s < ns; ++s) f[s] += dt / 6.0 * (k[0][s] + 2.0 * k[1][s] + 2.0 * k[2][s] + k[3][s]);
+        if (sumf) sumf[it + 1] = orc_sum(f, ns);
+    }
+    for (int j = 0; j < 4; ++j) free(k[j]);
+    free(y); free(d);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------------
  * Sampled evaluation straight from the problem definition (no list): I[s] for a few states, as the
  * ordered sum of Eq. 2 over every candidate pair that touches the state's k.  Used by the full-size
  * parity tests, where building the list for 1e8 channels is not wanted.

@@ -288,3 +288,86 @@ def test_p9_rt_conserves_particle_number_and_is_reproducible(small_win):
     assert np.array_equal(f1, f2) and np.array_equal(s1, s2)
     assert np.abs(s1 - s1[0]).max() <= 1e-12 * abs(s1[0])
     assert np.abs(f1 - p.f).max() > 1e-4          # the state did evolve
+
+
+# ---- drift term of Eq. 1 and transport post-processing (readings R-25, R-26) -----------------------------------
+def _full_grid_problem(grid, nb=2):
+    nq = grid[0] * grid[1] * grid[2]
+    return manual_problem(grid, E=np.zeros((nq, nb)), hw=np.full((nq, 1), 0.02), pairs=[], g2=np.zeros((0, 1, nb, nb)),
+                          sigma=0.01)
+
+
+def test_drift_closed_form_on_a_fourier_mode():
+    # f = A + B cos(2 pi x_i): the central difference is exact up to the factor N_i sin(2 pi / N_i):
+    # D = -(F_i / hbar) * (-B N_i sin(2 pi / N_i) sin(2 pi x_i))
+    grid = (6, 5, 8)
+    p = _full_grid_problem(grid)
+    idx = np.arange(p.nk)
+    c = [idx // (grid[1] * grid[2]), (idx // grid[2]) % grid[1], idx % grid[2]]
+    for i in range(3):
+        theta = 2 * np.pi * c[i] / grid[i]
+        f = np.repeat(0.3 + 0.2 * np.cos(theta), p.nb)
+        field = np.zeros(3); field[i] = 0.07
+        D = oracle.drift(p, f, field)
+        exp = np.repeat((0.07 / HBAR) * 0.2 * grid[i] * np.sin(2 * np.pi / grid[i]) * np.sin(theta), p.nb)
+        assert np.abs(D - exp).max() <= 1e-14 * np.abs(exp).max()
+        other = np.zeros(3); other[(i + 1) % 3] = 0.07               # a field along another axis sees no gradient
+        assert np.abs(oracle.drift(p, f, other)).max() <= 1e-15
+    # general f and field: linear in both, and the drift moves occupation without creating it (periodic grid)
+    rng = np.random.default_rng(3)
+    f = rng.uniform(0, 1, p.ns); g = rng.uniform(0, 1, p.ns)
+    F1, F2 = np.array([0.01, -0.02, 0.03]), np.array([0.05, 0.0, -0.01])
+    assert np.allclose(oracle.drift(p, 2 * f - g, F1 + F2), 2 * oracle.drift(p, f, F1) - oracle.drift(p, g, F1)
+                       + 2 * oracle.drift(p, f, F2) - oracle.drift(p, g, F2), rtol=0, atol=1e-13)
+    assert abs(oracle.drift(p, f, F1).sum()) <= 1e-12 * np.abs(oracle.drift(p, f, F1)).sum()
+
+
+def test_drift_treats_missing_neighbours_as_empty():
+    # active k = a slab of the grid: the neighbour outside it counts as f = 0 (reading R-25)
+    grid = (4, 1, 1)
+    p = manual_problem(grid, E=np.zeros((2, 1)), hw=np.full((4, 1), 0.02), pairs=[], g2=np.zeros((0, 1, 1, 1)), sigma=0.01,
+                       kfull=[1, 2])
+    D = oracle.drift(p, [0.5, 0.25], [0.1, 0.0, 0.0])
+    # k = 1: neighbours 2 (f = 0.25) and 0 (inactive, 0);  k = 2: neighbours 3 (inactive) and 1 (0.5); N_1 / 2 = 2
+    assert D[0] == pytest.approx(-(0.1 / HBAR) * 2 * (0.25 - 0.0), rel=1e-15)
+    assert D[1] == pytest.approx(-(0.1 / HBAR) * 2 * (0.0 - 0.5), rel=1e-15)
+
+
+def test_field_rk4_advects_a_fourier_mode():
+    # no channels: df/dt = D[f]; cos(theta - w t) with w = F N sin(2 pi / N) / hbar solves the discretised equation
+    # exactly, so RK4's error falls 16-fold when dt is halved
+    grid = (12, 1, 1)
+    p = _full_grid_problem(grid, nb=1)
+    L = oracle.OracleList(p)
+    assert L.nch == 0
+    theta = 2 * np.pi * np.arange(12) / 12
+    F = 0.2
+    w = F * 12 * np.sin(2 * np.pi / 12) / HBAR
+    errs = []
+    for nsteps in (40, 80):
+        dt = 4.0 / nsteps
+        f, sumf = oracle.rt_step_field(L, p, 0.5 + 0.3 * np.cos(theta), p.N, [F, 0, 0], dt, nsteps)
+        errs.append(np.abs(f - (0.5 + 0.3 * np.cos(theta - w * 4.0))).max())
+        assert np.abs(sumf - sumf[0]).max() <= 1e-13 * sumf[0]
+    assert errs[0] < 1e-4 and 12 < errs[0] / errs[1] < 20
+    # with the field off the driver is the plain rt_step
+    p2, L2 = make_problem("tiny", grid=(4, 4, 4), seed=5), None
+    L2 = oracle.OracleList(p2)
+    fa, sa = oracle.rt_step_field(L2, p2, p2.f, p2.N, [0, 0, 0], 1.0, 3)
+    fb, sb = L2.rt_step(p2.f, p2.N, 1.0, 3)
+    assert np.array_equal(fa, fb) and np.array_equal(sa, sb)
+
+
+def test_transport_moments_closed_form():
+    # states whose velocity points along one axis each, F = 2 v, f0 = 1/2: S = diag(count_al / 4 * 2), n = ns / 2
+    ns = 12
+    v = np.zeros((3, ns)); v[np.arange(ns) % 3, np.arange(ns)] = 1.0
+    S, n = oracle.transport_moments(np.full(ns, 0.5), v, 2 * v)
+    assert np.array_equal(S, np.diag([2.0, 2.0, 2.0])) and n == 6.0
+    # F = c v with any v: S is symmetric; one state with v = (1, 2, 3), F = (4, 5, 6), f0 = 0.2: outer product
+    rng = np.random.default_rng(5)
+    v = rng.normal(size=(3, 40)); f0 = rng.uniform(0, 1, 40)
+    S, _ = oracle.transport_moments(f0, v, 3.0 * v)
+    assert np.allclose(S, S.T, rtol=0, atol=1e-13)
+    S, n = oracle.transport_moments([0.2], [[1.0], [2.0], [3.0]], [[4.0], [5.0], [6.0]])
+    assert np.allclose(S, 0.16 * np.outer([1, 2, 3], [4, 5, 6]), rtol=1e-15) and n == 0.2
