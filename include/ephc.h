@@ -220,6 +220,21 @@ int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev
 int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
                  double *sumf_dev, void *stream);
 
+/* Drift term of Eq. 1: out[s] = -(1/hbar) F . grad_k f.  The paper gives no discretisation (its Methods
+ * section is missing); reading R-25 of DESIGN.md: central differences on the k grid in reduced coordinates,
+ * (grad f)_i ~ N_i/2 [f(n, k+e_i) - f(n, k-e_i)] with k +- e_i modulo the grid, a neighbour that is not an active k
+ * point counts as f = 0; field = 3 HOST doubles, the components of F along the reduced axes in eV. */
+int ephc_drift(ephc_handle *h, const double *f_dev, const double *field, double *out_dev, void *stream);
+/* ephc_rt_step with the drift term: RK4 on df/dt = -(1/hbar) F . grad_k f + I[f] (Eq. 1 as printed). */
+int ephc_rt_step_field(ephc_handle *h, double *f_dev, const double *N_dev, const double *field, double dt_fs,
+                       int nsteps, double *sumf_dev, void *stream);
+/* Post-processing of the transport solution (reading R-26): out10_dev[3 al + be] = sum_s f0_s (1 - f0_s) v[al][s] F[be][s]
+ * (al, be = x, y, z; -df0/dE = f0 (1 - f0) / k_B T for a Fermi-Dirac f0) and out10_dev[9] = sum_s f0_s, summed on the
+ * device in a fixed order.  Conductivity = e^2 / (Omega N_k k_B T) * S, mobility = e S / (k_B T n): the constants
+ * (cell volume, temperature) are the caller's. */
+int ephc_transport_moments(ephc_handle *h, const double *f0_dev, const double *v_dev, const double *F_dev,
+                           double *out10_dev, void *stream);
+
 /* One stage of the same RK4 step, for callers that exchange data between the stages (k-sharded handles):
  *   stage 1..3: y_out = f + a dt I[y_in] (a = 1/2, 1/2, 1), the handle accumulates b I[y_in];
  *   stage 4:    f += dt/6 (accumulated + I[y_in]) in place (y_out may be NULL).

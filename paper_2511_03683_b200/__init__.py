@@ -68,6 +68,9 @@ def _load():
         "ephc_build_channels_range": (i32, [C.POINTER(_Problem), i32, i32, C.POINTER(vp)]),
         "ephc_owned_states": (i32, [vp, C.POINTER(i64), C.POINTER(i64)]),
         "ephc_rt_stage": (i32, [vp, vp, vp, vp, dbl, i32, vp, vp]),
+        "ephc_drift": (i32, [vp, vp, C.POINTER(dbl), vp, vp]),
+        "ephc_rt_step_field": (i32, [vp, vp, vp, C.POINTER(dbl), dbl, i32, vp, vp]),
+        "ephc_transport_moments": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_query": (i32, [vp, C.POINTER(Counts)]),
         "ephc_export_channels": (i32, [vp] * 9),
         "ephc_export_diag": (i32, [vp] * 6),
@@ -280,6 +283,19 @@ class Handle:
         _check(_load().ephc_rt_stage(self._h, _dev_ptr(f, self.ns, "f"), _dev_ptr(y_in, self.ns, "y_in"),
                                      _dev_ptr(N, self.nq * self.nnu, "N"), float(dt_fs), int(stage),
                                      _dev_ptr(y_out, self.ns, "y_out"), _stream_ptr(stream)))
+
+    def drift(self, f, field, out, stream=None):
+        fld = (C.c_double * 3)(*[float(x) for x in field])
+        _check(_load().ephc_drift(self._h, _dev_ptr(f, self.ns, "f"), fld, _dev_ptr(out, self.ns, "out"), _stream_ptr(stream)))
+
+    def rt_step_field(self, f, N, field, dt_fs: float, nsteps: int, sumf=None, stream=None):
+        fld = (C.c_double * 3)(*[float(x) for x in field])
+        _check(_load().ephc_rt_step_field(self._h, _dev_ptr(f, self.ns, "f"), _dev_ptr(N, self.nq * self.nnu, "N"), fld,
+                                          float(dt_fs), int(nsteps), _dev_ptr(sumf, nsteps + 1, "sumf"), _stream_ptr(stream)))
+
+    def transport_moments(self, f0, v, F, out10, stream=None):
+        _check(_load().ephc_transport_moments(self._h, _dev_ptr(f0, self.ns, "f0"), _dev_ptr(v, 3 * self.ns, "v"),
+                                              _dev_ptr(F, 3 * self.ns, "F"), _dev_ptr(out10, 10, "out10"), _stream_ptr(stream)))
 
     def rt_step(self, f, N, dt_fs: float, nsteps: int, sumf=None, stream=None):
         _check(_load().ephc_rt_step(self._h, _dev_ptr(f, self.ns, "f"), _dev_ptr(N, self.nq * self.nnu, "N"),

@@ -41,6 +41,9 @@ struct ephc_handle {
     std::vector<double> E;               // copy of the band energies and window: the optional stores are built from them
     double emin = 0.0, emax = 0.0;
     bool tile_built = false, stream_built = false, res_built = false;
+    std::vector<int32_t> kfull;          // full-grid index of every active k (neighbour table of the drift term)
+    int32_t *d_nbr = nullptr;            // [6][nk] compact index of k +- e_i, -1 where that point is not active
+    double *d_drift = nullptr;           // drift term of the current RK stage
     bool ranged = false;                 // built by ephc_build_channels_range: owns the destination k in [d.k_lo, d.k_hi)
     RowHost rowhost;                     // kept only for EPHC_HOST_ONLY handles (ephc_export_rows)
     int variant = -1;  // -1: automatic (collision / rt_step on the tile store, transport on the gather store)
@@ -147,7 +150,7 @@ static void free_dev(ephc_handle *h) {
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
                     h->ds_blk_ent_off, h->dx_blob, h->dx_iqn, h->dx_tiles, h->dx_cta_ptr, h->dx_fc, h->dx_part,
                     h->dx_row_state, h->dx_state_row, h->dx_state_blk, h->dx_blk_row0, h->dx_blk_ent_ptr, h->dx_slot_off,
-                    h->dx_blk_ent_off, h->dp_ch, h->dp_ik, h->dp_ikq, h->dp_iq, h->dp_src, h->dp_targets, h->dp_sc_col};
+                    h->dx_blk_ent_off, h->dp_ch, h->dp_ik, h->dp_ikq, h->dp_iq, h->dp_src, h->dp_targets, h->dp_sc_col, h->d_nbr, h->d_drift};
     for (void *p : ptrs)
         if (p) cudaFree(p);
 }
@@ -505,6 +508,7 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
     }
     h->emin = p->emin;
     h->emax = p->emax;
+    h->kfull.assign(p->kfull, p->kfull + p->nk);
     h->g_entries = (int64_t)g.code.size();
     h->g_halfpairs = (int64_t)g.hp_k.size();
     h->n_wu = (int32_t)g.wus.size();
@@ -563,6 +567,26 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
              cudaMalloc((void **)&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, (ns + 255) / 256), 1) * 8) != cudaSuccess))
             rc = fail(EPHC_ENOMEM, "cudaMalloc (transport weights / RK4 scratch) failed");
         if (rc == EPHC_OK) h->bytes_transport += h->g_entries * 8 * (h->rows_ok ? 2 : 1);
+        if (rc == EPHC_OK) {  // neighbours of every active k along the three grid axes (drift term, reading R-25)
+            std::vector<int32_t> compact((size_t)nq, -1), nbr((size_t)6 * p->nk, -1);
+            for (int32_t k = 0; k < p->nk; ++k) compact[p->kfull[k]] = k;
+            const int32_t G0 = p->grid[0], G1 = p->grid[1], G2 = p->grid[2];
+            for (int32_t k = 0; k < p->nk; ++k) {
+                const int32_t kf = p->kfull[k];
+                const int32_t c[3] = {kf / (G1 * G2), (kf / G2) % G1, kf % G2};
+                const int32_t G[3] = {G0, G1, G2};
+                for (int i = 0; i < 3; ++i)
+                    for (int sgn = 0; sgn < 2; ++sgn) {
+                        int32_t cc[3] = {c[0], c[1], c[2]};
+                        cc[i] = (c[i] + (sgn ? G[i] - 1 : 1)) % G[i];
+                        nbr[(size_t)(2 * i + sgn) * p->nk + k] = compact[((int64_t)cc[0] * G1 + cc[1]) * G2 + cc[2]];
+                    }
+            }
+            int64_t bn = 0;
+            rc = upload(&h->d_nbr, nbr, &bn);
+            if (rc == EPHC_OK && cudaMalloc((void **)&h->d_drift, nb8) != cudaSuccess)
+                rc = fail(EPHC_ENOMEM, "cudaMalloc (drift term) failed");
+        }
     } else {
         h->bytes_gather = (int64_t)(g.code.size() * 4 + g.w.size() * 8 + g.hp_k.size() * 8 +
                                     g.tasks.size() * sizeof(Task) + g.rounds.size() * sizeof(Round) +
@@ -1542,10 +1566,24 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
 
 // One RK4 stage (reading R-18): k = I[y_in]; stage 1..3: y_out = f + a dt k and ksum accumulates b k; stage 4:
 // f += dt/6 (ksum + k) in place.  The axpy is the epilogue of the collision pass.
+static int launch_drift(ephc_handle *h, const double *f, const double *field, double *out, cudaStream_t s) {
+    const double c0 = field[0] * h->d.grid[0] / (2.0 * kHbar), c1 = field[1] * h->d.grid[1] / (2.0 * kHbar),
+                 c2 = field[2] * h->d.grid[2] / (2.0 * kHbar);
+    drift_kernel<<<(unsigned)((h->d.ns + 255) / 256), 256, 0, s>>>(f, h->d_nbr, c0, c1, c2, out, h->d.nk, h->d.nb);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
 static int rk_stage(ephc_handle *h, double *f_dev, const double *y_in, const double *N_dev, double dt_fs, int st, double *y_out,
-                    bool want_sum, cudaStream_t s) {
+                    bool want_sum, cudaStream_t s, const double *field = nullptr) {
     int rc;
     const int v = rt_variant(h);
+    const double *extra = nullptr;
+    if (field) {  // Eq. 1: k_j = D[y_j] + I[y_j]
+        if ((rc = launch_drift(h, y_in, field, h->d_drift, s))) return rc;
+        extra = h->d_drift;
+    }
     if (v >= 1) {
         FinishParams Fp;
         if (v >= 2) {
@@ -1564,6 +1602,7 @@ static int rk_stage(ephc_handle *h, double *f_dev, const double *y_in, const dou
         Fp.ynext = y_out;
         Fp.ksum = h->d_ksum;
         Fp.blk_sum = want_sum ? h->d_wusum : nullptr;
+        Fp.extra = extra;
         return launch_finish<kFRkStage>(h, Fp, s);
     }
     GatherParams P = base_params(h);
@@ -1572,6 +1611,7 @@ static int rk_stage(ephc_handle *h, double *f_dev, const double *y_in, const dou
     P.f0 = f_dev;
     P.ksum = h->d_ksum;
     P.wu_sum = want_sum ? h->d_wusum : nullptr;
+    P.extra = extra;
     P.stage = st;
     P.f = y_in;
     P.ynext = y_out;
@@ -1588,8 +1628,43 @@ extern "C" int ephc_rt_stage(ephc_handle *h, double *f_dev, const double *y_in_d
     return rk_stage(h, f_dev, y_in_dev, N_dev, dt_fs, stage, y_out_dev, false, (cudaStream_t)stream);
 }
 
+static int rt_step_impl(ephc_handle *h, double *f_dev, const double *N_dev, const double *field, double dt_fs, int nsteps,
+                        double *sumf_dev, void *stream);
+
 extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
                             double *sumf_dev, void *stream) {
+    return rt_step_impl(h, f_dev, N_dev, nullptr, dt_fs, nsteps, sumf_dev, stream);
+}
+
+extern "C" int ephc_rt_step_field(ephc_handle *h, double *f_dev, const double *N_dev, const double *field, double dt_fs,
+                                  int nsteps, double *sumf_dev, void *stream) {
+    if (!field || !std::isfinite(field[0]) || !std::isfinite(field[1]) || !std::isfinite(field[2]))
+        return fail(EPHC_EINVAL, "field: three finite components (host array) required");
+    return rt_step_impl(h, f_dev, N_dev, field, dt_fs, nsteps, sumf_dev, stream);
+}
+
+extern "C" int ephc_drift(ephc_handle *h, const double *f_dev, const double *field, double *out_dev, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f_dev || !out_dev || !field || !std::isfinite(field[0]) || !std::isfinite(field[1]) || !std::isfinite(field[2]))
+        return fail(EPHC_EINVAL, "null pointer or non-finite field");
+    if (f_dev == out_dev) return fail(EPHC_EINVAL, "ephc_drift is out of place");
+    return launch_drift(h, f_dev, field, out_dev, (cudaStream_t)stream);
+}
+
+extern "C" int ephc_transport_moments(ephc_handle *h, const double *f0_dev, const double *v_dev, const double *F_dev,
+                                      double *out10_dev, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!f0_dev || !v_dev || !F_dev || !out10_dev) return fail(EPHC_EINVAL, "null device pointer");
+    moments_kernel<<<1, 1024, 0, (cudaStream_t)stream>>>(f0_dev, v_dev, F_dev, h->d.ns, out10_dev);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
+
+static int rt_step_impl(ephc_handle *h, double *f_dev, const double *N_dev, const double *field, double dt_fs, int nsteps,
+                        double *sumf_dev, void *stream) {
     int rc = need_device(h);
     if (rc) return rc;
     if (!f_dev || !N_dev) return fail(EPHC_EINVAL, "null device pointer");
@@ -1607,7 +1682,7 @@ extern "C" int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, 
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
         for (int st = 0; st < 4; ++st)
-            if ((rc = rk_stage(h, f_dev, src[st], N_dev, dt_fs, st + 1, dst[st], sumf_dev != nullptr, s))) return rc;
+            if ((rc = rk_stage(h, f_dev, src[st], N_dev, dt_fs, st + 1, dst[st], sumf_dev != nullptr, s, field))) return rc;
         if (sumf_dev) {
             if (rt_variant(h) >= 1)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);

@@ -41,6 +41,7 @@ struct GatherParams {
     double *ynext;     // y_{j+1} (stages 1..3)
     double *ksum;      // k1 + 2 k2 + 2 k3
     double *wu_sum;    // per work unit: sum of the updated f over its rows (stage 4)
+    const double *extra;  // added to k_j per state (drift term of Eq. 1), may be null
     // transport
     double *gW;        // per ordered entry W(a<-b): written by setup, read by iter
     const double *F, *v, *tau;
@@ -204,7 +205,7 @@ __global__ void __launch_bounds__(kThreads) gather_kernel(const GatherParams P) 
             for (int al = 0; al < 3; ++al)
                 P.out[(int64_t)al * P.ns + a] = ta * (P.v[(int64_t)al * P.ns + a] + sAcc[i * 3 + al]);
         } else {  // RK4 stage (reading R-18): k_j = I[y_j]
-            const double k = -sAcc[i];
+            const double k = -sAcc[i] + (P.extra ? P.extra[a] : 0.0);
             const double f0 = P.f0[a];
             if (P.stage == 1) {
                 P.ksum[a] = k;
@@ -247,6 +248,53 @@ __global__ void __launch_bounds__(1024) sum_kernel(const double *x, int64_t n, d
         __syncthreads();
     }
     if (threadIdx.x == 0) *out = s[0];
+}
+
+// Drift term of Eq. 1, reading R-25: out[n,k] = -(1/hbar) sum_i F_i N_i/2 (f[n, k+e_i] - f[n, k-e_i]);
+// nbr[d][k] = compact index of k + e_i (d = 2i) / k - e_i (d = 2i+1), or -1 when that grid point is not an active k.
+// coef[i] = F_i N_i / (2 hbar).
+__global__ void __launch_bounds__(256) drift_kernel(const double *__restrict__ f, const int32_t *__restrict__ nbr, double c0, double c1,
+                                                    double c2, double *__restrict__ out, int nk, int nb) {
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= (int64_t)nk * nb) return;
+    const int k = (int)(s / nb), n = (int)(s - (int64_t)k * nb);
+    const double coef[3] = {c0, c1, c2};
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int kp = nbr[(size_t)(2 * i) * nk + k], km = nbr[(size_t)(2 * i + 1) * nk + k];
+        const double fp = kp >= 0 ? f[(int64_t)kp * nb + n] : 0.0, fm = km >= 0 ? f[(int64_t)km * nb + n] : 0.0;
+        acc += coef[i] * (fp - fm);
+    }
+    out[s] = -acc;
+}
+
+// Transport post-processing (reading R-26): out[3 al + be] = sum_s f0 (1 - f0) v[al][s] F[be][s], out[9] = sum_s f0;
+// one CTA, fixed order (strided per-thread sums, shared-memory tree).
+__global__ void __launch_bounds__(1024) moments_kernel(const double *__restrict__ f0, const double *__restrict__ v,
+                                                       const double *__restrict__ F, int64_t ns, double *__restrict__ out) {
+    __shared__ double s[1024];
+    double a[10];
+#pragma unroll
+    for (int j = 0; j < 10; ++j) a[j] = 0.0;
+    for (int64_t i = threadIdx.x; i < ns; i += 1024) {
+        const double x = f0[i], wgt = x * (1.0 - x);
+#pragma unroll
+        for (int al = 0; al < 3; ++al)
+#pragma unroll
+            for (int be = 0; be < 3; ++be) a[3 * al + be] += wgt * v[(int64_t)al * ns + i] * F[(int64_t)be * ns + i];
+        a[9] += x;
+    }
+    for (int j = 0; j < 10; ++j) {
+        s[threadIdx.x] = a[j];
+        __syncthreads();
+        for (int o = 512; o > 0; o >>= 1) {
+            if ((int)threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) out[j] = s[0];
+        __syncthreads();
+    }
 }
 
 // tau = 1/Gamma (0 where Gamma == 0); F0[al] = tau * v[al]

@@ -57,6 +57,7 @@ struct FinishParams {
     int32_t stage;
     double dt;
     double *f0, *ynext, *ksum, *blk_sum;
+    const double *extra;  // added to k_j per state (drift term of Eq. 1), may be null
     // transport
     const double *v, *tau;
     int *reset;  // tile counter of the stream kernel, set back to 0 for the next evaluation (may be null)
@@ -412,7 +413,7 @@ __global__ void __launch_bounds__(256) finish_kernel(const FinishParams P) {
 #pragma unroll
             for (int c = 0; c < C; ++c) P.out[(int64_t)c * P.ns + a] = ta * (P.v[(int64_t)c * P.ns + a] + sum[c]);
         } else {  // RK4 stage (reading R-18): k_j = I[y_j]
-            const double k = sum[0];
+            const double k = sum[0] + (P.extra ? P.extra[a] : 0.0);
             const double f0 = P.f0[a];
             if (P.stage == 1) {
                 P.ksum[a] = k;

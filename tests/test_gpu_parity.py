@@ -399,6 +399,50 @@ def test_k_sharded_handles_on_one_gpu():
         assert _relerr(fs[0].cpu().numpy(), L.rt_step(p.f, p.N, 1.0, 3)[0]) <= TOL
 
 
+def test_drift_and_field_dynamics_match_oracle():
+    # Eq. 1 with its first term (reading R-25): the drift term alone, RK4 with field + collisions on every
+    # collision variant, and the field-free limit
+    field = [0.004, -0.002, 0.003]
+    for p in (_small_problems()[2], _small_problems()[1], _small_problems()[0]):
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p)
+        f, N = dev(p.f), dev(p.N)
+        D = torch.full((p.ns,), float("nan"), device="cuda", dtype=torch.float64)
+        h.drift(f, field, D)
+        Do = oracle.drift(p, p.f, field)
+        assert np.abs(Do).max() > 0 and np.abs(D.cpu().numpy() - Do).max() <= 1e-13 * np.abs(Do).max()
+        fo, so = oracle.rt_step_field(L, p, p.f, p.N, field, 1.0, 6)
+        for variant in (-1, 0, 2, 3):
+            h.set_variant(variant)
+            fr = dev(p.f)
+            sumf = torch.zeros(7, device="cuda", dtype=torch.float64)
+            h.rt_step_field(fr, N, field, 1.0, 6, sumf)
+            assert _relerr(fr.cpu().numpy(), fo) <= TOL
+            assert np.abs(sumf.cpu().numpy() - so).max() <= 1e-12 * abs(so[0])
+        f1, f2 = dev(p.f), dev(p.f)
+        h.rt_step_field(f1, N, [0.0, 0.0, 0.0], 1.0, 3, None)
+        h.rt_step(f2, N, 1.0, 3, None)
+        assert torch.equal(f1, f2)
+        assert np.abs(fo - L.rt_step(p.f, p.N, 1.0, 6)[0]).max() > 1e-6 * np.abs(fo).max()     # the field matters
+
+
+def test_transport_moments_match_oracle():
+    for p in (_small_problems()[2], _small_problems()[4]):
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p)
+        F, G = np.zeros((3, p.ns)), np.zeros(p.ns)
+        h.transport_solve_host(p.f0, p.N, p.v, 5, F, G)
+        out = torch.zeros(10, device="cuda", dtype=torch.float64)
+        h.transport_moments(dev(p.f0), dev(p.v), dev(F), out)
+        So, no = oracle.transport_moments(p.f0, p.v, F)
+        got = out.cpu().numpy()
+        assert np.abs(got[:9].reshape(3, 3) - So).max() <= 1e-12 * np.abs(So).max()
+        assert got[9] == pytest.approx(no, rel=1e-13)
+        out2 = torch.zeros(10, device="cuda", dtype=torch.float64)
+        h.transport_moments(dev(p.f0), dev(p.v), dev(F), out2)
+        assert torch.equal(out, out2)
+
+
 def test_stream_argument_is_honoured():
     p = make_problem("si", grid=(12, 12, 12), pair_prob=0.3, seed=3)
     h = ephc.build_channels(p)
