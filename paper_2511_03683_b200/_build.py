@@ -34,6 +34,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-Xcompiler", "-fPIC,-fopenmp,-O2,-ffp-contract=off", "-shared", "-o", tmp]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("EPHC_BUILD_FLAGS", "").split()   # e.g. -DEPHC_RES_TIMING for a working build
     cmd += [os.path.join(CSRC, f) for f in SOURCES] + ["-lgomp"]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)

@@ -108,6 +108,7 @@ struct ephc_handle {
     ResHost rhost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_res)
     int32_t x_Ra = 0, x_Rcap = 0, x_RbMax = 0, x_ntile = 0, x_ncta = 0, x_nrows = 0;
     int64_t x_entries = 0, x_part_rows = 0, x_smem_tile = 0, bytes_res = 0;
+    int x_mode = 0;  // launch mode of res_kernel (kResModes)
     unsigned char *dx_blob = nullptr;
     uint32_t *dx_iqn = nullptr;
     ResTile *dx_tiles = nullptr;
@@ -131,7 +132,8 @@ struct ephc_handle {
     double *dr_W = nullptr, *dr_Fc = nullptr;
     int32_t r_nrows = 0;
     uint16_t *dr_idx = nullptr;
-    uint32_t *dr_perm = nullptr;
+    uint32_t *dr_meta = nullptr;  // per entry: (iq * nnu + mode) | kind << 31
+    double *dr_wst = nullptr;     // per entry: channel weight
     RowSeg *dr_segs = nullptr;
     RowTile *dr_tiles = nullptr;
     RowStrip *dr_strips = nullptr;
@@ -144,7 +146,7 @@ static void free_dev(ephc_handle *h) {
                     h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
-                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_idx, h->dr_perm, h->dr_segs, h->dr_tiles, h->dr_strips,
+                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_idx, h->dr_meta, h->dr_wst, h->dr_segs, h->dr_tiles, h->dr_strips,
                     h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
                     h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_order, h->ds_counter, h->ds_row_state,
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
@@ -301,19 +303,43 @@ static int make_stream_store(ephc_handle *h) {
     return rc;
 }
 
+// Launch modes of res_kernel: consumer threads, CTAs per SM, dynamic shared memory per CTA (the tile images are built
+// for that budget; 227 KB per SM minus 1 KB per CTA and the static barriers).
+struct ResMode {
+    int nl, ctas;
+    int64_t smem;
+};
+static const ResMode kResModes[] = {{256, 2, 112 * 1024}, {512, 1, 225 * 1024}, {256, 1, 225 * 1024}, {384, 1, 225 * 1024},
+                                    {128, 4, 55 * 1024},  {512, 2, 112 * 1024}, {768, 1, 225 * 1024}};
+constexpr int kResNModes = (int)(sizeof(kResModes) / sizeof(kResModes[0]));
+constexpr int kResDefaultMode = 0;
+
 static int make_res_store(ephc_handle *h) {
     if (h->res_built) return EPHC_OK;
     const ephc_problem q = problem_view(h);
     std::string err;
     ResHost xh;
-    int nshare = kResCtasPerSm * h->n_sm;
+    // Launch mode: two CTAs of 8 consumer warps per SM overlap best; when the rows of a half-size tile would carry fewer
+    // than about six entries (sparse, few channels per pair), one CTA of 16 warps with tiles twice as large wins.
+    h->x_mode = kResDefaultMode;
+    {
+        int64_t nrows = 0;
+        for (int64_t st = 0; st < h->d.ns; ++st) nrows += q.E[st] >= q.emin && q.E[st] <= q.emax;
+        const double per_pair = (double)h->can.nw / (double)std::max<int64_t>(1, h->can.npair_active);
+        const double rho = (double)h->can.nw / (0.5 * (double)nrows * (double)nrows + 1.0);
+        const double fit = 44000.0 / (15.5 + 8.0 * h->d.nnu / std::max(1.0, per_pair));
+        if (per_pair < 64.0 && std::sqrt(rho * fit) < 6.0) h->x_mode = 1;
+    }
+    if (const char *e = std::getenv("EPHC_RES_MODE")) h->x_mode = std::min(kResNModes - 1, std::max(0, std::atoi(e)));
+    const ResMode &md = kResModes[h->x_mode];
+    int nshare = md.ctas * h->n_sm;
     if (const char *e = std::getenv("EPHC_RES_CTAS")) nshare = std::max(1, std::atoi(e));
-    int64_t cap = kResSmemCap;
-    if (const char *e = std::getenv("EPHC_RES_SMEM")) cap = std::max(8192, std::atoi(e));
-    int rc = build_res(&q, h->d, h->can, nshare, cap, xh, err);
+    int64_t cap = md.smem;
+    if (const char *e = std::getenv("EPHC_RES_SMEM")) cap = std::min<int64_t>(md.smem, std::max(8192, std::atoi(e)));
+    int rc = build_res(&q, h->d, h->can, nshare, cap, md.nl / 32, xh, err);
     if (rc != EPHC_OK) return fail(rc, err);
     h->res_built = true;
-    h->res_ok = xh.supported && res_smem_total(xh.Ra, xh.Rcap, xh.RbMax, xh.smem_tile) <= kResSmemCap;
+    h->res_ok = xh.supported && res_smem_total(xh.Ra, xh.Rcap, xh.smem_tile) <= md.smem;
     h->res_why = xh.supported ? "shared-memory budget exceeded" : xh.why;
     h->x_ncta = xh.ncta;
     h->x_ntile = (int32_t)xh.tiles.size();
@@ -417,14 +443,13 @@ static int make_paper_store(ephc_handle *h) {
 }
 
 // Automatic choice for collision / RK stages (measured on B200): the two-sided gather store while
-// it stays resident in the 126 MB L2; beyond that the resident-tile store when a (k,k') pair carries many channels
-// (large cells: 4.99e7 channels, nb = 16, nnu = 36: 343 us vs 597 us on the stream store) and the stream store
-// otherwise (1.26e7 channels, nb = 4: 126 us vs 134 us; 1.94e8 channels, nb = 1: 2.44 ms vs 4.2 ms).
+// it stays resident in the 126 MB L2; beyond that the resident-tile store (round 2: 126 us vs 130 us on the stream store
+// at 1.26e7 channels, nb = 4; 2.12 ms vs 2.45 ms at 1.94e8 channels, nb = 1; 335 us vs 597 us at 4.99e7 channels,
+// nb = 16, nnu = 36); the stream store remains the fallback when a problem exceeds the tile format's limits.
 static int auto_coll_variant(const ephc_handle *h) {
     if (h->ranged) return 0;  // a k-sharded handle owns destinations: the two-sided, destination-sorted store
     if (h->g_entries * 12 <= (int64_t)96 << 20) return 0;
-    const double per_pair = (double)h->can.nw / (double)std::max<int64_t>(1, h->can.npair_active);
-    return per_pair >= 64.0 ? 3 : 2;
+    return 3;
 }
 
 static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ranged, ephc_handle **out);
@@ -529,7 +554,7 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         h->r_Rb = rh.Rb;
         h->r_Ra = rh.Ra;
         h->r_nrows = rh.nrows;
-        h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.perm.size() * 4 + rh.segs.size() * sizeof(RowSeg) +
+        h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.meta.size() * 4 + rh.wst.size() * 8 + rh.segs.size() * sizeof(RowSeg) +
                                   rh.tiles.size() * sizeof(RowTile) + rh.strips.size() * sizeof(RowStrip) +
                                   (rh.row_state.size() + rh.state_row.size()) * 4);
         if (h->host_only) h->rowhost = rh;
@@ -548,7 +573,8 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         if (rc == EPHC_OK && h->rows_ok) {
             int64_t br = 0;
             rc = upload(&h->dr_idx, rh.idx, &br);
-            if (rc == EPHC_OK) rc = upload(&h->dr_perm, rh.perm, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_meta, rh.meta, &br);
+            if (rc == EPHC_OK) rc = upload(&h->dr_wst, rh.wst, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_segs, rh.segs, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_tiles, rh.tiles, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_strips, rh.strips, &br);
@@ -561,12 +587,12 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         // enqueue work ("allocated once"): transport weights in gather and row order, RK4 scratch, sums
         const size_t nb8 = (size_t)ns * 8, ne8 = (size_t)std::max<int64_t>(1, h->g_entries) * 8;
         if (rc == EPHC_OK &&
-            (cudaMalloc((void **)&h->d_gW, ne8) != cudaSuccess || (h->rows_ok && cudaMalloc((void **)&h->dr_W, ne8) != cudaSuccess) ||
+            ((!h->rows_ok && cudaMalloc((void **)&h->d_gW, ne8) != cudaSuccess) || (h->rows_ok && cudaMalloc((void **)&h->dr_W, ne8) != cudaSuccess) ||
              cudaMalloc((void **)&h->d_y[0], nb8) != cudaSuccess || cudaMalloc((void **)&h->d_y[1], nb8) != cudaSuccess ||
              cudaMalloc((void **)&h->d_ksum, nb8) != cudaSuccess ||
              cudaMalloc((void **)&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, (ns + 255) / 256), 1) * 8) != cudaSuccess))
             rc = fail(EPHC_ENOMEM, "cudaMalloc (transport weights / RK4 scratch) failed");
-        if (rc == EPHC_OK) h->bytes_transport += h->g_entries * 8 * (h->rows_ok ? 2 : 1);
+        if (rc == EPHC_OK) h->bytes_transport += h->g_entries * 8;
         if (rc == EPHC_OK) {  // neighbours of every active k along the three grid axes (drift term, reading R-25)
             std::vector<int32_t> compact((size_t)nq, -1), nbr((size_t)6 * p->nk, -1);
             for (int32_t k = 0; k < p->nk; ++k) compact[p->kfull[k]] = k;
@@ -975,10 +1001,11 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
     const int nnu = h->d.nnu;
     if ((int32_t)t.cta_ptr.size() != t.ncta + 1 || t.cta_ptr[0] != 0 || t.cta_ptr[t.ncta] != (int32_t)t.tiles.size())
         return fail(EPHC_ESTATE, "internal: schedule does not list every tile");
-    if (res_smem_total(t.Ra, t.Rcap, t.RbMax, t.smem_tile) > kResSmemCap || t.Ra % 2 || t.Rcap % 2 || t.RbMax % 2)
+    if (res_smem_total(t.Ra, t.Rcap, t.smem_tile) > t.smem_cap || t.Ra % 2 || t.Rcap % 2 || t.RbMax % 2)
         return fail(EPHC_ESTATE, "internal: shared-memory plan");
     int64_t o = 0;
     std::vector<int32_t> owner, used;
+    std::vector<uint8_t> row_out, row_in;
     size_t irun = 0;
     for (int32_t cta = 0; cta < t.ncta; ++cta) {
         for (int32_t it = t.cta_ptr[cta]; it < t.cta_ptr[cta + 1]; ++it) {
@@ -997,12 +1024,15 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
                 return fail(EPHC_ESTATE, "internal: bad run / tile header");
             if (D.flags & 2) ++irun;
             ResTile Dl = D;
-            res_set_layout(Dl, t.nl, nnu);
+            res_set_layout(Dl, t.nwarp);
+            if (D.pad != 0 || D.o_sn_next != (it + 1 < t.cta_ptr[cta + 1] ? res_o_sn(t.tiles[it + 1]) : 0u))
+                return fail(EPHC_ESTATE, "internal: where the next tile's N rows go");
             const int32_t R = run.a_rows + D.b_rows;
             if (D.ne < 1 || std::memcmp(&Dl, &D, sizeof(D)) != 0 || (int64_t)D.a_off != t.slot_off[D.a_slot] ||
                 (D.b_slot >= 0 && (int64_t)D.b_off != t.slot_off[D.b_slot]) || D.blob_off % 128 != 0 || D.blob_off + D.blob_bytes > (int64_t)t.blob.size() ||
                 res_tile_smem(D, nnu) > t.smem_tile || R > t.Rcap || D.b_rows > t.RbMax || R > kResRowMax || D.nq * nnu > kResSlotMax ||
-                D.ne + D.npiece + D.npart > kResXMax || D.ngl1 > D.ne + D.npiece || D.ngl2 != D.npart ||
+                D.ne_pad % 32 || D.ng_pad % 32 || D.ne_pad > kResXMax - 1 || D.ne_pad / 32 > 1023 || D.ng_pad / 32 > 1023 || D.ne > D.ne_pad ||
+                D.ne > D.ng_pad || D.nslab1 < 1 || D.nslab2 < 1 ||
                 (D.b_rows > 0) != (D.b_slot >= 0) || (D.b_rows > 0 && (D.b_row0 < run.a_row0 + run.a_rows || D.b_row0 % 2 || run.a_rows % 2)) ||
                 (D.b_slot >= 0 && (t.slot_row0[D.b_slot] != D.b_row0 || t.slot_rows[D.b_slot] != D.b_rows)) ||
                 D.q0 < 0 || D.q0 + D.nq > (int64_t)t.iqn.size())
@@ -1012,98 +1042,87 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
             const unsigned char *B = t.blob.data() + D.blob_off;
             const uint32_t *code = reinterpret_cast<const uint32_t *>(B);
             const uint16_t *perm = reinterpret_cast<const uint16_t *>(B + D.o_perm);
-            const uint16_t *prow = reinterpret_cast<const uint16_t *>(B + D.o_prow);
-            const uint16_t *pf = reinterpret_cast<const uint16_t *>(B + D.o_pf);
-            const uint16_t *tf = reinterpret_cast<const uint16_t *>(B + D.o_tf);
-            const uint16_t *d1 = reinterpret_cast<const uint16_t *>(B + D.o_d1);
-            const uint16_t *d2 = reinterpret_cast<const uint16_t *>(B + D.o_d2);
-            const uint32_t *cols = reinterpret_cast<const uint32_t *>(B + D.o_cols);
+            const uint16_t *srow1 = reinterpret_cast<const uint16_t *>(B + D.o_srow1);
+            const uint32_t *shdr1 = reinterpret_cast<const uint32_t *>(B + D.o_shdr1);
+            const uint16_t *srow2 = reinterpret_cast<const uint16_t *>(B + D.o_srow2);
+            const uint32_t *shdr2 = reinterpret_cast<const uint32_t *>(B + D.o_shdr2);
             const double *wv = reinterpret_cast<const double *>(B + D.o_w);
+            const uint16_t *wptr = reinterpret_cast<const uint16_t *>(B + D.o_wptr);
             auto row_of = [&](int32_t loc) { return loc < run.a_rows ? run.a_row0 + loc : D.b_row0 + (loc - run.a_rows); };
-            // phase 1 exactly as the kernel walks it: owner[x] = local row that must receive X[x]
-            const int32_t nx = D.ne + D.npiece + D.npart;
-            owner.assign((size_t)nx, -1);
-            used.assign((size_t)nx, 0);
-            int32_t pieces_seen = 0;
-            for (int32_t l = 0; l < t.nl; ++l) {
-                int32_t piece = pf[l], combo_in = -1;
-                bool open = false;
-                for (int32_t j = 0; j < D.nc1; ++j) {
-                    const int32_t cnt = (int32_t)(cols[j] & 0xffffu), base = (int32_t)(cols[j] >> 16);
-                    if (l >= cnt) break;
-                    const int32_t e = base + l;
-                    if (piece >= D.npiece || prow[piece] >= R || e < 0 || e >= D.ne || owner[e] != -1)
-                        return fail(EPHC_ESTATE, "internal: entry visited twice / piece out of range");
-                    const uint32_t cd = code[e];
-                    const int32_t in_loc = (int32_t)((cd & 0xffffu) >> 3), slot = (int32_t)(cd >> 19);
-                    if ((cd & 4u) || (cd & 3u) == 3u || in_loc >= R || slot / nnu >= D.nq)
-                        return fail(EPHC_ESTATE, "internal: entry code out of range");
-                    if (combo_in >= 0 && combo_in != in_loc) return fail(EPHC_ESTATE, "internal: a combo mixes in rows");
-                    combo_in = (cd & 2u) ? in_loc : -1;
-                    owner[e] = (cd & 2u) ? -2 : in_loc;  // -2: its term is part of the combo that ends later in this lane
-                    const int32_t ro = row_of(prow[piece]), ri = row_of(in_loc);
-                    if (ro == ri) return fail(EPHC_ESTATE, "internal: entry with equal ends");
-                    const int64_t x = o + e;
-                    if (a) a[x] = t.row_state[std::min(ro, ri)];
-                    if (b) b[x] = t.row_state[std::max(ro, ri)];
-                    if (iq) iq[x] = (int32_t)(t.iqn[D.q0 + slot / nnu] / (uint32_t)nnu);
-                    if (nu) nu[x] = slot % nnu;
-                    if (kind) kind[x] = ro < ri ? 1 : 0;  // out = a: emission weight; out = b: absorption weight
-                    if (w) w[x] = wv[e];
-                    open = true;
-                    if (cd & 1u) {
-                        if (owner[D.ne + piece] >= 0) return fail(EPHC_ESTATE, "internal: piece closed twice");
-                        owner[D.ne + piece] = prow[piece];
-                        ++piece;
-                        ++pieces_seen;
-                        open = false;
-                    }
-                }
-                if (open) return fail(EPHC_ESTATE, "internal: a lane ends inside a piece");
-            }
-            if (pieces_seen != D.npiece) return fail(EPHC_ESTATE, "internal: piece count");
-            for (int32_t e = 0; e < D.ne; ++e)
-                if (owner[e] == -1) return fail(EPHC_ESTATE, "internal: entry not covered by any lane");
-            // phase 2: every X value is added exactly once, to its owner row (directly or through one partial sum)
-            std::vector<uint8_t> row_final((size_t)R, 0), task_seen((size_t)D.ntask1, 0);
-            for (int32_t l = 0; l < t.nl; ++l) {
-                int32_t task = tf[l], row = -1;
-                for (int32_t j = 0; j < D.nc2; ++j) {
-                    const int32_t cnt = (int32_t)(cols[D.nc1 + j] & 0xffffu), base = (int32_t)(cols[D.nc1 + j] >> 16);
-                    if (l >= cnt) break;
-                    const uint32_t wd = perm[base + l];
-                    const int32_t x = (int32_t)(wd & 0x7fffu);
-                    if (base + l >= D.ngl1 || x >= D.ne + D.npiece || owner[x] < 0 || used[x]++) return fail(EPHC_ESTATE, "internal: gather list");
-                    if (row < 0) row = owner[x];
-                    if (owner[x] != row) return fail(EPHC_ESTATE, "internal: gather task mixes rows");
-                    if (wd & 0x8000u) {
-                        if (task >= D.ntask1 || task_seen[task]++) return fail(EPHC_ESTATE, "internal: task index");
-                        const int32_t dst = d1[task++];
-                        if (dst & 0x8000) {
-                            if ((dst & 0x7fff) >= D.npart || owner[D.ne + D.npiece + (dst & 0x7fff)] >= 0)
-                                return fail(EPHC_ESTATE, "internal: partial index out of range");
-                            owner[D.ne + D.npiece + (dst & 0x7fff)] = row;
-                        } else if (dst != row || row_final[dst]++) {
-                            return fail(EPHC_ESTATE, "internal: final task of a row");
+            // Walks the slabs of one phase as the kernel does.  visit(row, position) is called for every position of a
+            // lane that owns a row; checks: the warps' slab ranges tile [0, nslab), the slabs tile [0, npos) in order,
+            // heights descend inside a warp, the lanes of a row are adjacent, in one slab only, and flagged.
+            auto walk = [&](const uint16_t *srow, const uint32_t *shdr, const uint16_t *wp, int32_t nslab, int32_t npos,
+                            std::vector<uint8_t> &row_seen, auto &&visit) -> bool {
+                row_seen.assign((size_t)R, 0);
+                int32_t next = 0;
+                if (wp[0] != 0 || wp[t.nwarp] != nslab) return false;
+                for (int32_t wi = 0; wi < t.nwarp; ++wi) {
+                    if (wp[wi + 1] < wp[wi]) return false;
+                    int32_t prevH = kResHMax + 1;
+                    for (int32_t sl = wp[wi]; sl < wp[wi + 1]; ++sl) {
+                        const uint32_t hd = shdr[sl];
+                        const int32_t base = (int32_t)(hd & 1023u) * 32, H = (int32_t)((hd >> kResHdrHShift) & kResHdrHMask);
+                        if (base != next || H > prevH || base + 32 * H > npos || (hd & ~(kResHdrMulti | 0x7ffffu))) return false;
+                        prevH = H;
+                        next = base + 32 * H;
+                        bool multi = false;
+                        for (int l = 0; l < 32; ++l) {
+                            const uint16_t u = srow[32 * sl + l];
+                            if (u == kResNoRow) continue;
+                            if (u >= R) return false;
+                            if (l > 0 && srow[32 * sl + l - 1] == u) {
+                                multi = true;
+                            } else if (row_seen[u]++) {
+                                return false;
+                            }
+                            for (int32_t j = 0; j < H; ++j)
+                                if (!visit(u, base + 32 * j + l)) return false;
                         }
-                        row = -1;
+                        if (multi && !(hd & kResHdrMulti)) return false;
                     }
                 }
-                if (row >= 0) return fail(EPHC_ESTATE, "internal: a lane ends inside a gather task");
-            }
-            for (int32_t tk = 0; tk < D.ntask2; ++tk) {
-                const int32_t row = d2[tk];
-                if (row >= R || row_final[row]++) return fail(EPHC_ESTATE, "internal: two final tasks for a row");
-                for (int32_t j = 0; j < D.nc3; ++j) {
-                    const int32_t cnt = (int32_t)(cols[D.nc1 + D.nc2 + j] & 0xffffu), base = (int32_t)(cols[D.nc1 + D.nc2 + j] >> 16);
-                    if (tk >= cnt) break;
-                    const int32_t x = perm[D.ngl1 + base + tk];
-                    if (base + tk >= D.ngl2 || x < D.ne + D.npiece || x >= nx || used[x]++ || owner[x] != row)
-                        return fail(EPHC_ESTATE, "internal: round-2 gather list");
-                }
-            }
-            for (int32_t x = 0; x < nx; ++x)
-                if (used[x] != (owner[x] == -2 ? 0 : 1)) return fail(EPHC_ESTATE, "internal: X value not gathered exactly once");
+                return next == npos;
+            };
+            // phase 1: owner[pos] = b row of the weight at pos (-1: padding, w == 0); every a row is a row of the strip
+            owner.assign((size_t)D.ne_pad, -1);
+            used.assign((size_t)D.ne_pad, 0);
+            int32_t real = 0;
+            const bool ok1 = walk(srow1, shdr1, wptr, D.nslab1, D.ne_pad, row_out, [&](int32_t u, int32_t pos) {
+                if (used[pos]++ || u >= run.a_rows) return false;
+                const uint32_t cd = code[pos];
+                const int32_t in_loc = (int32_t)((cd & 0xffffu) >> 3), slot = (int32_t)(cd >> 19);
+                if ((cd & 7u) || in_loc >= R || slot / nnu >= D.nq) return false;
+                if (wv[pos] == 0.0) return cd == 0u;  // padding reads f of row 0 and N slot 0
+                const int32_t ro = row_of(u), ri = row_of(in_loc);
+                if (ro >= ri || (D.b_rows > 0 && in_loc < run.a_rows)) return false;
+                owner[pos] = in_loc;
+                const int64_t x = o + real++;
+                if (x >= t.nent) return false;
+                if (a) a[x] = t.row_state[ro];
+                if (b) b[x] = t.row_state[ri];
+                if (iq) iq[x] = (int32_t)(t.iqn[D.q0 + slot / nnu] / (uint32_t)nnu);
+                if (nu) nu[x] = slot % nnu;
+                if (kind) kind[x] = wv[pos] > 0.0 ? 1 : 0;  // the sign carries the kind: +w emission, -w absorption
+                if (w) w[x] = std::fabs(wv[pos]);
+                return true;
+            });
+            if (!ok1 || real != D.ne || D.nslab1 < 1) return fail(EPHC_ESTATE, "internal: phase-1 slabs of a resident tile");
+            for (int32_t pos = 0; pos < D.ne_pad; ++pos)  // positions of lanes without a row hold padding
+                if (!used[pos] && (wv[pos] != 0.0 || code[pos] != 0u)) return fail(EPHC_ESTATE, "internal: weight in a lane without a row");
+            // phase 2: every T value is added exactly once, to its b row; off the diagonal every B row stores a sum
+            std::fill(used.begin(), used.end(), 0);
+            int32_t gathered = 0;
+            const bool ok2 = walk(srow2, shdr2, wptr + t.nwarp + 1, D.nslab2, D.ng_pad, row_in, [&](int32_t u, int32_t g) {
+                const int32_t x = perm[g];
+                if (x == D.ne_pad) return true;  // the zero
+                if (x > D.ne_pad || owner[x] != u || used[x]++) return false;
+                ++gathered;
+                return true;
+            });
+            if (!ok2 || gathered != D.ne) return fail(EPHC_ESTATE, "internal: phase-2 slabs of a resident tile");
+            for (int32_t r = run.a_rows; r < R; ++r)
+                if (!row_in[r]) return fail(EPHC_ESTATE, "internal: a B row of a tile has no lane");
             o += D.ne;
         }
     }
@@ -1168,8 +1187,15 @@ static int set_kernel_attributes(int device) {
     CUDA_TRY(cudaFuncSetAttribute(gather_kernel<kTransportIter>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)gather_smem_bytes(kTransportIter)));
     CUDA_TRY(cudaFuncSetAttribute(stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    CUDA_TRY(cudaFuncSetAttribute(res_kernel<kResLanes>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResSmemCap));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResModes[0].smem));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResModes[1].smem));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResModes[2].smem));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<384, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResModes[3].smem));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<128, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResModes[4].smem));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResModes[5].smem));
+    CUDA_TRY(cudaFuncSetAttribute(res_kernel<768, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResModes[6].smem));
     CUDA_TRY(cudaFuncSetAttribute(row_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    CUDA_TRY(cudaFuncSetAttribute(row_setup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
 #define EPHC_TILE_ATTR(NB_)                                                                                          \
     CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTCollision, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, big)); \
     CUDA_TRY(cudaFuncSetAttribute(tile_kernel<kTSetup, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));     \
@@ -1342,7 +1368,7 @@ static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStre
         P.Rcap = h->x_Rcap;
         P.RbMax = h->x_RbMax;
         P.nnu = h->d.nnu;
-        P.buf_bytes = (uint32_t)res_buf_bytes(h->x_Rcap, h->x_RbMax, h->x_smem_tile);
+        P.buf_bytes = (uint32_t)res_buf_bytes(h->x_Rcap, h->x_smem_tile);
         P.fixed_bytes = (uint32_t)res_fixed_bytes(h->x_Ra);
         P.gran16 = (h->d.nnu % 2 == 0) && ((reinterpret_cast<uintptr_t>(N) & 15) == 0);
         P.gran = P.gran16 ? h->d.nnu / 2 : h->d.nnu;
@@ -1352,25 +1378,34 @@ static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStre
         P.part = h->dx_part;
 #ifdef EPHC_RES_TIMING
         static long long *dbg = nullptr;
-        const size_t ndbg = (size_t)h->x_ncta * (kResLanes / 32) * 8;
+        const size_t ndbg = (size_t)h->x_ncta * (kResModes[h->x_mode].nl / 32 + 1) * 8;
         if (!dbg) cudaMalloc((void **)&dbg, ndbg * 8);
         cudaMemset(dbg, 0, ndbg * 8);
         P.dbg = dbg;
 #endif
-        res_kernel<kResLanes><<<(unsigned)h->x_ncta, kResLanes + 32,
-                                  (size_t)res_smem_total(h->x_Ra, h->x_Rcap, h->x_RbMax, h->x_smem_tile), s>>>(P);
+        const size_t smem = (size_t)res_smem_total(h->x_Ra, h->x_Rcap, h->x_smem_tile);
+        const unsigned grid = (unsigned)h->x_ncta;
+        switch (h->x_mode) {
+            case 0: res_kernel<256, 2><<<grid, 256 + 32, smem, s>>>(P); break;
+            case 1: res_kernel<512, 1><<<grid, 512 + 32, smem, s>>>(P); break;
+            case 2: res_kernel<256, 1><<<grid, 256 + 32, smem, s>>>(P); break;
+            case 3: res_kernel<384, 1><<<grid, 384 + 32, smem, s>>>(P); break;
+            case 4: res_kernel<128, 4><<<grid, 128 + 32, smem, s>>>(P); break;
+            case 5: res_kernel<512, 2><<<grid, 512 + 32, smem, s>>>(P); break;
+            default: res_kernel<768, 1><<<grid, 768 + 32, smem, s>>>(P); break;
+        }
         h->launches++;
 #ifdef EPHC_RES_TIMING
         if (std::getenv("EPHC_RES_TIMING_PRINT")) {
             std::vector<long long> hd(ndbg);
             cudaMemcpy(hd.data(), dbg, ndbg * 8, cudaMemcpyDeviceToHost);
-            const char *nm[8] = {"loop", "wait full", "phase 1", "barrier", "phase 2 r1", "round 2", "barrier", "copy-out"};
-            const int nw = kResLanes / 32;
+            const char *nm[8] = {"loop", "wait full", "phase 1", "barrier", "phase 2", "barrier", "copy-out", "release"};
+            const int nw = kResModes[h->x_mode].nl / 32;
             for (int k = 0; k < 8; ++k) {
                 double mean = 0, w0 = 0, wl = 0, mx = 0;
                 for (int c = 0; c < h->x_ncta; ++c)
                     for (int w = 0; w < nw; ++w) {
-                        const double v = (double)hd[((size_t)c * nw + w) * 8 + k];
+                        const double v = (double)hd[((size_t)c * (nw + 1) + w) * 8 + k];
                         mean += v;
                         mx = std::max(mx, v);
                         if (w == 0) w0 += v;
@@ -1378,6 +1413,12 @@ static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStre
                     }
                 std::fprintf(stderr, "res timing %-14s mean %9.0f  warp0 %9.0f  last warp %9.0f  max %9.0f cycles per CTA\n", nm[k],
                              mean / (h->x_ncta * nw), w0 / h->x_ncta, wl / h->x_ncta, mx);
+            }
+            const char *pn[6] = {"loop", "wait empty", "dir + bulk", "wait prev", "N staging", "until full"};
+            for (int k = 0; k < 6; ++k) {
+                double mean = 0;
+                for (int c = 0; c < h->x_ncta; ++c) mean += (double)hd[((size_t)c * (nw + 1) + nw) * 8 + k];
+                std::fprintf(stderr, "res producer %-12s mean %9.0f cycles per CTA (%d tiles)\n", pn[k], mean / h->x_ncta, h->x_ntile);
             }
         }
 #endif
@@ -1459,6 +1500,26 @@ extern "C" int ephc_collision(ephc_handle *h, const double *f_dev, const double 
     return launch_gather<kCollision>(h, P, (cudaStream_t)stream);
 }
 
+static RowParams row_params(const ephc_handle *h) {
+    RowParams R;
+    std::memset(&R, 0, sizeof(R));
+    R.W = h->dr_W;
+    R.wst = h->dr_wst;
+    R.meta = h->dr_meta;
+    R.idx = h->dr_idx;
+    R.segs = h->dr_segs;
+    R.tiles = h->dr_tiles;
+    R.strips = h->dr_strips;
+    R.row_state = h->dr_row_state;
+    R.state_row = h->dr_state_row;
+    R.Rb = h->r_Rb;
+    R.Ra = h->r_Ra;
+    R.nstrip = h->r_nstrip;
+    R.ns = h->d.ns;
+    R.Fc = h->dr_Fc;
+    return R;
+}
+
 extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const double *N_dev, double *Gamma_dev,
                                     void *stream) {
     int rc = need_device(h);
@@ -1478,17 +1539,26 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
         }
         return rc;
     }
-    GatherParams P = base_params(h);
-    P.f = f0_dev;
-    P.N = N_dev;
-    P.out = Gamma_dev;
-    rc = launch_gather<kTransportSetup>(h, P, (cudaStream_t)stream);
-    if (rc == EPHC_OK && h->rows_ok && h->g_entries > 0) {
-        // the iteration runs on the row store: same ordered terms, regrouped; bring the weights into its order
-        row_permute_kernel<<<(unsigned)((h->g_entries + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
-            h->d_gW, h->dr_perm, h->dr_W, h->g_entries);
+    if (h->rows_ok) {
+        // the row store holds every ordered term with its weight, N index and kind: weights and Gamma in one pass, written
+        // in the order row_iter_kernel streams them
+        const cudaStream_t s = (cudaStream_t)stream;
+        if (h->r_nrows > 0) {
+            row_compact1_kernel<<<(unsigned)((h->r_nrows + 255) / 256), 256, 0, s>>>(f0_dev, h->dr_row_state, h->dr_Fc, h->r_nrows);
+            h->launches++;
+        }
+        RowParams R = row_params(h);
+        R.N = N_dev;
+        R.out = Gamma_dev;
+        row_setup_kernel<<<(unsigned)std::max(h->r_nstrip, 1), kRowThreads, row_smem_bytes(h->r_Rb, h->r_Ra), s>>>(R);
         h->launches++;
         CUDA_TRY(cudaGetLastError());
+    } else {
+        GatherParams P = base_params(h);
+        P.f = f0_dev;
+        P.N = N_dev;
+        P.out = Gamma_dev;
+        rc = launch_gather<kTransportSetup>(h, P, (cudaStream_t)stream);
     }
     if (rc == EPHC_OK) {
         h->transport_ready = true;
@@ -1528,19 +1598,7 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
         return launch_finish<kFIter>(h, Fp, (cudaStream_t)stream);
     }
     if (h->rows_ok) {
-        RowParams R;
-        std::memset(&R, 0, sizeof(R));
-        R.W = h->dr_W;
-        R.idx = h->dr_idx;
-        R.segs = h->dr_segs;
-        R.tiles = h->dr_tiles;
-        R.strips = h->dr_strips;
-        R.row_state = h->dr_row_state;
-        R.state_row = h->dr_state_row;
-        R.Rb = h->r_Rb;
-        R.Ra = h->r_Ra;
-        R.nstrip = h->r_nstrip;
-        R.ns = h->d.ns;
+        RowParams R = row_params(h);
         if (h->r_nrows > 0) {
             row_compact_kernel<<<(unsigned)((h->r_nrows + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
                 F_dev, h->dr_row_state, h->dr_Fc, h->r_nrows, h->d.ns);

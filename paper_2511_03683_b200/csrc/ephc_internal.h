@@ -165,7 +165,9 @@ struct RowHost {
     int32_t Rb = 0, Ra = 0, nrows = 0;
     std::vector<int32_t> row_state, state_row;
     std::vector<uint16_t> idx;        // per entry: partner row - col0 of its tile
-    std::vector<uint32_t> perm;       // per entry: index of the same ordered term in the gather store (weights come from there)
+    std::vector<uint32_t> perm;       // per entry: index of the same ordered term in the gather store (host only: export / tests)
+    std::vector<double> wst;          // per entry: the channel weight |g|^2 delta of this ordered term (transport_setup reads it)
+    std::vector<uint32_t> meta;       // per entry: (iq * nnu + mode) | kind << 31 (kind as seen from the destination)
     std::vector<RowSeg> segs;
     std::vector<RowTile> tiles;
     std::vector<RowStrip> strips;
@@ -222,50 +224,55 @@ struct StreamHost {
 int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, StreamHost &t, std::string &err);
 
 // ---- resident-tile store (variant 3, collision / RK stages) -----------------------------------------------------
-// Every weight is stored ONCE as a directed "emission-form" entry (out -> in):
-//     T = w [ (f_out - f_in) N + f_out (1 - f_in) ],   I[out] -= T,   I[in] += T
-// A channel's emission weight gives out = (n,k), in = (m,k+q); its absorption weight gives the reversed entry,
-// because F_abs(a,b) = -F_em(b,a) (reading R-1), so no per-entry kind is needed.
-// Compact rows are cut into strips of Ra rows; a tile holds the entries between one strip (A rows) and a narrow range
-// of rows after it (B rows), or inside the strip (diagonal tile), sized so that TWO tile images fit in shared memory:
-// an image is one contiguous, 16-byte aligned blob that the CTA fetches with bulk copies (TMA) one tile ahead and
-// then works on in place.  Consecutive tiles of a strip form a run: the strip's accumulators stay in shared memory
-// for the whole run.  The tiles in strip-major order are cut into one contiguous share of equal work per CTA and are
-// stored in that order.  The image is laid out for a CTA of NL = kResLanes threads:
-//   phase 1 (paper step 2): the out rows of the tile are cut into pieces of at most ceil(E / NL) entries and the
-//            pieces are packed into NL lanes of (almost) equal load, longest piece first; a lane walks its pieces one
-//            after the other, keeps f_out and -sum(T) in registers and overwrites w by T in shared memory; entry j of
-//            lane l sits at col1[j].base + l (lanes sorted by descending load: column-major, no padding); bit 0 of an
-//            entry code marks the last entry of a piece, whose sum then goes to X[ne + piece].
-//   phase 2 (paper step 3): per row one gather task = the X positions of its in-entries (T) and of its out pieces
-//            (negated sums), the last one with bit 15 set; the tasks are packed into NL lanes in the same way (word j
-//            of lane l at col2[j].base + l); a lane's tasks are numbered consecutively from tf[l] and d1[task] is the
-//            destination (a row, or 0x8000 | index of a partial sum).  Rows with more
-//            inputs than a lane's share are cut into partial tasks whose sums a second, small round adds (one lane
-//            per row, column tables col3).  One owner per row and round, fixed order, no atomics.
-struct ResTile {           // 144 bytes (device directory)
+// Every weight is stored ONCE, with the channel's first end a = (n,k) as its owner and the second end b = (m,k+q) as
+// its partner; the kind rides in the sign of the stored weight (emission +w, absorption -w; weights are positive):
+//     T = |ws| (f_a - f_b) N + ws (x - f_a f_b),  x = f_a (ws > 0) or f_b (ws < 0);   I[a] -= T,   I[b] += T
+// which is w F_em resp. w F_abs of Eq. 2 (reading R-1).
+// Compact rows are cut into strips of Ra rows; a tile holds the entries between one strip (A rows, the a ends) and a
+// range of rows after it (B rows, the b ends), or inside the strip (diagonal tile), sized so that TWO tile images fit
+// in shared memory: an image is one contiguous, 16-byte aligned blob that the CTA fetches with bulk copies (TMA) one
+// tile ahead and then works on in place.  Consecutive tiles of a strip form a run: the strip's accumulators stay in
+// shared memory for the whole run.  The tiles in strip-major order are cut into one contiguous share of equal work
+// per CTA and are stored in that order.  Inside an image the work is laid out in SLABS of 32 lanes x H columns,
+// column-major (element j of lane l at base + 32 j + l: every warp access is one coalesced shared-memory wavefront):
+//   phase 1 (paper step 2): the entries of an a row are cut into pieces of at most Hcap entries, the pieces are
+//            sorted by descending length (pieces of one row adjacent) and dealt 32 per slab; a lane walks its piece with
+//            f_a and sum(T) in registers and overwrites w by T; shorter lanes are padded with w = 0 entries.  Lanes of
+//            a slab that share a row (flag "multi") are combined with a segmented warp-shuffle reduction before the
+//            first of them subtracts the sum from the row's accumulator in shared memory.
+//   phase 2 (paper step 3): the same slab layout over the b rows: perm[] holds, per (slab, column, lane), the position
+//            of a T value of that row (padding points at a zero behind the entries); the sum of a B row goes straight
+//            to the tile's partial-sum slot in global memory (every B row of the tile has a lane, rows without
+//            entries store 0), on a diagonal tile it is added to the strip's accumulator.
+// One owner per row and phase, fixed order, no atomics.  The slabs of a phase are dealt to the warps of the CTA by the
+// host (longest first, to the least loaded warp) and stored warp by warp: warp w takes slabs wptr[w] .. wptr[w+1].
+struct ResTile {           // 120 bytes (device directory)
     int64_t blob_off;      // byte offset of the image in the blob array (multiple of 128)
     int32_t blob_bytes;    // multiple of 16
-    int32_t ne;            // entries
-    int32_t npiece;        // out-row pieces
-    int32_t npart;         // round-1 partial tasks
-    int32_t ntask1, ntask2;// round-1 tasks (final + partial), round-2 tasks (rows whose inputs were cut)
-    int32_t nc1, nc2, nc3; // columns of phase 1, of round 1 (both padded to multiples of 4 with empty columns), of round 2
-    int32_t ngl1, ngl2;    // stream words of round 1 (positions + destinations), gather-list elements of round 2
+    int32_t ne;            // weights (real entries)
+    int32_t ne_pad;        // phase-1 positions = 32 * sum of the slab heights; X[ne_pad] is the zero that padding reads
+    int32_t ng_pad;        // phase-2 positions
+    int32_t nslab1, nslab2;
     int32_t q0, nq;        // pairs: iqn[q0 .. q0+nq) = iq * nnu of the tile's pairs
     int32_t nq_next;       // pairs of the next tile of the same CTA: their iq * nnu ride in this image (section nxt)
     int32_t b_row0, b_rows;// B rows (b_rows = 0 on a diagonal tile)
     int32_t b_slot;        // partial-sum slot of the B rows (-1 on a diagonal tile)
     int32_t a_row0, a_rows, a_slot;  // the run's strip and its partial-sum slot
     int32_t flags;         // bit 0: first tile of its run, bit 1: last tile of its run
-    // byte offsets of the sections inside the image (= inside the tile buffer), each 16-byte aligned; w comes last so
-    // that the X tail (piece sums, partial sums) and then the N rows can follow it in shared memory
-    uint32_t o_perm, o_prow, o_pf, o_tf, o_d1, o_d2, o_cols, o_nxt, o_w, o_sn;
+    // byte offsets of the sections inside the image (= inside the tile buffer), each 16-byte aligned; the code section
+    // is at offset 0 and w comes last so that the zero and then the N rows can follow it in shared memory
+    uint32_t o_perm, o_srow1, o_shdr1, o_srow2, o_shdr2, o_wptr, o_nxt, o_w;
     uint32_t a_off, b_off; // first element of the A / B slot in the partial-sum buffer
+    uint32_t o_sn_next;    // where the N rows of the next tile of the same CTA go in ITS buffer (res_o_sn of that tile)
     int32_t pad;
 };
-static_assert(sizeof(ResTile) == 144, "ResTile is copied word by word");
+static_assert(sizeof(ResTile) == 120 && sizeof(ResTile) / 4 <= 32, "ResTile is copied word by word by one warp");
 constexpr int kResTileWords = sizeof(ResTile) / 4;
+// slab header (uint32): first position / 32 (10 bits) | height H << 10 (9 bits) | multi << 31
+constexpr uint32_t kResHdrHShift = 10, kResHdrHMask = 0x1ff, kResHdrMulti = 0x80000000u;
+constexpr int kResHMax = 511;
+constexpr uint16_t kResNoRow = 0xffff;  // lane without a piece
+constexpr int kResWarpMax = 32;         // consumer warps per CTA
 struct ResRun {            // host only: consecutive tiles of one strip (indices into the scheduled tile sequence)
     int32_t t0, nt;
     int32_t a_row0, a_rows, a_slot;
@@ -273,31 +280,28 @@ struct ResRun {            // host only: consecutive tiles of one strip (indices
 };
 inline int32_t res_al16(int32_t x) { return (x + 15) & ~15; }
 // fills the section offsets and blob_bytes of D from its counts (code section first, at offset 0)
-inline void res_set_layout(ResTile &D, int nl, int nnu) {
-    (void)nnu;
-    D.o_perm = (uint32_t)res_al16(4 * D.ne);
-    D.o_prow = D.o_perm + (uint32_t)res_al16(2 * (D.ngl1 + D.ngl2));
-    D.o_pf = D.o_prow + (uint32_t)res_al16(2 * (D.npiece + 4));
-    D.o_tf = D.o_pf + (uint32_t)res_al16(2 * nl);
-    D.o_d1 = D.o_tf + (uint32_t)res_al16(2 * nl);
-    D.o_d2 = D.o_d1 + (uint32_t)res_al16(2 * D.ntask1);
-    D.o_cols = D.o_d2 + (uint32_t)res_al16(2 * D.ntask2);
-    D.o_nxt = D.o_cols + (uint32_t)res_al16(4 * (D.nc1 + D.nc2 + D.nc3));
+inline void res_set_layout(ResTile &D, int nwarp) {
+    D.o_perm = (uint32_t)res_al16(4 * D.ne_pad);
+    D.o_srow1 = D.o_perm + (uint32_t)res_al16(2 * D.ng_pad);
+    D.o_shdr1 = D.o_srow1 + (uint32_t)res_al16(2 * 32 * D.nslab1);
+    D.o_srow2 = D.o_shdr1 + (uint32_t)res_al16(4 * D.nslab1);
+    D.o_shdr2 = D.o_srow2 + (uint32_t)res_al16(2 * 32 * D.nslab2);
+    D.o_wptr = D.o_shdr2 + (uint32_t)res_al16(4 * D.nslab2);
+    D.o_nxt = D.o_wptr + (uint32_t)res_al16(2 * 2 * (nwarp + 1));
     D.o_w = D.o_nxt + (uint32_t)res_al16(4 * D.nq_next);
-    D.blob_bytes = (int32_t)D.o_w + res_al16(8 * D.ne);
-    D.o_sn = (uint32_t)res_al16((int32_t)D.o_w + 8 * (D.ne + D.npiece + D.npart));
+    D.blob_bytes = (int32_t)D.o_w + res_al16(8 * D.ne_pad);
 }
-// shared memory a tile needs behind the f / accumulator arrays: image, X tail, N rows of its pairs
-inline int64_t res_tile_smem(const ResTile &D, int nnu) { return (int64_t)D.o_sn + 8 * (int64_t)D.nq * nnu; }
+// the N rows of the tile's pairs follow the zero in shared memory
+inline uint32_t res_o_sn(const ResTile &D) { return (uint32_t)res_al16((int32_t)D.o_w + 8 * (D.ne_pad + 1)); }
+// shared memory a tile needs behind the f / accumulator arrays: image, the zero, N rows of its pairs
+inline int64_t res_tile_smem(const ResTile &D, int nnu) { return (int64_t)res_o_sn(D) + 8 * (int64_t)D.nq * nnu; }
 constexpr int kResSlotMax = 8192;     // N slots (pair * nnu + mode) per tile: slot * 8 fits the 16-bit field of the code
 constexpr int kResRowMax = 8192;      // rows (A + B) per tile: row * 8 fits the 16-bit field of the code
-constexpr int kResLanes = 256;        // threads of a persistent CTA of res_kernel = lanes of a tile image
-constexpr int kResCtasPerSm = 2;      // the phases of the two CTAs of an SM interleave
-constexpr int64_t kResSmemCap = 112 * 1024;  // dynamic shared memory per CTA (227 KB per SM incl. static and 1 KB per CTA)
-constexpr int kResXMax = 32767;       // X positions (entries + pieces + partials) per tile: 15 bits of a stream word
+constexpr int kResXMax = 32767;       // positions per tile (10-bit slab base in units of 32; uint16 perm)
 struct ResHost {
-    int32_t Ra = 0, RbMax = 0, Rcap = 0, rf = 0, nblk = 0, nrows = 0, nnu = 0, ncta = 0, nl = 0;
+    int32_t Ra = 0, RbMax = 0, Rcap = 0, rf = 0, nblk = 0, nrows = 0, nnu = 0, ncta = 0, nwarp = 0;
     int64_t smem_tile = 0;            // largest res_tile_smem of any tile
+    int64_t smem_cap = 0;             // shared-memory budget per CTA the store was built for
     std::vector<int32_t> blk_row0, row_state, state_row, state_blk;
     std::vector<unsigned char> blob;  // all tile images, in schedule order
     std::vector<uint32_t> iqn;        // per (tile, pair): iq * nnu
@@ -307,20 +311,16 @@ struct ResHost {
     std::vector<int64_t> slot_off;
     std::vector<int32_t> slot_row0, slot_rows, blk_ent_ptr;
     std::vector<int64_t> blk_ent_off;
-    int64_t part_rows = 0, nent = 0;
+    int64_t part_rows = 0, nent = 0, nent_pad = 0, ngather_pad = 0, nslab = 0;
     bool supported = false;
     std::string why;
 };
 // bytes of res_kernel's dynamic shared memory: strip accumulators, three directory entries, two tile buffers
-// (f of the A and B rows, accumulators of the B rows, image + X tail + N rows)
-inline int64_t res_buf_bytes(int Rcap, int RbMax, int64_t smem_tile) {
-    return ((int64_t)8 * Rcap + (int64_t)8 * RbMax + smem_tile + 127) & ~(int64_t)127;
-}
+// (f of the A and B rows, image + zero + N rows)
+inline int64_t res_buf_bytes(int Rcap, int64_t smem_tile) { return ((int64_t)8 * Rcap + smem_tile + 127) & ~(int64_t)127; }
 inline int64_t res_fixed_bytes(int Ra) { return ((int64_t)8 * Ra + 3 * (int64_t)sizeof(ResTile) + 127) & ~(int64_t)127; }
-inline int64_t res_smem_total(int Ra, int Rcap, int RbMax, int64_t smem_tile) {
-    return res_fixed_bytes(Ra) + 2 * res_buf_bytes(Rcap, RbMax, smem_tile);
-}
-int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, int64_t smem_cap, ResHost &t,
+inline int64_t res_smem_total(int Ra, int Rcap, int64_t smem_tile) { return res_fixed_bytes(Ra) + 2 * res_buf_bytes(Rcap, smem_tile); }
+int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, int64_t smem_cap, int nwarp, ResHost &t,
               std::string &err);
 
 }  // namespace ephc

@@ -16,8 +16,8 @@ namespace ephc {
 
 namespace {
 
-struct DEnt {          // directed entry: T = w F_em(f_out, f_in, N[iq, nu]); I[out] -= T; I[in] += T
-    int32_t out, in;   // compact rows
+struct DEnt {          // entry: T = |w| F_em or F_abs (sign of w)(f_out, f_in, N[iq, nu]); I[out] -= T; I[in] += T
+    int32_t out, in;   // compact rows of the channel's first end a and second end b
     int32_t ip;        // candidate pair (-> iq)
     int32_t nu;
     double w;
@@ -27,71 +27,98 @@ struct Image {
     ResTile dir;
     std::vector<unsigned char> blob;
     std::vector<uint32_t> iqn;
-    int64_t smem = 0;   // blob + X tail + N rows
+    int64_t smem = 0;   // blob + zero + N rows
     int64_t work = 0;
 };
 
 struct ImgParams {
     int32_t a_row0, a_rows, b_row0, b_rows;
-    int nnu, nl;
-    int qmul, lmul;     // longest piece / gather task in units of a lane's average load
+    int nnu, nwarp;
+    int hcap;           // pieces of at most this many elements (0: automatic)
+    bool bank_aware;    // order a lane's entries so that the gathers of a column spread over the shared-memory banks
     int32_t nq_cap;     // pairs per tile (bounds the iq list that rides in the previous tile's image)
-    int64_t budget;     // bytes available for image (without that list) + X tail + N rows
+    int64_t budget;     // bytes available for image (without that list) + zero + N rows
     const int32_t *pair_iq;
 };
 
 struct Scratch {
-    std::vector<int32_t> cnt, start, idx, pos_of, in_cnt, in_start, in_list;
+    std::vector<int32_t> cnt, start, idx, pos_of, in_start, in_list;
     std::vector<uint32_t> pair_local;
 };
 
-struct Item {
-    int32_t key, start, len;   // piece: out row / task: destination; first element; elements
+struct Piece {
+    int32_t row, start, len;   // local row; first element in the row-sorted list; elements
 };
 
-// Column tables of a set of lists sorted by descending length: col[j] = (number of lists longer than j) | (first
-// element of column j) << 16.
-static void make_cols(const std::vector<int32_t> &lens_desc, std::vector<uint32_t> &cols, int32_t &ncol) {
-    ncol = lens_desc.empty() ? 0 : lens_desc[0];
-    cols.assign((size_t)ncol, 0);
-    size_t n = lens_desc.size();
-    int32_t base = 0;
-    for (int32_t j = 0; j < ncol; ++j) {
-        while (n > 0 && lens_desc[n - 1] <= j) --n;
-        cols[j] = (uint32_t)n | ((uint32_t)base << 16);
-        base += (int32_t)n;
-    }
-}
+struct Slab {
+    int32_t base, H;           // first position; columns
+    bool multi;                // some row owns more than one lane
+    int32_t piece[32];         // piece per lane, -1 = none
+};
 
-// Packs items into nl lanes of (almost) equal load, longest item first (every item goes to the lane with the least
-// load so far); lanes are then sorted by descending load.  lanes[l] = the items of lane l in the order it walks them.
-static void pack_lanes(const std::vector<Item> &items, int nl, std::vector<std::vector<int32_t>> &lanes,
-                       std::vector<int32_t> &loads) {
-    std::vector<int32_t> order(items.size());
-    for (size_t i = 0; i < items.size(); ++i) order[i] = (int32_t)i;
-    std::stable_sort(order.begin(), order.end(), [&](int32_t x, int32_t y) { return items[x].len > items[y].len; });
-    std::vector<std::vector<int32_t>> bins((size_t)nl);
-    std::vector<std::pair<int32_t, int32_t>> heap;  // (-load, -bin): the top is the least loaded, lowest bin
-    for (int32_t b = 0; b < nl; ++b) heap.push_back({0, -b});
-    std::make_heap(heap.begin(), heap.end());
-    for (int32_t it : order) {
-        std::pop_heap(heap.begin(), heap.end());
-        auto top = heap.back();
-        bins[(size_t)(-top.second)].push_back(it);
-        heap.back() = {top.first - items[it].len, top.second};
-        std::push_heap(heap.begin(), heap.end());
+// Cuts the lists [start[r], start[r+1]) of the rows r0 .. r1 into pieces of at most hcap elements (equal parts), sorts
+// them by descending length with the pieces of one row adjacent, and deals them 32 per slab; the pieces of one row never
+// straddle two slabs (a row has at most 32 pieces).  With keep_empty, rows without elements get a lane too (a piece
+// of length 0).  The slabs are then dealt to nwarp warps, longest first to the least loaded warp, and come out warp by
+// warp (wptr[w] .. wptr[w+1]), each warp's slabs by descending height.
+static void make_slabs(const std::vector<int32_t> &start, int32_t r0, int32_t r1, bool keep_empty, int32_t hcap, int nwarp,
+                       std::vector<Piece> &pieces, std::vector<Slab> &slabs, std::vector<int32_t> &wptr, int32_t &npos) {
+    pieces.clear();
+    std::vector<Slab> tmp;
+    std::vector<std::pair<int32_t, int32_t>> rows;  // (first piece, pieces) per row
+    for (int32_t r = r0; r < r1; ++r) {
+        const int32_t c = start[r + 1] - start[r];
+        if (c == 0 && !keep_empty) continue;
+        int32_t npc = 1;  // a power of two, so that the lanes of whole rows fill a slab exactly
+        while (npc * hcap < c) npc *= 2;
+        const int32_t base = c / npc, rem = c % npc;
+        rows.push_back({(int32_t)pieces.size(), npc});
+        int32_t s = start[r];
+        for (int32_t k = 0; k < npc; ++k) {
+            const int32_t len = base + (k < rem ? 1 : 0);
+            pieces.push_back(Piece{r, s, len});
+            s += len;
+        }
     }
-    std::vector<int32_t> bl((size_t)nl, 0), bo((size_t)nl);
-    for (int32_t b = 0; b < nl; ++b) {
-        for (int32_t it : bins[b]) bl[b] += items[it].len;
-        bo[b] = b;
+    // rows by the length of their longest piece (the first), descending; ties by row
+    std::stable_sort(rows.begin(), rows.end(), [&](const std::pair<int32_t, int32_t> &x, const std::pair<int32_t, int32_t> &y) {
+        return pieces[x.first].len > pieces[y.first].len;
+    });
+    int32_t used = 32;
+    for (const auto &rw : rows) {
+        if (used + rw.second > 32) {
+            Slab sl;
+            sl.base = 0;
+            sl.H = pieces[rw.first].len;
+            sl.multi = false;
+            std::fill(sl.piece, sl.piece + 32, -1);
+            tmp.push_back(sl);
+            used = 0;
+        }
+        Slab &sl = tmp.back();
+        if (rw.second > 1) sl.multi = true;
+        for (int32_t k = 0; k < rw.second; ++k) sl.piece[used++] = rw.first + k;
     }
-    std::stable_sort(bo.begin(), bo.end(), [&](int32_t x, int32_t y) { return bl[x] > bl[y]; });
-    lanes.assign((size_t)nl, {});
-    loads.assign((size_t)nl, 0);
-    for (int32_t l = 0; l < nl; ++l) {
-        lanes[l].swap(bins[bo[l]]);
-        loads[l] = bl[bo[l]];
+    // tmp is sorted by descending height: longest first to the least loaded warp (cost: columns + a prologue)
+    std::vector<std::vector<int32_t>> mine((size_t)nwarp);
+    std::vector<int64_t> load((size_t)nwarp, 0);
+    for (size_t i = 0; i < tmp.size(); ++i) {
+        int best = 0;
+        for (int w = 1; w < nwarp; ++w)
+            if (load[w] < load[best]) best = w;
+        mine[best].push_back((int32_t)i);
+        load[best] += tmp[i].H + 2;
+    }
+    slabs.clear();
+    wptr.assign((size_t)nwarp + 1, 0);
+    npos = 0;
+    for (int w = 0; w < nwarp; ++w) {
+        for (int32_t i : mine[w]) {
+            slabs.push_back(tmp[i]);
+            slabs.back().base = npos;
+            npos += 32 * tmp[i].H;
+        }
+        wptr[w + 1] = (int32_t)slabs.size();
     }
 }
 
@@ -99,8 +126,7 @@ static void pack_lanes(const std::vector<Item> &items, int nl, std::vector<std::
 // shared-memory budget is exceeded (the caller then splits the entry range).
 static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S, Image &out) {
     const int32_t R = P.a_rows + P.b_rows;
-    const int nl = P.nl;
-    if (n > kResXMax || R > kResRowMax) return false;
+    if (n > kResXMax - 32 || R > kResRowMax) return false;
     auto loc = [&](int32_t row) {
         return (row >= P.a_row0 && row < P.a_row0 + P.a_rows) ? row - P.a_row0 : P.a_rows + (row - P.b_row0);
     };
@@ -113,191 +139,193 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
     }
     const int32_t nq = (int32_t)out.iqn.size();
     if ((int64_t)nq * P.nnu > kResSlotMax || nq > P.nq_cap) return false;
-    // ---- phase 1: out rows -> pieces of at most ceil(n / nl) entries -> lanes ------------------------------------------
+    // ---- phase 1: entries by a row (inside a row by b row, then canonical order) ------------------------------------
     S.cnt.assign((size_t)R + 1, 0);
     for (int64_t i = 0; i < n; ++i) S.cnt[loc(e[i].out) + 1]++;
     S.start.assign((size_t)R + 1, 0);
-    for (int32_t r = 0; r < R; ++r) S.start[r + 1] = S.start[r] + S.cnt[r + 1];
+    int32_t longest = 0;
+    for (int32_t r = 0; r < R; ++r) {
+        S.start[r + 1] = S.start[r] + S.cnt[r + 1];
+        longest = std::max(longest, S.cnt[r + 1]);
+    }
     S.idx.resize((size_t)n);
     {
         std::vector<int32_t> &cur = S.cnt;  // reuse as cursor
         for (int32_t r = 0; r < R; ++r) cur[r] = S.start[r];
         for (int64_t i = 0; i < n; ++i) S.idx[cur[loc(e[i].out)]++] = (int32_t)i;
     }
-    // inside an out row: by in row, so that the entries of one (out, in) combo (same rows, different modes) are adjacent
     for (int32_t r = 0; r < R; ++r)
         std::sort(S.idx.begin() + S.start[r], S.idx.begin() + S.start[r + 1], [&](int32_t x, int32_t y) {
             if (e[x].in != e[y].in) return e[x].in < e[y].in;
             return x < y;
         });
-    const int32_t Q1 = (int32_t)std::max<int64_t>(1, P.qmul * ((n + nl - 1) / nl));
-    std::vector<Item> pieces;
+    // b-row lists
+    S.in_start.assign((size_t)R + 1, 0);
+    for (int64_t i = 0; i < n; ++i) S.in_start[loc(e[i].in) + 1]++;
     for (int32_t r = 0; r < R; ++r) {
-        const int32_t c = S.start[r + 1] - S.start[r];
-        if (c == 0) continue;
-        const int32_t npc = (c + Q1 - 1) / Q1, base = c / npc, rem = c % npc;
-        int32_t s = S.start[r];
-        for (int32_t k = 0; k < npc; ++k) {
-            const int32_t len = base + (k < rem ? 1 : 0);
-            pieces.push_back(Item{r, s, len});
-            s += len;
-        }
+        longest = std::max(longest, S.in_start[r + 1]);
+        S.in_start[r + 1] += S.in_start[r];
     }
-    const int32_t npiece = (int32_t)pieces.size();
-    std::vector<std::vector<int32_t>> lanes1, lanes2;
-    std::vector<int32_t> loads1, loads2;
-    pack_lanes(pieces, nl, lanes1, loads1);
-    std::vector<uint32_t> cols1, cols2, cols3;
-    int32_t nc1 = 0, nc2 = 0, nc3 = 0;
-    make_cols(loads1, cols1, nc1);
-    while (nc1 % 4) {  // the kernel reads four columns at a time
-        cols1.push_back((uint32_t)n << 16);
-        ++nc1;
-    }
-    // pieces are numbered in the order the lanes walk them; entry positions; END flags
-    std::vector<int32_t> piece_no((size_t)npiece), pf((size_t)nl), prow((size_t)npiece + 4, 0);
-    std::vector<uint8_t> is_end((size_t)n, 0);  // bit 0: last entry of its piece; bit 1: the next entry of the piece has the same in row
-    S.pos_of.resize((size_t)n);
-    {
-        int32_t no = 0;
-        for (int32_t l = 0; l < nl; ++l) {
-            pf[l] = no;
-            int32_t j = 0;
-            for (int32_t ip : lanes1[l]) {
-                piece_no[ip] = no;
-                prow[no] = pieces[ip].key;
-                ++no;
-                for (int32_t k = 0; k < pieces[ip].len; ++k, ++j) {
-                    const int32_t ei = S.idx[pieces[ip].start + k];
-                    S.pos_of[ei] = (int32_t)(cols1[j] >> 16) + l;
-                    if (k + 1 == pieces[ip].len)
-                        is_end[ei] = 1;
-                    else if (e[S.idx[pieces[ip].start + k + 1]].in == e[ei].in)
-                        is_end[ei] = 2;
+    const int32_t hmin = (longest + 31) / 32;  // a row owns at most 32 lanes
+    if (hmin > kResHMax) return false;
+    std::vector<Piece> pc1, pc2;
+    std::vector<Slab> sl1, sl2;
+    std::vector<int32_t> wp1, wp2;
+    int32_t ne_pad = 0, ng_pad = 0;
+    // piece length: the candidate with the least padding and fewest slabs (positions + a prologue per slab)
+    int32_t hcap = std::max(P.hcap, hmin);
+    if (P.hcap <= 0) {
+        int64_t best = -1;
+        for (int32_t cand : {6, 8, 10, 12, 16, 20, 24, 32, 48, 64, 96, 128, 256, kResHMax}) {
+            if (cand < hmin) continue;
+            int32_t np1 = 0, np2 = 0;
+            make_slabs(S.start, 0, R, false, cand, P.nwarp, pc1, sl1, wp1, np1);
+            if (P.b_rows > 0)
+                make_slabs(S.in_start, P.a_rows, R, true, cand, P.nwarp, pc2, sl2, wp2, np2);
+            else
+                make_slabs(S.in_start, 0, R, false, cand, P.nwarp, pc2, sl2, wp2, np2);
+            // the slowest warp of each phase sets the pace
+            int64_t cost = 0;
+            for (int ph = 0; ph < 2; ++ph) {
+                const std::vector<Slab> &sl = ph ? sl2 : sl1;
+                const std::vector<int32_t> &wp = ph ? wp2 : wp1;
+                int64_t worst = 0;
+                for (int w = 0; w < P.nwarp; ++w) {
+                    int64_t ld = 0;
+                    for (int32_t k = wp[w]; k < wp[w + 1]; ++k) ld += (ph ? 2 : 5) * (int64_t)sl[k].H + 8;
+                    worst = std::max(worst, ld);
                 }
+                cost += worst * P.nwarp;
+            }
+            cost += 2 * ((int64_t)np1 + np2) / 3;  // and the bytes moved
+            if (best < 0 || cost < best) {
+                best = cost;
+                hcap = cand;
             }
         }
     }
-    // ---- phase 2: inputs of every row: positions of its in-entries (ascending), then of its out pieces --------------------
-    S.in_cnt.assign((size_t)R + 1, 0);
-    int32_t ncombo = 0;
-    for (int64_t i = 0; i < n; ++i)
-        if (!(is_end[i] & 2)) {  // the term of a combo sits at its last entry
-            S.in_cnt[loc(e[i].in) + 1]++;
-            ++ncombo;
+    make_slabs(S.start, 0, R, false, hcap, P.nwarp, pc1, sl1, wp1, ne_pad);
+    if (ne_pad > kResXMax - 1 || ne_pad / 32 > 1023) return false;
+    // Order of a lane's entries: a warp gathers f_b and N of a column with 8-byte loads, 16 lanes per shared-memory
+    // wavefront, and every extra lane on a bank pair (address / 8 mod 16) costs another wavefront.  Column by column,
+    // lanes with the fewest entries left choose first, each the entry that lands on the least used bank pairs.
+    if (P.bank_aware) {
+        auto bank_f = [&](int32_t ei) { return loc(e[ei].in) & 15; };
+        auto bank_n = [&](int32_t ei) { return (int32_t)((S.pair_local[ei] * (uint32_t)P.nnu + (uint32_t)e[ei].nu) & 15u); };
+        int32_t order[16];
+        for (const Slab &sl : sl1)
+            for (int32_t j = 0; j + 1 < sl.H; ++j)
+                for (int half = 0; half < 2; ++half) {
+                    int32_t cf[16] = {0}, cn[16] = {0}, nl = 0;
+                    for (int l = 16 * half; l < 16 * half + 16; ++l)
+                        if (sl.piece[l] >= 0 && pc1[sl.piece[l]].len > j) order[nl++] = l;
+                    std::sort(order, order + nl, [&](int32_t x, int32_t y) { return pc1[sl.piece[x]].len < pc1[sl.piece[y]].len; });
+                    for (int32_t k = 0; k < nl; ++k) {
+                        const Piece &pc = pc1[sl.piece[order[k]]];
+                        int32_t best = j, bc = 1 << 30;
+                        for (int32_t m = j; m < pc.len; ++m) {
+                            const int32_t ei = S.idx[pc.start + m], c = cf[bank_f(ei)] + cn[bank_n(ei)];
+                            if (c < bc) bc = c, best = m;
+                        }
+                        std::swap(S.idx[pc.start + j], S.idx[pc.start + best]);
+                        const int32_t ei = S.idx[pc.start + j];
+                        cf[bank_f(ei)]++;
+                        cn[bank_n(ei)]++;
+                    }
+                }
+    }
+    S.pos_of.resize((size_t)n);
+    for (const Slab &sl : sl1)
+        for (int l = 0; l < 32; ++l) {
+            if (sl.piece[l] < 0) continue;
+            const Piece &pc = pc1[sl.piece[l]];
+            for (int32_t k = 0; k < pc.len; ++k) S.pos_of[S.idx[pc.start + k]] = sl.base + 32 * k + l;
         }
-    for (int32_t p = 0; p < npiece; ++p) S.in_cnt[pieces[p].key + 1]++;
-    S.in_start.assign((size_t)R + 1, 0);
-    for (int32_t r = 0; r < R; ++r) S.in_start[r + 1] = S.in_start[r] + S.in_cnt[r + 1];
-    S.in_list.resize((size_t)ncombo + npiece);
-    int32_t nrow_in = 0;
+    // ---- phase 2: positions of the entries of every b row, ascending; off the diagonal every B row gets a lane ------
+    S.in_list.resize((size_t)n);
     {
-        std::vector<int32_t> &cur = S.in_cnt;
-        for (int32_t r = 0; r < R; ++r) cur[r] = S.in_start[r];
-        for (int64_t i = 0; i < n; ++i)
-            if (!(is_end[i] & 2)) S.in_list[cur[loc(e[i].in)]++] = S.pos_of[i];
-        for (int32_t r = 0; r < R; ++r) std::sort(S.in_list.begin() + S.in_start[r], S.in_list.begin() + cur[r]);
-        for (int32_t p = 0; p < npiece; ++p) S.in_list[cur[pieces[p].key]++] = (int32_t)n + piece_no[p];
-        for (int32_t r = 0; r < R; ++r) nrow_in += S.in_start[r + 1] > S.in_start[r];
+        std::vector<int32_t> cur(S.in_start.begin(), S.in_start.end() - 1);
+        for (int64_t i = 0; i < n; ++i) S.in_list[cur[loc(e[i].in)]++] = S.pos_of[i];
+        for (int32_t r = 0; r < R; ++r) std::sort(S.in_list.begin() + S.in_start[r], S.in_list.begin() + S.in_start[r + 1]);
     }
-    // gather tasks: a row with at most Lcap inputs is one final task; longer rows are cut into partial tasks whose
-    // sums a round-2 task adds
-    const int32_t Lcap = (int32_t)std::max<int64_t>(2, P.lmul * (((int64_t)ncombo + npiece + nl - 1) / nl));
-    std::vector<Item> t1, t2;
-    std::vector<int32_t> list2;
-    int32_t npart = 0;
-    for (int32_t r = 0; r < R; ++r) {
-        const int32_t L = S.in_start[r + 1] - S.in_start[r];
-        if (L == 0) continue;
-        if (L <= Lcap) {
-            t1.push_back(Item{r, S.in_start[r], L});
-            continue;
-        }
-        const int32_t nchunk = (L + Lcap - 1) / Lcap, base = L / nchunk, rem = L % nchunk;
-        int32_t s = S.in_start[r];
-        t2.push_back(Item{r, (int32_t)list2.size(), nchunk});
-        for (int32_t k = 0; k < nchunk; ++k) {
-            const int32_t len = base + (k < rem ? 1 : 0);
-            t1.push_back(Item{0x8000 | npart, s, len});
-            list2.push_back((int32_t)n + npiece + npart);
-            ++npart;
-            s += len;
-        }
-    }
-    if (npart > 0x7fff || n + npiece + npart > kResXMax) return false;
-    const int32_t ntask1 = (int32_t)t1.size(), ntask2 = (int32_t)t2.size();
-    pack_lanes(t1, nl, lanes2, loads2);
-    make_cols(loads2, cols2, nc2);
-    while (nc2 % 4) {
-        cols2.push_back((uint32_t)(ncombo + npiece) << 16);
-        ++nc2;
-    }
-    std::stable_sort(t2.begin(), t2.end(), [](const Item &x, const Item &y) { return x.len > y.len; });
-    {
-        std::vector<int32_t> lens((size_t)ntask2);
-        for (int32_t t = 0; t < ntask2; ++t) lens[t] = t2[t].len;
-        make_cols(lens, cols3, nc3);
+    if (P.b_rows > 0)
+        make_slabs(S.in_start, P.a_rows, R, true, hcap, P.nwarp, pc2, sl2, wp2, ng_pad);
+    else
+        make_slabs(S.in_start, 0, R, false, hcap, P.nwarp, pc2, sl2, wp2, ng_pad);
+    if (ng_pad / 32 > 1023) return false;
+    if (P.bank_aware) {  // the same for the T values a lane of phase 2 gathers: bank pair = position mod 16
+        int32_t order[16];
+        for (const Slab &sl : sl2)
+            for (int32_t j = 0; j + 1 < sl.H; ++j)
+                for (int half = 0; half < 2; ++half) {
+                    int32_t cx[16] = {0}, nl = 0;
+                    for (int l = 16 * half; l < 16 * half + 16; ++l)
+                        if (sl.piece[l] >= 0 && pc2[sl.piece[l]].len > j) order[nl++] = l;
+                    std::sort(order, order + nl, [&](int32_t x, int32_t y) { return pc2[sl.piece[x]].len < pc2[sl.piece[y]].len; });
+                    for (int32_t k = 0; k < nl; ++k) {
+                        const Piece &pc = pc2[sl.piece[order[k]]];
+                        int32_t best = j, bc = 1 << 30;
+                        for (int32_t m = j; m < pc.len; ++m) {
+                            const int32_t c = cx[S.in_list[pc.start + m] & 15];
+                            if (c < bc) bc = c, best = m;
+                        }
+                        std::swap(S.in_list[pc.start + j], S.in_list[pc.start + best]);
+                        cx[S.in_list[pc.start + j] & 15]++;
+                    }
+                }
     }
     ResTile &D = out.dir;
     std::memset(&D, 0, sizeof(D));
     D.ne = (int32_t)n;
-    D.npiece = npiece;
-    D.npart = npart;
-    D.ntask1 = ntask1;
-    D.ntask2 = ntask2;
-    D.nc1 = nc1;
-    D.nc2 = nc2;
-    D.nc3 = nc3;
-    D.ngl1 = ncombo + npiece;
-    D.ngl2 = (int32_t)list2.size();
+    D.ne_pad = ne_pad;
+    D.ng_pad = ng_pad;
+    D.nslab1 = (int32_t)sl1.size();
+    D.nslab2 = (int32_t)sl2.size();
     D.nq = nq;
     D.nq_next = 0;
     D.b_row0 = P.b_row0;
     D.b_rows = P.b_rows;
     D.b_slot = -1;
-    res_set_layout(D, nl, P.nnu);
+    res_set_layout(D, P.nwarp);
     out.smem = res_tile_smem(D, P.nnu);
     if (out.smem > P.budget) return false;
     // ---- fill the blob ---------------------------------------------------------------------------------------------
     out.blob.assign((size_t)D.blob_bytes, 0);
     uint32_t *code = reinterpret_cast<uint32_t *>(out.blob.data());
     uint16_t *perm = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_perm);
-    uint16_t *prow_o = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_prow);
-    uint16_t *pf_o = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_pf);
-    uint16_t *tf_o = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_tf);
-    uint16_t *d1 = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_d1);
-    uint16_t *d2 = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_d2);
-    uint32_t *cols = reinterpret_cast<uint32_t *>(out.blob.data() + D.o_cols);
+    uint16_t *srow1 = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_srow1);
+    uint32_t *shdr1 = reinterpret_cast<uint32_t *>(out.blob.data() + D.o_shdr1);
+    uint16_t *srow2 = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_srow2);
+    uint32_t *shdr2 = reinterpret_cast<uint32_t *>(out.blob.data() + D.o_shdr2);
+    uint16_t *wptr = reinterpret_cast<uint16_t *>(out.blob.data() + D.o_wptr);
     double *w = reinterpret_cast<double *>(out.blob.data() + D.o_w);
+    // padding entries: w = 0, partner row 0, N slot 0 (both always staged)
     for (int64_t i = 0; i < n; ++i) {
         const int32_t pos = S.pos_of[i];
-        code[pos] = ((uint32_t)loc(e[i].in) << 3) | ((S.pair_local[i] * (uint32_t)P.nnu + (uint32_t)e[i].nu) << 19) | is_end[i];
+        code[pos] = ((uint32_t)loc(e[i].in) << 3) | ((S.pair_local[i] * (uint32_t)P.nnu + (uint32_t)e[i].nu) << 19);
         w[pos] = e[i].w;
     }
-    for (int32_t p = 0; p < npiece + 4; ++p) prow_o[p] = (uint16_t)prow[p];  // four pad entries: the kernel reads three pieces ahead
-    for (int32_t l = 0; l < nl; ++l) pf_o[l] = (uint16_t)pf[l];
-    {
-        int32_t no = 0;
-        for (int32_t l = 0; l < nl; ++l) {
-            tf_o[l] = (uint16_t)no;
-            int32_t j = 0;
-            for (int32_t it : lanes2[l]) {
-                d1[no++] = (uint16_t)t1[it].key;
-                for (int32_t k = 0; k < t1[it].len; ++k, ++j)
-                    perm[(cols2[j] >> 16) + l] = (uint16_t)(S.in_list[t1[it].start + k] | (k + 1 == t1[it].len ? 0x8000 : 0));
-            }
+    for (size_t s = 0; s < sl1.size(); ++s) {
+        shdr1[s] = (uint32_t)(sl1[s].base / 32) | ((uint32_t)sl1[s].H << kResHdrHShift) | (sl1[s].multi ? kResHdrMulti : 0u);
+        for (int l = 0; l < 32; ++l) srow1[32 * s + l] = sl1[s].piece[l] < 0 ? kResNoRow : (uint16_t)pc1[sl1[s].piece[l]].row;
+    }
+    for (int32_t g = 0; g < ng_pad; ++g) perm[g] = (uint16_t)ne_pad;  // the zero
+    for (size_t s = 0; s < sl2.size(); ++s) {
+        shdr2[s] = (uint32_t)(sl2[s].base / 32) | ((uint32_t)sl2[s].H << kResHdrHShift) | (sl2[s].multi ? kResHdrMulti : 0u);
+        for (int l = 0; l < 32; ++l) {
+            srow2[32 * s + l] = kResNoRow;
+            if (sl2[s].piece[l] < 0) continue;
+            const Piece &pc = pc2[sl2[s].piece[l]];
+            srow2[32 * s + l] = (uint16_t)pc.row;
+            for (int32_t k = 0; k < pc.len; ++k) perm[sl2[s].base + 32 * k + l] = (uint16_t)S.in_list[pc.start + k];
         }
     }
-    for (int32_t t = 0; t < ntask2; ++t) {
-        d2[t] = (uint16_t)t2[t].key;
-        for (int32_t j = 0; j < t2[t].len; ++j) perm[D.ngl1 + (cols3[j] >> 16) + t] = (uint16_t)list2[t2[t].start + j];
+    for (int w_ = 0; w_ <= P.nwarp; ++w_) {
+        wptr[w_] = (uint16_t)wp1[w_];
+        wptr[P.nwarp + 1 + w_] = (uint16_t)wp2[w_];
     }
-    std::copy(cols1.begin(), cols1.end(), cols);
-    std::copy(cols2.begin(), cols2.end(), cols + nc1);
-    std::copy(cols3.begin(), cols3.end(), cols + nc1 + nc2);
-    // cost model of a tile for the shares (entries, row pieces / tasks, staged N rows, fixed)
-    out.work = n + 2 * (int64_t)(npiece + ntask1 + ntask2) + 3 * (int64_t)nq + 600;
-    (void)nrow_in;
+    // cost model of a tile for the shares, in phase-1 positions: positions, gathers, per-slab prologues, staged N rows
+    out.work = ne_pad + (2 * (int64_t)ng_pad) / 5 + 45 * (int64_t)(D.nslab1 + D.nslab2) + 3 * (int64_t)nq + 600;
     return true;
 }
 
@@ -328,12 +356,13 @@ static int env_int(const char *name, int dflt) {
 
 }  // namespace
 
-int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, int64_t smem_cap, ResHost &t,
+int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, int64_t smem_cap, int nwarp, ResHost &t,
               std::string &err) {
     const int nb = d.nb, nnu = d.nnu;
     const int64_t npair = p->npair;
     t = ResHost();
     t.nnu = nnu;
+    t.smem_cap = smem_cap;
     if (ncta < 1) ncta = 1;
     try {
         t.state_row.assign((size_t)d.ns, -1);
@@ -347,17 +376,27 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
         t.nent = nent;
         // ---- geometry: strips of Ra rows, B ranges of <= RbMax rows in units of fine blocks of Rf rows --------------
         int Ra = env_int("EPHC_RES_ROWS", 1024), RbMax = env_int("EPHC_RES_ROWS_B", 512);
-        const int nl = kResLanes;
-        const int qmul = std::max(1, env_int("EPHC_RES_QMUL", 1)), lmul = std::max(1, env_int("EPHC_RES_LMUL", 1));
+        const int hcap = std::max(0, env_int("EPHC_RES_HCAP", 0));
         Ra = std::max(1, std::min(Ra, kResRowMax / 2));
         RbMax = std::max(1, std::min(RbMax, kResRowMax / 2));
+        const double rho = (double)std::max<int64_t>(nent, 1) / (0.5 * (double)t.nrows * (double)t.nrows + 1.0);  // entries per row pair
+        const double bytes_per_entry = 15.5 + 8.0 * nnu / std::max(1.0, (double)nent / std::max<int64_t>(1, c.npair_active));
         if (!std::getenv("EPHC_RES_ROWS")) {
+            // square tiles give both ends of a channel equally long rows: Ra = Rb = sqrt(entries that fit / density); the
+            // f values of both row ranges may take a quarter of a buffer
+            Ra = 1024;
+            for (int iter = 0; iter < 3; ++iter) {
+                const double buf = (double)(smem_cap - res_fixed_bytes(Ra)) / 2 - 8.0 * 3.0 * Ra - 256;
+                const double rstar = std::sqrt(std::max(64.0, buf) / bytes_per_entry / rho);
+                Ra = (int)std::max(32.0, std::min({rstar, 2048.0, (double)smem_cap / (2 * 4 * 8 * 3.0)}));
+            }
+            RbMax = std::min(2 * Ra, kResRowMax / 2);
             // small problems: enough strips that every CTA gets a few runs
             while (Ra > 16 && (int64_t)(t.nrows / Ra) * (t.nrows / Ra) < 8 * (int64_t)ncta) Ra /= 2;
         }
         // two tile buffers: f of the A and B rows, accumulators of the B rows, image + X tail + N rows; a tenth of what
         // is left may hold N rows of pairs, which bounds the next tile's iq list that an image carries
-        const int64_t per_buf = (smem_cap - res_fixed_bytes(Ra)) / 2 - 8 * (int64_t)(Ra + RbMax) - 8 * (int64_t)RbMax - 256;
+        const int64_t per_buf = (smem_cap - res_fixed_bytes(Ra)) / 2 - 8 * (int64_t)(Ra + RbMax) - 256;
         const int32_t nq_cap = (int32_t)std::max<int64_t>(1, std::min<int64_t>(kResSlotMax / nnu, per_buf / (3 * 8 * (int64_t)nnu)));
         const int64_t budget = per_buf - 4 * (int64_t)nq_cap - 16;
         if (budget < 2048) {
@@ -367,8 +406,7 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
         int Rf = env_int("EPHC_RES_FINE", 0);
         if (Rf <= 0) {
             // an atom (strip x fine block) should hold about a sixth of what fits in a tile
-            const double rho = (double)std::max<int64_t>(nent, 1) / (0.5 * (double)t.nrows * (double)t.nrows + 1.0);
-            const double per_row = std::max(1e-9, rho * Ra) * (14.5 + 8.0 * nnu / std::max(1.0, (double)nent / std::max<int64_t>(1, c.npair_active)));
+            const double per_row = std::max(1e-9, rho * Ra) * bytes_per_entry;
             Rf = 128;
             while (Rf > 4 && Rf * per_row > (double)budget / 6.0) Rf /= 2;
         }
@@ -420,7 +458,7 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
             int64_t est;
         };
         auto est_bytes = [&](int64_t E, int64_t Pq, int64_t rows_) {
-            return 14 * E + 8 * (int64_t)nnu * Pq + 16 * std::min<int64_t>(rows_, 2 * E) + 16 * (int64_t)nl + 512;
+            return 15 * E + 8 * (int64_t)nnu * Pq + 5 * std::min<int64_t>(rows_, 2 * E) + 1024;
         };
         auto make_inits = [&](int32_t I, double scale, std::vector<Init> &inits) {
             const int32_t a_rows = std::min(t.nrows, (I + 1) * Ra) - std::min(t.nrows, I * Ra);
@@ -468,9 +506,9 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                         if (!strip_on[a / Ra]) continue;
                         const int64_t it = atom_init[atom_of(a, b)];
                         if (it < 0) continue;
-                        // emission weight: out = a, in = b; absorption weight: out = b, in = a (F_abs(a,b) = -F_em(b,a))
+                        // owner a, partner b; emission weight stored as +w, absorption weight as -w
                         if (c.ch_wem[j] != 0.0) ents[cur[it]++] = DEnt{a, b, (int32_t)ip, nu, c.ch_wem[j]};
-                        if (c.ch_wabs[j] != 0.0) ents[cur[it]++] = DEnt{b, a, (int32_t)ip, nu, c.ch_wabs[j]};
+                        if (c.ch_wabs[j] != 0.0) ents[cur[it]++] = DEnt{a, b, (int32_t)ip, nu, -c.ch_wabs[j]};
                     }
                 }
                 for (int64_t it = 0; it < ninit; ++it)
@@ -497,9 +535,9 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                         P.b_rows = t.blk_row0[j1 + 1] - P.b_row0;
                     }
                     P.nnu = nnu;
-                    P.nl = nl;
-                    P.qmul = qmul;
-                    P.lmul = lmul;
+                    P.nwarp = nwarp;
+                    P.hcap = hcap;
+                    P.bank_aware = !std::getenv("EPHC_RES_NO_BANKS");
                     P.nq_cap = nq_cap;
                     P.budget = budget;
                     P.pair_iq = c.pair_iq.data();
@@ -627,19 +665,21 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
             for (int32_t i = t.cta_ptr[cta]; i + 1 < t.cta_ptr[cta + 1]; ++i) t.tiles[i].nq_next = t.tiles[i + 1].nq;
         for (int64_t i = 0; i < ntile; ++i) {
             ResTile &D = t.tiles[i];
-            res_set_layout(D, nl, nnu);
+            res_set_layout(D, nwarp);
             D.blob_off = boff;
             boff += (D.blob_bytes + 127) & ~127;
             t.smem_tile = std::max(t.smem_tile, res_tile_smem(D, nnu));
             t.Rcap = std::max(t.Rcap, D.a_rows + D.b_rows);
         }
+        for (int32_t cta = 0; cta < ncta; ++cta)
+            for (int32_t i = t.cta_ptr[cta]; i + 1 < t.cta_ptr[cta + 1]; ++i) t.tiles[i].o_sn_next = res_o_sn(t.tiles[i + 1]);
         if (t.smem_tile > per_buf) {
             err = "internal: resident tile exceeds its shared-memory budget";
             return EPHC_ESTATE;
         }
         t.Rcap = (t.Rcap + 1) & ~1;
         t.RbMax = RbMax;
-        t.nl = nl;
+        t.nwarp = nwarp;
         t.iqn.resize((size_t)nqtot);
         t.blob.assign((size_t)boff + 128, 0);
 #pragma omp parallel for schedule(dynamic, 16)
@@ -675,14 +715,15 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                 for (int32_t b = t.slot_row0[sl] / Rf; b * Rf < t.slot_row0[sl] + t.slot_rows[sl]; ++b)
                     t.blk_ent_off[cur[b]++] = t.slot_off[sl] + (t.blk_row0[b] - t.slot_row0[sl]);
         }
+        for (const ResTile &D : t.tiles) {
+            t.nent_pad += D.ne_pad;
+            t.ngather_pad += D.ng_pad;
+            t.nslab += D.nslab1 + D.nslab2;
+        }
         if (std::getenv("EPHC_DEBUG")) {
-            double ne = 0, np = 0, nt1 = 0, nt2 = 0, nq = 0, bb = 0, br = 0, sm = 0;
+            double nq = 0, bb = 0, br = 0, sm = 0;
             for (const ResTile &D : t.tiles) {
                 sm += (double)res_tile_smem(D, nnu);
-                ne += D.ne;
-                np += D.npiece;
-                nt1 += D.ntask1;
-                nt2 += D.ntask2;
                 nq += D.nq;
                 bb += D.blob_bytes;
                 br += D.b_rows;
@@ -692,18 +733,19 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                 for (int32_t cta = 0; cta < ncta; ++cta) {
                     double wk = 0;
                     for (int32_t i = t.cta_ptr[cta]; i < t.cta_ptr[cta + 1]; ++i)
-                        wk += t.tiles[i].ne + 2.0 * (t.tiles[i].npiece + t.tiles[i].ntask1 + t.tiles[i].ntask2) + 3.0 * t.tiles[i].nq + 600;
+                        wk += t.tiles[i].ne_pad + 0.4 * t.tiles[i].ng_pad + 45.0 * (t.tiles[i].nslab1 + t.tiles[i].nslab2) + 3.0 * t.tiles[i].nq + 600;
                     mn = std::min(mn, wk);
                     mx = std::max(mx, wk);
                 }
                 std::fprintf(stderr, "res schedule: %d CTAs, work %.0f .. %.0f\n", ncta, mn, mx);
             }
-            const double n = (double)std::max<size_t>(t.tiles.size(), 1);
+            const double n = (double)std::max<size_t>(t.tiles.size(), 1), ne = (double)std::max<int64_t>(nent, 1);
             std::fprintf(stderr,
-                         "res store: Ra %d Rf %d RbMax %d budget %lld scale %.3f | %zu tiles in %zu runs, per tile: %.0f entries, %.0f pieces, "
-                         "%.0f + %.0f tasks, %.0f pairs, %.0f B rows, %.0f blob bytes (%.2f B/entry), smem avg %.0f max %lld, part rows %lld\n",
-                         Ra, Rf, RbMax, (long long)budget, scale, t.tiles.size(), t.runs.size(), ne / n, np / n, nt1 / n, nt2 / n,
-                         nq / n, br / n, bb / n, bb / std::max(ne, 1.0), sm / n, (long long)t.smem_tile, (long long)t.part_rows);
+                         "res store: Ra %d Rf %d RbMax %d budget %lld scale %.3f | %zu tiles in %zu runs, per tile: %.0f entries (+%.1f%% padding), "
+                         "%.0f gathers (+%.1f%%), %.1f slabs, %.0f pairs, %.0f B rows, %.0f blob bytes (%.2f B/entry), smem avg %.0f max %lld, part rows %lld\n",
+                         Ra, Rf, RbMax, (long long)budget, scale, t.tiles.size(), t.runs.size(), ne / n, 100.0 * (t.nent_pad - ne) / ne,
+                         (double)t.ngather_pad / n, 100.0 * (t.ngather_pad - ne) / ne, (double)t.nslab / n, nq / n, br / n, bb / n, bb / ne,
+                         sm / n, (long long)t.smem_tile, (long long)t.part_rows);
         }
     } catch (const std::bad_alloc &) {
         err = "host allocation failed (resident-tile store)";

@@ -94,21 +94,37 @@ __device__ __forceinline__ void mbar_arrive_cp_async(uint64_t *bar) {
 }
 __device__ __forceinline__ void consumer_sync(int nthreads) { asm volatile("bar.sync 1, %0;\n" ::"r"(nthreads) : "memory"); }
 
-// NL consumer threads (= lanes of a tile image) + one producer warp
-template <int NL>
-__global__ void __launch_bounds__(NL + 32, kResCtasPerSm) res_kernel(const ResParams P) {
+// Segmented sum over the lanes of a slab that own the same row (adjacent lanes): afterwards the first lane of every
+// group holds the group's sum (fixed tree order).  `same` = lanes with this lane's row.
+__device__ __forceinline__ double res_group_sum(double acc, unsigned same, int lane) {
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const double v = __shfl_down_sync(0xffffffffu, acc, d);
+        if (lane + d < 32 && ((same >> (lane + d)) & 1u)) acc += v;
+    }
+    return acc;
+}
+
+// Eq. 2 summand of one stored weight (reading R-1): ws > 0 emission weight, ws < 0 absorption weight
+__device__ __forceinline__ double res_term(double ws, double fa, double fb, double N) {
+    const double x = __double2hiint(ws) < 0 ? fb : fa;
+    return fma(fabs(ws), (fa - fb) * N, ws * fma(-fa, fb, x));
+}
+
+// NL consumer threads + one producer warp
+template <int NL, int CTAS>
+__global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
     extern __shared__ __align__(128) unsigned char res_smem[];
     double *sAccA = reinterpret_cast<double *>(res_smem);                  // accumulators of the strip (run)
     ResTile *sD = reinterpret_cast<ResTile *>(res_smem + 8 * P.Ra);        // directory entries of tiles i, i+1, i+2
     __shared__ __align__(8) uint64_t sFull[2], sEmpty[2];
-    __shared__ double sDummy;
-    const int tid = threadIdx.x, wbase = tid & ~31;
+    const int tid = threadIdx.x;
     const int nnu = P.nnu;
     const int i0 = P.cta_ptr[blockIdx.x], n = P.cta_ptr[blockIdx.x + 1] - i0;
     if (n <= 0) return;
     if (tid == 0) {
-        mbar_init(&sFull[0], 33);        // the producer's expect_tx arrive + the cp.async arrives of its 32 lanes
-        mbar_init(&sFull[1], 33);
+        mbar_init(&sFull[0], NL + 1);    // the producer's expect_tx arrive + the cp.async arrives of the consumers (N rows)
+        mbar_init(&sFull[1], NL + 1);
         mbar_init(&sEmpty[0], NL / 32);  // one arrive per consumer warp
         mbar_init(&sEmpty[1], NL / 32);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
@@ -123,25 +139,37 @@ __global__ void __launch_bounds__(NL + 32, kResCtasPerSm) res_kernel(const ResPa
         uint64_t pol_stream, pol_keep;
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol_stream));  // the store is read once
         asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol_keep));     // f is read by every tile
+#ifdef EPHC_RES_TIMING
+        long long pacc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pprev = clock64();
+#define EPHC_PTICK(k)                        \
+    {                                        \
+        const long long tn_ = clock64();     \
+        pacc[k] += tn_ - pprev;              \
+        pprev = tn_;                         \
+    }
+#else
+#define EPHC_PTICK(k)
+#endif
+        auto load_dir = [&](int j) {  // directory entry of tile j, word by word
+            const int32_t *src = reinterpret_cast<const int32_t *>(&P.tiles[i0 + j]);
+            int32_t *dst = reinterpret_cast<int32_t *>(&sD[j % 3]);
+            if (lane < kResTileWords) dst[lane] = src[lane];
+        };
+        load_dir(0);
         for (int j = 0; j < n; ++j) {
             const int b = j & 1;
+            EPHC_PTICK(0)
             if (j >= 2) mbar_wait(&sEmpty[b], (unsigned)((j >> 1) - 1) & 1u);  // the consumers are done with tile j - 2
-            {   // directory entry of tile j, word by word
-                const int32_t *src = reinterpret_cast<const int32_t *>(&P.tiles[i0 + j]);
-                int32_t *dst = reinterpret_cast<int32_t *>(&sD[j % 3]);
-                dst[lane] = src[lane];
-                if (lane + 32 < kResTileWords) dst[lane + 32] = src[lane + 32];
-            }
+            EPHC_PTICK(1)
             __syncwarp();
             const ResTile &D = sD[j % 3];
             unsigned char *buf = buf_of(b);
             double *sF = reinterpret_cast<double *>(buf);
-            double *sAccB = sF + P.Rcap;
-            unsigned char *sBlob = reinterpret_cast<unsigned char *>(sAccB + P.RbMax);
-            double *sN = reinterpret_cast<double *>(sBlob + D.o_sn);
+            unsigned char *sBlob = reinterpret_cast<unsigned char *>(sF + P.Rcap);
             if (lane == 0) {
                 const int a_rows = D.a_rows, b_rows = D.b_rows, bytes = D.blob_bytes;
                 const unsigned fa = (unsigned)((8 * a_rows + 15) & ~15), fb = (unsigned)((8 * b_rows + 15) & ~15);
+                *reinterpret_cast<double *>(sBlob + D.o_w + 8 * (size_t)D.ne_pad) = 0.0;  // the zero that padding reads
                 asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
                 mbar_expect_tx(&sFull[b], (unsigned)bytes + fa + fb);
                 const unsigned char *src = P.blob + D.blob_off;
@@ -149,25 +177,26 @@ __global__ void __launch_bounds__(NL + 32, kResCtasPerSm) res_kernel(const ResPa
                 bulk_g2s(sF, P.fc + D.a_row0, fa, &sFull[b], pol_keep);
                 if (fb) bulk_g2s(sF + a_rows, P.fc + D.b_row0, fb, &sFull[b], pol_keep);
             }
-            for (int k = lane; k < D.b_rows; k += 32) sAccB[k] = 0.0;
-            // N[iq, :] of the tile's pairs; their iq * nnu came with the image of the previous tile
-            const uint32_t *iq = P.iqn + D.q0;
-            if (j > 0) {
-                mbar_wait(&sFull[b ^ 1], (unsigned)((j - 1) >> 1) & 1u);
-                const unsigned char *prev = buf_of(b ^ 1) + 8 * (size_t)(P.Rcap + P.RbMax);
-                iq = reinterpret_cast<const uint32_t *>(prev + sD[(j - 1) % 3].o_nxt);
+            EPHC_PTICK(2)
+            // the directory entry of the next tile (its slot was last used by tile j - 2), and its image on the way to the L2
+            if (j + 1 < n) {
+                load_dir(j + 1);
+                __syncwarp();
+                if (lane == 0) {
+                    const ResTile &Dn = sD[(j + 1) % 3];
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(P.blob + Dn.blob_off), "r"((unsigned)Dn.blob_bytes) : "memory");
+                }
             }
-            const int total = D.nq * P.gran;
-            for (int g = lane; g < total; g += 32) {
-                const int pr = P.gran_magic ? (int)__umulhi((unsigned)g, P.gran_magic) : g, part = g - pr * P.gran;
-                const double *src = P.N + (size_t)iq[pr];
-                if (P.gran16)
-                    cp_async16(sN + pr * nnu + 2 * part, src + 2 * part);
-                else
-                    res_cp_async8(sN + pr * nnu + part, src + part);
-            }
-            mbar_arrive_cp_async(&sFull[b]);
+            EPHC_PTICK(3)
+#ifdef EPHC_RES_TIMING
+            mbar_wait(&sFull[b], (unsigned)(j >> 1) & 1u);  // working build only: how long until the tile is complete
+            EPHC_PTICK(5)
+#endif
         }
+#ifdef EPHC_RES_TIMING
+        if (P.dbg && lane == 0)
+            for (int k = 0; k < 8; ++k) P.dbg[((size_t)blockIdx.x * (NL / 32 + 1) + NL / 32) * 8 + k] = pacc[k];
+#endif
         return;
     }
 
@@ -183,174 +212,187 @@ __global__ void __launch_bounds__(NL + 32, kResCtasPerSm) res_kernel(const ResPa
 #else
 #define EPHC_TICK(k)
 #endif
+    const int lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = NL / 32;
+    // N[iq, :] of a tile's pairs -> the tile's buffer, by all consumer threads, one tile ahead; counted on its full barrier
+    auto stage_N = [&](const uint32_t *iq, int nq, double *sN, uint64_t *bar) {
+        const int total = nq * P.gran;
+        for (int g = tid; g < total; g += NL) {
+            const int pr = P.gran_magic ? (int)__umulhi((unsigned)g, P.gran_magic) : g, part = g - pr * P.gran;
+            const double *src = P.N + (size_t)iq[pr];
+            if (P.gran16)
+                cp_async16(sN + pr * nnu + 2 * part, src + 2 * part);
+            else
+                res_cp_async8(sN + pr * nnu + part, src + part);
+        }
+        mbar_arrive_cp_async(bar);
+    };
+    {   // first tile: its pair list comes from global memory
+        const ResTile &G = P.tiles[i0];
+        const unsigned o_sn0 = (G.o_w + 8u * (unsigned)(G.ne_pad + 1) + 15u) & ~15u;
+        stage_N(P.iqn + G.q0, G.nq, reinterpret_cast<double *>(buf_of(0) + 8 * (size_t)P.Rcap + o_sn0), &sFull[0]);
+    }
     for (int i = 0; i < n; ++i) {
         const int b = i & 1;
         unsigned char *buf = buf_of(b);
         double *sF = reinterpret_cast<double *>(buf);
-        double *sAccB = sF + P.Rcap;
-        unsigned char *sBlob = reinterpret_cast<unsigned char *>(sAccB + P.RbMax);
+        unsigned char *sBlob = reinterpret_cast<unsigned char *>(sF + P.Rcap);
         EPHC_TICK(0)
         mbar_wait(&sFull[b], (unsigned)(i >> 1) & 1u);
         EPHC_TICK(1)
         const ResTile &D = sD[i % 3];
-        const int ne = D.ne, npiece = D.npiece, a_rows = D.a_rows, nc1 = D.nc1, nc2 = D.nc2;
+        const int a_rows = D.a_rows;
         double *X = reinterpret_cast<double *>(sBlob + D.o_w);
         const uint32_t *code = reinterpret_cast<const uint32_t *>(sBlob);
-        const uint16_t *perm = reinterpret_cast<const uint16_t *>(sBlob + D.o_perm);
-        const uint16_t *prow = reinterpret_cast<const uint16_t *>(sBlob + D.o_prow);
-        const uint32_t *cols = reinterpret_cast<const uint32_t *>(sBlob + D.o_cols);
         const unsigned char *sFb = reinterpret_cast<const unsigned char *>(sF);
-        const unsigned char *sNb = sBlob + D.o_sn;
-        // ---- phase 1: Eq. 2 summand per entry; a lane walks the pieces packed into it, four columns per step: all loads
-        //      of a step are issued before its arithmetic, which is branch-free ------------------------------------------------
+        const unsigned char *sNb = sBlob + ((D.o_w + 8u * (unsigned)(D.ne_pad + 1) + 15u) & ~15u);
+        const uint16_t *wptr = reinterpret_cast<const uint16_t *>(sBlob + D.o_wptr);
+        // ---- phase 1 (paper step 2): Eq. 2 summand per entry; a lane walks one piece of an a row ---------------------------
         {
-            int piece = reinterpret_cast<const uint16_t *>(sBlob + D.o_pf)[tid];
-            // f_out of the current piece and of the next two, row of the third: a sliding window that is refilled at every
-            // piece end, so that no load sits between a piece end and the next entry
-            double xo = sF[prow[piece]], xo1 = sF[prow[piece + 1]], xo2 = sF[prow[piece + 2]];
-            int rn = prow[piece + 3];
-            double s0 = 0.0, s1 = 0.0;  // sum of w and of w N over the current combo
-            double acc = 0.0;
-            for (int j = 0; j < nc1; j += 4) {
-                const uint4 c4 = *reinterpret_cast<const uint4 *>(cols + j);
-                if (wbase >= (int)(c4.x & 0xffffu)) break;  // lanes descend in load: nothing left for this warp
-                const bool a0 = tid < (int)(c4.x & 0xffffu), a1 = tid < (int)(c4.y & 0xffffu), a2 = tid < (int)(c4.z & 0xffffu),
-                           a3 = tid < (int)(c4.w & 0xffffu);
-                const int e0 = a0 ? (int)(c4.x >> 16) + tid : 0, e1 = a1 ? (int)(c4.y >> 16) + tid : 0,
-                          e2 = a2 ? (int)(c4.z >> 16) + tid : 0, e3 = a3 ? (int)(c4.w >> 16) + tid : 0;
-                // an inactive lane reads entry 0 and treats it as "inside a combo" (no store, no sums)
-                const uint32_t cd0 = a0 ? code[e0] : 2u, cd1 = a1 ? code[e1] : 2u, cd2 = a2 ? code[e2] : 2u, cd3 = a3 ? code[e3] : 2u;
-                const double w0 = a0 ? X[e0] : 0.0, w1 = a1 ? X[e1] : 0.0, w2 = a2 ? X[e2] : 0.0, w3 = a3 ? X[e3] : 0.0;
-                // f_in is needed only where a combo (entries of one lane with the same out and in rows) ends
-                const double xi0 = (cd0 & 2u) ? 0.0 : *reinterpret_cast<const double *>(sFb + (cd0 & 0xfff8u));
-                const double xi1 = (cd1 & 2u) ? 0.0 : *reinterpret_cast<const double *>(sFb + (cd1 & 0xfff8u));
-                const double xi2 = (cd2 & 2u) ? 0.0 : *reinterpret_cast<const double *>(sFb + (cd2 & 0xfff8u));
-                const double xi3 = (cd3 & 2u) ? 0.0 : *reinterpret_cast<const double *>(sFb + (cd3 & 0xfff8u));
-                const double N0 = *reinterpret_cast<const double *>(sNb + (cd0 >> 16));
-                const double N1 = *reinterpret_cast<const double *>(sNb + (cd1 >> 16));
-                const double N2 = *reinterpret_cast<const double *>(sNb + (cd2 >> 16));
-                const double N3 = *reinterpret_cast<const double *>(sNb + (cd3 >> 16));
-                // sum_e w_e [(xo - xi) N_e + xo (1 - xi)] = (xo - xi) sum w_e N_e + xo (1 - xi) sum w_e over a combo
-#define EPHC_RES_STEP(E, CD, W, XI, NN)                                                        \
-    {                                                                                          \
-        s1 = fma(W, NN, s1);                                                                   \
-        s0 += W;                                                                               \
-        const bool ce = !(CD & 2u), pe = (CD & 1u) != 0; /* last entry of a combo / piece */   \
-        const double T = fma(xo - XI, s1, s0 * fma(-xo, XI, xo));                              \
-        if (ce) X[E] = T;                                                                      \
-        acc += ce ? T : 0.0;                                                                   \
-        s1 = ce ? 0.0 : s1;                                                                    \
-        s0 = ce ? 0.0 : s0;                                                                    \
-        if (pe) X[ne + piece] = -acc;                                                          \
-        acc = pe ? 0.0 : acc;                                                                  \
-        piece += pe ? 1 : 0;                                                                   \
-        xo = pe ? xo1 : xo;                                                                    \
-        xo1 = pe ? xo2 : xo1;                                                                  \
-        if (pe) xo2 = sF[rn];                                                                  \
-        if (pe) rn = prow[piece + 3];                                                          \
-    }
-                EPHC_RES_STEP(e0, cd0, w0, xi0, N0)
-                EPHC_RES_STEP(e1, cd1, w1, xi1, N1)
-                EPHC_RES_STEP(e2, cd2, w2, xi2, N2)
-                EPHC_RES_STEP(e3, cd3, w3, xi3, N3)
-#undef EPHC_RES_STEP
+            const uint16_t *srow = reinterpret_cast<const uint16_t *>(sBlob + D.o_srow1);
+            const uint32_t *shdr = reinterpret_cast<const uint32_t *>(sBlob + D.o_shdr1);
+            const int s1 = wptr[warp + 1];
+            int s = wptr[warp];
+            // header, row and f_a of the next slab are fetched while the current one is computed
+            uint32_t hd = 0;
+            unsigned u = kResNoRow;
+            double xo = 0.0;
+            if (s < s1) {
+                hd = shdr[s];
+                u = srow[32 * s + lane];
+                xo = u != kResNoRow ? sF[u] : 0.0;
+            }
+            for (; s < s1; ++s) {
+                const bool more = s + 1 < s1;
+                const uint32_t hd_n = more ? shdr[s + 1] : 0u;
+                const unsigned u_n = more ? srow[32 * (s + 1) + lane] : (unsigned)kResNoRow;
+                const int base = (int)(hd & 1023u) * 32 + lane, H = (int)((hd >> kResHdrHShift) & kResHdrHMask);
+                const uint32_t *c = code + base;
+                double *x = X + base;
+                double acc = 0.0;
+                // columns in groups of four: the codes and weights of the next group are loaded before the current group's
+                // gathers and arithmetic
+                uint32_t c0 = c[0], c1 = 1 < H ? c[32] : 0u, c2 = 2 < H ? c[64] : 0u, c3 = 3 < H ? c[96] : 0u;
+                double w0 = x[0], w1 = 1 < H ? x[32] : 0.0, w2 = 2 < H ? x[64] : 0.0, w3 = 3 < H ? x[96] : 0.0;
+                for (int j = 0; j < H; j += 4) {
+                    const bool q0 = j + 4 < H, q1 = j + 5 < H, q2 = j + 6 < H, q3 = j + 7 < H;
+                    const uint32_t n0 = q0 ? c[128] : 0u, n1 = q1 ? c[160] : 0u, n2 = q2 ? c[192] : 0u, n3 = q3 ? c[224] : 0u;
+                    const double v0 = q0 ? x[128] : 0.0, v1 = q1 ? x[160] : 0.0, v2 = q2 ? x[192] : 0.0, v3 = q3 ? x[224] : 0.0;
+                    const double b0 = *reinterpret_cast<const double *>(sFb + (c0 & 0xfff8u)), b1 = *reinterpret_cast<const double *>(sFb + (c1 & 0xfff8u)),
+                                 b2 = *reinterpret_cast<const double *>(sFb + (c2 & 0xfff8u)), b3 = *reinterpret_cast<const double *>(sFb + (c3 & 0xfff8u));
+                    const double N0 = *reinterpret_cast<const double *>(sNb + (c0 >> 16)), N1 = *reinterpret_cast<const double *>(sNb + (c1 >> 16)),
+                                 N2 = *reinterpret_cast<const double *>(sNb + (c2 >> 16)), N3 = *reinterpret_cast<const double *>(sNb + (c3 >> 16));
+                    const double T0 = res_term(w0, xo, b0, N0), T1 = res_term(w1, xo, b1, N1), T2 = res_term(w2, xo, b2, N2),
+                                 T3 = res_term(w3, xo, b3, N3);
+                    x[0] = T0;
+                    if (j + 1 < H) x[32] = T1;
+                    if (j + 2 < H) x[64] = T2;
+                    if (j + 3 < H) x[96] = T3;
+                    acc += T0;
+                    acc += T1;  // columns past H carry w = 0: T = 0
+                    acc += T2;
+                    acc += T3;
+                    c0 = n0, c1 = n1, c2 = n2, c3 = n3;
+                    w0 = v0, w1 = v1, w2 = v2, w3 = v3;
+                    c += 128;
+                    x += 128;
+                }
+                const double xo_n = u_n != kResNoRow ? sF[u_n] : 0.0;
+                bool head = true;
+                if (hd & kResHdrMulti) {
+                    const unsigned same = __match_any_sync(0xffffffffu, u);
+                    acc = res_group_sum(acc, same, lane);
+                    head = (same & ((1u << lane) - 1u)) == 0u;
+                }
+                if (u != kResNoRow && head) sAccA[u] -= acc;  // a rows are rows of the strip
+                hd = hd_n;
+                u = u_n;
+                xo = xo_n;
             }
         }
         EPHC_TICK(2)
         consumer_sync(NL);
+        // every warp has left tile i - 1 (it arrived here): its buffer takes the N rows of tile i + 1, whose pair list came
+        // with this tile's image
+        if (i + 1 < n)
+            stage_N(reinterpret_cast<const uint32_t *>(sBlob + D.o_nxt), D.nq_next,
+                    reinterpret_cast<double *>(buf_of(b ^ 1) + 8 * (size_t)P.Rcap + D.o_sn_next), &sFull[b ^ 1]);
         EPHC_TICK(3)
-        // ---- phase 2, round 1: a lane walks the gather tasks packed into it, four columns per step ----------------------------
+        // ---- phase 2 (paper step 3): a lane sums the T values listed for one piece of a b row -------------------------------
         {
-            const uint32_t *cols2 = cols + nc1;
-            const uint16_t *d1 = reinterpret_cast<const uint16_t *>(sBlob + D.o_d1);
-            int task = reinterpret_cast<const uint16_t *>(sBlob + D.o_tf)[tid];
-            int dn = d1[task];  // destination of the current task, loaded one task ahead
-            // the add of a finished task into its row's accumulator is completed at the next task end (or after the loop),
-            // so that the warp never waits for the accumulator's old value
-            double *pptr = &sDummy;
-            double pold = 0.0, pacc = 0.0, acc = 0.0;
-            for (int j = 0; j < nc2; j += 4) {
-                const uint4 c4 = *reinterpret_cast<const uint4 *>(cols2 + j);
-                if (wbase >= (int)(c4.x & 0xffffu)) break;
-                const bool a0 = tid < (int)(c4.x & 0xffffu), a1 = tid < (int)(c4.y & 0xffffu), a2 = tid < (int)(c4.z & 0xffffu),
-                           a3 = tid < (int)(c4.w & 0xffffu);
-                const uint32_t wd0 = a0 ? perm[(int)(c4.x >> 16) + tid] : 0u, wd1 = a1 ? perm[(int)(c4.y >> 16) + tid] : 0u,
-                               wd2 = a2 ? perm[(int)(c4.z >> 16) + tid] : 0u, wd3 = a3 ? perm[(int)(c4.w >> 16) + tid] : 0u;
-                const double v0 = a0 ? X[wd0 & 0x7fffu] : 0.0, v1 = a1 ? X[wd1 & 0x7fffu] : 0.0, v2 = a2 ? X[wd2 & 0x7fffu] : 0.0,
-                             v3 = a3 ? X[wd3 & 0x7fffu] : 0.0;
-#define EPHC_RES_STEP(WD, V)                                                                   \
-    {                                                                                          \
-        acc += V;                                                                              \
-        if (WD & 0x8000u) { /* last input of a task */                                         \
-            *pptr = pold + pacc;                                                               \
-            const int dst = dn;                                                                \
-            dn = d1[++task];                                                                   \
-            pptr = (dst & 0x8000) ? X + (ne + npiece + (dst & 0x7fff))                         \
-                                  : (dst < a_rows ? sAccA + dst : sAccB + (dst - a_rows));     \
-            pold = *pptr;                                                                      \
-            if (dst & 0x8000) pold = 0.0;                                                      \
-            pacc = acc;                                                                        \
-            acc = 0.0;                                                                         \
-        }                                                                                      \
-    }
-                EPHC_RES_STEP(wd0, v0)
-                EPHC_RES_STEP(wd1, v1)
-                EPHC_RES_STEP(wd2, v2)
-                EPHC_RES_STEP(wd3, v3)
-#undef EPHC_RES_STEP
+            const uint16_t *srow = reinterpret_cast<const uint16_t *>(sBlob + D.o_srow2);
+            const uint32_t *shdr = reinterpret_cast<const uint32_t *>(sBlob + D.o_shdr2);
+            const uint16_t *perm = reinterpret_cast<const uint16_t *>(sBlob + D.o_perm);
+            double *bdst = P.part + D.b_off - a_rows;  // partial sum of local row u >= a_rows
+            const int s1 = wptr[NW + 1 + warp + 1];
+            int s = wptr[NW + 1 + warp];
+            uint32_t hd = 0;
+            unsigned u = kResNoRow;
+            if (s < s1) {
+                hd = shdr[s];
+                u = srow[32 * s + lane];
             }
-            *pptr = pold + pacc;
+            for (; s < s1; ++s) {
+                const bool more = s + 1 < s1;
+                const uint32_t hd_n = more ? shdr[s + 1] : 0u;
+                const unsigned u_n = more ? srow[32 * (s + 1) + lane] : (unsigned)kResNoRow;
+                const int base = (int)(hd & 1023u) * 32 + lane, H = (int)((hd >> kResHdrHShift) & kResHdrHMask);
+                const uint16_t *g = perm + base;
+                double acc = 0.0;
+                const unsigned zero = (unsigned)D.ne_pad;
+                unsigned p0 = 0 < H ? g[0] : zero, p1 = 1 < H ? g[32] : zero, p2 = 2 < H ? g[64] : zero, p3 = 3 < H ? g[96] : zero;
+                for (int j = 0; j < H; j += 4) {
+                    const unsigned n0 = j + 4 < H ? g[128] : zero, n1 = j + 5 < H ? g[160] : zero, n2 = j + 6 < H ? g[192] : zero,
+                                   n3 = j + 7 < H ? g[224] : zero;
+                    const double v0 = X[p0], v1 = X[p1], v2 = X[p2], v3 = X[p3];
+                    acc += v0;
+                    acc += v1;
+                    acc += v2;
+                    acc += v3;
+                    p0 = n0, p1 = n1, p2 = n2, p3 = n3;
+                    g += 128;
+                }
+                bool head = true;
+                if (hd & kResHdrMulti) {
+                    const unsigned same = __match_any_sync(0xffffffffu, u);
+                    acc = res_group_sum(acc, same, lane);
+                    head = (same & ((1u << lane) - 1u)) == 0u;
+                }
+                if (u != kResNoRow && head) {
+                    if ((int)u < a_rows)
+                        sAccA[u] += acc;   // diagonal tile: both ends in the strip
+                    else
+                        bdst[u] = acc;     // the only contribution of this tile to the row
+                }
+                hd = hd_n;
+                u = u_n;
+            }
         }
         EPHC_TICK(4)
-        if (D.ntask2 > 0) {  // rows whose inputs were cut: their partial sums are added in a second round
-            consumer_sync(NL);
-            const uint32_t *cols3 = cols + nc1 + nc2;
-            const uint16_t *perm2 = perm + D.ngl1;
-            const uint16_t *d2 = reinterpret_cast<const uint16_t *>(sBlob + D.o_d2);
-            const int ntask2 = D.ntask2, nc3 = D.nc3;
-            for (int t = tid; t < ((ntask2 + 31) & ~31); t += NL) {
-                const int s0 = t & ~31;
-                double acc = 0.0;
-                for (int j = 0; j < nc3; ++j) {
-                    const uint32_t c = cols3[j];
-                    const int cnt = (int)(c & 0xffffu);
-                    if (s0 >= cnt) break;
-                    if (t < cnt) acc += X[perm2[(int)(c >> 16) + t]];
-                }
-                if (t < ntask2) {
-                    const int dst = d2[t];
-                    if (dst < a_rows)
-                        sAccA[dst] += acc;
-                    else
-                        sAccB[dst - a_rows] += acc;
-                }
-            }
-        }
+        // the strip's accumulators are touched by phase 2 (diagonal tile) or flushed (end of a run): order that against
+        // the next tile's phase 1
+        const int flags = D.flags, b_rows = D.b_rows;
+        if (b_rows == 0 || (flags & 2)) consumer_sync(NL);
         EPHC_TICK(5)
-        consumer_sync(NL);
-        EPHC_TICK(6)
-        const int b_rows = D.b_rows;
-        if (b_rows > 0) {
-            double *dst = P.part + D.b_off;
-            for (int k = tid; k < b_rows; k += NL) dst[k] = sAccB[k];
-        }
-        if (D.flags & 2) {  // last tile of its run: the strip's sums go to their slot
+        if (flags & 2) {  // last tile of its run: the strip's sums go to their slot
             double *dst = P.part + D.a_off;
             for (int k = tid; k < a_rows; k += NL) {
                 dst[k] = sAccA[k];
                 sAccA[k] = 0.0;
             }
+            consumer_sync(NL);
         }
+        EPHC_TICK(6)
         // this warp is done with the buffer and with the directory entry: T was written over w, order it before the
         // producer's next bulk copy
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(&sEmpty[b]);
+        if (lane == 0) mbar_arrive(&sEmpty[b]);
         EPHC_TICK(7)
     }
 #ifdef EPHC_RES_TIMING
-    if (P.dbg && (tid & 31) == 0)
-        for (int k = 0; k < 8; ++k) P.dbg[((size_t)blockIdx.x * (NL / 32) + (tid >> 5)) * 8 + k] = tacc[k];
+    if (P.dbg && lane == 0)
+        for (int k = 0; k < 8; ++k) P.dbg[((size_t)blockIdx.x * (NW + 1) + warp) * 8 + k] = tacc[k];
 #endif
 }
 

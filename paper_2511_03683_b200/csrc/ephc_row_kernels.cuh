@@ -26,7 +26,10 @@ constexpr int kRowGroup = 8;  // lanes per destination row
 constexpr int kRowBatch = EPHC_ROW_BATCH;
 
 struct RowParams {
-    const double *W;        // per entry, row-store order
+    double *W;              // per entry, row-store order: written by row_setup_kernel, read by row_iter_kernel
+    const double *wst;      // per entry: channel weight (setup)
+    const uint32_t *meta;   // per entry: (iq * nnu + mode) | kind << 31 (setup)
+    const double *N;        // setup: phonon occupations [nq][nnu]
     const uint16_t *idx;
     const RowSeg *segs;
     const RowTile *tiles;
@@ -66,6 +69,99 @@ __device__ __forceinline__ void cp_async_wait() {
 __global__ void __launch_bounds__(256) row_permute_kernel(const double *gW, const uint32_t *perm, double *W, int64_t n) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) W[i] = __ldg(gW + __ldcs(perm + i));
+}
+
+// f0[ns] -> f0 of the compact rows (the rows a tile stages are then one contiguous block)
+__global__ void __launch_bounds__(256) row_compact1_kernel(const double *f, const int32_t *row_state, double *fc, int nrows) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < nrows) fc[r] = f[row_state[r]];
+}
+
+// transport_setup on the row store (reading R-16): per ordered term a <- b
+//     W(a<-b) = w (1 + N - f0_b)  (emission as seen from a)   or   w (N + f0_b)  (absorption),
+// written in row-store order for row_iter_kernel, and Gamma_a = sum_b W(a<-b).  Same walk as row_iter_kernel (one CTA per
+// strip of destination rows, partner ranges staged in shared memory -- here f0, 8 bytes per row --, 8 lanes per
+// destination row); N[iq, nu] comes from the L2-resident table.
+__global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_setup_kernel(const RowParams P) {
+    extern __shared__ double smem[];
+    double *sF = smem;                   // staged f0 of the partner rows [Rb]
+    double *sAcc = smem + (P.Rb + 2);    // [Ra]
+    int *sNext = reinterpret_cast<int *>(sAcc + P.Ra);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int sub = lane / kRowGroup, gl = lane % kRowGroup;
+    constexpr int GPW = 32 / kRowGroup;
+    for (int64_t s = (int64_t)blockIdx.x * kRowThreads + tid; s < P.ns; s += (int64_t)gridDim.x * kRowThreads)
+        if (P.state_row[s] < 0) P.out[s] = 0.0;  // states outside the window scatter nowhere
+    if ((int)blockIdx.x >= P.nstrip) return;
+    const RowStrip st = P.strips[blockIdx.x];
+    for (int i = tid; i < st.nrows; i += kRowThreads) sAcc[i] = 0.0;
+    const double *wb = P.wst + st.e0;
+    const uint32_t *mb = P.meta + st.e0;
+    const uint16_t *Ib = P.idx + st.e0;
+    double *Wb = P.W + st.e0;
+    for (int t = st.t0; t < st.t1; ++t) {
+        const RowTile tl = P.tiles[t];
+        __syncthreads();
+        {
+            const double *src = P.Fc + tl.col0;  // col0 is even: 16-byte aligned
+            const int n16 = (tl.ncols + 1) / 2;
+            for (int i = tid; i < n16; i += kRowThreads) cp_async16(sF + 2 * i, src + 2 * i);
+            cp_async_commit();
+            if (tid == 0) *sNext = 0;
+            cp_async_wait<0>();
+        }
+        __syncthreads();
+        for (;;) {
+            int g = 0;
+            if (lane == 0) g = atomicAdd(sNext, GPW);
+            const int sg0 = __shfl_sync(0xffffffffu, g, 0);
+            if (sg0 >= tl.nseg) break;
+            uint32_t start = 0, len = 0, row = 0;
+            if (sg0 + sub < tl.nseg) {
+                const uint4 q = __ldg(reinterpret_cast<const uint4 *>(P.segs + tl.seg0 + sg0 + sub));
+                start = q.x;
+                len = q.y;
+                row = q.z;
+            }
+            uint32_t lmax = len;
+            lmax = max(lmax, __shfl_xor_sync(0xffffffffu, lmax, 8));
+            lmax = max(lmax, __shfl_xor_sync(0xffffffffu, lmax, 16));
+            double acc = 0.0;
+            constexpr int U = 4;
+            for (uint32_t ib = 0; ib < lmax; ib += U * kRowGroup) {
+                double wv[U], Nv[U];
+                uint32_t mv[U];
+                unsigned jv[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const uint32_t ii = ib + gl + u * kRowGroup;
+                    wv[u] = 0.0;
+                    mv[u] = 0;
+                    jv[u] = 0;
+                    if (ii < len) {
+                        wv[u] = __ldcs(wb + start + ii);
+                        mv[u] = __ldcs(mb + start + ii);
+                        jv[u] = __ldcs(Ib + start + ii);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u) Nv[u] = __ldg(P.N + (mv[u] & 0x7fffffffu));
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const uint32_t ii = ib + gl + u * kRowGroup;
+                    const double fb = sF[jv[u]];
+                    const double W = (mv[u] >> 31) ? wv[u] * (1.0 + Nv[u] - fb) : wv[u] * (Nv[u] + fb);
+                    if (ii < len) __stcs(Wb + start + ii, W);
+                    acc += W;  // lanes past the end carry w = 0
+                }
+            }
+#pragma unroll
+            for (int o = kRowGroup / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            if (gl == 0 && sg0 + sub < tl.nseg) sAcc[row] += acc;  // the only writer of this row in this tile
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < st.nrows; i += kRowThreads) P.out[P.row_state[st.row0 + i]] = sAcc[i];
 }
 
 __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kernel(const RowParams P) {

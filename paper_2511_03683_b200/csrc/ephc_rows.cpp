@@ -37,6 +37,11 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
 
         // destination / partner row of every gather entry (walk work units -> rounds -> tasks as the kernels do)
         std::vector<int32_t> drow((size_t)nent), prow((size_t)nent);
+        std::vector<uint32_t> pmeta((size_t)nent);  // (iq * nnu + mode) | kind << 31: what transport_setup needs besides w
+        if ((int64_t)d.nq * d.nnu >= 0x80000000LL) {
+            err = "row store: N table with 2^31 or more elements";
+            return EPHC_ELIMIT;
+        }
         const int64_t nwu = (int64_t)g.wus.size();
 #pragma omp parallel for schedule(dynamic, 16)
         for (int64_t iw = 0; iw < nwu; ++iw) {
@@ -50,6 +55,8 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
                         const int32_t ps = g.hp_k[rd.hp0 + (c & kPairMask)] * nb + (int32_t)((c >> kBandShift) & 15);
                         drow[e] = r.state_row[tk.row];
                         prow[e] = r.state_row[ps];
+                        pmeta[e] = ((uint32_t)g.hp_q[rd.hp0 + (c & kPairMask)] * (uint32_t)d.nnu + ((c >> kModeShift) & 63u)) |
+                                   (((c >> kKindBit) & 1u) << 31);
                     }
                 }
             }
@@ -125,11 +132,15 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
         // scatter the entries (gather order inside a segment)
         r.idx.resize((size_t)nent);
         r.perm.resize((size_t)nent);
+        r.wst.resize((size_t)nent);
+        r.meta.resize((size_t)nent);
         for (int64_t e = 0; e < nent; ++e) {
             const int32_t c = prow[e] / Rb;
             const int64_t o = seg_abs[(size_t)drow[e] * nrange + c]++;
             r.idx[o] = (uint16_t)(prow[e] - c * Rb);
             r.perm[o] = (uint32_t)e;
+            r.wst[o] = g.w[e];
+            r.meta[o] = pmeta[e];
         }
     } catch (const std::bad_alloc &) {
         err = "host allocation failed (row store)";

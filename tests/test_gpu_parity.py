@@ -260,16 +260,18 @@ def test_stream_geometry_on_gpu(monkeypatch, rows, fine, ctas):
         assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
 
 
-@pytest.mark.parametrize("rows,fine,smem,lp,lg,ctas", [(16, 4, 16000, 3, 2, 3), (64, 8, 24000, 2, 3, 40), (512, 128, None, None, None, 1),
-                                                       (32, 32, 20000, 16, 4, 7)])
-def test_res_geometry_on_gpu(monkeypatch, rows, fine, smem, lp, lg, ctas):
-    # resident-tile store: many tiny tiles, tiles split by the shared-memory budget, out rows cut into pieces, rows that
-    # need the second gather round, runs longer than one tile, one CTA for everything
+@pytest.mark.parametrize("rows,fine,smem,hcap,mode,ctas", [(16, 4, 16000, 1, 0, 3), (64, 8, 24000, 2, 4, 40), (512, 128, None, 3, 1, 1),
+                                                           (32, 32, 20000, 200, 2, 7), (128, 16, None, None, 6, 5), (64, 16, 30000, 4, 5, 300),
+                                                           (256, 32, None, None, 3, 148)])
+def test_res_geometry_on_gpu(monkeypatch, rows, fine, smem, hcap, mode, ctas):
+    # resident-tile store: many tiny tiles, tiles split by the shared-memory budget, rows cut into one- to three-element
+    # pieces (several lanes per row, combined by shuffles), runs longer than one tile, one CTA for everything, every
+    # launch mode of res_kernel
     monkeypatch.setenv("EPHC_RES_ROWS", str(rows))
     monkeypatch.setenv("EPHC_RES_ROWS_B", str(rows))
     monkeypatch.setenv("EPHC_RES_FINE", str(fine))
     monkeypatch.setenv("EPHC_RES_CTAS", str(ctas))
-    for k, v in (("EPHC_RES_SMEM", smem), ("EPHC_RES_LP", lp), ("EPHC_RES_LG", lg)):
+    for k, v in (("EPHC_RES_SMEM", smem), ("EPHC_RES_HCAP", hcap), ("EPHC_RES_MODE", mode)):
         if v is not None:
             monkeypatch.setenv(k, str(v))
     for p in _small_problems()[:5]:

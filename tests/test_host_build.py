@@ -197,21 +197,21 @@ def test_stream_store_holds_every_channel_once(prob, rows, fine, ctas, monkeypat
     assert np.abs(I - Io).max() <= 1e-12 * np.abs(Io).max()
 
 
-@pytest.mark.parametrize("rows,fine,smem,lp,lg", [(None, None, None, None, None), (16, 4, 16000, 3, 2), (64, 8, 24000, 2, 3),
-                                                  (512, 128, None, None, None), (32, 32, 20000, 16, 4)])
-def test_res_store_holds_every_weight_once(prob, rows, fine, smem, lp, lg, monkeypatch):
+@pytest.mark.parametrize("rows,fine,smem,hcap,mode", [(None, None, None, None, None), (16, 4, 16000, 1, 1), (64, 8, 24000, 2, 4),
+                                                      (512, 128, None, 3, 6), (32, 32, 20000, 200, 2)])
+def test_res_store_holds_every_weight_once(prob, rows, fine, smem, hcap, mode, monkeypatch):
     # resident-tile store (variant 3): default geometry, and forced geometries with many tiny tiles, tiles split by
-    # the shared-memory budget, out rows cut into pieces and rows whose inputs need the second gather round
+    # the shared-memory budget, rows cut into many one- to three-element pieces (several lanes per row), other launch modes
     if rows is not None:
         monkeypatch.setenv("EPHC_RES_ROWS", str(rows))
         monkeypatch.setenv("EPHC_RES_ROWS_B", str(rows))
         monkeypatch.setenv("EPHC_RES_FINE", str(fine))
-    for k, v in (("EPHC_RES_SMEM", smem), ("EPHC_RES_LP", lp), ("EPHC_RES_LG", lg)):
+    for k, v in (("EPHC_RES_SMEM", smem), ("EPHC_RES_HCAP", hcap), ("EPHC_RES_MODE", mode)):
         if v is not None:
             monkeypatch.setenv(k, str(v))
     L = oracle.OracleList(prob)
     h = ephc.build_channels(prob, flags=ephc.HOST_ONLY)
-    t = h.export_res()        # also checks the tile images: column tables, pieces, gather lists, slots, coverage
+    t = h.export_res()        # also checks the tile images: slabs of both phases, padding, gather lists, slots, coverage
     ch = L.export()
     assert len(t["w"]) == L.nw
     a = ch["ik"] * prob.nb + ch["n"]
