@@ -300,7 +300,7 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
              3: "res_compact_kernel + res_kernel + finish_kernel<0>"}[variant]
     rname = {0: "gather_kernel<1>", 1: "tile_kernel<0> + finish_kernel<1>", 2: "stream_kernel + finish_kernel<1>",
              3: "res_compact_kernel + res_kernel + finish_kernel<1>"}[variant]
-    sname, iname = "gather_kernel<2> + row_permute_kernel", "row_compact_kernel + row_iter_kernel"
+    sname, iname = "row_compact1_kernel + row_setup_kernel", "row_compact_kernel + row_iter_kernel"
     if os.environ.get("EPHC_NO_ROWS"):
         sname, iname = "gather_kernel<2>", "gather_kernel<3>"
     if tvariant == 1:
@@ -391,7 +391,7 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
     if variant != 0 and tvariant == 0:
         sb += q["store_bytes_gather"]
     names = {0: "gather", 1: "tiles", 2: "stream", 3: "resident tiles"}
-    tname = names[tvariant] if (tvariant == 1 or os.environ.get("EPHC_NO_ROWS")) else "rows (setup on gather)"
+    tname = names[tvariant] if (tvariant == 1 or os.environ.get("EPHC_NO_ROWS")) else "rows"
     coll_mb = (q["store_bytes_scatter"] if variant else q["store_bytes_gather"]) / 1e6
     l2 = ("no flush: every collision evaluation streams its %.0f MB store, larger than the 126 MB L2" % coll_mb
           if coll_mb > 126 else "no flush: the %.0f MB collision store FITS the 126 MB L2 (L2-resident after warm-up; the roofline fraction is not an HBM figure)" % coll_mb)

@@ -465,7 +465,7 @@ def test_full_size_bench_workload_matches_oracle():
     p = make_problem("si")
     L = oracle.OracleList(p)
     h = ephc.build_channels(p)
-    assert h.query()["nch"] == L.nch > 1.0e7 and h.get_variant() == 2 and h.get_transport_variant() == 0
+    assert h.query()["nch"] == L.nch > 1.0e7 and h.get_variant() == 3 and h.get_transport_variant() == 0
     a, b = h.export_channels(), L.export()                 # the list, bit for bit, at full size
     for k in ("ik", "ikq", "iq", "n", "m", "nu"):
         assert np.array_equal(a[k], b[k]), k
