@@ -394,10 +394,10 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
             // small problems: enough strips that every CTA gets a few runs
             while (Ra > 16 && (int64_t)(t.nrows / Ra) * (t.nrows / Ra) < 8 * (int64_t)ncta) Ra /= 2;
         }
-        // two tile buffers: f of the A and B rows, accumulators of the B rows, image + X tail + N rows; a tenth of what
-        // is left may hold N rows of pairs, which bounds the next tile's iq list that an image carries
+        // two tile buffers: f of the A and B rows, image + zero + N rows; three fifths of a buffer may hold N rows of pairs
+        // (few channels per pair: the N rows outweigh the entries), which bounds the next tile's iq list that an image carries
         const int64_t per_buf = (smem_cap - res_fixed_bytes(Ra)) / 2 - 8 * (int64_t)(Ra + RbMax) - 256;
-        const int32_t nq_cap = (int32_t)std::max<int64_t>(1, std::min<int64_t>(kResSlotMax / nnu, per_buf / (3 * 8 * (int64_t)nnu)));
+        const int32_t nq_cap = (int32_t)std::max<int64_t>(1, std::min<int64_t>(kResSlotMax / nnu, (per_buf * 3 / 5) / (8 * (int64_t)nnu)));
         const int64_t budget = per_buf - 4 * (int64_t)nq_cap - 16;
         if (budget < 2048) {
             t.why = "resident-tile store: shared-memory budget too small";
