@@ -340,17 +340,18 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
                 const uint16_t *g = perm + base;
                 double acc = 0.0;
                 const unsigned zero = (unsigned)D.ne_pad;
-                unsigned p0 = 0 < H ? g[0] : zero, p1 = 1 < H ? g[32] : zero, p2 = 2 < H ? g[64] : zero, p3 = 3 < H ? g[96] : zero;
-                for (int j = 0; j < H; j += 4) {
-                    const unsigned n0 = j + 4 < H ? g[128] : zero, n1 = j + 5 < H ? g[160] : zero, n2 = j + 6 < H ? g[192] : zero,
-                                   n3 = j + 7 < H ? g[224] : zero;
-                    const double v0 = X[p0], v1 = X[p1], v2 = X[p2], v3 = X[p3];
-                    acc += v0;
-                    acc += v1;
-                    acc += v2;
-                    acc += v3;
-                    p0 = n0, p1 = n1, p2 = n2, p3 = n3;
-                    g += 128;
+                // eight columns per step: all positions, then all T values, then the adds (the lists are short: latency, not
+                // bandwidth, bounds this phase)
+                for (int j = 0; j < H; j += 8) {
+                    unsigned p[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) p[k] = j + k < H ? g[32 * k] : zero;
+                    double v[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) v[k] = X[p[k]];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) acc += v[k];
+                    g += 256;
                 }
                 bool head = true;
                 if (hd & kResHdrMulti) {
