@@ -156,18 +156,19 @@ int64_t ephc_stream_entries(const ephc_handle *h);
 
 /* Decoded image of the resident-tile store (variant 3), same conditions as ephc_export_gather.  Arrays of length
  * ephc_res_entries(h) (= nw) in store order (runs in hand-out order -> tiles -> entry positions): state a = (n,k),
- * state b = (m,k'), canonical iq, mode, kind (0: w_abs, stored as the directed entry b -> a; 1: w_em, stored as
- * a -> b), weight.  Walks the tile images exactly as the kernel does (column tables, pieces, gather lists of both
- * rounds) and checks that every term T reaches both of its rows exactly once. */
+ * state b = (m,k'), canonical iq, mode, kind (0: w_abs, stored as -w; 1: w_em, stored as +w), weight.  Walks the
+ * tile images exactly as the kernel does (the slabs of both phases warp by warp, padding, gather lists) and checks that
+ * every term T reaches both of its rows exactly once and that every B row of a tile stores a sum. */
 int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
                     double *w);
 int64_t ephc_res_entries(const ephc_handle *h);
 
 /* Decoded image of the row store (the destination-sorted store ephc_transport_iter runs on), same conditions as
  * ephc_export_gather.  Arrays of length gather_entries in store order (strips -> partner-range tiles -> segments):
- * destination state, partner state, position of the same ordered term in the gather store (whose weights
- * ephc_transport_setup brings into this order).  Checks that the strips partition the destination rows, that a row has
- * one segment per tile with segments in descending length, and that the positions are a permutation. */
+ * destination state, partner state, position of the same ordered term in the gather store (the row store carries its
+ * own copy of the weight, N index and kind of every ordered term).  Checks that the strips partition the destination
+ * rows, that a row has one segment per tile with segments in descending length, and that the positions are a
+ * permutation. */
 int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *partner, int64_t *gather_pos);
 
 /* Choice of algorithm:
@@ -179,18 +180,19 @@ int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *partner, int6
  *   2 = stream  : once-stored channels in the same tiles, one lane per ENTRY; the per-entry terms stay in shared
  *                 memory and are summed per k row and per k' row of a chunk by one thread each (no atomics).
  *                 Collision / rt only (transport calls then use the gather + row stores); any nb, nnu.
- *   3 = resident tiles: once-stored DIRECTED entries (an absorption weight is the reversed emission entry, so no
- *                 per-entry kind), tiles whose whole image is bulk-copied (TMA) into shared memory and processed in
- *                 place: one lane per out row piece writes the terms over the weights, one lane per row gathers them.
- *                 Collision / rt only (transport calls then use the gather + row stores); any nb, nnu.
+ *   3 = resident tiles: once-stored entries (owner = the channel's first end, the kind in the sign of the weight),
+ *                 tiles whose whole image is bulk-copied (TMA) into shared memory and processed in place: slabs of
+ *                 32 lanes, one lane per piece of an owner row writes the terms over the weights, one lane per piece
+ *                 of a partner row gathers them (no atomics, fixed order).
+ *                 Collision / rt only (transport calls then use the row store); any nb, nnu.
  *   4 = paper layout: the data structure and the two GPU steps of PAPER.md:84-102 as two plain kernels (scatter /
  *                 scatter_channels rows, step 2 writes the per-channel scratch sc_col to HBM, step 3 sums it per
  *                 target through stargets_sources / targets).  ephc_collision only, for the A/B comparison with the
  *                 library's own stores on the same GPU; never chosen automatically.
  *  -1 = automatic (default): ephc_collision / ephc_rt_step use the gather store while it fits the L2 cache
- *                 (<= 96 MB) and the resident-tile store beyond that; ephc_transport_setup runs on the gather store and
- *                 ephc_transport_iter on the row store built from it (the faster choice per call as measured on
- *                 B200).
+ *                 (<= 96 MB) and the resident-tile store beyond that (the stream store if the problem exceeds the tile
+ *                 format); ephc_transport_setup and ephc_transport_iter run on the row store built from the gather
+ *                 store (the faster choice per call as measured on B200).
  * A store that the automatic choice does not use is built and uploaded by the first ephc_set_variant that asks for
  * it (that call allocates and copies; ephc_build_channels builds only what the automatic choice needs).
  * ephc_transport_setup must be called again after a change of variant.  ephc_get_variant returns the variant

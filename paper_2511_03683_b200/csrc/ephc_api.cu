@@ -127,6 +127,7 @@ struct ephc_handle {
     double *dp_sc_col = nullptr;
     // row store (transport_iter of the gather path)
     bool rows_ok = false;
+    bool gather_dev = false;  // the gather store is in device memory (uploaded when a call path needs it)
     int32_t r_nstrip = 0, r_Rb = 0, r_Ra = 0;
     int64_t bytes_rows = 0;
     double *dr_W = nullptr, *dr_Fc = nullptr;
@@ -184,6 +185,38 @@ static ephc_problem problem_view(const ephc_handle *h) {  // what the store buil
     q.pair_ik = h->pair_ik.data();
     q.pair_ikq = h->pair_ikq.data();
     return q;
+}
+
+// The two-sided gather store in device memory.  ephc_build_channels uploads it when the automatic choice computes on it
+// (L2-resident problems, k-sharded handles, no row store); otherwise the first ephc_set_variant(0) rebuilds it from the
+// canonical list and uploads it (that call allocates and copies).
+static int upload_gather(ephc_handle *h, const GatherHost &g) {
+    if (h->gather_dev) return EPHC_OK;
+    int64_t b = 0;
+    int rc = upload(&h->d_code, g.code, &b);
+    if (rc == EPHC_OK) rc = upload(&h->d_w, g.w, &b);
+    if (rc == EPHC_OK) rc = upload(&h->d_hp_k, g.hp_k, &b);
+    if (rc == EPHC_OK) rc = upload(&h->d_hp_q, g.hp_q, &b);
+    if (rc == EPHC_OK) rc = upload(&h->d_tasks, g.tasks, &b);
+    if (rc == EPHC_OK) rc = upload(&h->d_rounds, g.rounds, &b);
+    if (rc == EPHC_OK) rc = upload(&h->d_wus, g.wus, &b);
+    if (rc == EPHC_OK && !h->rows_ok && !h->d_gW &&
+        cudaMalloc((void **)&h->d_gW, (size_t)std::max<int64_t>(1, h->g_entries) * 8) != cudaSuccess)
+        rc = fail(EPHC_ENOMEM, "cudaMalloc (transport weights) failed");
+    if (rc == EPHC_OK) {
+        h->bytes_gather = b;
+        h->gather_dev = true;
+    }
+    return rc;
+}
+static int make_gather_device(ephc_handle *h) {
+    if (h->gather_dev) return EPHC_OK;
+    const ephc_problem q = problem_view(h);
+    std::string err;
+    GatherHost g;
+    int rc = build_gather(&q, h->d, h->can, g, err);
+    if (rc != EPHC_OK) return fail(rc, err);
+    return upload_gather(h, g);
 }
 
 static int make_tile_store(ephc_handle *h) {
@@ -453,6 +486,8 @@ static int auto_coll_variant(const ephc_handle *h) {
 }
 
 static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ranged, ephc_handle **out);
+static inline int coll_variant(const ephc_handle *h);
+static inline int rt_variant(const ephc_handle *h);
 
 extern "C" int ephc_build_channels(const ephc_problem *p, ephc_handle **out) {
     if (out) *out = nullptr;
@@ -561,15 +596,8 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
     }
     h->bytes_gather = 0;
     if (!h->host_only) {
-        int64_t b = 0;
-        rc = upload(&h->d_code, g.code, &b);
-        if (rc == EPHC_OK) rc = upload(&h->d_w, g.w, &b);
-        if (rc == EPHC_OK) rc = upload(&h->d_hp_k, g.hp_k, &b);
-        if (rc == EPHC_OK) rc = upload(&h->d_hp_q, g.hp_q, &b);
-        if (rc == EPHC_OK) rc = upload(&h->d_tasks, g.tasks, &b);
-        if (rc == EPHC_OK) rc = upload(&h->d_rounds, g.rounds, &b);
-        if (rc == EPHC_OK) rc = upload(&h->d_wus, g.wus, &b);
-        h->bytes_gather = b;
+        // the gather store itself goes to the device only when a call path computes on it
+        if (h->ranged || !h->rows_ok || auto_coll_variant(h) == 0) rc = upload_gather(h, g);
         if (rc == EPHC_OK && h->rows_ok) {
             int64_t br = 0;
             rc = upload(&h->dr_idx, rh.idx, &br);
@@ -587,7 +615,7 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         // enqueue work ("allocated once"): transport weights in gather and row order, RK4 scratch, sums
         const size_t nb8 = (size_t)ns * 8, ne8 = (size_t)std::max<int64_t>(1, h->g_entries) * 8;
         if (rc == EPHC_OK &&
-            ((!h->rows_ok && cudaMalloc((void **)&h->d_gW, ne8) != cudaSuccess) || (h->rows_ok && cudaMalloc((void **)&h->dr_W, ne8) != cudaSuccess) ||
+            ((h->rows_ok && cudaMalloc((void **)&h->dr_W, ne8) != cudaSuccess) ||
              cudaMalloc((void **)&h->d_y[0], nb8) != cudaSuccess || cudaMalloc((void **)&h->d_y[1], nb8) != cudaSuccess ||
              cudaMalloc((void **)&h->d_ksum, nb8) != cudaSuccess ||
              cudaMalloc((void **)&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, (ns + 255) / 256), 1) * 8) != cudaSuccess))
@@ -627,6 +655,7 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         if (rc == EPHC_OK && (h->host_only || av == 2 || (av == 3 && !h->res_ok))) rc = make_stream_store(h);
         if (rc == EPHC_OK && (h->host_only || (av >= 2 && !h->res_ok && !h->stream_ok))) rc = make_tile_store(h);
     }
+    if (rc == EPHC_OK && !h->host_only && !h->gather_dev && (coll_variant(h) == 0 || rt_variant(h) == 0)) rc = make_gather_device(h);
     if (rc != EPHC_OK) {
         const std::string msg = g_err;
         if (!h->host_only) free_dev(h);
@@ -1163,6 +1192,7 @@ extern "C" int ephc_set_variant(ephc_handle *h, int variant) {
     if (variant == 1 && !h->tile_ok)
         return fail(EPHC_ESTATE, "tile store not available for this problem: " + h->thost.why);
     h->variant = variant;
+    if (!h->host_only && (coll_variant(h) == 0 || rt_variant(h) == 0)) return make_gather_device(h);
     return EPHC_OK;
 }
 
