@@ -62,6 +62,9 @@ extern "C" {
 
 /* flags of ephc_problem.flags */
 #define EPHC_HOST_ONLY 1u /* build the store on the host only (no device needed): query/export work, compute fails */
+#define EPHC_SELECT_GPU 2u /* channel selection on the device: count / prefix sum / fill over the candidate
+                              pairs; the same canonical list as the host selection (indices bit-exact, weights within the
+                              two exp implementations); the stores are still laid out on the host */
 
 typedef struct ephc_handle ephc_handle;
 
@@ -71,7 +74,7 @@ typedef struct ephc_problem {
     int32_t nk;              /* number of active k points (>= 1) */
     int32_t nb;              /* bands, 1..16 */
     int32_t nnu;             /* phonon modes, 1..64 */
-    uint32_t flags;          /* EPHC_HOST_ONLY or 0 */
+    uint32_t flags;          /* EPHC_HOST_ONLY, EPHC_SELECT_GPU or 0 */
     const int32_t *kfull;    /* [nk] full-grid index of each active k, strictly ascending */
     const double *E;         /* [nk*nb] band energies, eV */
     double emin, emax;       /* energy window, inclusive; a channel needs both end states inside */

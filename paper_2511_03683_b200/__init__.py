@@ -16,9 +16,10 @@ import numpy as np
 
 from . import _build
 
-__all__ = ["EphcError", "Handle", "build_channels", "lib_path", "HOST_ONLY", "version"]
+__all__ = ["EphcError", "Handle", "build_channels", "lib_path", "HOST_ONLY", "SELECT_GPU", "version"]
 
 HOST_ONLY = 1
+SELECT_GPU = 2
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
 

@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libephc.so")
 SOURCES = ("ephc_build.cpp", "ephc_tiles.cpp", "ephc_rows.cpp", "ephc_stream.cpp", "ephc_res.cpp", "ephc_api.cu")
-HEADERS = ("ephc_internal.h", "ephc_kernels.cuh", "ephc_tile_kernels.cuh", "ephc_row_kernels.cuh", "ephc_stream_kernels.cuh", "ephc_res_kernels.cuh", "ephc_paper_kernels.cuh", os.path.join("..", "..", "include", "ephc.h"))
+HEADERS = ("ephc_internal.h", "ephc_select_kernels.cuh", "ephc_kernels.cuh", "ephc_tile_kernels.cuh", "ephc_row_kernels.cuh", "ephc_stream_kernels.cuh", "ephc_res_kernels.cuh", "ephc_paper_kernels.cuh", os.path.join("..", "..", "include", "ephc.h"))
 
 
 def _stale() -> bool:

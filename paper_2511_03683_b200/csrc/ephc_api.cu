@@ -17,6 +17,7 @@
 #include "ephc_row_kernels.cuh"
 #include "ephc_stream_kernels.cuh"
 #include "ephc_res_kernels.cuh"
+#include "ephc_select_kernels.cuh"
 #include "ephc_paper_kernels.cuh"
 
 using namespace ephc;
@@ -485,6 +486,129 @@ static int auto_coll_variant(const ephc_handle *h) {
     return 3;
 }
 
+// Channel selection on the device (EPHC_SELECT_GPU): uploads the problem, counts the active channels of
+// every candidate pair, prefix-sums the counts on the host, fills the canonical list on the device and brings it back.
+// Same list as build_canonical (bit-exact indices; weights within the two exp implementations).
+static int build_canonical_gpu(const ephc_problem *p, const Dims &d, Canonical &c, std::string &err) {
+    int rc = validate_problem(p, d, err);
+    if (rc != EPHC_OK) return rc;
+    const int64_t npair = p->npair, blk = (int64_t)d.nnu * d.nb * d.nb;
+    std::vector<void *> owned;
+    auto dev_alloc = [&](size_t bytes) -> void * {
+        void *q = nullptr;
+        if (cudaMalloc(&q, std::max<size_t>(bytes, 8)) != cudaSuccess) return nullptr;
+        owned.push_back(q);
+        return q;
+    };
+    auto cleanup = [&]() {
+        for (void *q : owned) cudaFree(q);
+    };
+    auto dev_copy = [&](const void *src, size_t bytes) -> void * {
+        void *q = dev_alloc(bytes);
+        if (q && bytes && cudaMemcpy(q, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return nullptr;
+        return q;
+    };
+    SelectParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.pair_ik = (const int32_t *)dev_copy(p->pair_ik, (size_t)npair * 4);
+    P.pair_ikq = (const int32_t *)dev_copy(p->pair_ikq, (size_t)npair * 4);
+    P.kfull = (const int32_t *)dev_copy(p->kfull, (size_t)d.nk * 4);
+    P.E = (const double *)dev_copy(p->E, (size_t)d.ns * 8);
+    P.hw = (const double *)dev_copy(p->hw, (size_t)d.nq * d.nnu * 8);
+    P.g2 = (const double *)dev_copy(p->g2, (size_t)(npair * blk) * 8);
+    P.cnt_ch = (uint32_t *)dev_alloc((size_t)npair * 4);
+    P.cnt_dg = (uint32_t *)dev_alloc((size_t)npair * 4);
+    P.pair_iq = (int32_t *)dev_alloc((size_t)npair * 4);
+    int64_t *d_ch0 = (int64_t *)dev_alloc((size_t)(npair + 1) * 8), *d_dg0 = (int64_t *)dev_alloc((size_t)(npair + 1) * 8);
+    if (!P.pair_ik || !P.pair_ikq || !P.kfull || !P.E || !P.hw || !P.g2 || !P.cnt_ch || !P.cnt_dg || !P.pair_iq || !d_ch0 || !d_dg0) {
+        cleanup();
+        err = "device allocation or copy failed (channel selection)";
+        return EPHC_ENOMEM;
+    }
+    P.nb = d.nb;
+    P.nnu = d.nnu;
+    P.g0 = d.grid[0];
+    P.g1 = d.grid[1];
+    P.g2n = d.grid[2];
+    P.emin = p->emin;
+    P.emax = p->emax;
+    P.sigma = p->sigma;
+    P.cut = p->ncut * p->sigma;
+    P.g2_cut = p->g2_cut;
+    P.C = d.C;
+    P.npair = npair;
+    const unsigned grid = (unsigned)((npair + 127) / 128);
+    try {
+        std::vector<uint32_t> cch((size_t)npair), cdg((size_t)npair);
+        c.pair_iq.assign((size_t)npair, 0);
+        c.pair_ch0.assign((size_t)npair + 1, 0);
+        c.pair_dg0.assign((size_t)npair + 1, 0);
+        if (npair > 0) {
+            select_kernel<false><<<grid, 128>>>(P);
+            if (cudaMemcpy(cch.data(), P.cnt_ch, (size_t)npair * 4, cudaMemcpyDeviceToHost) != cudaSuccess ||
+                cudaMemcpy(cdg.data(), P.cnt_dg, (size_t)npair * 4, cudaMemcpyDeviceToHost) != cudaSuccess ||
+                cudaMemcpy(c.pair_iq.data(), P.pair_iq, (size_t)npair * 4, cudaMemcpyDeviceToHost) != cudaSuccess) {
+                cleanup();
+                err = std::string("channel selection (count pass): ") + cudaGetErrorString(cudaGetLastError());
+                return EPHC_ECUDA;
+            }
+        }
+        int64_t npa = 0;
+        for (int64_t ip = 0; ip < npair; ++ip) {
+            npa += (cch[ip] + cdg[ip]) > 0;
+            c.pair_ch0[ip + 1] = c.pair_ch0[ip] + cch[ip];
+            c.pair_dg0[ip + 1] = c.pair_dg0[ip] + cdg[ip];
+        }
+        c.nch = c.pair_ch0[npair];
+        c.ndiag = c.pair_dg0[npair];
+        c.npair_active = npa;
+        c.ch_code.resize((size_t)c.nch);
+        c.ch_wabs.resize((size_t)c.nch);
+        c.ch_wem.resize((size_t)c.nch);
+        c.dg_s.resize((size_t)c.ndiag);
+        c.dg_nu.resize((size_t)c.ndiag);
+        c.dg_wabs.resize((size_t)c.ndiag);
+        c.dg_wem.resize((size_t)c.ndiag);
+        P.ch_code = (uint16_t *)dev_alloc((size_t)c.nch * 2);
+        P.ch_wabs = (double *)dev_alloc((size_t)c.nch * 8);
+        P.ch_wem = (double *)dev_alloc((size_t)c.nch * 8);
+        P.dg_s = (int32_t *)dev_alloc((size_t)c.ndiag * 4);
+        P.dg_nu = (int32_t *)dev_alloc((size_t)c.ndiag * 4);
+        P.dg_wabs = (double *)dev_alloc((size_t)c.ndiag * 8);
+        P.dg_wem = (double *)dev_alloc((size_t)c.ndiag * 8);
+        P.ch0 = d_ch0;
+        P.dg0 = d_dg0;
+        bool ok = P.ch_code && P.ch_wabs && P.ch_wem && P.dg_s && P.dg_nu && P.dg_wabs && P.dg_wem &&
+                  cudaMemcpy(d_ch0, c.pair_ch0.data(), (size_t)(npair + 1) * 8, cudaMemcpyHostToDevice) == cudaSuccess &&
+                  cudaMemcpy(d_dg0, c.pair_dg0.data(), (size_t)(npair + 1) * 8, cudaMemcpyHostToDevice) == cudaSuccess;
+        if (ok && npair > 0) {
+            select_kernel<true><<<grid, 128>>>(P);
+            ok = cudaMemcpy(c.ch_code.data(), P.ch_code, (size_t)c.nch * 2, cudaMemcpyDeviceToHost) == cudaSuccess &&
+                 cudaMemcpy(c.ch_wabs.data(), P.ch_wabs, (size_t)c.nch * 8, cudaMemcpyDeviceToHost) == cudaSuccess &&
+                 cudaMemcpy(c.ch_wem.data(), P.ch_wem, (size_t)c.nch * 8, cudaMemcpyDeviceToHost) == cudaSuccess &&
+                 cudaMemcpy(c.dg_s.data(), P.dg_s, (size_t)c.ndiag * 4, cudaMemcpyDeviceToHost) == cudaSuccess &&
+                 cudaMemcpy(c.dg_nu.data(), P.dg_nu, (size_t)c.ndiag * 4, cudaMemcpyDeviceToHost) == cudaSuccess &&
+                 cudaMemcpy(c.dg_wabs.data(), P.dg_wabs, (size_t)c.ndiag * 8, cudaMemcpyDeviceToHost) == cudaSuccess &&
+                 cudaMemcpy(c.dg_wem.data(), P.dg_wem, (size_t)c.ndiag * 8, cudaMemcpyDeviceToHost) == cudaSuccess;
+        }
+        cleanup();
+        if (!ok) {
+            err = std::string("channel selection (fill pass): ") + cudaGetErrorString(cudaGetLastError());
+            return EPHC_ECUDA;
+        }
+    } catch (const std::bad_alloc &) {
+        cleanup();
+        err = "host allocation failed (canonical channel list)";
+        return EPHC_ENOMEM;
+    }
+    int64_t nw = 0;
+#pragma omp parallel for reduction(+ : nw) schedule(static)
+    for (int64_t j = 0; j < c.nch; ++j) nw += (c.ch_wabs[j] != 0.0) + (c.ch_wem[j] != 0.0);
+    c.nw = nw;
+    c.iq0 = 0;
+    return EPHC_OK;
+}
+
 static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ranged, ephc_handle **out);
 static inline int coll_variant(const ephc_handle *h);
 static inline int rt_variant(const ephc_handle *h);
@@ -551,7 +675,11 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
     }
 
     std::string err;
-    int rc = build_canonical(p, h->d, h->can, err);
+    if ((p->flags & EPHC_SELECT_GPU) && h->host_only) {
+        delete h;
+        return fail(EPHC_EINVAL, "EPHC_SELECT_GPU needs a device handle (not EPHC_HOST_ONLY)");
+    }
+    int rc = (p->flags & EPHC_SELECT_GPU) ? build_canonical_gpu(p, h->d, h->can, err) : build_canonical(p, h->d, h->can, err);
     GatherHost g;
     if (rc == EPHC_OK) rc = build_gather(p, h->d, h->can, g, err);
     if (rc != EPHC_OK) {

@@ -79,10 +79,9 @@ inline int select_pair(const ephc_problem *p, const Dims &d, const uint8_t *inwi
 
 }  // namespace
 
-int build_canonical(const ephc_problem *p, const Dims &d, Canonical &c, std::string &err) {
+int validate_problem(const ephc_problem *p, const Dims &d, std::string &err) {
     const int nb = d.nb, nnu = d.nnu;
     const int64_t npair = p->npair;
-    // ---- validation ------------------------------------------------------------------------------
     for (int32_t k = 0; k < d.nk; ++k) {
         if (p->kfull[k] < 0 || p->kfull[k] >= d.nq || (k > 0 && p->kfull[k] <= p->kfull[k - 1])) {
             err = "kfull must be strictly ascending full-grid indices";
@@ -124,7 +123,17 @@ int build_canonical(const ephc_problem *p, const Dims &d, Canonical &c, std::str
         err = "g2 must be finite and >= 0";
         return EPHC_EINVAL;
     }
+    return EPHC_OK;
+}
 
+int build_canonical(const ephc_problem *p, const Dims &d, Canonical &c, std::string &err) {
+    const int nb = d.nb, nnu = d.nnu;
+    const int64_t npair = p->npair;
+    {
+        const int rc = validate_problem(p, d, err);
+        if (rc != EPHC_OK) return rc;
+    }
+    const int64_t blk = (int64_t)nnu * nb * nb;
     // ---- window flags (R-7: inclusive, state level) -------------------------------------------------
     std::vector<uint8_t> inwin((size_t)d.ns);
     for (int64_t i = 0; i < d.ns; ++i) inwin[i] = (p->E[i] >= p->emin && p->E[i] <= p->emax) ? 1 : 0;

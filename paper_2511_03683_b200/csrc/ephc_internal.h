@@ -75,6 +75,7 @@ struct Dims {
 };
 
 // host builder (ephc_build.cu)
+int validate_problem(const ephc_problem *p, const Dims &d, std::string &err);
 int build_canonical(const ephc_problem *p, const Dims &d, Canonical &c, std::string &err);
 int build_gather(const ephc_problem *p, const Dims &d, const Canonical &c, GatherHost &g, std::string &err);
 

@@ -292,6 +292,32 @@ def test_res_geometry_on_gpu(monkeypatch, rows, fine, smem, hcap, mode, ctas):
         assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
 
 
+def test_gpu_channel_selection_matches_oracle_list():
+    # EPHC_SELECT_GPU: the canonical list selected on the device equals the oracle's
+    # list bit for bit (indices) and within 4 ulp (weights: two exp implementations), diagonal terms included; the
+    # collision integral and Gamma computed from it match the oracle
+    for p in _small_problems() + [make_problem("si", grid=(20, 20, 20), pair_prob=0.2, seed=12)]:
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p, flags=ephc.SELECT_GPU)
+        hh = ephc.build_channels(p)
+        q, qh = h.query(), hh.query()
+        for k in ("nch", "nw", "ndiag", "npair_active", "gather_entries"):
+            assert q[k] == qh[k], k
+        a, b = h.export_channels(), L.export()
+        assert len(a["w_abs"]) == L.nch
+        for k in ("ik", "ikq", "iq", "n", "m", "nu"):
+            assert np.array_equal(a[k], b[k]), k
+        for k in ("w_abs", "w_em"):
+            assert np.all(np.abs(a[k] - b[k]) <= 4 * np.spacing(np.maximum(np.abs(a[k]), np.abs(b[k])))), k
+            assert np.array_equal(a[k] == 0.0, b[k] == 0.0), k        # the same deltas are cut off
+        I = np.zeros(p.ns)
+        h.collision_host(p.f, p.N, I)
+        assert _relerr(I, L.collision(p.f, p.N)) <= TOL
+        F, G = np.zeros((3, p.ns)), np.zeros(p.ns)
+        h.transport_solve_host(p.f0, p.N, p.v, 1, F, G)
+        assert _relerr(G, L.transport_setup(p.f0, p.N)) <= TOL
+
+
 @pytest.mark.parametrize("rng_rows,strips", [(32, 1), (64, 3), (32, 40)])
 def test_row_geometry_on_gpu(monkeypatch, rng_rows, strips):
     # row store (transport_iter): several partner ranges per strip (restaging between tiles), one strip for everything,
