@@ -400,7 +400,25 @@ __global__ void __launch_bounds__(256) finish_kernel(const FinishParams P) {
         if (cr >= 0) {
             const int b = P.state_blk[a];
             const int64_t r = cr - P.blk_row0[b];
-            for (int i = P.blk_ent_ptr[b]; i < P.blk_ent_ptr[b + 1]; ++i) {
+            // eight slots per step: all offsets, then all values, then the adds in list order (the loads are independent;
+            // one at a time this loop is a chain of L2 latencies)
+            const int i1 = P.blk_ent_ptr[b + 1];
+            int i = P.blk_ent_ptr[b];
+            for (; i + 8 <= i1; i += 8) {
+                int64_t off[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) off[u] = __ldg(P.blk_ent_off + i + u);
+                double val[8][C];
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+#pragma unroll
+                    for (int c = 0; c < C; ++c) val[u][c] = __ldcs(P.part + (off[u] + r) * C + c);
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+#pragma unroll
+                    for (int c = 0; c < C; ++c) sum[c] += val[u][c];
+            }
+            for (; i < i1; ++i) {
                 const double *src = P.part + (P.blk_ent_off[i] + r) * C;
 #pragma unroll
                 for (int c = 0; c < C; ++c) sum[c] += src[c];
