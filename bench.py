@@ -299,7 +299,7 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
     cname = {0: "gather_kernel<0>", 1: "tile_kernel<0> + finish_kernel<0>", 2: "stream_kernel + finish_kernel<0>",
              3: "res_compact_kernel + res_kernel + finish_kernel<0>"}[variant]
     rname = {0: "gather_kernel<1>", 1: "tile_kernel<0> + finish_kernel<1>", 2: "stream_kernel + finish_kernel<1>",
-             3: "res_compact_kernel + res_kernel + finish_kernel<1>"}[variant]
+             3: "res_kernel + finish_kernel<1>, which also writes the next stage's compact f"}[variant]
     sname, iname = "row_compact1_kernel + row_setup_kernel", "row_compact_kernel + row_iter_kernel"
     if os.environ.get("EPHC_NO_ROWS"):
         sname, iname = "gather_kernel<2>", "gather_kernel<3>"

@@ -1511,10 +1511,13 @@ static int launch_stream(ephc_handle *h, const double *f, const double *N, cudaS
     return EPHC_OK;
 }
 
-static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStream_t s) {
+// fc_ready: the compact copy of f (dx_fc) was already written by the finish kernel of the previous RK stage
+static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStream_t s, bool fc_ready = false) {
     if (h->x_ntile > 0) {
-        res_compact_kernel<<<(unsigned)((h->x_nrows + 255) / 256), 256, 0, s>>>(f, h->dx_row_state, h->dx_fc, h->x_nrows);
-        h->launches++;
+        if (!fc_ready) {
+            res_compact_kernel<<<(unsigned)((h->x_nrows + 255) / 256), 256, 0, s>>>(f, h->dx_row_state, h->dx_fc, h->x_nrows);
+            h->launches++;
+        }
         ResParams P;
         std::memset(&P, 0, sizeof(P));
         P.blob = h->dx_blob;
@@ -1791,8 +1794,10 @@ static int launch_drift(ephc_handle *h, const double *f, const double *field, do
     return EPHC_OK;
 }
 
+// chained: the caller runs the stages back to back (ephc_rt_step): on the resident-tile store the finish kernel then
+// also writes the compact copy that the next stage reads, and fc_ready says that the previous stage did so
 static int rk_stage(ephc_handle *h, double *f_dev, const double *y_in, const double *N_dev, double dt_fs, int st, double *y_out,
-                    bool want_sum, cudaStream_t s, const double *field = nullptr) {
+                    bool want_sum, cudaStream_t s, const double *field = nullptr, bool chained = false, bool fc_ready = false) {
     int rc;
     const int v = rt_variant(h);
     const double *extra = nullptr;
@@ -1803,7 +1808,7 @@ static int rk_stage(ephc_handle *h, double *f_dev, const double *y_in, const dou
     if (v >= 1) {
         FinishParams Fp;
         if (v >= 2) {
-            if ((rc = (v == 3) ? launch_res(h, y_in, N_dev, s) : launch_stream(h, y_in, N_dev, s))) return rc;
+            if ((rc = (v == 3) ? launch_res(h, y_in, N_dev, s, chained && fc_ready) : launch_stream(h, y_in, N_dev, s))) return rc;
             Fp = (v == 3) ? finish_params_res(h) : finish_params_stream(h);
         } else {
             TileParams T = tile_params(h);
@@ -1819,6 +1824,7 @@ static int rk_stage(ephc_handle *h, double *f_dev, const double *y_in, const dou
         Fp.ksum = h->d_ksum;
         Fp.blk_sum = want_sum ? h->d_wusum : nullptr;
         Fp.extra = extra;
+        Fp.fc_next = (chained && v == 3) ? h->dx_fc : nullptr;
         return launch_finish<kFRkStage>(h, Fp, s);
     }
     GatherParams P = base_params(h);
@@ -1898,7 +1904,8 @@ static int rt_step_impl(ephc_handle *h, double *f_dev, const double *N_dev, cons
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
         for (int st = 0; st < 4; ++st)
-            if ((rc = rk_stage(h, f_dev, src[st], N_dev, dt_fs, st + 1, dst[st], sumf_dev != nullptr, s, field))) return rc;
+            if ((rc = rk_stage(h, f_dev, src[st], N_dev, dt_fs, st + 1, dst[st], sumf_dev != nullptr, s, field, true, it > 0 || st > 0)))
+                return rc;
         if (sumf_dev) {
             if (rt_variant(h) >= 1)
                 sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);

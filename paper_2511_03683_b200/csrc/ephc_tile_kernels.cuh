@@ -57,6 +57,7 @@ struct FinishParams {
     int32_t stage;
     double dt;
     double *f0, *ynext, *ksum, *blk_sum;
+    double *fc_next;      // compact-row copy of what the next evaluation reads (resident-tile store), may be null
     const double *extra;  // added to k_j per state (drift term of Eq. 1), may be null
     // transport
     const double *v, *tau;
@@ -397,6 +398,7 @@ __global__ void __launch_bounds__(256) finish_kernel(const FinishParams P) {
     double fsum = 0.0;
     if (a < P.ns) {
         const int cr = P.state_row[a];
+        double ynew = 0.0;  // rk stage: y_{j+1} (or the new f) of this state
         if (cr >= 0) {
             const int b = P.state_blk[a];
             const int64_t r = cr - P.blk_row0[b];
@@ -435,18 +437,19 @@ __global__ void __launch_bounds__(256) finish_kernel(const FinishParams P) {
             const double f0 = P.f0[a];
             if (P.stage == 1) {
                 P.ksum[a] = k;
-                P.ynext[a] = f0 + 0.5 * P.dt * k;
+                P.ynext[a] = ynew = f0 + 0.5 * P.dt * k;
             } else if (P.stage == 2) {
                 P.ksum[a] += 2.0 * k;
-                P.ynext[a] = f0 + 0.5 * P.dt * k;
+                P.ynext[a] = ynew = f0 + 0.5 * P.dt * k;
             } else if (P.stage == 3) {
                 P.ksum[a] += 2.0 * k;
-                P.ynext[a] = f0 + P.dt * k;
+                P.ynext[a] = ynew = f0 + P.dt * k;
             } else {
                 const double fn = f0 + P.dt / 6.0 * (P.ksum[a] + k);
-                P.f0[a] = fn;
+                P.f0[a] = ynew = fn;
                 fsum = fn;
             }
+            if (P.fc_next != nullptr && cr >= 0) P.fc_next[cr] = ynew;  // the next stage's gather reads compact rows
         }
     }
     if (FMODE == kFRkStage) {
