@@ -219,6 +219,12 @@ int ephc_transport_start(ephc_handle *h, const double *Gamma_dev, const double *
 int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
                         double *Fout_dev, void *stream);
 
+/* niter >= 1 chained iterations, Fout = result of the last one (F_dev is not modified; F_dev != Fout_dev).  Same
+ * arithmetic as niter calls of ephc_transport_iter (bit-identical result); on the row store the intermediate F stay in
+ * compact row order in the handle's scratch instead of going through the API layout. */
+int ephc_transport_iters(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
+                         double *Fout_dev, int niter, void *stream);
+
 /* nsteps classical RK4 steps of df/dt = I[f] with N fixed (reading R-18), f updated in place.
  * sumf_dev (may be NULL): [nsteps+1], sum_s f_s before the first step and after every step.
  * The axpy of every stage is fused into the collision kernel's epilogue. */

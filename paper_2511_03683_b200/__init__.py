@@ -89,6 +89,7 @@ def _load():
         "ephc_transport_setup": (i32, [vp, vp, vp, vp, vp]),
         "ephc_transport_start": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_transport_iter": (i32, [vp, vp, vp, vp, vp, vp]),
+        "ephc_transport_iters": (i32, [vp, vp, vp, vp, vp, i32, vp]),
         "ephc_rt_step": (i32, [vp, vp, vp, dbl, i32, vp, vp]),
         "ephc_collision_host": (i32, [vp, vp, vp, vp]),
         "ephc_transport_solve_host": (i32, [vp, vp, vp, vp, i32, vp, vp]),
@@ -274,6 +275,11 @@ class Handle:
         _check(_load().ephc_transport_iter(self._h, _dev_ptr(F, 3 * self.ns, "F"), _dev_ptr(v, 3 * self.ns, "v"),
                                            _dev_ptr(tau, self.ns, "tau"), _dev_ptr(Fout, 3 * self.ns, "Fout"),
                                            _stream_ptr(stream)))
+
+    def transport_iters(self, F, v, tau, Fout, niter: int, stream=None):
+        _check(_load().ephc_transport_iters(self._h, _dev_ptr(F, 3 * self.ns, "F"), _dev_ptr(v, 3 * self.ns, "v"),
+                                            _dev_ptr(tau, self.ns, "tau"), _dev_ptr(Fout, 3 * self.ns, "Fout"),
+                                            int(niter), _stream_ptr(stream)))
 
     def owned_states(self):
         lo, hi = C.c_int64(), C.c_int64()

@@ -131,7 +131,8 @@ struct ephc_handle {
     bool gather_dev = false;  // the gather store is in device memory (uploaded when a call path needs it)
     int32_t r_nstrip = 0, r_Rb = 0, r_Ra = 0;
     int64_t bytes_rows = 0;
-    double *dr_W = nullptr, *dr_Fc = nullptr;
+    double *dr_W = nullptr, *dr_Fc = nullptr, *dr_Fc2 = nullptr;  // Fc / Fc2: compact F of chained iterations (ping-pong)
+    double *d_Fscr = nullptr;  // [3][ns] scratch of ephc_transport_iters on the stores without a compact copy
     int32_t r_nrows = 0;
     uint16_t *dr_idx = nullptr;
     uint32_t *dr_meta = nullptr;  // per entry: (iq * nnu + mode) | kind << 31
@@ -148,7 +149,7 @@ static void free_dev(ephc_handle *h) {
                     h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
-                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_idx, h->dr_meta, h->dr_wst, h->dr_segs, h->dr_tiles, h->dr_strips,
+                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_Fc2, h->d_Fscr, h->dr_idx, h->dr_meta, h->dr_wst, h->dr_segs, h->dr_tiles, h->dr_strips,
                     h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
                     h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_order, h->ds_counter, h->ds_row_state,
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
@@ -736,7 +737,8 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
             if (rc == EPHC_OK) rc = upload(&h->dr_strips, rh.strips, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_row_state, rh.row_state, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_state_row, rh.state_row, &br);
-            if (rc == EPHC_OK && cudaMalloc((void **)&h->dr_Fc, ((size_t)rh.nrows * 3 + 4) * 8) != cudaSuccess)
+            if (rc == EPHC_OK && (cudaMalloc((void **)&h->dr_Fc, ((size_t)rh.nrows * 3 + 4) * 8) != cudaSuccess ||
+                                  cudaMalloc((void **)&h->dr_Fc2, ((size_t)rh.nrows * 3 + 4) * 8) != cudaSuccess))
                 rc = fail(EPHC_ENOMEM, "cudaMalloc (compact F) failed");
         }
         // everything the device entry points write besides the caller's buffers is allocated here, so that they only
@@ -745,7 +747,7 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         if (rc == EPHC_OK &&
             ((h->rows_ok && cudaMalloc((void **)&h->dr_W, ne8) != cudaSuccess) ||
              cudaMalloc((void **)&h->d_y[0], nb8) != cudaSuccess || cudaMalloc((void **)&h->d_y[1], nb8) != cudaSuccess ||
-             cudaMalloc((void **)&h->d_ksum, nb8) != cudaSuccess ||
+             cudaMalloc((void **)&h->d_ksum, nb8) != cudaSuccess || cudaMalloc((void **)&h->d_Fscr, 3 * nb8) != cudaSuccess ||
              cudaMalloc((void **)&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, (ns + 255) / 256), 1) * 8) != cudaSuccess))
             rc = fail(EPHC_ENOMEM, "cudaMalloc (transport weights / RK4 scratch) failed");
         if (rc == EPHC_OK) h->bytes_transport += h->g_entries * 8;
@@ -1783,6 +1785,47 @@ extern "C" int ephc_transport_iter(ephc_handle *h, const double *F_dev, const do
     return launch_gather<kTransportIter>(h, P, (cudaStream_t)stream);
 }
 
+extern "C" int ephc_transport_iters(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
+                                    double *Fout_dev, int niter, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!F_dev || !v_dev || !tau_dev || !Fout_dev || niter < 1) return fail(EPHC_EINVAL, "null device pointer or niter < 1");
+    if (F_dev == Fout_dev) return fail(EPHC_EINVAL, "transport_iters is out of place: F_dev and Fout_dev must differ");
+    if (!h->transport_ready || h->transport_variant != tr_variant(h))
+        return fail(EPHC_ESTATE, "call ephc_transport_setup (with the current variant) before ephc_transport_iters");
+    if (tr_variant(h) == 0 && h->rows_ok) {
+        // chained on the row store: F is brought into compact row order once, every iteration writes the compact copy the
+        // next one stages, the last one writes the API layout
+        const cudaStream_t s = (cudaStream_t)stream;
+        RowParams R = row_params(h);
+        if (h->r_nrows > 0) {
+            row_compact_kernel<<<(unsigned)((h->r_nrows + 255) / 256), 256, 0, s>>>(F_dev, h->dr_row_state, h->dr_Fc, h->r_nrows, h->d.ns);
+            h->launches++;
+        }
+        R.v = v_dev;
+        R.tau = tau_dev;
+        double *buf[2] = {h->dr_Fc, h->dr_Fc2};
+        for (int it = 0; it < niter; ++it) {
+            const bool last = it + 1 == niter;
+            R.Fc = buf[it & 1];
+            R.Fc_out = last ? nullptr : buf[(it + 1) & 1];
+            R.out = last ? Fout_dev : nullptr;
+            row_iter_kernel<<<(unsigned)std::max(h->r_nstrip, 1), kRowThreads, row_smem_bytes(h->r_Rb, h->r_Ra), s>>>(R);
+            h->launches++;
+        }
+        CUDA_TRY(cudaGetLastError());
+        return EPHC_OK;
+    }
+    // other stores: plain iterations through the scratch vector, ending in Fout
+    const double *src = F_dev;
+    for (int it = 0; it < niter; ++it) {
+        double *dst = ((niter - 1 - it) & 1) ? h->d_Fscr : Fout_dev;
+        if ((rc = ephc_transport_iter(h, src, v_dev, tau_dev, dst, stream))) return rc;
+        src = dst;
+    }
+    return EPHC_OK;
+}
+
 // One RK4 stage (reading R-18): k = I[y_in]; stage 1..3: y_out = f + a dt k and ksum accumulates b k; stage 4:
 // f += dt/6 (ksum + k) in place.  The axpy is the epilogue of the collision pass.
 static int launch_drift(ephc_handle *h, const double *f, const double *field, double *out, cudaStream_t s) {
@@ -1955,12 +1998,10 @@ extern "C" int ephc_transport_solve_host(ephc_handle *h, const double *f0_host, 
     if (rc) return rc;
     rc = ephc_transport_start(h, Gam, v, tau, Fa, nullptr);
     if (rc) return rc;
-    for (int it = 0; it < niter; ++it) {
-        rc = ephc_transport_iter(h, Fa, v, tau, Fb, nullptr);
+    if (niter > 0) {
+        rc = ephc_transport_iters(h, Fa, v, tau, Fb, niter, nullptr);
         if (rc) return rc;
-        double *t = Fa;
         Fa = Fb;
-        Fb = t;
     }
     CUDA_TRY(cudaMemcpyAsync(F_host, Fa, 3 * nf, cudaMemcpyDeviceToHost, 0));
     if (Gamma_host) CUDA_TRY(cudaMemcpyAsync(Gamma_host, Gam, nf, cudaMemcpyDeviceToHost, 0));

@@ -39,7 +39,8 @@ struct RowParams {
     int64_t ns;
     const double *Fc;       // F of the compact rows, [nrows][3] (row_compact_kernel), padded by 2 doubles
     const double *v, *tau;
-    double *out;
+    double *out;            // API layout [3][ns] (Gamma [ns] in setup); the iteration may pass null between chained iterations
+    double *Fc_out;         // iteration: compact [nrows][3] copy of the result for the next chained iteration, may be null
 };
 
 inline size_t row_smem_bytes(int Rb, int Ra) { return ((size_t)Rb + (size_t)Ra) * 3 * sizeof(double) + 48; }
@@ -174,12 +175,13 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kern
     constexpr int GPW = 32 / kRowGroup;  // row groups per warp
 
     // states outside the window receive no contribution: F' = tau v (grid-stride over all states)
-    for (int64_t s = (int64_t)blockIdx.x * kRowThreads + tid; s < P.ns; s += (int64_t)gridDim.x * kRowThreads)
-        if (P.state_row[s] < 0) {
-            const double ta = P.tau[s];
+    if (P.out != nullptr)
+        for (int64_t s = (int64_t)blockIdx.x * kRowThreads + tid; s < P.ns; s += (int64_t)gridDim.x * kRowThreads)
+            if (P.state_row[s] < 0) {
+                const double ta = P.tau[s];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) P.out[(int64_t)c * P.ns + s] = ta * P.v[(int64_t)c * P.ns + s];
-        }
+                for (int c = 0; c < 3; ++c) P.out[(int64_t)c * P.ns + s] = ta * P.v[(int64_t)c * P.ns + s];
+            }
     if ((int)blockIdx.x >= P.nstrip) return;
     const RowStrip st = P.strips[blockIdx.x];
     for (int i = tid; i < st.nrows * 3; i += kRowThreads) sAcc[i] = 0.0;
@@ -282,7 +284,11 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kern
         const int64_t s = P.row_state[st.row0 + i];
         const double ta = P.tau[s];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) P.out[(int64_t)c * P.ns + s] = ta * (P.v[(int64_t)c * P.ns + s] + sAcc[i * 3 + c]);
+        for (int c = 0; c < 3; ++c) {
+            const double val = ta * (P.v[(int64_t)c * P.ns + s] + sAcc[i * 3 + c]);
+            if (P.out != nullptr) P.out[(int64_t)c * P.ns + s] = val;
+            if (P.Fc_out != nullptr) P.Fc_out[(int64_t)(st.row0 + i) * 3 + c] = val;
+        }
     }
 }
 

@@ -107,6 +107,16 @@ def test_transport_matches_oracle(case):
         Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau_o)
     assert _relerr(Gh, Go) <= TOL
     assert _relerr(Fh, Fr) <= 1e-10                                    # 20 chained iterations
+    # ephc_transport_iters: the same arithmetic as repeated ephc_transport_iter calls, bit for bit (1, 2 and 5 iterations)
+    va, ta = dev(v), dev(tau_o)
+    for n in (1, 2, 5):
+        A, B = dev(F), torch.empty(3 * p.ns, device="cuda", dtype=torch.float64)
+        for _ in range(n):
+            h.transport_iter(A, va, ta, B)
+            A, B = B, A
+        Fc = torch.full((3 * p.ns,), np.nan, device="cuda", dtype=torch.float64)
+        h.transport_iters(dev(F), va, ta, Fc, n)
+        assert torch.equal(Fc, A), n
 
 
 def test_rt_step_matches_oracle(case):
