@@ -518,9 +518,13 @@ def test_full_size_bench_workload_matches_oracle():
     st = np.random.default_rng(5).choice(np.flatnonzero(Io != 0.0), 24, replace=False).astype(np.int32)
     Is = oracle.collision_sampled(p, p.f, p.N, st)
     assert np.abs(got[st] - Is).max() <= TOL * np.abs(Io).max()
+    # one owner per element and a fixed order of additions: 200 back-to-back evaluations, the same bits
+    # every time (a missed barrier or an early release of a tile buffer would show up here)
     I2 = torch.empty_like(I)
-    h.collision(f, N, I2)
-    assert torch.equal(I, I2)
+    for _ in range(200):
+        I2.fill_(float("nan"))
+        h.collision(f, N, I2)
+        assert torch.equal(I, I2)
     # transport: Gamma and two iterations from F0 = tau v
     G = torch.empty(p.ns, device="cuda", dtype=torch.float64)
     h.transport_setup(dev(p.f0), N, G)
@@ -535,6 +539,16 @@ def test_full_size_bench_workload_matches_oracle():
         Fa, Fb = Fb, Fa
         Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau_o)
     assert _relerr(Fa.cpu().numpy().reshape(3, -1), Fr) <= TOL
+    # config 2's schedule at full size: 20 chained iterations (ephc_transport_iters), against 18 more oracle iterations;
+    # twice, bit-identical
+    F20 = [torch.full((3 * p.ns,), np.nan, device="cuda", dtype=torch.float64) for _ in range(2)]
+    F0 = dev(tau_o[None, :] * p.v)
+    for k in range(2):
+        h.transport_iters(F0, v, tau, F20[k], 20)
+    assert torch.equal(F20[0], F20[1])
+    for _ in range(18):
+        Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau_o)
+    assert _relerr(F20[0].cpu().numpy().reshape(3, -1), Fr) <= 1e-10      # reading R-27
     # rt-BTE (config 5's initial condition is make_problem("rt"); same channel set): 2 RK4 steps
     pr = make_problem("rt")
     fr = dev(pr.f)
