@@ -78,6 +78,12 @@ __global__ void __launch_bounds__(256) row_compact1_kernel(const double *f, cons
     if (r < nrows) fc[r] = f[row_state[r]];
 }
 
+__device__ __forceinline__ double ld_keep(const double *p, uint64_t policy) {
+    double v;
+    asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;\n" : "=d"(v) : "l"(p), "l"(policy));
+    return v;
+}
+
 // transport_setup on the row store (reading R-16): per ordered term a <- b
 //     W(a<-b) = w (1 + N - f0_b)  (emission as seen from a)   or   w (N + f0_b)  (absorption),
 // written in row-store order for row_iter_kernel, and Gamma_a = sum_b W(a<-b).  Same walk as row_iter_kernel (one CTA per
@@ -96,6 +102,8 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_setup_ker
     if ((int)blockIdx.x >= P.nstrip) return;
     const RowStrip st = P.strips[blockIdx.x];
     for (int i = tid; i < st.nrows; i += kRowThreads) sAcc[i] = 0.0;
+    uint64_t pol_keep;  // the N table is gathered by every strip while 22 bytes per entry stream through the L2
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol_keep));
     const double *wb = P.wst + st.e0;
     const uint32_t *mb = P.meta + st.e0;
     const uint16_t *Ib = P.idx + st.e0;
@@ -146,7 +154,7 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_setup_ker
                     }
                 }
 #pragma unroll
-                for (int u = 0; u < U; ++u) Nv[u] = __ldg(P.N + (mv[u] & 0x7fffffffu));
+                for (int u = 0; u < U; ++u) Nv[u] = ld_keep(P.N + (mv[u] & 0x7fffffffu), pol_keep);
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
                     const uint32_t ii = ib + gl + u * kRowGroup;
