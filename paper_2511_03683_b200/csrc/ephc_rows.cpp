@@ -142,6 +142,46 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
             r.wst[o] = g.w[e];
             r.meta[o] = pmeta[e];
         }
+        // inside a segment: by partner row (stable), so that the ordered terms of one (destination, partner) state pair --
+        // its modes and kinds -- are adjacent (the mode-collapsed specialisation sums them)
+        if (!std::getenv("EPHC_ROW_NO_SORT")) {
+            const int64_t nstrips = (int64_t)r.strips.size();
+#pragma omp parallel
+            {
+                std::vector<uint32_t> ord;
+                std::vector<uint16_t> t_idx;
+                std::vector<uint32_t> t_perm, t_meta;
+                std::vector<double> t_w;
+#pragma omp for schedule(dynamic, 1)
+                for (int64_t is = 0; is < nstrips; ++is) {
+                    const RowStrip &st = r.strips[is];
+                    for (int32_t t = st.t0; t < st.t1; ++t)
+                        for (int32_t sg = r.tiles[t].seg0; sg < r.tiles[t].seg0 + r.tiles[t].nseg; ++sg) {
+                            const uint32_t len = r.segs[sg].len;
+                            const int64_t e0 = st.e0 + r.segs[sg].start;
+                            ord.resize(len);
+                            for (uint32_t i = 0; i < len; ++i) ord[i] = i;
+                            std::stable_sort(ord.begin(), ord.end(), [&](uint32_t x, uint32_t y) { return r.idx[e0 + x] < r.idx[e0 + y]; });
+                            t_idx.resize(len);
+                            t_perm.resize(len);
+                            t_meta.resize(len);
+                            t_w.resize(len);
+                            for (uint32_t i = 0; i < len; ++i) {
+                                t_idx[i] = r.idx[e0 + ord[i]];
+                                t_perm[i] = r.perm[e0 + ord[i]];
+                                t_meta[i] = r.meta[e0 + ord[i]];
+                                t_w[i] = r.wst[e0 + ord[i]];
+                            }
+                            for (uint32_t i = 0; i < len; ++i) {
+                                r.idx[e0 + i] = t_idx[i];
+                                r.perm[e0 + i] = t_perm[i];
+                                r.meta[e0 + i] = t_meta[i];
+                                r.wst[e0 + i] = t_w[i];
+                            }
+                        }
+                }
+            }
+        }
     } catch (const std::bad_alloc &) {
         err = "host allocation failed (row store)";
         return EPHC_ENOMEM;
