@@ -216,7 +216,7 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
     p = make_workload(a2, seed_offset=rank)       # replicas: an independent problem per rank
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
-    h = ephc.build_channels(p)
+    h = ephc.build_channels(p, flags=ephc.TRANSPORT_COLLAPSE)   # + the mode-collapsed row store, timed separately below
     t_build = time.perf_counter() - t0
     if args.variant >= 0:
         h.set_variant(args.variant)
@@ -327,6 +327,36 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
             "not part of the step: PAPER.md:84-102 as two plain kernels on the same problem, for comparison; its own layout moves "
             "about %.0f B per channel" % ((24 * q["nw"] + 8 * q["nw"] * 2 + 8 * q["nw"] * 2) / max(nch, 1)))
         h.set_variant(args.variant)
+
+    # the mode-collapsed transport specialisation (SURVEY.md 8(d) honesty note): 20 chained iterations on one weight per
+    # (destination, partner) state pair.  Fewer bytes per claimed channel-term: reported here, never part of `value`.
+    if with_paper and h.collapsed_entries() > 0 and tvariant == 0 and not os.environ.get("EPHC_NO_ROWS"):
+        ec0, ec1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ec0.record(stream)
+        h.transport_collapse(stream)          # sums the weights of the last transport_setup per state pair; switches over
+        ec1.record(stream)
+        for _ in range(2):
+            h.transport_iters(Fa, v, tau, Fb, N_TRANSPORT_ITERS, stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(3):
+            h.transport_iters(Fa, v, tau, Fb, N_TRANSPORT_ITERS, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        h.set_transport_collapsed(False)
+        ms_c = e0.elapsed_time(e1) / (3 * N_TRANSPORT_ITERS)
+        nc = h.collapsed_entries()
+        bytes_c = 10 * nc + (3 * 8 * 3 + 8) * ns
+        kern["transport_iter, mode-collapsed specialisation (row_iter_kernel on one weight per state pair)"] = {
+            "bound": "hbm", "achieved": bytes_c / (ms_c * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+            "frac": bytes_c / (ms_c * 1e-3) / 1e9 / peak, "traffic": None, "alg_bytes_per_launch": int(bytes_c),
+            "us_per_launch": 1e3 * ms_c, "share_of_step": 0.0, "channel_terms_per_s": nch / (ms_c * 1e-3),
+            "state_pairs": int(nc), "ordered_terms": int(q["gather_entries"]),
+            "note": "not part of the step or of `value`: a specialisation that moves %.1f B per channel-term instead of %.1f; "
+                    "`achieved` counts ITS bytes (10 B per state pair + the vectors), `channel_terms_per_s` the channel terms it "
+                    "stands for; general path: %.1f us per iteration; summing the weights once per setup (row_collapse_kernel): %.1f us"
+                    % (bytes_c / max(nch, 1), q["alg_bytes_transport"] / max(nch, 1), 1e3 * ms_iter / N_TRANSPORT_ITERS,
+                       1e3 * ec0.elapsed_time(ec1))}
 
     # ---- end to end: the same step through host buffers ------------------------------------------------
     e2e = None

@@ -62,6 +62,7 @@ extern "C" {
 
 /* flags of ephc_problem.flags */
 #define EPHC_HOST_ONLY 1u /* build the store on the host only (no device needed): query/export work, compute fails */
+#define EPHC_TRANSPORT_COLLAPSE 4u /* also build the mode-collapsed row store (ephc_set_transport_collapsed) */
 #define EPHC_SELECT_GPU 2u /* channel selection on the device: count / prefix sum / fill over the candidate
                               pairs; the same canonical list as the host selection (indices bit-exact, weights within the
                               two exp implementations); the stores are still laid out on the host */
@@ -74,7 +75,7 @@ typedef struct ephc_problem {
     int32_t nk;              /* number of active k points (>= 1) */
     int32_t nb;              /* bands, 1..16 */
     int32_t nnu;             /* phonon modes, 1..64 */
-    uint32_t flags;          /* EPHC_HOST_ONLY, EPHC_SELECT_GPU or 0 */
+    uint32_t flags;          /* EPHC_HOST_ONLY, EPHC_SELECT_GPU, EPHC_TRANSPORT_COLLAPSE or 0 */
     const int32_t *kfull;    /* [nk] full-grid index of each active k, strictly ascending */
     const double *E;         /* [nk*nb] band energies, eV */
     double emin, emax;       /* energy window, inclusive; a channel needs both end states inside */
@@ -224,6 +225,19 @@ int ephc_transport_iter(ephc_handle *h, const double *F_dev, const double *v_dev
  * compact row order in the handle's scratch instead of going through the API layout. */
 int ephc_transport_iters(ephc_handle *h, const double *F_dev, const double *v_dev, const double *tau_dev,
                          double *Fout_dev, int niter, void *stream);
+
+/* Mode-collapsed transport specialisation (SURVEY.md 8(d) honesty note, 8(f) NEXT-3).  In the iteration the ordered terms
+ * of one (destination, partner) state pair -- its phonon modes and kinds -- enter through the SUM of their weights only,
+ * so after ephc_transport_setup the iteration can run on one weight per state pair.  Handles built with
+ * EPHC_TRANSPORT_COLLAPSE carry that second store (same strips and tiles as the row store).  After
+ * ephc_transport_setup, ephc_transport_collapse sums the current weights into it (one small kernel) and switches
+ * ephc_transport_iter / ephc_transport_iters over to it; ephc_set_transport_collapsed(h, 0 / 1) switches back and forth;
+ * the next ephc_transport_setup switches back to the general store.  The result is the same F' up to the order of
+ * additions.  It moves fewer bytes per channel-term than the general path, so bench.py reports its rate separately and
+ * never as the headline.  ephc_collapsed_entries = state pairs stored. */
+int ephc_transport_collapse(ephc_handle *h, void *stream);
+int ephc_set_transport_collapsed(ephc_handle *h, int on);
+int64_t ephc_collapsed_entries(const ephc_handle *h);
 
 /* nsteps classical RK4 steps of df/dt = I[f] with N fixed (reading R-18), f updated in place.
  * sumf_dev (may be NULL): [nsteps+1], sum_s f_s before the first step and after every step.

@@ -16,10 +16,11 @@ import numpy as np
 
 from . import _build
 
-__all__ = ["EphcError", "Handle", "build_channels", "lib_path", "HOST_ONLY", "SELECT_GPU", "version"]
+__all__ = ["EphcError", "Handle", "build_channels", "lib_path", "HOST_ONLY", "SELECT_GPU", "TRANSPORT_COLLAPSE", "version"]
 
 HOST_ONLY = 1
 SELECT_GPU = 2
+TRANSPORT_COLLAPSE = 4
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
 
@@ -90,6 +91,9 @@ def _load():
         "ephc_transport_start": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_transport_iter": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_transport_iters": (i32, [vp, vp, vp, vp, vp, i32, vp]),
+        "ephc_transport_collapse": (i32, [vp, vp]),
+        "ephc_set_transport_collapsed": (i32, [vp, i32]),
+        "ephc_collapsed_entries": (i64, [vp]),
         "ephc_rt_step": (i32, [vp, vp, vp, dbl, i32, vp, vp]),
         "ephc_collision_host": (i32, [vp, vp, vp, vp]),
         "ephc_transport_solve_host": (i32, [vp, vp, vp, vp, i32, vp, vp]),
@@ -280,6 +284,15 @@ class Handle:
         _check(_load().ephc_transport_iters(self._h, _dev_ptr(F, 3 * self.ns, "F"), _dev_ptr(v, 3 * self.ns, "v"),
                                             _dev_ptr(tau, self.ns, "tau"), _dev_ptr(Fout, 3 * self.ns, "Fout"),
                                             int(niter), _stream_ptr(stream)))
+
+    def transport_collapse(self, stream=None):
+        _check(_load().ephc_transport_collapse(self._h, _stream_ptr(stream)))
+
+    def set_transport_collapsed(self, on: bool):
+        _check(_load().ephc_set_transport_collapsed(self._h, 1 if on else 0))
+
+    def collapsed_entries(self) -> int:
+        return int(_load().ephc_collapsed_entries(self._h))
 
     def owned_states(self):
         lo, hi = C.c_int64(), C.c_int64()

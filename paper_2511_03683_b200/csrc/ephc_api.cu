@@ -135,6 +135,15 @@ struct ephc_handle {
     double *d_Fscr = nullptr;  // [3][ns] scratch of ephc_transport_iters on the stores without a compact copy
     int32_t r_nrows = 0;
     uint16_t *dr_idx = nullptr;
+    // mode-collapsed row store (EPHC_TRANSPORT_COLLAPSE): built on request, used after ephc_set_transport_collapsed(h, 1)
+    bool collapse_built = false, collapse_on = false, collapse_ready = false;  // ready: summed from the current weights
+    int64_t c_nent = 0, bytes_collapsed = 0;
+    uint16_t *dc_idx = nullptr, *dc_count = nullptr;
+    uint32_t *dc_first = nullptr;
+    double *dc_W = nullptr;
+    RowSeg *dc_segs = nullptr;
+    RowTile *dc_tiles = nullptr;
+    RowStrip *dc_strips = nullptr;
     uint32_t *dr_meta = nullptr;  // per entry: (iq * nnu + mode) | kind << 31
     double *dr_wst = nullptr;     // per entry: channel weight
     RowSeg *dr_segs = nullptr;
@@ -149,7 +158,7 @@ static void free_dev(ephc_handle *h) {
                     h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
-                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_Fc2, h->d_Fscr, h->dr_idx, h->dr_meta, h->dr_wst, h->dr_segs, h->dr_tiles, h->dr_strips,
+                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_Fc2, h->d_Fscr, h->dr_idx, h->dc_idx, h->dc_count, h->dc_first, h->dc_W, h->dc_segs, h->dc_tiles, h->dc_strips, h->dr_meta, h->dr_wst, h->dr_segs, h->dr_tiles, h->dr_strips,
                     h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
                     h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_order, h->ds_counter, h->ds_row_state,
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
@@ -737,6 +746,23 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
             if (rc == EPHC_OK) rc = upload(&h->dr_strips, rh.strips, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_row_state, rh.row_state, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_state_row, rh.state_row, &br);
+            if (rc == EPHC_OK && (p->flags & EPHC_TRANSPORT_COLLAPSE)) {
+                RowCollapsed rc2;
+                rc = build_rows_collapsed(rh, rc2, err);
+                if (rc != EPHC_OK) rc = fail(rc, err);
+                int64_t bc = 0;
+                if (rc == EPHC_OK) rc = upload(&h->dc_idx, rc2.idx, &bc);
+                if (rc == EPHC_OK) rc = upload(&h->dc_first, rc2.first, &bc);
+                if (rc == EPHC_OK) rc = upload(&h->dc_count, rc2.count, &bc);
+                if (rc == EPHC_OK) rc = upload(&h->dc_segs, rc2.segs, &bc);
+                if (rc == EPHC_OK) rc = upload(&h->dc_tiles, rc2.tiles, &bc);
+                if (rc == EPHC_OK) rc = upload(&h->dc_strips, rc2.strips, &bc);
+                h->c_nent = (int64_t)rc2.idx.size();
+                if (rc == EPHC_OK && cudaMalloc((void **)&h->dc_W, (size_t)std::max<int64_t>(1, h->c_nent) * 8) != cudaSuccess)
+                    rc = fail(EPHC_ENOMEM, "cudaMalloc (collapsed transport weights) failed");
+                h->bytes_collapsed = bc + h->c_nent * 8;
+                h->collapse_built = rc == EPHC_OK;
+            }
             if (rc == EPHC_OK && (cudaMalloc((void **)&h->dr_Fc, ((size_t)rh.nrows * 3 + 4) * 8) != cudaSuccess ||
                                   cudaMalloc((void **)&h->dr_Fc2, ((size_t)rh.nrows * 3 + 4) * 8) != cudaSuccess))
                 rc = fail(EPHC_ENOMEM, "cudaMalloc (compact F) failed");
@@ -1680,8 +1706,41 @@ static RowParams row_params(const ephc_handle *h) {
     R.nstrip = h->r_nstrip;
     R.ns = h->d.ns;
     R.Fc = h->dr_Fc;
+    if (h->collapse_on) {  // the mode-collapsed specialisation: same walk, one entry per state pair
+        R.W = h->dc_W;
+        R.idx = h->dc_idx;
+        R.segs = h->dc_segs;
+        R.tiles = h->dc_tiles;
+        R.strips = h->dc_strips;
+    }
     return R;
 }
+
+extern "C" int ephc_transport_collapse(ephc_handle *h, void *stream) {
+    int rc = need_device(h);
+    if (rc) return rc;
+    if (!h->collapse_built)
+        return fail(EPHC_ESTATE, "no mode-collapsed row store: build the handle with EPHC_TRANSPORT_COLLAPSE (row store required)");
+    if (!h->transport_ready || h->transport_variant != 0 || tr_variant(h) != 0)
+        return fail(EPHC_ESTATE, "call ephc_transport_setup (automatic or gather variant) before ephc_transport_collapse");
+    if (h->c_nent > 0) {
+        row_collapse_kernel<<<(unsigned)((h->c_nent + 255) / 256), 256, 0, (cudaStream_t)stream>>>(h->dr_W, h->dc_first, h->dc_count,
+                                                                                               h->dc_W, h->c_nent);
+        h->launches++;
+        CUDA_TRY(cudaGetLastError());
+    }
+    h->collapse_ready = true;
+    h->collapse_on = true;
+    return EPHC_OK;
+}
+extern "C" int ephc_set_transport_collapsed(ephc_handle *h, int on) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (on && !h->collapse_ready)
+        return fail(EPHC_ESTATE, "no collapsed weights: call ephc_transport_collapse after ephc_transport_setup");
+    h->collapse_on = on != 0;
+    return EPHC_OK;
+}
+extern "C" int64_t ephc_collapsed_entries(const ephc_handle *h) { return (h && h->collapse_built) ? h->c_nent : 0; }
 
 extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const double *N_dev, double *Gamma_dev,
                                     void *stream) {
@@ -1710,11 +1769,16 @@ extern "C" int ephc_transport_setup(ephc_handle *h, const double *f0_dev, const 
             row_compact1_kernel<<<(unsigned)((h->r_nrows + 255) / 256), 256, 0, s>>>(f0_dev, h->dr_row_state, h->dr_Fc, h->r_nrows);
             h->launches++;
         }
+        const bool was_on = h->collapse_on;
+        h->collapse_on = false;  // the weights are computed per ordered term on the full row store
         RowParams R = row_params(h);
+        h->collapse_on = was_on;
         R.N = N_dev;
         R.out = Gamma_dev;
         row_setup_kernel<<<(unsigned)std::max(h->r_nstrip, 1), kRowThreads, row_smem_bytes(h->r_Rb, h->r_Ra), s>>>(R);
         h->launches++;
+        h->collapse_ready = false;  // new weights: ephc_transport_collapse sums them again
+        h->collapse_on = false;
         CUDA_TRY(cudaGetLastError());
     } else {
         GatherParams P = base_params(h);

@@ -174,6 +174,21 @@ struct RowHost {
     std::vector<RowStrip> strips;
 };
 int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int nstrip, RowHost &r, std::string &err);
+// Mode-collapsed row store (transport specialisation, SURVEY.md 8(d) honesty note / 8(f) NEXT-3): in
+// F'_a = tau_a (v_a + sum_b W(a<-b) F_b) the ordered terms of one (a, b) state pair -- its modes and kinds -- enter
+// through the SUM of their weights only, so the iteration can run on one weight per state pair.  Same strips, ranges and
+// tiles as the row store; one entry per (destination, partner) pair of a segment (the row store keeps them adjacent);
+// first[] / count[] locate the terms whose weights transport_setup sums into it.  Fewer bytes per channel-term than the
+// general path: reported separately, never chosen by default.
+struct RowCollapsed {
+    std::vector<uint16_t> idx;        // per collapsed entry: partner row - col0 of its tile
+    std::vector<uint32_t> first;      // per collapsed entry: first ordered term in the row store (absolute position)
+    std::vector<uint16_t> count;      // per collapsed entry: ordered terms summed
+    std::vector<RowSeg> segs;
+    std::vector<RowTile> tiles;
+    std::vector<RowStrip> strips;
+};
+int build_rows_collapsed(const RowHost &r, RowCollapsed &c, std::string &err);
 
 // ---- stream store (variant 2, collision / RK stages): one LANE per ENTRY ------------------------------------------
 // Same tiles and partial-sum slots as the tile store (strip of k rows x range of k' rows, both staged in shared

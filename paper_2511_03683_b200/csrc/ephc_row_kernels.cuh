@@ -173,6 +173,19 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_setup_ker
     for (int i = tid; i < st.nrows; i += kRowThreads) P.out[P.row_state[st.row0 + i]] = sAcc[i];
 }
 
+// mode-collapsed specialisation: weight of a (destination, partner) state pair = sum of the weights of its ordered terms
+// (adjacent in the row store), in store order
+__global__ void __launch_bounds__(256) row_collapse_kernel(const double *__restrict__ W, const uint32_t *__restrict__ first,
+                                                           const uint16_t *__restrict__ count, double *__restrict__ Wc, int64_t n) {
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n) return;
+    const double *src = W + first[c];
+    const int cnt = count[c];
+    double s = 0.0;
+    for (int j = 0; j < cnt; ++j) s += src[j];
+    Wc[c] = s;
+}
+
 __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kernel(const RowParams P) {
     extern __shared__ double smem[];
     double *sF = smem;                       // staged partner rows [Rb][3]

@@ -189,4 +189,67 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
     return EPHC_OK;
 }
 
+int build_rows_collapsed(const RowHost &r, RowCollapsed &c, std::string &err) {
+    c = RowCollapsed();
+    try {
+        c.strips.resize(r.strips.size());
+        int64_t e_run = 0;
+        std::vector<std::pair<uint32_t, int32_t>> order;  // (collapsed length, segment) of a tile
+        std::vector<uint32_t> clen(r.segs.size(), 0);
+        for (size_t is = 0; is < r.strips.size(); ++is) {  // collapsed length of every segment
+            const RowStrip &st = r.strips[is];
+            for (int32_t t = st.t0; t < st.t1; ++t)
+                for (int32_t sg = r.tiles[t].seg0; sg < r.tiles[t].seg0 + r.tiles[t].nseg; ++sg) {
+                    const int64_t e0 = st.e0 + r.segs[sg].start;
+                    uint32_t n = 0;
+                    for (uint32_t i = 0; i < r.segs[sg].len; ++i) n += (i == 0 || r.idx[e0 + i] != r.idx[e0 + i - 1]);
+                    clen[sg] = n;
+                }
+        }
+        for (size_t is = 0; is < r.strips.size(); ++is) {
+            const RowStrip &st = r.strips[is];
+            RowStrip &cs = c.strips[is];
+            cs = st;
+            cs.e0 = e_run;
+            cs.t0 = (int32_t)c.tiles.size();
+            for (int32_t t = st.t0; t < st.t1; ++t) {
+                RowTile tl = r.tiles[t];
+                order.clear();
+                for (int32_t sg = tl.seg0; sg < tl.seg0 + tl.nseg; ++sg) order.emplace_back(clen[sg], sg);
+                std::stable_sort(order.begin(), order.end(),
+                                 [](const std::pair<uint32_t, int32_t> &x, const std::pair<uint32_t, int32_t> &y) { return x.first > y.first; });
+                tl.seg0 = (int32_t)c.segs.size();
+                for (const auto &q : order) {
+                    const RowSeg &sg = r.segs[q.second];
+                    const int64_t e0 = st.e0 + sg.start;
+                    if (e_run - cs.e0 > 0xffffffffLL || e0 + sg.len > 0xffffffffLL) {
+                        err = "collapsed row store: more than 2^32 entries";
+                        return EPHC_ELIMIT;
+                    }
+                    c.segs.push_back(RowSeg{(uint32_t)(e_run - cs.e0), q.first, sg.row, 0u});
+                    for (uint32_t i = 0; i < sg.len;) {
+                        uint32_t j = i + 1;
+                        while (j < sg.len && r.idx[e0 + j] == r.idx[e0 + i]) ++j;
+                        if (j - i > 0xffffu) {
+                            err = "collapsed row store: more than 65535 terms on one state pair";
+                            return EPHC_ELIMIT;
+                        }
+                        c.idx.push_back(r.idx[e0 + i]);
+                        c.first.push_back((uint32_t)(e0 + i));
+                        c.count.push_back((uint16_t)(j - i));
+                        ++e_run;
+                        i = j;
+                    }
+                }
+                c.tiles.push_back(tl);
+            }
+            cs.t1 = (int32_t)c.tiles.size();
+        }
+    } catch (const std::bad_alloc &) {
+        err = "host allocation failed (collapsed row store)";
+        return EPHC_ENOMEM;
+    }
+    return EPHC_OK;
+}
+
 }  // namespace ephc

@@ -302,6 +302,45 @@ def test_res_geometry_on_gpu(monkeypatch, rows, fine, smem, hcap, mode, ctas):
         assert _relerr(f, fo) <= TOL and np.abs(s - so).max() <= 1e-12 * abs(so[0])
 
 
+def test_mode_collapsed_transport_matches_oracle():
+    # SURVEY.md 8(d) honesty note / 8(f) NEXT-3: the iteration on one weight per (destination, partner) state pair gives
+    # the same F' as the general row store (sums reordered) and as the oracle; Gamma is unchanged
+    for p in _small_problems():
+        L = oracle.OracleList(p)
+        h = ephc.build_channels(p, flags=ephc.TRANSPORT_COLLAPSE)
+        nc, ne = h.collapsed_entries(), h.query()["gather_entries"]
+        assert 0 < nc <= ne and (p.nnu == 1 or nc < ne)
+        f0, N, v = dev(p.f0), dev(p.N), dev(p.v)
+        G = torch.empty(p.ns, device="cuda", dtype=torch.float64)
+        h.transport_setup(f0, N, G)
+        Go = L.transport_setup(p.f0, p.N)
+        assert _relerr(G.cpu().numpy(), Go) <= TOL
+        tau_o = np.where(Go > 0, 1.0 / np.where(Go > 0, Go, 1.0), 0.0)
+        F0 = tau_o[None, :] * p.v
+        Fr = F0
+        for _ in range(3):
+            Fr = L.transport_iter(p.f0, p.N, Fr, p.v, tau_o)
+        with pytest.raises(ephc.EphcError):
+            h.set_transport_collapsed(True)  # the collapsed weights have not been summed yet
+        h.transport_collapse()
+        out = {}
+        for on in (False, True, False):
+            h.set_transport_collapsed(on)
+            Fo = torch.full((3 * p.ns,), np.nan, device="cuda", dtype=torch.float64)
+            h.transport_iters(dev(F0), v, dev(tau_o), Fo, 3)
+            assert _relerr(Fo.cpu().numpy().reshape(3, -1), Fr) <= TOL
+            if on in out:
+                assert torch.equal(out[on], Fo)
+            out[on] = Fo
+        Fs = torch.empty(3 * p.ns, device="cuda", dtype=torch.float64)
+        h.set_transport_collapsed(True)
+        h.transport_iter(dev(F0), v, dev(tau_o), Fs)
+        assert _relerr(Fs.cpu().numpy().reshape(3, -1), L.transport_iter(p.f0, p.N, F0, p.v, tau_o)) <= TOL
+    h = ephc.build_channels(_small_problems()[0])
+    with pytest.raises(ephc.EphcError):
+        h.transport_collapse()               # not built with EPHC_TRANSPORT_COLLAPSE
+
+
 def test_gpu_channel_selection_matches_oracle_list():
     # EPHC_SELECT_GPU: the canonical list selected on the device equals the oracle's
     # list bit for bit (indices) and within 4 ulp (weights: two exp implementations), diagonal terms included; the
