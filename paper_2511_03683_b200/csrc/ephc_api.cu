@@ -47,7 +47,7 @@ struct ephc_handle {
     double *d_drift = nullptr;           // drift term of the current RK stage
     bool ranged = false;                 // built by ephc_build_channels_range: owns the destination k in [d.k_lo, d.k_hi)
     RowHost rowhost;                     // kept only for EPHC_HOST_ONLY handles (ephc_export_rows)
-    int variant = -1;  // -1: automatic (collision / rt_step on the tile store, transport on the gather store)
+    int variant = -1;  // -1: automatic (collision / rt_step: gather store while it fits the L2, resident tiles beyond; transport: rows)
     Canonical can;
     GatherHost ghost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_gather)
     std::vector<int32_t> pair_ik, pair_ikq;  // copy of the candidate pair list (export)
