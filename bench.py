@@ -500,16 +500,36 @@ def measure_sharded(args, ephc, torch, rank, local, dist):
     lo, hi = S.h.owned_states()
     own = [None] * world
     dist.all_gather_object(own, [lo, hi, int(S.h.query()["gather_entries"])])
+    # the collision call alone (every rank: it ends in a collective)
+    ec = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    for _ in range(3):
+        S.collision(f, N, I, stream)
+    barrier()
+    ec[0].record(stream)
+    for _ in range(10):
+        S.collision(f, N, I, stream)
+    ec[1].record(stream)
+    barrier()
+    ms_c = ec[0].elapsed_time(ec[1]) / 10
     if rank != 0:
         return None
     exchanges = 1 + 1 + N_TRANSPORT_ITERS * 3 + 4
     cfg = workload_config(args, p, nch)
-    cfg.update({"variant": "collision/rt: gather (destination-sorted, two-sided), transport: rows (setup on gather)",
+    cfg.update({"variant": "collision/rt: gather (destination-sorted, two-sided), transport: rows",
                 "parallelism": f"k-sharded over {world} GPUs: contiguous ranges of destination k balanced by half-pair count; "
                                f"{exchanges} all-gathers of the owned slices per step (NCCL), <= {8 * ns} bytes each",
                 "owned_states_and_ordered_entries_per_rank": own, "generate_s": t_gen, "build_channels_s": t_build,
                 "l2": "no flush: every rank streams its share of the two-sided store in every evaluation"})
     val = nch * EVALS_PER_STEP * args.steps / (ms_total * 1e-3)
+    # roofline of the collision call on this rank's share (gather_kernel<0> + the all-gather of the owned slice): the
+    # algorithmic bytes of the whole problem times the share of the ordered terms rank 0 owns
+    share0 = own[0][2] / max(sum(o[2] for o in own), 1)
+    peak, peak_src = peaks()
+    gbs = q["alg_bytes_collision"] * share0 / (ms_c * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                "kernel": "collision on rank 0's share (gather_kernel<0> + NCCL all-gather of the owned slice)",
+                "alg_bytes_per_launch": int(q["alg_bytes_collision"] * share0), "us_per_launch": 1e3 * ms_c,
+                "share_of_ordered_terms": share0, "peak_source": peak_src}
     e2e = None
     if ms_e2e is not None:
         e2e = {"value": nch * EVALS_PER_STEP * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
@@ -518,7 +538,7 @@ def measure_sharded(args, ephc, torch, rank, local, dist):
     return {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / max(args.steps, 1), "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": cfg, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": None, "cpu_baseline": None}
+            "roofline": roofline, "cpu_baseline": None}
 
 
 def load_traffic(config_name):
