@@ -241,7 +241,9 @@ int64_t ephc_collapsed_entries(const ephc_handle *h);
 
 /* nsteps classical RK4 steps of df/dt = I[f] with N fixed (reading R-18), f updated in place.
  * sumf_dev (may be NULL): [nsteps+1], sum_s f_s before the first step and after every step.
- * The axpy of every stage is fused into the collision kernel's epilogue. */
+ * The axpy of every stage is the epilogue of the collision pass.  For runs of four or more steps the steady-state step
+ * (its 8-9 launches have fixed arguments) is captured once into a CUDA graph on a stream the handle owns and replayed on
+ * `stream` (EPHC_NO_GRAPH=1: plain launches). */
 int ephc_rt_step(ephc_handle *h, double *f_dev, const double *N_dev, double dt_fs, int nsteps,
                  double *sumf_dev, void *stream);
 

@@ -65,6 +65,16 @@ struct ephc_handle {
     bool transport_ready = false;
     // scratch for rt_step / host variants (allocated lazily, freed in destroy)
     double *d_y[2] = {nullptr, nullptr}, *d_ksum = nullptr, *d_wusum = nullptr;
+    // CUDA graph of one steady-state RK4 step of ephc_rt_step (captured on cap_stream, replayed on the caller's stream)
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t rk_graph = nullptr;
+    double *d_sumstep = nullptr;  // sum_s f_s of the step the graph has just run
+    struct RkKey {
+        const void *f, *N;
+        double dt, field[3];
+        int has_field, want_sum, variant;
+    } rk_key = {nullptr, nullptr, 0.0, {0.0, 0.0, 0.0}, 0, 0, -99};
+    int rk_graph_launches = 0;
     double *d_hf = nullptr, *d_hN = nullptr, *d_hI = nullptr;  // host-variant staging: f, N, I
     double *d_tr[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // Gamma, tau, v, F, F'
     double *d_sumf = nullptr;
@@ -167,6 +177,9 @@ static void free_dev(ephc_handle *h) {
                     h->dx_blk_ent_off, h->dp_ch, h->dp_ik, h->dp_ikq, h->dp_iq, h->dp_src, h->dp_targets, h->dp_sc_col, h->d_nbr, h->d_drift};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    if (h->d_sumstep) cudaFree(h->d_sumstep);
+    if (h->rk_graph) cudaGraphExecDestroy(h->rk_graph);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
 }
 
 template <class T>
@@ -774,6 +787,8 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
             ((h->rows_ok && cudaMalloc((void **)&h->dr_W, ne8) != cudaSuccess) ||
              cudaMalloc((void **)&h->d_y[0], nb8) != cudaSuccess || cudaMalloc((void **)&h->d_y[1], nb8) != cudaSuccess ||
              cudaMalloc((void **)&h->d_ksum, nb8) != cudaSuccess || cudaMalloc((void **)&h->d_Fscr, 3 * nb8) != cudaSuccess ||
+             cudaMalloc((void **)&h->d_sumstep, 8) != cudaSuccess ||
+             cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess ||
              cudaMalloc((void **)&h->d_wusum, (size_t)std::max<int64_t>(std::max<int64_t>(h->n_wu, (ns + 255) / 256), 1) * 8) != cudaSuccess))
             rc = fail(EPHC_ENOMEM, "cudaMalloc (transport weights / RK4 scratch) failed");
         if (rc == EPHC_OK) h->bytes_transport += h->g_entries * 8;
@@ -2005,24 +2020,75 @@ static int rt_step_impl(ephc_handle *h, double *f_dev, const double *N_dev, cons
         sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev);
         h->launches++;
     }
-    for (int it = 0; it < nsteps; ++it) {
-        // stage 1 gathers f, writes y2 -> y[0]; stage 2 gathers y[0], writes y3 -> y[1];
-        // stage 3 gathers y[1], writes y4 -> y[0]; stage 4 gathers y[0], updates f in place.
+    // one step: stage 1 gathers f, writes y2 -> y[0]; stage 2 gathers y[0], writes y3 -> y[1]; stage 3 gathers y[1],
+    // writes y4 -> y[0]; stage 4 gathers y[0], updates f in place; then sum_s f_s -> sum_out
+    auto one_step = [&](cudaStream_t st_, bool fc_ready0, double *sum_out) -> int {
         const double *src[4] = {f_dev, h->d_y[0], h->d_y[1], h->d_y[0]};
         double *dst[4] = {h->d_y[0], h->d_y[1], h->d_y[0], nullptr};
-        for (int st = 0; st < 4; ++st)
-            if ((rc = rk_stage(h, f_dev, src[st], N_dev, dt_fs, st + 1, dst[st], sumf_dev != nullptr, s, field, true, it > 0 || st > 0)))
-                return rc;
-        if (sumf_dev) {
+        for (int st = 0; st < 4; ++st) {
+            const int r = rk_stage(h, f_dev, src[st], N_dev, dt_fs, st + 1, dst[st], sumf_dev != nullptr, st_, field, true, fc_ready0 || st > 0);
+            if (r) return r;
+        }
+        if (sum_out) {
             if (rt_variant(h) >= 1)
-                sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, finish_grid(h), sumf_dev + it + 1);
+                sum_kernel<<<1, 1024, 0, st_>>>(h->d_wusum, finish_grid(h), sum_out);
             else if (h->n_wu > 0)
-                sum_kernel<<<1, 1024, 0, s>>>(h->d_wusum, h->n_wu, sumf_dev + it + 1);
+                sum_kernel<<<1, 1024, 0, st_>>>(h->d_wusum, h->n_wu, sum_out);
             else
-                sum_kernel<<<1, 1024, 0, s>>>(f_dev, h->d.ns, sumf_dev + it + 1);
+                sum_kernel<<<1, 1024, 0, st_>>>(f_dev, h->d.ns, sum_out);
             h->launches++;
         }
+        return EPHC_OK;
+    };
+    int it = 0;
+    if (nsteps > 0) {
+        if ((rc = one_step(s, false, sumf_dev ? sumf_dev + 1 : nullptr))) return rc;
+        it = 1;
     }
+#ifndef EPHC_RES_TIMING
+    // Long runs (config 5: 1000 steps): the steady-state step -- 8 or 9 launches with fixed arguments -- is captured once
+    // into a CUDA graph on the handle's own stream and replayed on the caller's stream; the step's sum goes to a scratch
+    // double and is copied to its slot.  Any failure on the way falls back to plain launches.
+    if (nsteps - it >= 3 && std::getenv("EPHC_NO_GRAPH") == nullptr && h->cap_stream) {
+        ephc_handle::RkKey key = {f_dev, N_dev, dt_fs, {field ? field[0] : 0.0, field ? field[1] : 0.0, field ? field[2] : 0.0},
+                                  field != nullptr, sumf_dev != nullptr, rt_variant(h)};
+        const ephc_handle::RkKey &k0 = h->rk_key;
+        const bool same = k0.f == key.f && k0.N == key.N && k0.dt == key.dt && k0.field[0] == key.field[0] && k0.field[1] == key.field[1] &&
+                          k0.field[2] == key.field[2] && k0.has_field == key.has_field && k0.want_sum == key.want_sum &&
+                          k0.variant == key.variant;
+        if (!h->rk_graph || !same) {
+            if (h->rk_graph) cudaGraphExecDestroy(h->rk_graph);
+            h->rk_graph = nullptr;
+            const int64_t l0 = h->launches;
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                const int r = one_step(h->cap_stream, true, sumf_dev ? h->d_sumstep : nullptr);
+                const cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
+                if (r == EPHC_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&h->rk_graph, graph, 0) == cudaSuccess) {
+                    h->rk_key = key;
+                    h->rk_graph_launches = (int)(h->launches - l0);
+                } else {
+                    h->rk_graph = nullptr;
+                }
+                if (graph) cudaGraphDestroy(graph);
+            }
+            h->launches = l0;  // nothing ran during the capture
+            cudaGetLastError();
+        }
+        if (h->rk_graph) {
+            for (; it < nsteps; ++it) {
+                if (cudaGraphLaunch(h->rk_graph, s) != cudaSuccess) {
+                    cudaGetLastError();
+                    break;  // the remaining steps run as plain launches
+                }
+                h->launches += h->rk_graph_launches;
+                if (sumf_dev) CUDA_TRY(cudaMemcpyAsync(sumf_dev + it + 1, h->d_sumstep, 8, cudaMemcpyDeviceToDevice, s));
+            }
+        }
+    }
+#endif
+    for (; it < nsteps; ++it)
+        if ((rc = one_step(s, true, sumf_dev ? sumf_dev + it + 1 : nullptr))) return rc;
     CUDA_TRY(cudaGetLastError());
     return EPHC_OK;
 }
