@@ -175,6 +175,12 @@ int64_t ephc_res_entries(const ephc_handle *h);
  * permutation. */
 int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *partner, int64_t *gather_pos);
 
+/* Decoded image of the mode-collapsed row store (handles built with EPHC_HOST_ONLY | EPHC_TRANSPORT_COLLAPSE): arrays of
+ * length ephc_collapsed_entries(h) in store order: destination state, partner state, number of ordered terms summed.
+ * Checks that it has the row store's strips and tiles, one entry per partner of a segment, and that the entries cover
+ * every ordered term of the row store exactly once, each with its own partner. */
+int ephc_export_rows_collapsed(const ephc_handle *h, int32_t *dest, int32_t *partner, int32_t *count);
+
 /* Choice of algorithm:
  *   0 = gather  : destination-sorted two-sided store, one kernel, every ordered term read once
  *   1 = tiles   : once-stored channels grouped into (k-strip, k'-range) tiles; one lane per (k,k') pair updates

@@ -82,6 +82,7 @@ def _load():
         "ephc_stream_entries": (i64, [vp]),
         "ephc_export_res": (i32, [vp] * 7),
         "ephc_export_rows": (i32, [vp] * 4),
+        "ephc_export_rows_collapsed": (i32, [vp] * 4),
         "ephc_res_entries": (i64, [vp]),
         "ephc_set_variant": (i32, [vp, i32]),
         "ephc_get_variant": (i32, [vp]),
@@ -241,6 +242,13 @@ class Handle:
         dest, partner, pos = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int64)
         _check(_load().ephc_export_rows(self._h, dest.ctypes.data, partner.ctypes.data, pos.ctypes.data))
         return {"dest": dest[:ne], "partner": partner[:ne], "gather_pos": pos[:ne]}
+
+    def export_rows_collapsed(self) -> dict:
+        nc = self.collapsed_entries()
+        n = max(nc, 1)
+        dest, partner, count = (np.zeros(n, np.int32) for _ in range(3))
+        _check(_load().ephc_export_rows_collapsed(self._h, dest.ctypes.data, partner.ctypes.data, count.ctypes.data))
+        return {"dest": dest[:nc], "partner": partner[:nc], "count": count[:nc]}
 
     def set_variant(self, variant: int):
         _check(_load().ephc_set_variant(self._h, int(variant)))

@@ -47,6 +47,7 @@ struct ephc_handle {
     double *d_drift = nullptr;           // drift term of the current RK stage
     bool ranged = false;                 // built by ephc_build_channels_range: owns the destination k in [d.k_lo, d.k_hi)
     RowHost rowhost;                     // kept only for EPHC_HOST_ONLY handles (ephc_export_rows)
+    RowCollapsed chost;                  // the same for the mode-collapsed row store (ephc_export_rows_collapsed)
     int variant = -1;  // -1: automatic (collision / rt_step: gather store while it fits the L2, resident tiles beyond; transport: rows)
     Canonical can;
     GatherHost ghost;  // kept only for EPHC_HOST_ONLY handles (ephc_export_gather)
@@ -743,7 +744,18 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.meta.size() * 4 + rh.wst.size() * 8 + rh.segs.size() * sizeof(RowSeg) +
                                   rh.tiles.size() * sizeof(RowTile) + rh.strips.size() * sizeof(RowStrip) +
                                   (rh.row_state.size() + rh.state_row.size()) * 4);
-        if (h->host_only) h->rowhost = rh;
+        if (h->host_only) {
+            if ((p->flags & EPHC_TRANSPORT_COLLAPSE) && h->rows_ok) {
+                rc = build_rows_collapsed(rh, h->chost, err);
+                if (rc != EPHC_OK) {
+                    delete h;
+                    return fail(rc, err);
+                }
+                h->collapse_built = true;
+                h->c_nent = (int64_t)h->chost.idx.size();
+            }
+            h->rowhost = rh;
+        }
     }
     h->bytes_gather = 0;
     if (!h->host_only) {
@@ -1187,6 +1199,56 @@ extern "C" int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *pa
     if (next_row != r.nrows || next_tile != (int32_t)r.tiles.size()) return fail(EPHC_ESTATE, "internal: rows or tiles left over");
     for (uint8_t v : seen)
         if (!v) return fail(EPHC_ESTATE, "internal: row entry not covered by any segment");
+    return EPHC_OK;
+}
+
+extern "C" int ephc_export_rows_collapsed(const ephc_handle *h, int32_t *dest, int32_t *partner, int32_t *count) {
+    if (!h) return fail(EPHC_EINVAL, "null handle");
+    if (!h->host_only) return fail(EPHC_ESTATE, "ephc_export_rows_collapsed needs a handle built with EPHC_HOST_ONLY");
+    if (!h->collapse_built) return fail(EPHC_ESTATE, "no mode-collapsed row store: build with EPHC_TRANSPORT_COLLAPSE");
+    const RowHost &r = h->rowhost;
+    const RowCollapsed &c = h->chost;
+    const int64_t nc = (int64_t)c.idx.size(), nent = (int64_t)r.idx.size();
+    if ((int64_t)c.first.size() != nc || (int64_t)c.count.size() != nc || c.strips.size() != r.strips.size() || c.tiles.size() != r.tiles.size() ||
+        c.segs.size() != r.segs.size())
+        return fail(EPHC_ESTATE, "internal: collapsed row store size");
+    std::vector<uint8_t> covered((size_t)nent, 0);
+    int64_t x = 0;
+    for (size_t is = 0; is < c.strips.size(); ++is) {
+        const RowStrip &st = c.strips[is], &rs = r.strips[is];
+        if (st.row0 != rs.row0 || st.nrows != rs.nrows || st.t1 - st.t0 != rs.t1 - rs.t0 || st.e0 != x)
+            return fail(EPHC_ESTATE, "internal: collapsed strips differ from the row store's");
+        for (int32_t it = st.t0; it < st.t1; ++it) {
+            const RowTile &tl = c.tiles[it], &rt = r.tiles[rs.t0 + (it - st.t0)];
+            if (tl.col0 != rt.col0 || tl.ncols != rt.ncols || tl.nseg != rt.nseg) return fail(EPHC_ESTATE, "internal: collapsed tiles differ");
+            uint32_t last_len = 0xffffffffu;
+            for (int32_t ig = tl.seg0; ig < tl.seg0 + tl.nseg; ++ig) {
+                const RowSeg &sg = c.segs[ig];
+                if (sg.len < 1 || sg.len > last_len || (int32_t)sg.row >= st.nrows || st.e0 + sg.start != x)
+                    return fail(EPHC_ESTATE, "internal: collapsed segments must be contiguous and descend in length");
+                last_len = sg.len;
+                int32_t last_idx = -1;
+                for (uint32_t k = 0; k < sg.len; ++k, ++x) {
+                    // one entry per partner of the segment, ascending; its terms are adjacent in the row store, have this
+                    // partner, and belong to a segment of the same destination row in the same tile
+                    if (x >= nc || (int32_t)c.idx[x] <= last_idx || c.idx[x] >= tl.ncols || c.count[x] < 1 ||
+                        (int64_t)c.first[x] + c.count[x] > nent)
+                        return fail(EPHC_ESTATE, "internal: collapsed entry out of range");
+                    last_idx = c.idx[x];
+                    for (uint32_t j = 0; j < c.count[x]; ++j) {
+                        const int64_t o = (int64_t)c.first[x] + j;
+                        if (r.idx[o] != c.idx[x] || covered[o]++) return fail(EPHC_ESTATE, "internal: collapsed entry sums a foreign term");
+                    }
+                    if (dest) dest[x] = r.row_state[st.row0 + (int32_t)sg.row];
+                    if (partner) partner[x] = r.row_state[tl.col0 + c.idx[x]];
+                    if (count) count[x] = c.count[x];
+                }
+            }
+        }
+    }
+    if (x != nc) return fail(EPHC_ESTATE, "internal: collapsed entries left over");
+    for (uint8_t v : covered)
+        if (!v) return fail(EPHC_ESTATE, "internal: ordered term not covered by any collapsed entry");
     return EPHC_OK;
 }
 

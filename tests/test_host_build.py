@@ -258,6 +258,26 @@ def test_row_store_is_a_regrouping_of_the_gather_store(prob, rng_rows, strips, m
     assert inside[r["dest"]].all() and inside[r["partner"]].all()
 
 
+@pytest.mark.parametrize("rng_rows,strips", [(None, None), (32, 3), (64, 40)])
+def test_collapsed_row_store_sums_every_ordered_term_once(prob, rng_rows, strips, monkeypatch):
+    # mode-collapsed specialisation: one entry per (destination, partner) state pair of a segment; the counts are the
+    # multiplicities of the pairs in the row store; coverage and adjacency checked in C (ephc_export_rows_collapsed)
+    if rng_rows is not None:
+        monkeypatch.setenv("EPHC_ROW_RANGE", str(rng_rows))
+        monkeypatch.setenv("EPHC_ROW_STRIPS", str(strips))
+    h = ephc.build_channels(prob, flags=ephc.HOST_ONLY | ephc.TRANSPORT_COLLAPSE)
+    r, c = h.export_rows(), h.export_rows_collapsed()
+    assert 0 < len(c["dest"]) <= len(r["dest"]) and c["count"].sum() == len(r["dest"])
+    ns = prob.nk * prob.nb
+    key_r = r["dest"].astype(np.int64) * ns + r["partner"]
+    key_c = c["dest"].astype(np.int64) * ns + c["partner"]
+    uniq, cnt = np.unique(key_r, return_counts=True)
+    order = np.argsort(key_c, kind="stable")
+    assert np.array_equal(key_c[order], uniq) and np.array_equal(c["count"][order], cnt)   # one entry per state pair
+    with pytest.raises(ephc.EphcError):
+        ephc.build_channels(prob, flags=ephc.HOST_ONLY).export_rows_collapsed()
+
+
 def test_launch_geometry_limits():
     # a segment with more half-pairs than one round can stage (tiny 8x8x8: 512 partners per k, 5 doubles each)
     # and a dense many-band block: both must split into rounds/tasks within the kernel's limits
