@@ -35,6 +35,7 @@ struct ImgParams {
     int32_t a_row0, a_rows, b_row0, b_rows;
     int nnu, nwarp;
     int hcap;           // pieces of at most this many elements (0: automatic)
+    bool stats;         // EPHC_DEBUG: count the gather wavefronts of the layout
     bool bank_aware;    // order a lane's entries so that the gathers of a column spread over the shared-memory banks
     int32_t nq_cap;     // pairs per tile (bounds the iq list that rides in the previous tile's image)
     int64_t budget;     // bytes available for image (without that list) + zero + N rows
@@ -45,6 +46,9 @@ struct Scratch {
     std::vector<int32_t> cnt, start, idx, pos_of, in_start, in_list;
     std::vector<uint32_t> pair_local;
 };
+
+// working statistics (EPHC_DEBUG): shared-memory wavefronts of the 8-byte gathers as laid out, and their lower bound
+static long long g_wf_f = 0, g_wf_n = 0, g_wf_t = 0, g_wf_ideal1 = 0, g_wf_ideal2 = 0;
 
 struct Piece {
     int32_t row, start, len;   // local row; first element in the row-sorted list; elements
@@ -234,6 +238,37 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
                     }
                 }
     }
+    if (P.stats) {  // wavefronts of the f_b and N gathers: per column and half-warp, the largest number of DISTINCT addresses on a bank pair
+        long long wf = 0, wn = 0, wi = 0;
+        for (const Slab &sl : sl1)
+            for (int32_t j = 0; j < sl.H; ++j)
+                for (int half = 0; half < 2; ++half) {
+                    int32_t af[16][16], an[16][16], cf[16] = {0}, cn[16] = {0};
+                    bool any = false;
+                    for (int l = 16 * half; l < 16 * half + 16; ++l) {
+                        if (sl.piece[l] < 0 || pc1[sl.piece[l]].len <= j) continue;
+                        any = true;
+                        const int32_t ei = S.idx[pc1[sl.piece[l]].start + j];
+                        const int32_t fa = loc(e[ei].in), na = (int32_t)(S.pair_local[ei] * (uint32_t)P.nnu + (uint32_t)e[ei].nu);
+                        bool dup = false;
+                        for (int k = 0; k < cf[fa & 15]; ++k) dup |= af[fa & 15][k] == fa;
+                        if (!dup) af[fa & 15][cf[fa & 15]++] = fa;
+                        dup = false;
+                        for (int k = 0; k < cn[na & 15]; ++k) dup |= an[na & 15][k] == na;
+                        if (!dup) an[na & 15][cn[na & 15]++] = na;
+                    }
+                    if (!any) continue;
+                    wf += *std::max_element(cf, cf + 16);
+                    wn += *std::max_element(cn, cn + 16);
+                    wi += 1;
+                }
+#pragma omp critical
+        {
+            g_wf_f += wf;
+            g_wf_n += wn;
+            g_wf_ideal1 += wi;
+        }
+    }
     S.pos_of.resize((size_t)n);
     for (const Slab &sl : sl1)
         for (int l = 0; l < 32; ++l) {
@@ -273,6 +308,28 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
                         cx[S.in_list[pc.start + j] & 15]++;
                     }
                 }
+    }
+    if (P.stats) {
+        long long wt = 0, wi = 0;
+        for (const Slab &sl : sl2)
+            for (int32_t j = 0; j < sl.H; ++j)
+                for (int half = 0; half < 2; ++half) {
+                    int32_t cx[16] = {0};
+                    bool any = false;
+                    for (int l = 16 * half; l < 16 * half + 16; ++l) {
+                        if (sl.piece[l] < 0 || pc2[sl.piece[l]].len <= j) continue;
+                        any = true;
+                        cx[S.in_list[pc2[sl.piece[l]].start + j] & 15]++;
+                    }
+                    if (!any) continue;
+                    wt += *std::max_element(cx, cx + 16);
+                    wi += 1;
+                }
+#pragma omp critical
+        {
+            g_wf_t += wt;
+            g_wf_ideal2 += wi;
+        }
     }
     ResTile &D = out.dir;
     std::memset(&D, 0, sizeof(D));
@@ -538,6 +595,7 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                     P.nwarp = nwarp;
                     P.hcap = hcap;
                     P.bank_aware = !std::getenv("EPHC_RES_NO_BANKS");
+                    P.stats = std::getenv("EPHC_DEBUG") != nullptr;
                     P.nq_cap = nq_cap;
                     P.budget = budget;
                     P.pair_iq = c.pair_iq.data();
@@ -739,6 +797,10 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                 }
                 std::fprintf(stderr, "res schedule: %d CTAs, work %.0f .. %.0f\n", ncta, mn, mx);
             }
+            std::fprintf(stderr, "res gathers (wavefronts per half-warp column, 1 = conflict-free; calibration tiles included): f_b %.3f, N %.3f, T %.3f\n",
+                         (double)g_wf_f / std::max<long long>(g_wf_ideal1, 1), (double)g_wf_n / std::max<long long>(g_wf_ideal1, 1),
+                         (double)g_wf_t / std::max<long long>(g_wf_ideal2, 1));
+            g_wf_f = g_wf_n = g_wf_t = g_wf_ideal1 = g_wf_ideal2 = 0;
             const double n = (double)std::max<size_t>(t.tiles.size(), 1), ne = (double)std::max<int64_t>(nent, 1);
             std::fprintf(stderr,
                          "res store: Ra %d Rf %d RbMax %d budget %lld scale %.3f | %zu tiles in %zu runs, per tile: %.0f entries (+%.1f%% padding), "
