@@ -289,6 +289,8 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
         kern[f"{call} ({kernels})"] = {
             "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
             "traffic": tr["bytes"] if tr else None, "traffic_source": tr["source"] if tr else None,
+            "frac_of_nominal_8TBs": gbs / 8000.0,
+            "frac_dram_traffic": (tr["bytes"] / (ms_launch * 1e-3) / 1e9 / peak) if (tr and ms_launch > 0) else None,
             "alg_bytes_per_launch": int(alg_bytes), "us_per_launch": 1e3 * ms_launch, "share_of_step": share,
             "channel_terms_per_s": nch / (ms_launch * 1e-3) if ms_launch > 0 else 0.0}
 
