@@ -429,8 +429,11 @@ def measure(args, ephc, torch, config_name, steps, warmup, rank, local, dist, wi
                 "generate_s": t_gen, "build_channels_s": t_build, "store_bytes": sb + q["store_bytes_transport"],
                 "store_bytes_per_channel": (sb + q["store_bytes_transport"]) / max(nch, 1)})
     h.close()
+    # the kernel with the largest share of the step (the transport iteration), beside the collision call in `roofline`
+    dom_key = max((k for k in kern if kern[k]["share_of_step"] > 0), key=lambda k: kern[k]["share_of_step"])
     return {"value": value, "ms_per_step": ms_step, "config": cfg, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline, "kernels": kern, "cpu_baseline": cpu,
+            "roofline": roofline, "roofline_dominant": dict(kern[dom_key], kernel=dom_key, peak_source=peak_src), "kernels": kern,
+            "cpu_baseline": cpu,
             "collision_channel_terms_per_s": nch_all / (ms_coll * 1e-3) if ms_coll > 0 else 0.0}
 
 
@@ -604,6 +607,7 @@ def main():
                "warmup": args.warmup, "ms_per_step": main_res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": main_res["config"], "e2e": main_res["e2e"],
                "gpu_launches": main_res["gpu_launches"], "clocks": main_res["clocks"], "roofline": main_res["roofline"],
+               "roofline_dominant": main_res["roofline_dominant"],
                "collision_channel_terms_per_s": main_res["collision_channel_terms_per_s"],
                "kernels": main_res["kernels"], "cpu_baseline": main_res["cpu_baseline"], "per_config": per_config}
         print(json.dumps(out))
