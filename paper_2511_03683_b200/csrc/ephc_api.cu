@@ -1287,14 +1287,14 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
             if (D.flags & 2) ++irun;
             ResTile Dl = D;
             res_set_layout(Dl, t.nwarp);
-            if (D.pad != 0 || D.o_sn_next != (it + 1 < t.cta_ptr[cta + 1] ? res_o_sn(t.tiles[it + 1]) : 0u))
+            if (D.ncombo < 1 || D.ncombo > D.ne || D.o_sn_next != (it + 1 < t.cta_ptr[cta + 1] ? res_o_sn(t.tiles[it + 1]) : 0u))
                 return fail(EPHC_ESTATE, "internal: where the next tile's N rows go");
             const int32_t R = run.a_rows + D.b_rows;
             if (D.ne < 1 || std::memcmp(&Dl, &D, sizeof(D)) != 0 || (int64_t)D.a_off != t.slot_off[D.a_slot] ||
                 (D.b_slot >= 0 && (int64_t)D.b_off != t.slot_off[D.b_slot]) || D.blob_off % 128 != 0 || D.blob_off + D.blob_bytes > (int64_t)t.blob.size() ||
                 res_tile_smem(D, nnu) > t.smem_tile || R > t.Rcap || D.b_rows > t.RbMax || R > kResRowMax || D.nq * nnu > kResSlotMax ||
                 D.ne_pad % 32 || D.ng_pad % 32 || D.ne_pad > kResXMax - 1 || D.ne_pad / 32 > 1023 || D.ng_pad / 32 > 1023 || D.ne > D.ne_pad ||
-                D.ne > D.ng_pad || D.nslab1 < 1 || D.nslab2 < 1 ||
+                D.ncombo > D.ng_pad || D.nslab1 < 1 || D.nslab2 < 1 ||
                 (D.b_rows > 0) != (D.b_slot >= 0) || (D.b_rows > 0 && (D.b_row0 < run.a_row0 + run.a_rows || D.b_row0 % 2 || run.a_rows % 2)) ||
                 (D.b_slot >= 0 && (t.slot_row0[D.b_slot] != D.b_row0 || t.slot_rows[D.b_slot] != D.b_rows)) ||
                 D.q0 < 0 || D.q0 + D.nq > (int64_t)t.iqn.size())
@@ -1339,26 +1339,37 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
                                 return false;
                             }
                             for (int32_t j = 0; j < H; ++j)
-                                if (!visit(u, base + 32 * j + l)) return false;
+                                if (!visit(u, base + 32 * j + l, j, j + 1 == H)) return false;
                         }
                         if (multi && !(hd & kResHdrMulti)) return false;
                     }
                 }
                 return next == npos;
             };
-            // phase 1: owner[pos] = b row of the weight at pos (-1: padding, w == 0); every a row is a row of the strip
+            // phase 1: a lane's entries come in combos (same partner, closed by bit 0 of the code); owner[pos] = b row of the
+            // term at a combo's last position (-2: inside a combo, -1: padding, w == 0); every a row is a row of the strip
             owner.assign((size_t)D.ne_pad, -1);
             used.assign((size_t)D.ne_pad, 0);
-            int32_t real = 0;
-            const bool ok1 = walk(srow1, shdr1, wptr, D.nslab1, D.ne_pad, row_out, [&](int32_t u, int32_t pos) {
+            int32_t real = 0, combos = 0, open_in = -1;
+            const bool ok1 = walk(srow1, shdr1, wptr, D.nslab1, D.ne_pad, row_out, [&](int32_t u, int32_t pos, int32_t col, bool last_col) {
+                if (col == 0) open_in = -1;
                 if (used[pos]++ || u >= run.a_rows) return false;
                 const uint32_t cd = code[pos];
                 const int32_t in_loc = (int32_t)((cd & 0xffffu) >> 3), slot = (int32_t)(cd >> 19);
-                if ((cd & 7u) || in_loc >= R || slot / nnu >= D.nq) return false;
-                if (wv[pos] == 0.0) return cd == 0u;  // padding reads f of row 0 and N slot 0
+                if ((cd & 6u) || in_loc >= R || slot / nnu >= D.nq) return false;
+                if (wv[pos] == 0.0) return cd == 0u && open_in < 0;  // padding (after the lane's last combo) reads N slot 0
                 const int32_t ro = row_of(u), ri = row_of(in_loc);
                 if (ro >= ri || (D.b_rows > 0 && in_loc < run.a_rows)) return false;
-                owner[pos] = in_loc;
+                if (open_in >= 0 && open_in != in_loc) return false;  // a combo has one partner
+                if (cd & 1u) {
+                    owner[pos] = in_loc;
+                    open_in = -1;
+                    ++combos;
+                } else {
+                    if (last_col) return false;  // a lane must not end inside a combo
+                    owner[pos] = -2;
+                    open_in = in_loc;
+                }
                 const int64_t x = o + real++;
                 if (x >= t.nent) return false;
                 if (a) a[x] = t.row_state[ro];
@@ -1369,20 +1380,20 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
                 if (w) w[x] = std::fabs(wv[pos]);
                 return true;
             });
-            if (!ok1 || real != D.ne || D.nslab1 < 1) return fail(EPHC_ESTATE, "internal: phase-1 slabs of a resident tile");
+            if (!ok1 || real != D.ne || combos != D.ncombo || D.nslab1 < 1) return fail(EPHC_ESTATE, "internal: phase-1 slabs of a resident tile");
             for (int32_t pos = 0; pos < D.ne_pad; ++pos)  // positions of lanes without a row hold padding
                 if (!used[pos] && (wv[pos] != 0.0 || code[pos] != 0u)) return fail(EPHC_ESTATE, "internal: weight in a lane without a row");
             // phase 2: every T value is added exactly once, to its b row; off the diagonal every B row stores a sum
             std::fill(used.begin(), used.end(), 0);
             int32_t gathered = 0;
-            const bool ok2 = walk(srow2, shdr2, wptr + t.nwarp + 1, D.nslab2, D.ng_pad, row_in, [&](int32_t u, int32_t g) {
+            const bool ok2 = walk(srow2, shdr2, wptr + t.nwarp + 1, D.nslab2, D.ng_pad, row_in, [&](int32_t u, int32_t g, int32_t, bool) {
                 const int32_t x = perm[g];
                 if (x == D.ne_pad) return true;  // the zero
-                if (x > D.ne_pad || owner[x] != u || used[x]++) return false;
+                if (x > D.ne_pad || owner[x] < 0 || owner[x] != u || used[x]++) return false;
                 ++gathered;
                 return true;
             });
-            if (!ok2 || gathered != D.ne) return fail(EPHC_ESTATE, "internal: phase-2 slabs of a resident tile");
+            if (!ok2 || gathered != D.ncombo) return fail(EPHC_ESTATE, "internal: phase-2 slabs of a resident tile");
             for (int32_t r = run.a_rows; r < R; ++r)
                 if (!row_in[r]) return fail(EPHC_ESTATE, "internal: a B row of a tile has no lane");
             o += D.ne;

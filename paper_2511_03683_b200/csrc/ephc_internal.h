@@ -253,11 +253,15 @@ int build_stream(const ephc_problem *p, const Dims &d, const Canonical &c, int n
 // column-major (element j of lane l at base + 32 j + l: every warp access is one coalesced shared-memory wavefront):
 //   phase 1 (paper step 2): the entries of an a row are cut into pieces of at most Hcap entries, the pieces are
 //            sorted by descending length (pieces of one row adjacent) and dealt 32 per slab; a lane walks its piece with
-//            f_a and sum(T) in registers and overwrites w by T; shorter lanes are padded with w = 0 entries.  Lanes of
-//            a slab that share a row (flag "multi") are combined with a segmented warp-shuffle reduction before the
-//            first of them subtracts the sum from the row's accumulator in shared memory.
+//            f_a in a register.  The entries of one (a, b) state pair inside a piece -- a COMBO: its modes and kinds --
+//            are adjacent; the lane sums |ws| N, the emission and the absorption weights over the combo and forms ONE
+//            term T at its last entry (bit 0 of the code), written over that entry's weight:
+//                T = (f_a - f_b) sum|ws|N + (f_a - f_a f_b) sum_em ws + (f_b - f_a f_b) sum_abs ws.
+//            Shorter lanes are padded with w = 0 entries.  Lanes of a slab that share a row (flag "multi") are combined
+//            with a segmented warp-shuffle reduction before the first of them subtracts the sum from the row's
+//            accumulator in shared memory.
 //   phase 2 (paper step 3): the same slab layout over the b rows: perm[] holds, per (slab, column, lane), the position
-//            of a T value of that row (padding points at a zero behind the entries); the sum of a B row goes straight
+//            of a term T of that row (padding points at a zero behind the entries); the sum of a B row goes straight
 //            to the tile's partial-sum slot in global memory (every B row of the tile has a lane, rows without
 //            entries store 0), on a diagonal tile it is added to the strip's accumulator.
 // One owner per row and phase, fixed order, no atomics.  The slabs of a phase are dealt to the warps of the CTA by the
@@ -280,7 +284,7 @@ struct ResTile {           // 120 bytes (device directory)
     uint32_t o_perm, o_srow1, o_shdr1, o_srow2, o_shdr2, o_wptr, o_nxt, o_w;
     uint32_t a_off, b_off; // first element of the A / B slot in the partial-sum buffer
     uint32_t o_sn_next;    // where the N rows of the next tile of the same CTA go in ITS buffer (res_o_sn of that tile)
-    int32_t pad;
+    int32_t ncombo;        // terms T (one per combo = run of a lane's entries with the same partner): what phase 2 gathers
 };
 static_assert(sizeof(ResTile) == 120 && sizeof(ResTile) / 4 <= 32, "ResTile is copied word by word by one warp");
 constexpr int kResTileWords = sizeof(ResTile) / 4;

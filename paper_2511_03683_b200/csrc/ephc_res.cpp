@@ -163,7 +163,7 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
             if (e[x].in != e[y].in) return e[x].in < e[y].in;
             return x < y;
         });
-    // b-row lists
+    // b-row lists (an upper bound on their lengths for the piece length: one term per entry)
     S.in_start.assign((size_t)R + 1, 0);
     for (int64_t i = 0; i < n; ++i) S.in_start[loc(e[i].in) + 1]++;
     for (int32_t r = 0; r < R; ++r) {
@@ -210,9 +210,13 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
     }
     make_slabs(S.start, 0, R, false, hcap, P.nwarp, pc1, sl1, wp1, ne_pad);
     if (ne_pad > kResXMax - 1 || ne_pad / 32 > 1023) return false;
-    // Order of a lane's entries: a warp gathers f_b and N of a column with 8-byte loads, 16 lanes per shared-memory
-    // wavefront, and every extra lane on a bank pair (address / 8 mod 16) costs another wavefront.  Column by column,
-    // lanes with the fewest entries left choose first, each the entry that lands on the least used bank pairs.
+    // Order of a lane's entries.  The entries of one (owner, partner) state pair inside a piece -- a COMBO: its modes and
+    // kinds -- stay adjacent: the kernel sums their weights and forms ONE term at the combo's last entry, so f_b is
+    // gathered, T stored and T gathered again once per combo.  Inside that constraint the order is free (combos as
+    // blocks, entries inside a combo): a warp gathers N (every entry) and f_b (combo ends) of a column with 8-byte loads,
+    // 16 lanes per shared-memory wavefront, and every extra lane on a bank pair (address / 8 mod 16) costs another
+    // wavefront.  Column by column, lanes with the fewest entries left choose first: an entry of the lane's open combo,
+    // or of any combo if none is open, that lands on the least used bank pairs.
     if (P.bank_aware) {
         auto bank_f = [&](int32_t ei) { return loc(e[ei].in) & 15; };
         auto bank_n = [&](int32_t ei) { return (int32_t)((S.pair_local[ei] * (uint32_t)P.nnu + (uint32_t)e[ei].nu) & 15u); };
@@ -226,18 +230,40 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
                     std::sort(order, order + nl, [&](int32_t x, int32_t y) { return pc1[sl.piece[x]].len < pc1[sl.piece[y]].len; });
                     for (int32_t k = 0; k < nl; ++k) {
                         const Piece &pc = pc1[sl.piece[order[k]]];
-                        int32_t best = j, bc = 1 << 30;
+                        // the open combo: entries left with the partner of the entry just placed
+                        int32_t open_in = -1;
+                        if (j > 0) {
+                            const int32_t pin = e[S.idx[pc.start + j - 1]].in;
+                            for (int32_t m = j; m < pc.len && open_in < 0; ++m)
+                                if (e[S.idx[pc.start + m]].in == pin) open_in = pin;
+                        }
+                        int32_t best = -1, bc = 1 << 30;
                         for (int32_t m = j; m < pc.len; ++m) {
-                            const int32_t ei = S.idx[pc.start + m], c = cf[bank_f(ei)] + cn[bank_n(ei)];
+                            const int32_t ei = S.idx[pc.start + m];
+                            if (open_in >= 0 && e[ei].in != open_in) continue;
+                            int32_t left = 0;  // entries of this combo still to place (including this one)
+                            for (int32_t m2 = j; m2 < pc.len; ++m2) left += e[S.idx[pc.start + m2]].in == e[ei].in;
+                            const int32_t c = cn[bank_n(ei)] + (left == 1 ? cf[bank_f(ei)] : 0);
                             if (c < bc) bc = c, best = m;
                         }
                         std::swap(S.idx[pc.start + j], S.idx[pc.start + best]);
                         const int32_t ei = S.idx[pc.start + j];
-                        cf[bank_f(ei)]++;
                         cn[bank_n(ei)]++;
+                        bool last = true;
+                        for (int32_t m2 = j + 1; m2 < pc.len; ++m2) last &= e[S.idx[pc.start + m2]].in != e[ei].in;
+                        if (last) cf[bank_f(ei)]++;
                     }
                 }
     }
+    // combo ends: the last entry of a piece, or the next entry has another partner
+    std::vector<uint8_t> is_end((size_t)n, 0);
+    int32_t ncombo = 0;
+    for (const Piece &pc : pc1)
+        for (int32_t k = 0; k < pc.len; ++k)
+            if (k + 1 == pc.len || e[S.idx[pc.start + k + 1]].in != e[S.idx[pc.start + k]].in) {
+                is_end[S.idx[pc.start + k]] = 1;
+                ++ncombo;
+            }
     if (P.stats) {  // wavefronts of the f_b and N gathers: per column and half-warp, the largest number of DISTINCT addresses on a bank pair
         long long wf = 0, wn = 0, wi = 0;
         for (const Slab &sl : sl1)
@@ -250,7 +276,7 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
                         any = true;
                         const int32_t ei = S.idx[pc1[sl.piece[l]].start + j];
                         const int32_t fa = loc(e[ei].in), na = (int32_t)(S.pair_local[ei] * (uint32_t)P.nnu + (uint32_t)e[ei].nu);
-                        bool dup = false;
+                        bool dup = !is_end[ei];  // f_b is read at combo ends only
                         for (int k = 0; k < cf[fa & 15]; ++k) dup |= af[fa & 15][k] == fa;
                         if (!dup) af[fa & 15][cf[fa & 15]++] = fa;
                         dup = false;
@@ -276,11 +302,16 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
             const Piece &pc = pc1[sl.piece[l]];
             for (int32_t k = 0; k < pc.len; ++k) S.pos_of[S.idx[pc.start + k]] = sl.base + 32 * k + l;
         }
-    // ---- phase 2: positions of the entries of every b row, ascending; off the diagonal every B row gets a lane ------
-    S.in_list.resize((size_t)n);
+    // ---- phase 2: positions of the combo terms of every b row, ascending; off the diagonal every B row gets a lane ---
+    S.in_start.assign((size_t)R + 1, 0);
+    for (int64_t i = 0; i < n; ++i)
+        if (is_end[i]) S.in_start[loc(e[i].in) + 1]++;
+    for (int32_t r = 0; r < R; ++r) S.in_start[r + 1] += S.in_start[r];
+    S.in_list.resize((size_t)ncombo);
     {
         std::vector<int32_t> cur(S.in_start.begin(), S.in_start.end() - 1);
-        for (int64_t i = 0; i < n; ++i) S.in_list[cur[loc(e[i].in)]++] = S.pos_of[i];
+        for (int64_t i = 0; i < n; ++i)
+            if (is_end[i]) S.in_list[cur[loc(e[i].in)]++] = S.pos_of[i];
         for (int32_t r = 0; r < R; ++r) std::sort(S.in_list.begin() + S.in_start[r], S.in_list.begin() + S.in_start[r + 1]);
     }
     if (P.b_rows > 0)
@@ -334,6 +365,7 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
     ResTile &D = out.dir;
     std::memset(&D, 0, sizeof(D));
     D.ne = (int32_t)n;
+    D.ncombo = ncombo;
     D.ne_pad = ne_pad;
     D.ng_pad = ng_pad;
     D.nslab1 = (int32_t)sl1.size();
@@ -359,7 +391,7 @@ static bool build_image(const DEnt *e, int64_t n, const ImgParams &P, Scratch &S
     // padding entries: w = 0, partner row 0, N slot 0 (both always staged)
     for (int64_t i = 0; i < n; ++i) {
         const int32_t pos = S.pos_of[i];
-        code[pos] = ((uint32_t)loc(e[i].in) << 3) | ((S.pair_local[i] * (uint32_t)P.nnu + (uint32_t)e[i].nu) << 19);
+        code[pos] = ((uint32_t)loc(e[i].in) << 3) | ((S.pair_local[i] * (uint32_t)P.nnu + (uint32_t)e[i].nu) << 19) | is_end[i];
         w[pos] = e[i].w;
     }
     for (size_t s = 0; s < sl1.size(); ++s) {

@@ -105,12 +105,6 @@ __device__ __forceinline__ double res_group_sum(double acc, unsigned same, int l
     return acc;
 }
 
-// Eq. 2 summand of one stored weight (reading R-1): ws > 0 emission weight, ws < 0 absorption weight
-__device__ __forceinline__ double res_term(double ws, double fa, double fb, double N) {
-    const double x = __double2hiint(ws) < 0 ? fb : fa;
-    return fma(fabs(ws), (fa - fb) * N, ws * fma(-fa, fb, x));
-}
-
 // NL consumer threads + one producer warp
 template <int NL, int CTAS>
 __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
@@ -270,6 +264,7 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
                 const uint32_t *c = code + base;
                 double *x = X + base;
                 double acc = 0.0;
+                double S1 = 0.0, Se = 0.0, Sa = 0.0;  // over the open combo: sum |ws| N, sum of emission / absorption weights
                 // columns in groups of four: the codes and weights of the next group are loaded before the current group's
                 // gathers and arithmetic
                 uint32_t c0 = c[0], c1 = 1 < H ? c[32] : 0u, c2 = 2 < H ? c[64] : 0u, c3 = 3 < H ? c[96] : 0u;
@@ -278,20 +273,31 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
                     const bool q0 = j + 4 < H, q1 = j + 5 < H, q2 = j + 6 < H, q3 = j + 7 < H;
                     const uint32_t n0 = q0 ? c[128] : 0u, n1 = q1 ? c[160] : 0u, n2 = q2 ? c[192] : 0u, n3 = q3 ? c[224] : 0u;
                     const double v0 = q0 ? x[128] : 0.0, v1 = q1 ? x[160] : 0.0, v2 = q2 ? x[192] : 0.0, v3 = q3 ? x[224] : 0.0;
-                    const double b0 = *reinterpret_cast<const double *>(sFb + (c0 & 0xfff8u)), b1 = *reinterpret_cast<const double *>(sFb + (c1 & 0xfff8u)),
-                                 b2 = *reinterpret_cast<const double *>(sFb + (c2 & 0xfff8u)), b3 = *reinterpret_cast<const double *>(sFb + (c3 & 0xfff8u));
                     const double N0 = *reinterpret_cast<const double *>(sNb + (c0 >> 16)), N1 = *reinterpret_cast<const double *>(sNb + (c1 >> 16)),
                                  N2 = *reinterpret_cast<const double *>(sNb + (c2 >> 16)), N3 = *reinterpret_cast<const double *>(sNb + (c3 >> 16));
-                    const double T0 = res_term(w0, xo, b0, N0), T1 = res_term(w1, xo, b1, N1), T2 = res_term(w2, xo, b2, N2),
-                                 T3 = res_term(w3, xo, b3, N3);
-                    x[0] = T0;
-                    if (j + 1 < H) x[32] = T1;
-                    if (j + 2 < H) x[64] = T2;
-                    if (j + 3 < H) x[96] = T3;
-                    acc += T0;
-                    acc += T1;  // columns past H carry w = 0: T = 0
-                    acc += T2;
-                    acc += T3;
+                    // f_b is needed where a combo ends only (bit 0; padding never ends one)
+                    const double b0 = (c0 & 1u) ? *reinterpret_cast<const double *>(sFb + (c0 & 0xfff8u)) : 0.0,
+                                 b1 = (c1 & 1u) ? *reinterpret_cast<const double *>(sFb + (c1 & 0xfff8u)) : 0.0,
+                                 b2 = (c2 & 1u) ? *reinterpret_cast<const double *>(sFb + (c2 & 0xfff8u)) : 0.0,
+                                 b3 = (c3 & 1u) ? *reinterpret_cast<const double *>(sFb + (c3 & 0xfff8u)) : 0.0;
+#define EPHC_RES_ENTRY(CD, W, NN, FB, OFF)                                                              \
+    {                                                                                                   \
+        S1 = fma(fabs(W), NN, S1);                                                                      \
+        Se += fmax(W, 0.0);                                                                             \
+        Sa += fmin(W, 0.0);                                                                             \
+        if ((CD) & 1u) { /* Eq. 2 summed over the combo (reading R-1; the sign of ws carries the kind) */ \
+            const double p = xo * (FB);                                                                 \
+            const double T = fma(xo - (FB), S1, fma(xo - p, Se, ((FB) - p) * Sa));                      \
+            x[OFF] = T;                                                                                 \
+            acc += T;                                                                                   \
+            S1 = Se = Sa = 0.0;                                                                         \
+        }                                                                                               \
+    }
+                    EPHC_RES_ENTRY(c0, w0, N0, b0, 0)
+                    EPHC_RES_ENTRY(c1, w1, N1, b1, 32)
+                    EPHC_RES_ENTRY(c2, w2, N2, b2, 64)
+                    EPHC_RES_ENTRY(c3, w3, N3, b3, 96)
+#undef EPHC_RES_ENTRY
                     c0 = n0, c1 = n1, c2 = n2, c3 = n3;
                     w0 = v0, w1 = v1, w2 = v2, w3 = v3;
                     c += 128;
