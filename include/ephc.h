@@ -161,8 +161,9 @@ int64_t ephc_stream_entries(const ephc_handle *h);
 /* Decoded image of the resident-tile store (variant 3), same conditions as ephc_export_gather.  Arrays of length
  * ephc_res_entries(h) (= nw) in store order (runs in hand-out order -> tiles -> entry positions): state a = (n,k),
  * state b = (m,k'), canonical iq, mode, kind (0: w_abs, stored as -w; 1: w_em, stored as +w), weight.  Walks the
- * tile images exactly as the kernel does (the slabs of both phases warp by warp, padding, gather lists) and checks that
- * every term T reaches both of its rows exactly once and that every B row of a tile stores a sum. */
+ * tile images exactly as the kernel does (the slabs of both phases warp by warp, combos, padding, gather lists) and checks
+ * that every weight belongs to one combo with one partner, that every combo term T reaches both of its rows exactly once
+ * and that every B row of a tile stores a sum. */
 int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int32_t *iq, int32_t *nu, int32_t *kind,
                     double *w);
 int64_t ephc_res_entries(const ephc_handle *h);
