@@ -1663,13 +1663,13 @@ static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStre
         const size_t smem = (size_t)res_smem_total(h->x_Ra, h->x_Rcap, h->x_smem_tile);
         const unsigned grid = (unsigned)h->x_ncta;
         switch (h->x_mode) {
-            case 0: res_kernel<256, 2><<<grid, 256 + 32, smem, s>>>(P); break;
-            case 1: res_kernel<512, 1><<<grid, 512 + 32, smem, s>>>(P); break;
-            case 2: res_kernel<256, 1><<<grid, 256 + 32, smem, s>>>(P); break;
-            case 3: res_kernel<384, 1><<<grid, 384 + 32, smem, s>>>(P); break;
-            case 4: res_kernel<128, 4><<<grid, 128 + 32, smem, s>>>(P); break;
-            case 5: res_kernel<512, 2><<<grid, 512 + 32, smem, s>>>(P); break;
-            default: res_kernel<768, 1><<<grid, 768 + 32, smem, s>>>(P); break;
+            case 0: res_kernel<256, 2><<<grid, 256 + kResProducerThreads, smem, s>>>(P); break;
+            case 1: res_kernel<512, 1><<<grid, 512 + kResProducerThreads, smem, s>>>(P); break;
+            case 2: res_kernel<256, 1><<<grid, 256 + kResProducerThreads, smem, s>>>(P); break;
+            case 3: res_kernel<384, 1><<<grid, 384 + kResProducerThreads, smem, s>>>(P); break;
+            case 4: res_kernel<128, 4><<<grid, 128 + kResProducerThreads, smem, s>>>(P); break;
+            case 5: res_kernel<512, 2><<<grid, 512 + kResProducerThreads, smem, s>>>(P); break;
+            default: res_kernel<768, 1><<<grid, 768 + kResProducerThreads, smem, s>>>(P); break;
         }
         h->launches++;
 #ifdef EPHC_RES_TIMING

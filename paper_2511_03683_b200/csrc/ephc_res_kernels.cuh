@@ -106,8 +106,12 @@ __device__ __forceinline__ double res_group_sum(double acc, unsigned same, int l
 }
 
 // NL consumer threads + one producer warp
+constexpr int kResProducerWarps = 4;  // one of them loads the tile image and f; all of them stage the N rows of the tile's pairs
+constexpr int kResProducerThreads = 32 * kResProducerWarps;
+__device__ __forceinline__ void producer_sync() { asm volatile("bar.sync 2, %0;\n" ::"n"(kResProducerThreads) : "memory"); }
+
 template <int NL, int CTAS>
-__global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
+__global__ void __launch_bounds__(NL + kResProducerThreads, CTAS) res_kernel(const ResParams P) {
     extern __shared__ __align__(128) unsigned char res_smem[];
     double *sAccA = reinterpret_cast<double *>(res_smem);                  // accumulators of the strip (run)
     ResTile *sD = reinterpret_cast<ResTile *>(res_smem + 8 * P.Ra);        // directory entries of tiles i, i+1, i+2
@@ -117,19 +121,20 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
     const int i0 = P.cta_ptr[blockIdx.x], n = P.cta_ptr[blockIdx.x + 1] - i0;
     if (n <= 0) return;
     if (tid == 0) {
-        mbar_init(&sFull[0], NL + 1);    // the producer's expect_tx arrive + the cp.async arrives of the consumers (N rows)
-        mbar_init(&sFull[1], NL + 1);
+        mbar_init(&sFull[0], kResProducerThreads + 1);  // the loader's expect_tx arrive + the cp.async arrives of the producer threads (N rows)
+        mbar_init(&sFull[1], kResProducerThreads + 1);
         mbar_init(&sEmpty[0], NL / 32);  // one arrive per consumer warp
         mbar_init(&sEmpty[1], NL / 32);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    for (int r = tid; r < P.Ra; r += NL + 32) sAccA[r] = 0.0;
+    for (int r = tid; r < P.Ra; r += NL + kResProducerThreads) sAccA[r] = 0.0;
     __syncthreads();
     auto buf_of = [&](int b) { return res_smem + P.fixed_bytes + (size_t)b * P.buf_bytes; };
 
     if (tid >= NL) {
-        // ===== producer warp: everything a tile needs, up to two tiles ahead of the consumers ==============================
-        const int lane = tid - NL;
+        // ===== producer warps: everything a tile needs, up to two tiles ahead of the consumers; the N rows are staged while
+        // the consumers compute (their cp.async wavefronts fill the LSU cycles that the latency-bound phases leave idle) ======
+        const int ptid = tid - NL, lane = ptid & 31, pw = ptid >> 5;
         uint64_t pol_stream, pol_keep;
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol_stream));  // the store is read once
         asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol_keep));     // f is read by every tile
@@ -149,18 +154,18 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
             int32_t *dst = reinterpret_cast<int32_t *>(&sD[j % 3]);
             if (lane < kResTileWords) dst[lane] = src[lane];
         };
-        load_dir(0);
+        if (pw == 0) load_dir(0);
         for (int j = 0; j < n; ++j) {
             const int b = j & 1;
             EPHC_PTICK(0)
             if (j >= 2) mbar_wait(&sEmpty[b], (unsigned)((j >> 1) - 1) & 1u);  // the consumers are done with tile j - 2
             EPHC_PTICK(1)
-            __syncwarp();
+            producer_sync();  // the directory entry of tile j (written by the loader warp one tile ago) is visible to all of them
             const ResTile &D = sD[j % 3];
             unsigned char *buf = buf_of(b);
             double *sF = reinterpret_cast<double *>(buf);
             unsigned char *sBlob = reinterpret_cast<unsigned char *>(sF + P.Rcap);
-            if (lane == 0) {
+            if (ptid == 0) {
                 const int a_rows = D.a_rows, b_rows = D.b_rows, bytes = D.blob_bytes;
                 const unsigned fa = (unsigned)((8 * a_rows + 15) & ~15), fb = (unsigned)((8 * b_rows + 15) & ~15);
                 *reinterpret_cast<double *>(sBlob + D.o_w + 8 * (size_t)D.ne_pad) = 0.0;  // the zero that padding reads
@@ -173,7 +178,7 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
             }
             EPHC_PTICK(2)
             // the directory entry of the next tile (its slot was last used by tile j - 2), and its image on the way to the L2
-            if (j + 1 < n) {
+            if (pw == 0 && j + 1 < n) {
                 load_dir(j + 1);
                 __syncwarp();
                 if (lane == 0) {
@@ -182,13 +187,34 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
                 }
             }
             EPHC_PTICK(3)
+            // N[iq, :] of the tile's pairs; their iq * nnu came with the image of the previous tile
+            {
+                double *sN = reinterpret_cast<double *>(sBlob + ((D.o_w + 8u * (unsigned)(D.ne_pad + 1) + 15u) & ~15u));
+                const uint32_t *iq = P.iqn + D.q0;
+                if (j > 0) {
+                    mbar_wait(&sFull[b ^ 1], (unsigned)((j - 1) >> 1) & 1u);
+                    const unsigned char *prev = buf_of(b ^ 1) + 8 * (size_t)P.Rcap;
+                    iq = reinterpret_cast<const uint32_t *>(prev + sD[(j - 1) % 3].o_nxt);
+                }
+                const int total = D.nq * P.gran;
+                for (int g = ptid; g < total; g += kResProducerThreads) {
+                    const int pr = P.gran_magic ? (int)__umulhi((unsigned)g, P.gran_magic) : g, part = g - pr * P.gran;
+                    const double *src = P.N + (size_t)iq[pr];
+                    if (P.gran16)
+                        cp_async16(sN + pr * nnu + 2 * part, src + 2 * part);
+                    else
+                        res_cp_async8(sN + pr * nnu + part, src + part);
+                }
+                mbar_arrive_cp_async(&sFull[b]);
+            }
+            EPHC_PTICK(4)
 #ifdef EPHC_RES_TIMING
             mbar_wait(&sFull[b], (unsigned)(j >> 1) & 1u);  // working build only: how long until the tile is complete
             EPHC_PTICK(5)
 #endif
         }
 #ifdef EPHC_RES_TIMING
-        if (P.dbg && lane == 0)
+        if (P.dbg && ptid == 0)
             for (int k = 0; k < 8; ++k) P.dbg[((size_t)blockIdx.x * (NL / 32 + 1) + NL / 32) * 8 + k] = pacc[k];
 #endif
         return;
@@ -208,24 +234,6 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
 #endif
     const int lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NL / 32;
-    // N[iq, :] of a tile's pairs -> the tile's buffer, by all consumer threads, one tile ahead; counted on its full barrier
-    auto stage_N = [&](const uint32_t *iq, int nq, double *sN, uint64_t *bar) {
-        const int total = nq * P.gran;
-        for (int g = tid; g < total; g += NL) {
-            const int pr = P.gran_magic ? (int)__umulhi((unsigned)g, P.gran_magic) : g, part = g - pr * P.gran;
-            const double *src = P.N + (size_t)iq[pr];
-            if (P.gran16)
-                cp_async16(sN + pr * nnu + 2 * part, src + 2 * part);
-            else
-                res_cp_async8(sN + pr * nnu + part, src + part);
-        }
-        mbar_arrive_cp_async(bar);
-    };
-    {   // first tile: its pair list comes from global memory
-        const ResTile &G = P.tiles[i0];
-        const unsigned o_sn0 = (G.o_w + 8u * (unsigned)(G.ne_pad + 1) + 15u) & ~15u;
-        stage_N(P.iqn + G.q0, G.nq, reinterpret_cast<double *>(buf_of(0) + 8 * (size_t)P.Rcap + o_sn0), &sFull[0]);
-    }
     for (int i = 0; i < n; ++i) {
         const int b = i & 1;
         unsigned char *buf = buf_of(b);
@@ -318,11 +326,6 @@ __global__ void __launch_bounds__(NL + 32, CTAS) res_kernel(const ResParams P) {
         }
         EPHC_TICK(2)
         consumer_sync(NL);
-        // every warp has left tile i - 1 (it arrived here): its buffer takes the N rows of tile i + 1, whose pair list came
-        // with this tile's image
-        if (i + 1 < n)
-            stage_N(reinterpret_cast<const uint32_t *>(sBlob + D.o_nxt), D.nq_next,
-                    reinterpret_cast<double *>(buf_of(b ^ 1) + 8 * (size_t)P.Rcap + D.o_sn_next), &sFull[b ^ 1]);
         EPHC_TICK(3)
         // ---- phase 2 (paper step 3): a lane sums the T values listed for one piece of a b row -------------------------------
         {
