@@ -1,21 +1,22 @@
 // ephc_res_kernels.cuh -- sm_100a kernel of the resident-tile store (variant 3): collision integral with once-stored
-// directed entries (step 2 "contribution of every channel" and step 3 "sum over the channels of a
-// state" in one kernel; the per-channel terms -- the paper's sc_col -- overwrite the weights in shared memory and
-// never reach HBM).
+// entries (step 2 "contribution of every channel" and step 3 "sum over the channels of a state" in one
+// kernel; the per-channel terms -- the paper's sc_col -- overwrite the weights in shared memory and never reach HBM).
+// Layout of a tile image: ephc_internal.h "resident-tile store".
 //
-// One persistent CTA per SM walks its host-assigned sequence of tiles with two tile buffers in shared memory.
-// While tile i is computed, tile i+1 is loaded: one elected thread issues bulk copies (TMA, UBLKCP) of the tile
-// image (codes, gather lists, row tables, weights: one contiguous blob) and of the compact f values of its A and B
-// rows, all completing on the buffer's mbarrier; all threads stage N[iq,:] of its pairs with cp.async, reading the
-// pairs' iq from a list that came with the image of tile i.  Per tile:
-//   phase 1  one lane per out-row piece: T = w [(f_out - f_in) N + f_out (1 - f_in)] (Eq. 2, reading R-1, emission
-//            form; absorption weights are stored as the reversed entry), T overwrites w, the lane's -sum(T) goes to the
-//            X tail;
-//   phase 2  one lane per gather task: sums the X values listed for one row (T of its in-entries, sums of its out
-//            pieces) and adds them to the row's accumulator (one owner per row and round: no atomics, fixed order,
-//            bit-reproducible).
-// The accumulators of the strip (A rows) stay in shared memory for a run of tiles; B rows go to their partial-sum slot
-// after every tile, A rows at the end of the run; finish_kernel (ephc_tile_kernels.cuh) adds the slots per state.
+// Persistent CTAs (one or two per SM) walk their host-assigned sequence of tiles with two tile buffers in shared memory.
+// While the consumer warps compute tile i, four producer warps load tile i+1: one elected thread issues bulk copies (TMA,
+// UBLKCP) of the tile image (codes, gather lists, slab tables, weights: one contiguous blob) and of the compact f values
+// of its A and B rows, all completing on the buffer's mbarrier; all producer threads stage N[iq,:] of its pairs with
+// cp.async (counted on the same mbarrier), reading the pairs' iq from a list that came with the image of tile i.  Per tile:
+//   phase 1  a lane owns one piece of an owner row a (32 pieces per slab, column-major): per entry it gathers N and sums
+//            |ws| N and the emission / absorption weights over the open combo (the entries with one partner b); at the
+//            combo's last entry it gathers f_b and forms T (Eq. 2 with reading R-1, summed over the combo), written over
+//            that entry's weight; the lane's sum of T is subtracted from the strip's accumulator of row a;
+//   phase 2  a lane owns one piece of a partner row b: it gathers the terms T listed for it and stores their sum to the
+//            tile's partial-sum slot (global memory), or adds it to the strip's accumulator on a diagonal tile.
+// One owner per row and phase: no atomics, fixed order, bit-reproducible.  The accumulators of the strip
+// (A rows) stay in shared memory for a run of tiles and go to their slot at the end of the run; finish_kernel
+// (ephc_tile_kernels.cuh) adds the slots per state.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -106,7 +107,10 @@ __device__ __forceinline__ double res_group_sum(double acc, unsigned same, int l
 }
 
 // NL consumer threads + one producer warp
-constexpr int kResProducerWarps = 4;  // one of them loads the tile image and f; all of them stage the N rows of the tile's pairs
+#ifndef EPHC_RES_PRODUCERS
+#define EPHC_RES_PRODUCERS 4  // 2: Si 127 us, GaAs 1622 us; 4: 104, 1541; 8: 102, 1620 (collision call)
+#endif
+constexpr int kResProducerWarps = EPHC_RES_PRODUCERS;  // one of them loads the tile image and f; all of them stage the N rows of the tile's pairs
 constexpr int kResProducerThreads = 32 * kResProducerWarps;
 __device__ __forceinline__ void producer_sync() { asm volatile("bar.sync 2, %0;\n" ::"n"(kResProducerThreads) : "memory"); }
 
