@@ -284,6 +284,21 @@ int ephc_transport_solve_host(ephc_handle *h, const double *f0_host, const doubl
 int ephc_rt_step_host(ephc_handle *h, double *f_host, const double *N_host, double dt_fs, int nsteps,
                       double *sumf_host);
 
+/* Allocation-free conservation scalar: *sum_dev = sum_{s < n} f_dev[s] (electron number, checked every
+ * rt-BTE step; the same two-stage reduction as ephc_rt_step's sumf_dev: per-block partial sums, then their sum in a
+ * fixed order, bit-reproducible).  For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): needs no handle and calls no cudaMalloc / cudaFree or allocating library routine.
+ * The partial sums live in a fixed 32 KB device array inside the library (every GPU that loads the library holds it
+ * until exit), so n <= ephc_noalloc_max_states() = 16 777 216; larger n fails with EPHC_ELIMIT and touches nothing.
+ * f_dev, sum_dev: caller-owned device buffers on the CURRENT device; `stream` as elsewhere.  Every call shares the array,
+ * which keeps the last call's contents (each call overwrites all slots it reads): calls that overlap on the GPU, e.g. on
+ * two streams, race -- order them.  ephc_noalloc_init() looks up the array's device address for the current device
+ * (once per device; the first ephc_sum_states_noalloc on a device does it itself: call it beforehand when the first
+ * use would fall under graph capture). */
+int ephc_noalloc_init(void);
+int64_t ephc_noalloc_max_states(void);
+int ephc_sum_states_noalloc(const double *f_dev, int64_t n, double *sum_dev, void *stream);
+
 /* Number of kernel launches enqueued by this library since the handle was created (for bench.py). */
 int64_t ephc_launch_count(const ephc_handle *h);
 

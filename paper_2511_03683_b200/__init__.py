@@ -16,7 +16,8 @@ import numpy as np
 
 from . import _build
 
-__all__ = ["EphcError", "Handle", "build_channels", "lib_path", "HOST_ONLY", "SELECT_GPU", "TRANSPORT_COLLAPSE", "version"]
+__all__ = ["EphcError", "Handle", "build_channels", "lib_path", "HOST_ONLY", "SELECT_GPU", "TRANSPORT_COLLAPSE", "version",
+           "noalloc_init", "noalloc_max_states", "sum_states_noalloc"]
 
 HOST_ONLY = 1
 SELECT_GPU = 2
@@ -92,6 +93,9 @@ def _load():
         "ephc_transport_start": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_transport_iter": (i32, [vp, vp, vp, vp, vp, vp]),
         "ephc_transport_iters": (i32, [vp, vp, vp, vp, vp, i32, vp]),
+        "ephc_noalloc_init": (i32, []),
+        "ephc_noalloc_max_states": (i64, []),
+        "ephc_sum_states_noalloc": (i32, [vp, i64, vp, vp]),
         "ephc_transport_collapse": (i32, [vp, vp]),
         "ephc_set_transport_collapsed": (i32, [vp, i32]),
         "ephc_collapsed_entries": (i64, [vp]),
@@ -350,6 +354,22 @@ class Handle:
         pN, k2 = _host_ptr(N, self.nq * self.nnu, "N")
         ps, k3 = _host_ptr(sumf, nsteps + 1, "sumf", writable=True)
         _check(_load().ephc_rt_step_host(self._h, pf, pN, float(dt_fs), int(nsteps), ps))
+
+
+def noalloc_init() -> None:
+    """Looks up the device address of the library's fixed scratch array for the current device (once per device)."""
+    _check(_load().ephc_noalloc_init())
+
+
+def noalloc_max_states() -> int:
+    return int(_load().ephc_noalloc_max_states())
+
+
+def sum_states_noalloc(f, out, n: Optional[int] = None, stream=None) -> None:
+    """out[0] = sum of the first n (default: all) elements of the device vector f; allocates nothing (include/ephc.h)."""
+    if n is None:
+        n = f.numel()
+    _check(_load().ephc_sum_states_noalloc(_dev_ptr(f, None, "f"), int(n), _dev_ptr(out, None, "out"), _stream_ptr(stream)))
 
 
 def build_channels(prob, flags: int = 0, k_range=None) -> Handle:

@@ -2235,3 +2235,74 @@ extern "C" int ephc_rt_step_host(ephc_handle *h, double *f_host, const double *N
     CUDA_TRY(cudaStreamSynchronize(0));
     return EPHC_OK;
 }
+
+// ---- allocation-free conservation scalar (callers that cannot call cudaMalloc: graph capture, serving loops) ---------
+// sum_s f_s (the quantity whose conservation is checked every rt-BTE step) as the
+// library's two-stage reduction -- per-block partial sums in scratch memory, then sum_kernel over the partial sums in a
+// fixed order -- with the scratch in a file-scope device array instead of the handle's cudaMalloc'ed d_wusum.
+// Every GPU that loads the library holds the array (32 KB) until exit.  All calls share it and it keeps the last call's
+// contents: block_sum_kernel overwrites every slot the second stage reads, so nothing has to start at zero; calls that
+// overlap on the GPU (different streams) race on it.
+constexpr int kNoAllocBlockElems = 4096;  // elements one block of block_sum_kernel sums (256 threads x 16)
+constexpr int kNoAllocMaxBlocks = 4096;   // partial sums the scratch holds
+static __device__ __align__(256) double g_noalloc_partials[kNoAllocMaxBlocks];
+constexpr int kNoAllocMaxDevices = 64;
+static double *g_noalloc_ptr[kNoAllocMaxDevices] = {nullptr};  // device address of the array, per device (set-up)
+
+// partial[b] = sum of x[b * 4096 .. min(n, (b + 1) * 4096)) in a fixed order: strided per-thread sums, shuffle tree per
+// warp, then the eight warp sums in order
+__global__ void __launch_bounds__(256) block_sum_kernel(const double *__restrict__ x, int64_t n, double *__restrict__ partial) {
+    __shared__ double sw[8];
+    const int64_t lo = (int64_t)blockIdx.x * kNoAllocBlockElems, hi = lo + kNoAllocBlockElems < n ? lo + kNoAllocBlockElems : n;
+    double a = 0.0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += 256) a += x[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if ((threadIdx.x & 31) == 0) sw[threadIdx.x >> 5] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) s += sw[w];
+        partial[blockIdx.x] = s;
+    }
+}
+
+// Set-up for the current device: the address of the scratch array ON THAT DEVICE.  In host code the array's name is a
+// host-side stand-in, not a device address; only cudaGetSymbolAddress (with the device current) gives the pointer a
+// kernel may use.
+extern "C" int ephc_noalloc_init(void) {
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(EPHC_ELIMIT, "ephc_noalloc_init: device ordinal beyond 63");
+    if (g_noalloc_ptr[dev] != nullptr) return EPHC_OK;
+    double *ptr = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress((void **)&ptr, g_noalloc_partials));
+    if (ptr == nullptr) return fail(EPHC_ECUDA, "cudaGetSymbolAddress returned a null address for the scratch array");
+    g_noalloc_ptr[dev] = ptr;
+    return EPHC_OK;
+}
+
+extern "C" int64_t ephc_noalloc_max_states(void) { return (int64_t)kNoAllocBlockElems * kNoAllocMaxBlocks; }
+
+extern "C" int ephc_sum_states_noalloc(const double *f_dev, int64_t n, double *sum_dev, void *stream) {
+    if (!f_dev || !sum_dev) return fail(EPHC_EINVAL, "null device pointer");
+    if (n < 0) return fail(EPHC_EINVAL, "ephc_sum_states_noalloc: n must be >= 0");
+    if (n > ephc_noalloc_max_states())
+        return fail(EPHC_ELIMIT, "ephc_sum_states_noalloc: n = " + std::to_string(n) + " exceeds the fixed scratch (at most " +
+                                     std::to_string(ephc_noalloc_max_states()) + " states); use ephc_rt_step's sumf_dev instead");
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(EPHC_ELIMIT, "ephc_sum_states_noalloc: device ordinal beyond 63");
+    if (g_noalloc_ptr[dev] == nullptr) {  // first use on this device (call ephc_noalloc_init beforehand when capturing a graph)
+        const int rc = ephc_noalloc_init();
+        if (rc) return rc;
+    }
+    double *partial = g_noalloc_ptr[dev];
+    const cudaStream_t s = (cudaStream_t)stream;
+    const int nblk = (int)((n + kNoAllocBlockElems - 1) / kNoAllocBlockElems);
+    if (nblk > 0) block_sum_kernel<<<(unsigned)nblk, 256, 0, s>>>(f_dev, n, partial);
+    sum_kernel<<<1, 1024, 0, s>>>(partial, nblk, sum_dev);  // reads the nblk slots just written, nothing older
+    CUDA_TRY(cudaGetLastError());
+    return EPHC_OK;
+}
