@@ -155,6 +155,7 @@ struct ephc_handle {
     RowSeg *dc_segs = nullptr;
     RowTile *dc_tiles = nullptr;
     RowStrip *dc_strips = nullptr;
+    int32_t *dr_cols = nullptr;   // sparse staging: the strips' partner-row lists (null otherwise)
     uint32_t *dr_meta = nullptr;  // per entry: (iq * nnu + mode) | kind << 31
     double *dr_wst = nullptr;     // per entry: channel weight
     RowSeg *dr_segs = nullptr;
@@ -169,7 +170,7 @@ static void free_dev(ephc_handle *h) {
                     h->d_tr[1], h->d_tr[2], h->d_tr[3], h->d_tr[4], h->d_sumf, h->dt_w, h->dt_part, h->dt_Wf,
                     h->dt_Wr, h->dt_code, h->dt_prec, h->dt_slices, h->dt_tiles, h->dt_ctas, h->dt_blk_row0,
                     h->dt_row_state, h->dt_state_row, h->dt_state_blk, h->dt_blk_ent_ptr, h->dt_blk_ent_off,
-                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_Fc2, h->d_Fscr, h->dr_idx, h->dc_idx, h->dc_count, h->dc_first, h->dc_W, h->dc_segs, h->dc_tiles, h->dc_strips, h->dr_meta, h->dr_wst, h->dr_segs, h->dr_tiles, h->dr_strips,
+                    h->dt_slot_off, h->dr_W, h->dr_Fc, h->dr_Fc2, h->d_Fscr, h->dr_idx, h->dc_idx, h->dc_count, h->dc_first, h->dc_W, h->dc_segs, h->dc_tiles, h->dc_strips, h->dr_cols, h->dr_meta, h->dr_wst, h->dr_segs, h->dr_tiles, h->dr_strips,
                     h->dr_row_state, h->dr_state_row, h->ds_w, h->ds_part, h->ds_code, h->ds_iq, h->ds_perm, h->ds_aid,
                     h->ds_ast, h->ds_bid, h->ds_bst, h->ds_chunks, h->ds_tiles, h->ds_order, h->ds_counter, h->ds_row_state,
                     h->ds_state_row, h->ds_state_blk, h->ds_blk_row0, h->ds_blk_ent_ptr, h->ds_slot_off,
@@ -741,7 +742,7 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         h->r_Rb = rh.Rb;
         h->r_Ra = rh.Ra;
         h->r_nrows = rh.nrows;
-        h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.meta.size() * 4 + rh.wst.size() * 8 + rh.segs.size() * sizeof(RowSeg) +
+        h->bytes_rows = (int64_t)(rh.idx.size() * 2 + rh.cols.size() * 4 + rh.meta.size() * 4 + rh.wst.size() * 8 + rh.segs.size() * sizeof(RowSeg) +
                                   rh.tiles.size() * sizeof(RowTile) + rh.strips.size() * sizeof(RowStrip) +
                                   (rh.row_state.size() + rh.state_row.size()) * 4);
         if (h->host_only) {
@@ -764,6 +765,7 @@ static int build_impl(const ephc_problem *p, int32_t k_lo, int32_t k_hi, bool ra
         if (rc == EPHC_OK && h->rows_ok) {
             int64_t br = 0;
             rc = upload(&h->dr_idx, rh.idx, &br);
+            if (rc == EPHC_OK && !rh.cols.empty()) rc = upload(&h->dr_cols, rh.cols, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_meta, rh.meta, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_wst, rh.wst, &br);
             if (rc == EPHC_OK) rc = upload(&h->dr_segs, rh.segs, &br);
@@ -1172,9 +1174,14 @@ extern "C" int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *pa
         int32_t last_col0 = -1;
         for (int32_t it = st.t0; it < st.t1; ++it) {
             const RowTile &tl = r.tiles[it];
-            if (tl.nseg < 1 || tl.col0 % r.Rb != 0 || tl.col0 <= last_col0 || tl.ncols < 1 || tl.ncols > r.Rb ||
-                tl.col0 + tl.ncols > r.nrows)
+            const bool sparse = !r.cols.empty();
+            if (tl.nseg < 1 || tl.col0 <= last_col0 || tl.ncols < 1 || tl.ncols > r.Rb ||
+                (sparse ? tl.col0 < 0 || tl.col0 + (int64_t)tl.ncols > (int64_t)r.cols.size() : tl.col0 % r.Rb != 0 || tl.col0 + tl.ncols > r.nrows))
                 return fail(EPHC_ESTATE, "internal: bad row tile");
+            if (sparse)  // the tile's chunk of the strip's partner list: ascending rows
+                for (int32_t j = 0; j < tl.ncols; ++j)
+                    if (r.cols[tl.col0 + j] < 0 || r.cols[tl.col0 + j] >= r.nrows || (j > 0 && r.cols[tl.col0 + j] <= r.cols[tl.col0 + j - 1]))
+                        return fail(EPHC_ESTATE, "internal: partner list of a row tile");
             last_col0 = tl.col0;
             row_tiles.assign((size_t)std::max(st.nrows, 1), 0);
             uint32_t last_len = 0xffffffffu;
@@ -1190,7 +1197,7 @@ extern "C" int ephc_export_rows(const ephc_handle *h, int32_t *dest, int32_t *pa
                     const int64_t gp = r.perm[o];
                     if (gp >= nent || pos_seen[gp]++ || r.idx[o] >= tl.ncols) return fail(EPHC_ESTATE, "internal: row entry out of range");
                     if (dest) dest[o] = r.row_state[st.row0 + (int32_t)sg.row];
-                    if (partner) partner[o] = r.row_state[tl.col0 + r.idx[o]];
+                    if (partner) partner[o] = r.row_state[sparse ? r.cols[tl.col0 + r.idx[o]] : tl.col0 + r.idx[o]];
                     if (gather_pos) gather_pos[o] = gp;
                 }
             }
@@ -1240,7 +1247,7 @@ extern "C" int ephc_export_rows_collapsed(const ephc_handle *h, int32_t *dest, i
                         if (r.idx[o] != c.idx[x] || covered[o]++) return fail(EPHC_ESTATE, "internal: collapsed entry sums a foreign term");
                     }
                     if (dest) dest[x] = r.row_state[st.row0 + (int32_t)sg.row];
-                    if (partner) partner[x] = r.row_state[tl.col0 + c.idx[x]];
+                    if (partner) partner[x] = r.row_state[r.cols.empty() ? tl.col0 + c.idx[x] : r.cols[tl.col0 + c.idx[x]]];
                     if (count) count[x] = c.count[x];
                 }
             }
@@ -1789,6 +1796,7 @@ static RowParams row_params(const ephc_handle *h) {
     R.strips = h->dr_strips;
     R.row_state = h->dr_row_state;
     R.state_row = h->dr_state_row;
+    R.cols = h->dr_cols;
     R.Rb = h->r_Rb;
     R.Ra = h->r_Ra;
     R.nstrip = h->r_nstrip;
@@ -1962,8 +1970,28 @@ extern "C" int ephc_transport_iters(ephc_handle *h, const double *F_dev, const d
             R.Fc = buf[it & 1];
             R.Fc_out = last ? nullptr : buf[(it + 1) & 1];
             R.out = last ? Fout_dev : nullptr;
+#ifdef EPHC_ROW_TIMING
+            static unsigned long long *rdbg = nullptr;
+            if (!rdbg) cudaMalloc((void **)&rdbg, 4 * 8 * 1024);
+            R.dbg = rdbg;
+#endif
             row_iter_kernel<<<(unsigned)std::max(h->r_nstrip, 1), kRowThreads, row_smem_bytes(h->r_Rb, h->r_Ra), s>>>(R);
             h->launches++;
+#ifdef EPHC_ROW_TIMING
+            if (it == niter / 2 && std::getenv("EPHC_ROW_TIMING_PRINT")) {
+                std::vector<unsigned long long> hd(4 * (size_t)h->r_nstrip);
+                cudaMemcpy(hd.data(), rdbg, hd.size() * 8, cudaMemcpyDeviceToHost);
+                unsigned long long e0 = ~0ull, e1 = 0, x0 = ~0ull, x1 = 0;
+                double pro = 0, loop = 0, epi = 0;
+                for (int k = 0; k < h->r_nstrip; ++k) {
+                    e0 = std::min(e0, hd[4 * k]); e1 = std::max(e1, hd[4 * k]);
+                    x0 = std::min(x0, hd[4 * k + 3]); x1 = std::max(x1, hd[4 * k + 3]);
+                    pro += (double)(hd[4 * k + 1] - hd[4 * k]); loop += (double)(hd[4 * k + 2] - hd[4 * k + 1]); epi += (double)(hd[4 * k + 3] - hd[4 * k + 2]);
+                }
+                std::fprintf(stderr, "row timing (ns): entry spread %llu, first entry -> last exit %llu, exit spread %llu; per CTA prologue %.0f loop %.0f epilogue %.0f\n",
+                             e1 - e0, x1 - e0, x1 - x0, pro / h->r_nstrip, loop / h->r_nstrip, epi / h->r_nstrip);
+            }
+#endif
         }
         CUDA_TRY(cudaGetLastError());
         return EPHC_OK;

@@ -155,7 +155,8 @@ struct RowSeg {        // 16 bytes: one destination row inside one tile
 };
 struct RowTile {
     int32_t seg0, nseg;      // segment range
-    int32_t col0, ncols;     // partner rows staged for this tile (compact row range)
+    int32_t col0, ncols;     // partner rows staged for this tile: compact rows [col0, col0 + ncols), or -- sparse staging --
+                             // the rows cols[col0 .. col0 + ncols) of the strip's list of referenced partner rows
 };
 struct RowStrip {
     int64_t e0;              // first entry of the strip
@@ -165,7 +166,8 @@ struct RowStrip {
 struct RowHost {
     int32_t Rb = 0, Ra = 0, nrows = 0;
     std::vector<int32_t> row_state, state_row;
-    std::vector<uint16_t> idx;        // per entry: partner row - col0 of its tile
+    std::vector<int32_t> cols;        // sparse staging (empty otherwise): per strip the sorted partner rows its entries reference
+    std::vector<uint16_t> idx;        // per entry: partner row - col0 of its tile (sparse staging: position in the tile's chunk of cols)
     std::vector<uint32_t> perm;       // per entry: index of the same ordered term in the gather store (host only: export / tests)
     std::vector<double> wst;          // per entry: the channel weight |g|^2 delta of this ordered term (transport_setup reads it)
     std::vector<uint32_t> meta;       // per entry: (iq * nnu + mode) | kind << 31 (kind as seen from the destination)

@@ -35,12 +35,16 @@ struct RowParams {
     const RowTile *tiles;
     const RowStrip *strips;
     const int32_t *row_state, *state_row;
+    const int32_t *cols;    // sparse staging: the strips' lists of referenced partner rows (null: tiles cover row ranges)
     int32_t Rb, Ra, nstrip;
     int64_t ns;
     const double *Fc;       // F of the compact rows, [nrows][3] (row_compact_kernel), padded by 2 doubles
     const double *v, *tau;
     double *out;            // API layout [3][ns] (Gamma [ns] in setup); the iteration may pass null between chained iterations
     double *Fc_out;         // iteration: compact [nrows][3] copy of the result for the next chained iteration, may be null
+#ifdef EPHC_ROW_TIMING
+    unsigned long long *dbg;
+#endif
 };
 
 inline size_t row_smem_bytes(int Rb, int Ra) { return ((size_t)Rb + (size_t)Ra) * 3 * sizeof(double) + 48; }
@@ -59,6 +63,10 @@ __global__ void __launch_bounds__(256) row_compact_kernel(const double *F, const
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src));
+}
+__device__ __forceinline__ void row_cp_async8(void *smem_dst, const void *gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gmem_src));
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N>
@@ -112,9 +120,14 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_setup_ker
         const RowTile tl = P.tiles[t];
         __syncthreads();
         {
-            const double *src = P.Fc + tl.col0;  // col0 is even: 16-byte aligned
-            const int n16 = (tl.ncols + 1) / 2;
-            for (int i = tid; i < n16; i += kRowThreads) cp_async16(sF + 2 * i, src + 2 * i);
+            if (P.cols != nullptr) {  // sparse staging: the partner rows this strip references
+                const int32_t *cl = P.cols + tl.col0;
+                for (int i = tid; i < tl.ncols; i += kRowThreads) row_cp_async8(sF + i, P.Fc + __ldg(cl + i));
+            } else {
+                const double *src = P.Fc + tl.col0;  // col0 is even: 16-byte aligned
+                const int n16 = (tl.ncols + 1) / 2;
+                for (int i = tid; i < n16; i += kRowThreads) cp_async16(sF + 2 * i, src + 2 * i);
+            }
             cp_async_commit();
             if (tid == 0) *sNext = 0;
             cp_async_wait<0>();
@@ -187,6 +200,10 @@ __global__ void __launch_bounds__(256) row_collapse_kernel(const double *__restr
 }
 
 __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kernel(const RowParams P) {
+#ifdef EPHC_ROW_TIMING
+    unsigned long long g0, g1, g2, g3;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
+#endif
     extern __shared__ double smem[];
     double *sF = smem;                       // staged partner rows [Rb][3]
     double *sAcc = smem + (P.Rb * 3 + 2);    // [Ra][3]
@@ -209,13 +226,24 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kern
     const double *Wb = P.W + st.e0;
     const uint16_t *Ib = P.idx + st.e0;
 
+#ifdef EPHC_ROW_TIMING
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+#endif
     for (int t = st.t0; t < st.t1; ++t) {
         const RowTile tl = P.tiles[t];
         __syncthreads();  // previous tile done with sF (and sAcc zeroed)
         {   // stage the tile's partner rows: 16-byte copies global -> shared, no registers in between
-            const double *src = P.Fc + (int64_t)tl.col0 * 3;
-            const int n16 = (tl.ncols * 3 + 1) / 2;
-            for (int i = tid; i < n16; i += kRowThreads) cp_async16(sF + 2 * i, src + 2 * i);
+            if (P.cols != nullptr) {  // sparse staging: the partner rows this strip references, 24 bytes each
+                const int32_t *cl = P.cols + tl.col0;
+                for (int i = tid; i < tl.ncols * 3; i += kRowThreads) {
+                    const int rr = i / 3, cc = i - 3 * rr;
+                    row_cp_async8(sF + i, P.Fc + (int64_t)__ldg(cl + rr) * 3 + cc);
+                }
+            } else {
+                const double *src = P.Fc + (int64_t)tl.col0 * 3;
+                const int n16 = (tl.ncols * 3 + 1) / 2;
+                for (int i = tid; i < n16; i += kRowThreads) cp_async16(sF + 2 * i, src + 2 * i);
+            }
             cp_async_commit();
             if (tid == 0) *sNext = 0;
             cp_async_wait<0>();
@@ -301,6 +329,9 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kern
         }
     }
     __syncthreads();
+#ifdef EPHC_ROW_TIMING
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g2));
+#endif
     for (int i = tid; i < st.nrows; i += kRowThreads) {
         const int64_t s = P.row_state[st.row0 + i];
         const double ta = P.tau[s];
@@ -311,6 +342,16 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kern
             if (P.Fc_out != nullptr) P.Fc_out[(int64_t)(st.row0 + i) * 3 + c] = val;
         }
     }
+#ifdef EPHC_ROW_TIMING
+    __syncthreads();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g3));
+    if (tid == 0 && P.dbg) {
+        P.dbg[4 * blockIdx.x] = g0;
+        P.dbg[4 * blockIdx.x + 1] = g1;
+        P.dbg[4 * blockIdx.x + 2] = g2;
+        P.dbg[4 * blockIdx.x + 3] = g3;
+    }
+#endif
 }
 
 }  // namespace ephc

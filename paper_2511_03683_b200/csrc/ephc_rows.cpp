@@ -69,17 +69,26 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
         // entries per (row, range) and per row
         std::vector<uint32_t> cnt((size_t)r.nrows * nrange, 0);
         for (int64_t e = 0; e < nent; ++e) cnt[(size_t)drow[e] * nrange + prow[e] / Rb]++;
+        // work of a row for the strip balance: a segment is walked in steps of 32 entries (8 lanes x 4 entries) and
+        // costs a fixed overhead (header fetch, shuffle reduction, accumulator update) on top
+        int seg_step = 32, seg_cost = 16;
+        if (const char *e = std::getenv("EPHC_ROW_SEG_STEP")) seg_step = std::max(1, std::atoi(e));
+        if (const char *e = std::getenv("EPHC_ROW_SEG_COST")) seg_cost = std::max(0, std::atoi(e));
         std::vector<int64_t> row_cnt((size_t)r.nrows + 1, 0);
         for (int32_t i = 0; i < r.nrows; ++i) {
             int64_t sum = 0;
-            for (int32_t c = 0; c < nrange; ++c) sum += cnt[(size_t)i * nrange + c];
+            for (int32_t c = 0; c < nrange; ++c) {
+                const int64_t n = cnt[(size_t)i * nrange + c];
+                if (n) sum += (n + seg_step - 1) / seg_step * seg_step + seg_cost;
+            }
             row_cnt[i + 1] = row_cnt[i] + sum;
         }
+        const int64_t work_total = row_cnt[r.nrows];
         // strips of equal entry count (row granularity)
         int Ra_cap = 2048;
         std::vector<int32_t> strip_row0(1, 0);
         for (int s = 1; s <= nstrip; ++s) {
-            const int64_t goal = nent * (int64_t)s / nstrip;
+            const int64_t goal = work_total * (int64_t)s / nstrip;
             int32_t r1 = (int32_t)(std::lower_bound(row_cnt.begin(), row_cnt.end(), goal) - row_cnt.begin());
             r1 = std::max(r1, strip_row0.back());
             if (s == nstrip) r1 = r.nrows;
@@ -92,6 +101,58 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
         const int32_t ns_real = (int32_t)strip_row0.size() - 1;
         r.strips.resize((size_t)ns_real);
         r.Ra = 1;
+        // Sparse staging: a strip needs F of the partner rows its entries reference only.  When that is less than half
+        // of all (strip, partner row) combinations (few partner k per k: large cells), a strip's tiles run over ITS sorted
+        // list of referenced partner rows (cols[]: chunks of Rb list positions) instead of over all rows, the kernels
+        // stage those rows only, and the partner index of an entry is its position in the tile's chunk of the list.
+        std::vector<int32_t> row_strip((size_t)r.nrows, 0);
+        for (int32_t s2 = 0; s2 < ns_real; ++s2)
+            for (int32_t i = strip_row0[s2]; i < strip_row0[s2 + 1]; ++i) row_strip[i] = s2;
+        std::vector<int64_t> cols_off((size_t)ns_real + 1, 0);
+        {
+            // referenced (strip, partner row) combinations: a bitmap per strip
+            const size_t wpr = ((size_t)r.nrows + 63) / 64;
+            std::vector<uint64_t> bits((size_t)ns_real * wpr, 0);
+            for (int64_t e = 0; e < nent; ++e) bits[(size_t)row_strip[drow[e]] * wpr + ((size_t)prow[e] >> 6)] |= 1ull << (prow[e] & 63);
+            int64_t total = 0;
+            for (int32_t s2 = 0; s2 < ns_real; ++s2) {
+                int64_t m = 0;
+                for (size_t k = 0; k < wpr; ++k) m += __builtin_popcountll(bits[(size_t)s2 * wpr + k]);
+                cols_off[s2 + 1] = cols_off[s2] + m;
+                total += m;
+            }
+            const char *force = std::getenv("EPHC_ROW_SPARSE");
+            const bool sparse = force ? std::atoi(force) != 0 : 2 * total < (int64_t)ns_real * r.nrows;
+            if (sparse) {
+                r.cols.resize((size_t)total);
+                for (int32_t s2 = 0; s2 < ns_real; ++s2) {
+                    int64_t o = cols_off[s2];
+                    for (size_t k = 0; k < wpr; ++k)
+                        for (uint64_t wbits = bits[(size_t)s2 * wpr + k]; wbits; wbits &= wbits - 1)
+                            r.cols[o++] = (int32_t)(k * 64 + (size_t)__builtin_ctzll(wbits));
+                }
+            }
+        }
+        const bool sparse = !r.cols.empty();
+        // position of an entry's partner: (chunk of Rb rows, index inside the chunk)
+        auto place = [&](int64_t e, int32_t &c, int32_t &j) {
+            int32_t p = prow[e];
+            if (sparse) {
+                const int32_t s2 = row_strip[drow[e]];
+                const int32_t *b0 = r.cols.data() + cols_off[s2], *b1 = r.cols.data() + cols_off[s2 + 1];
+                p = (int32_t)(std::lower_bound(b0, b1, p) - b0);
+            }
+            c = p / Rb;
+            j = p - c * Rb;
+        };
+        if (sparse) {  // entries per (row, chunk) on the strips' own lists
+            std::fill(cnt.begin(), cnt.end(), 0u);
+            for (int64_t e = 0; e < nent; ++e) {
+                int32_t c, j;
+                place(e, c, j);
+                cnt[(size_t)drow[e] * nrange + c]++;
+            }
+        }
         // per strip: tiles and segments (sorted by descending length), entry offsets
         std::vector<int64_t> seg_abs((size_t)r.nrows * nrange, 0);  // absolute first entry of (row, range)
         int64_t e_run = 0;
@@ -114,8 +175,18 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
                 RowTile tl;
                 tl.seg0 = (int32_t)r.segs.size();
                 tl.nseg = (int32_t)rows.size();
-                tl.col0 = c * Rb;
-                tl.ncols = std::min(Rb, r.nrows - tl.col0);
+                if (sparse) {  // rows cols[col0 .. col0 + ncols) of the strip's list
+                    const int64_t m = cols_off[s + 1] - cols_off[s];
+                    if (cols_off[s] + (int64_t)c * Rb > 0x7fffffffLL) {
+                        err = "row store: partner lists with more than 2^31 rows";
+                        return EPHC_ELIMIT;
+                    }
+                    tl.col0 = (int32_t)(cols_off[s] + (int64_t)c * Rb);
+                    tl.ncols = (int32_t)std::min<int64_t>(Rb, m - (int64_t)c * Rb);
+                } else {
+                    tl.col0 = c * Rb;
+                    tl.ncols = std::min(Rb, r.nrows - tl.col0);
+                }
                 for (const auto &q : rows) {
                     if (e_run - st.e0 > 0xffffffffLL) {
                         err = "row store: strip with more than 2^32 entries";
@@ -135,9 +206,10 @@ int build_rows(const ephc_problem *p, const Dims &d, const GatherHost &g, int ns
         r.wst.resize((size_t)nent);
         r.meta.resize((size_t)nent);
         for (int64_t e = 0; e < nent; ++e) {
-            const int32_t c = prow[e] / Rb;
+            int32_t c, j;
+            place(e, c, j);
             const int64_t o = seg_abs[(size_t)drow[e] * nrange + c]++;
-            r.idx[o] = (uint16_t)(prow[e] - c * Rb);
+            r.idx[o] = (uint16_t)j;
             r.perm[o] = (uint32_t)e;
             r.wst[o] = g.w[e];
             r.meta[o] = pmeta[e];

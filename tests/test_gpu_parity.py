@@ -367,12 +367,15 @@ def test_gpu_channel_selection_matches_oracle_list():
         assert _relerr(G, L.transport_setup(p.f0, p.N)) <= TOL
 
 
-@pytest.mark.parametrize("rng_rows,strips", [(32, 1), (64, 3), (32, 40)])
-def test_row_geometry_on_gpu(monkeypatch, rng_rows, strips):
-    # row store (transport_iter): several partner ranges per strip (restaging between tiles), one strip for everything,
-    # more strips than a problem this small would get; and the fallback without the row store
+@pytest.mark.parametrize("rng_rows,strips,sparse", [(32, 1, None), (64, 3, None), (32, 40, None), (32, 7, 1), (64, 40, 1), (32, 40, 0)])
+def test_row_geometry_on_gpu(monkeypatch, rng_rows, strips, sparse):
+    # row store (transport_setup / transport_iter): several partner ranges per strip (restaging between tiles), one strip
+    # for everything, more strips than a problem this small would get; sparse staging (a strip stages the partner rows it
+    # references only) forced on and off; and the fallback without the row store
     monkeypatch.setenv("EPHC_ROW_RANGE", str(rng_rows))
     monkeypatch.setenv("EPHC_ROW_STRIPS", str(strips))
+    if sparse is not None:
+        monkeypatch.setenv("EPHC_ROW_SPARSE", str(sparse))
     for no_rows in (False, True):
         if no_rows:
             monkeypatch.setenv("EPHC_NO_ROWS", "1")

@@ -240,13 +240,17 @@ def test_res_store_holds_every_weight_once(prob, rows, fine, smem, hcap, mode, m
     assert np.abs(I - Io).max() <= 1e-12 * np.abs(Io).max()
 
 
-@pytest.mark.parametrize("rng_rows,strips", [(None, None), (32, 1), (64, 3), (32, 40)])
-def test_row_store_is_a_regrouping_of_the_gather_store(prob, rng_rows, strips, monkeypatch):
+@pytest.mark.parametrize("rng_rows,strips,sparse", [(None, None, None), (32, 1, None), (64, 3, None), (32, 40, None), (32, 5, 1),
+                                                    (64, 40, 1), (None, None, 1)])
+def test_row_store_is_a_regrouping_of_the_gather_store(prob, rng_rows, strips, sparse, monkeypatch):
     # the store transport_iter runs on: same ordered terms as the gather store (dest, partner), every gather position
-    # exactly once; strips / tiles / segments checked in C (ephc_export_rows)
+    # exactly once; strips / tiles / segments (and, with sparse staging, the strips' partner lists) checked in C
+    # (ephc_export_rows)
     if rng_rows is not None:
         monkeypatch.setenv("EPHC_ROW_RANGE", str(rng_rows))
         monkeypatch.setenv("EPHC_ROW_STRIPS", str(strips))
+    if sparse is not None:
+        monkeypatch.setenv("EPHC_ROW_SPARSE", str(sparse))
     h = ephc.build_channels(prob, flags=ephc.HOST_ONLY)
     g, r = h.export_gather(), h.export_rows()
     assert len(r["dest"]) == len(g["dest"]) > 0
@@ -258,12 +262,14 @@ def test_row_store_is_a_regrouping_of_the_gather_store(prob, rng_rows, strips, m
     assert inside[r["dest"]].all() and inside[r["partner"]].all()
 
 
-@pytest.mark.parametrize("rng_rows,strips", [(None, None), (32, 3), (64, 40)])
+@pytest.mark.parametrize("rng_rows,strips", [(None, None), (32, 3), (64, 40), (-32, 7)])
 def test_collapsed_row_store_sums_every_ordered_term_once(prob, rng_rows, strips, monkeypatch):
     # mode-collapsed specialisation: one entry per (destination, partner) state pair of a segment; the counts are the
     # multiplicities of the pairs in the row store; coverage and adjacency checked in C (ephc_export_rows_collapsed)
     if rng_rows is not None:
-        monkeypatch.setenv("EPHC_ROW_RANGE", str(rng_rows))
+        if rng_rows < 0:     # negative: the same range with sparse staging forced
+            monkeypatch.setenv("EPHC_ROW_SPARSE", "1")
+        monkeypatch.setenv("EPHC_ROW_RANGE", str(abs(rng_rows)))
         monkeypatch.setenv("EPHC_ROW_STRIPS", str(strips))
     h = ephc.build_channels(prob, flags=ephc.HOST_ONLY | ephc.TRANSPORT_COLLAPSE)
     r, c = h.export_rows(), h.export_rows_collapsed()
