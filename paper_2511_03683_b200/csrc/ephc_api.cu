@@ -1698,6 +1698,21 @@ static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStre
                 std::fprintf(stderr, "res timing %-14s mean %9.0f  warp0 %9.0f  last warp %9.0f  max %9.0f cycles per CTA\n", nm[k],
                              mean / (h->x_ncta * nw), w0 / h->x_ncta, wl / h->x_ncta, mx);
             }
+            {   // per CTA: cycles of warp 0 over all sections
+                double mn = 1e30, mx = 0, sum = 0;
+                int imx = 0;
+                for (int c = 0; c < h->x_ncta; ++c) {
+                    double tt = 0;
+                    for (int k = 0; k < 8; ++k) tt += (double)hd[((size_t)c * (nw + 1)) * 8 + k];
+                    if (tt > mx) mx = tt, imx = c;
+                    mn = std::min(mn, tt);
+                    sum += tt;
+                }
+                std::fprintf(stderr, "res timing per CTA total: min %.0f mean %.0f max %.0f (CTA %d) cycles\n", mn, sum / h->x_ncta, mx, imx);
+                std::fprintf(stderr, "res timing slowest CTA %d sections:", imx);
+                for (int k = 0; k < 8; ++k) std::fprintf(stderr, " %lld", hd[((size_t)imx * (nw + 1)) * 8 + k]);
+                std::fprintf(stderr, "\n");
+            }
             const char *pn[6] = {"loop", "wait empty", "dir + bulk", "wait prev", "N staging", "until full"};
             for (int k = 0; k < 6; ++k) {
                 double mean = 0;
