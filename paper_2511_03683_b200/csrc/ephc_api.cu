@@ -373,6 +373,11 @@ static const ResMode kResModes[] = {{256, 2, 112 * 1024}, {512, 1, 225 * 1024}, 
 constexpr int kResNModes = (int)(sizeof(kResModes) / sizeof(kResModes[0]));
 constexpr int kResDefaultMode = 0;
 
+static int upload_res(ephc_handle *h, const ResHost &xh);
+static int calibrate_res(ephc_handle *h, ResHost &xh);
+static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStream_t s, bool fc_ready, long long *tile_cycles);
+static int set_kernel_attributes(int device);
+
 static int make_res_store(ephc_handle *h) {
     if (h->res_built) return EPHC_OK;
     const ephc_problem q = problem_view(h);
@@ -411,11 +416,34 @@ static int make_res_store(ephc_handle *h) {
     h->x_smem_tile = xh.smem_tile;
     h->bytes_res = (int64_t)(xh.blob.size() + xh.iqn.size() * 4 + xh.tiles.size() * sizeof(ResTile) + xh.cta_ptr.size() * 4);
     if (h->host_only) {
+        if (const char *e = std::getenv("EPHC_RES_TEST_RECUT")) {  // structural tests of res_reschedule: pseudo-random tile costs
+            std::vector<double> cost(xh.tiles.size());
+            uint32_t x = (uint32_t)std::atoi(e) * 2654435761u + 12345u;
+            for (double &c : cost) {
+                x = x * 1664525u + 1013904223u;
+                c = 1.0 + (double)(x >> 8) / 65536.0;
+            }
+            rc = res_reschedule(xh, cost, err);
+            if (rc != EPHC_OK) return fail(rc, err);
+        }
         h->rhost = std::move(xh);
         return EPHC_OK;
     }
     if (!h->res_ok) return EPHC_OK;
+    rc = upload_res(h, xh);
+    // Calibration: the shares of the static schedule are re-cut from cycles measured on this device at build (the cost
+    // model of the builder is off by 10-20 % for the slowest CTA).  This build-time step allocates and frees scratch.
+    // Only where a CTA has an SM to itself: with two CTAs per SM a share's time depends on its neighbour and the iteration
+    // does not settle (measured: GaAs 1559 -> 1617 us, large cell 285 -> 297 us; one CTA per SM: Si 104 -> 98.5 us).
+    if (rc == EPHC_OK && h->res_ok && md.ctas == 1 && std::getenv("EPHC_RES_NO_CALIBRATE") == nullptr && xh.tiles.size() > 1)
+        rc = calibrate_res(h, xh);
+    return rc;
+}
+
+static int upload_res(ephc_handle *h, const ResHost &xh) {
+    int rc;
     int64_t bx = 0;
+    h->x_part_rows = xh.part_rows;
     rc = upload(&h->dx_blob, xh.blob, &bx);
     if (rc == EPHC_OK) rc = upload(&h->dx_iqn, xh.iqn, &bx);
     if (rc == EPHC_OK) rc = upload(&h->dx_tiles, xh.tiles, &bx);
@@ -433,6 +461,84 @@ static int make_res_store(ephc_handle *h) {
                           cudaMemset(h->dx_fc, 0, ((size_t)xh.nrows + 4) * 8) != cudaSuccess))
         rc = fail(EPHC_ENOMEM, "cudaMalloc (compact f) failed");
     if (rc != EPHC_OK) h->res_ok = false;
+    return rc;
+}
+
+template <class T>
+static int reupload(T **dst, const std::vector<T> &src) {  // replaces a device array of the handle
+    if (*dst) cudaFree(*dst);
+    *dst = nullptr;
+    int64_t b = 0;
+    return upload(dst, src, &b);
+}
+
+static int calibrate_res(ephc_handle *h, ResHost &xh) {
+    const int64_t ntile = (int64_t)xh.tiles.size();
+    const size_t nN = (size_t)h->d.nq * h->d.nnu * 8;
+    long long *d_cyc = nullptr;
+    double *d_N = nullptr;
+    int rc = EPHC_OK;
+    if (cudaMalloc((void **)&d_cyc, (size_t)ntile * 8) != cudaSuccess || cudaMalloc((void **)&d_N, nN) != cudaSuccess ||
+        cudaMemset(d_N, 0, nN) != cudaSuccess || cudaMemset(d_cyc, 0, (size_t)ntile * 8) != cudaSuccess) {
+        cudaGetLastError();
+        if (d_cyc) cudaFree(d_cyc);
+        if (d_N) cudaFree(d_N);
+        return EPHC_OK;  // no memory for the measurement: the model's schedule stays
+    }
+    if ((rc = set_kernel_attributes(h->device)) == EPHC_OK) {
+        // Fixed-point iteration on the shares: the model's tile costs are scaled by (measured cycles / model work) of
+        // the share they are in, the shares are re-cut, and again.  Sums over a share are robust where single tile
+        // times are not (two CTAs share an SM; waits depend on the neighbours in the pipeline).
+        std::vector<double> cost = xh.tile_work;
+        std::vector<long long> cyc((size_t)ntile);
+        const int64_t launches0 = h->launches;
+        int rounds = 3;
+        if (const char *e = std::getenv("EPHC_RES_CALIB_ROUNDS")) rounds = std::max(0, std::atoi(e));
+        for (int round = 0; round < rounds && rc == EPHC_OK; ++round) {
+            std::vector<double> meas((size_t)ntile, 0.0);
+            for (int r = 0; r < 3 && rc == EPHC_OK; ++r) {  // the first launch warms up
+                rc = launch_res(h, nullptr, d_N, nullptr, true, d_cyc);  // f = 0 (the compact copy was zeroed at upload)
+                if (rc == EPHC_OK && cudaMemcpy(cyc.data(), d_cyc, (size_t)ntile * 8, cudaMemcpyDeviceToHost) != cudaSuccess)
+                    rc = fail(EPHC_ECUDA, "calibration of the resident-tile schedule failed");
+                if (r > 0)
+                    for (int64_t i = 0; i < ntile; ++i) meas[i] += (double)cyc[i];
+            }
+            if (rc != EPHC_OK) break;
+            double tot_m = 0.0, tot_c = 0.0, worst = 0.0;
+            for (int64_t i = 0; i < ntile; ++i) tot_m += meas[i], tot_c += cost[i];
+            for (int32_t c = 0; c < xh.ncta; ++c) {
+                double m = 0.0, w = 0.0;
+                for (int32_t i = xh.cta_ptr[c]; i < xh.cta_ptr[c + 1]; ++i) m += meas[i], w += cost[i];
+                if (w <= 0.0 || m <= 0.0) continue;
+                const double fac = (m / tot_m) / (w / tot_c);  // > 1: this share takes longer than the model says
+                worst = std::max(worst, m);
+                for (int32_t i = xh.cta_ptr[c]; i < xh.cta_ptr[c + 1]; ++i) cost[i] *= fac;
+            }
+            if (std::getenv("EPHC_DEBUG"))
+                std::fprintf(stderr, "res calibration round %d: slowest share %.0f cycles, mean %.0f\n", round, worst / 2, tot_m / 2 / xh.ncta);
+            std::string err;
+            if ((rc = res_reschedule(xh, cost, err)) != EPHC_OK) {
+                rc = fail(rc, err);
+                break;
+            }
+            h->x_part_rows = xh.part_rows;
+            rc = reupload(&h->dx_tiles, xh.tiles);
+            if (rc == EPHC_OK) rc = reupload(&h->dx_cta_ptr, xh.cta_ptr);
+            if (rc == EPHC_OK) rc = reupload(&h->dx_blk_ent_ptr, xh.blk_ent_ptr);
+            if (rc == EPHC_OK) rc = reupload(&h->dx_blk_ent_off, xh.blk_ent_off);
+            if (rc == EPHC_OK) rc = reupload(&h->dx_slot_off, xh.slot_off);
+            if (rc == EPHC_OK) {
+                cudaFree(h->dx_part);
+                h->dx_part = nullptr;
+                if (cudaMalloc((void **)&h->dx_part, (size_t)std::max<int64_t>(1, xh.part_rows) * 8) != cudaSuccess)
+                    rc = fail(EPHC_ENOMEM, "cudaMalloc (resident-tile partial sums) failed");
+            }
+            if (rc != EPHC_OK) h->res_ok = false;
+        }
+        h->launches = launches0;  // build-time launches are not part of the count the callers see
+    }
+    cudaFree(d_cyc);
+    cudaFree(d_N);
     return rc;
 }
 
@@ -1289,12 +1395,12 @@ extern "C" int ephc_export_res(const ephc_handle *h, int32_t *a, int32_t *b, int
             if (((D.flags & 2) != 0) != (it == run.t0 + run.nt - 1) || run.a_row0 % t.Ra != 0 || run.a_rows < 1 || run.a_rows > t.Ra ||
                 D.a_row0 != run.a_row0 || D.a_rows != run.a_rows || D.a_slot != run.a_slot || run.a_slot < 0 ||
                 t.slot_row0[run.a_slot] != run.a_row0 || t.slot_rows[run.a_slot] != run.a_rows ||
-                (it + 1 < t.cta_ptr[cta + 1] ? D.nq_next != t.tiles[it + 1].nq : D.nq_next != 0))
+                (it + 1 < (int32_t)t.tiles.size() ? D.nq_next != t.tiles[it + 1].nq : D.nq_next != 0))
                 return fail(EPHC_ESTATE, "internal: bad run / tile header");
             if (D.flags & 2) ++irun;
             ResTile Dl = D;
             res_set_layout(Dl, t.nwarp);
-            if (D.ncombo < 1 || D.ncombo > D.ne || D.o_sn_next != (it + 1 < t.cta_ptr[cta + 1] ? res_o_sn(t.tiles[it + 1]) : 0u))
+            if (D.ncombo < 1 || D.ncombo > D.ne || D.o_sn_next != (it + 1 < (int32_t)t.tiles.size() ? res_o_sn(t.tiles[it + 1]) : 0u))
                 return fail(EPHC_ESTATE, "internal: where the next tile's N rows go");
             const int32_t R = run.a_rows + D.b_rows;
             if (D.ne < 1 || std::memcmp(&Dl, &D, sizeof(D)) != 0 || (int64_t)D.a_off != t.slot_off[D.a_slot] ||
@@ -1635,7 +1741,7 @@ static int launch_stream(ephc_handle *h, const double *f, const double *N, cudaS
 }
 
 // fc_ready: the compact copy of f (dx_fc) was already written by the finish kernel of the previous RK stage
-static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStream_t s, bool fc_ready = false) {
+static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStream_t s, bool fc_ready = false, long long *tile_cycles = nullptr) {
     if (h->x_ntile > 0) {
         if (!fc_ready) {
             res_compact_kernel<<<(unsigned)((h->x_nrows + 255) / 256), 256, 0, s>>>(f, h->dx_row_state, h->dx_fc, h->x_nrows);
@@ -1660,6 +1766,7 @@ static int launch_res(ephc_handle *h, const double *f, const double *N, cudaStre
         P.fc = h->dx_fc;
         P.N = N;
         P.part = h->dx_part;
+        P.tile_cycles = tile_cycles;
 #ifdef EPHC_RES_TIMING
         static long long *dbg = nullptr;
         const size_t ndbg = (size_t)h->x_ncta * (kResModes[h->x_mode].nl / 32 + 1) * 8;

@@ -329,6 +329,7 @@ struct ResHost {
     std::vector<uint32_t> iqn;        // per (tile, pair): iq * nnu
     std::vector<ResTile> tiles;       // in schedule order: the tiles of CTA c are tiles[cta_ptr[c] .. cta_ptr[c+1])
     std::vector<int32_t> cta_ptr;
+    std::vector<double> tile_work;    // cost-model work of every tile (storage order)
     std::vector<ResRun> runs;
     std::vector<int64_t> slot_off;
     std::vector<int32_t> slot_row0, slot_rows, blk_ent_ptr;
@@ -344,5 +345,6 @@ inline int64_t res_fixed_bytes(int Ra) { return ((int64_t)8 * Ra + 3 * (int64_t)
 inline int64_t res_smem_total(int Ra, int Rcap, int64_t smem_tile) { return res_fixed_bytes(Ra) + 2 * res_buf_bytes(Rcap, smem_tile); }
 int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta, int64_t smem_cap, int nwarp, ResHost &t,
               std::string &err);
+int res_reschedule(ResHost &t, const std::vector<double> &cost, std::string &err);
 
 }  // namespace ephc

@@ -733,6 +733,7 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                         D.b_off = (uint32_t)t.slot_off[D.b_slot];
                     }
                     t.tiles.push_back(D);
+                    t.tile_work.push_back((double)imgs[r.tl[k].first][r.tl[k].second].work);
                     src.push_back(r.tl[k]);
                 }
             }
@@ -751,8 +752,9 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
                 return EPHC_ELIMIT;
             }
         }
-        for (int32_t cta = 0; cta < ncta; ++cta)
-            for (int32_t i = t.cta_ptr[cta]; i + 1 < t.cta_ptr[cta + 1]; ++i) t.tiles[i].nq_next = t.tiles[i + 1].nq;
+        // the pair list of the NEXT tile in storage order rides in every image (the shares are contiguous pieces of that
+        // order, wherever their boundaries are: res_reschedule may move them)
+        for (int64_t i = 0; i + 1 < ntile; ++i) t.tiles[i].nq_next = t.tiles[i + 1].nq;
         for (int64_t i = 0; i < ntile; ++i) {
             ResTile &D = t.tiles[i];
             res_set_layout(D, nwarp);
@@ -761,8 +763,7 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
             t.smem_tile = std::max(t.smem_tile, res_tile_smem(D, nnu));
             t.Rcap = std::max(t.Rcap, D.a_rows + D.b_rows);
         }
-        for (int32_t cta = 0; cta < ncta; ++cta)
-            for (int32_t i = t.cta_ptr[cta]; i + 1 < t.cta_ptr[cta + 1]; ++i) t.tiles[i].o_sn_next = res_o_sn(t.tiles[i + 1]);
+        for (int64_t i = 0; i + 1 < ntile; ++i) t.tiles[i].o_sn_next = res_o_sn(t.tiles[i + 1]);
         if (t.smem_tile > per_buf) {
             err = "internal: resident tile exceeds its shared-memory budget";
             return EPHC_ESTATE;
@@ -782,11 +783,10 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
             std::memcpy(dst + D.o_w, im.blob.data() + D0.o_w, (size_t)(D0.blob_bytes - (int32_t)D0.o_w));
             std::copy(im.iqn.begin(), im.iqn.end(), t.iqn.begin() + D.q0);
         }
-        for (int32_t cta = 0; cta < ncta; ++cta)  // the next tile's iq list rides in the image of its predecessor
-            for (int32_t i = t.cta_ptr[cta]; i + 1 < t.cta_ptr[cta + 1]; ++i) {
-                const ResTile &D = t.tiles[i], &Dn = t.tiles[i + 1];
-                std::memcpy(t.blob.data() + D.blob_off + D.o_nxt, t.iqn.data() + Dn.q0, (size_t)Dn.nq * 4);
-            }
+        for (int64_t i = 0; i + 1 < ntile; ++i) {  // the next tile's iq list rides in the image of its predecessor
+            const ResTile &D = t.tiles[i], &Dn = t.tiles[i + 1];
+            std::memcpy(t.blob.data() + D.blob_off + D.o_nxt, t.iqn.data() + Dn.q0, (size_t)Dn.nq * 4);
+        }
         imgs.clear();
         t.part_rows = rows;
         if (rows > 0xffffffffLL) {
@@ -846,6 +846,90 @@ int build_res(const ephc_problem *p, const Dims &d, const Canonical &c, int ncta
         return EPHC_ENOMEM;
     }
     t.supported = true;
+    return EPHC_OK;
+}
+
+// Re-cuts the static schedule: the tiles keep their storage order and images; the contiguous shares get new boundaries
+// of equal cost (cost[i] per stored tile, e.g. cycles measured on the device), and what depends on the boundaries -- the
+// runs (consecutive tiles of one strip inside a share), their flags, the partial-sum slots and the per-block slot
+// lists of the finish kernel -- is rebuilt.  Order of additions: per state still fixed by the tables, so a handle is
+// bit-reproducible from call to call; two handles with different boundaries group the partial sums differently.
+int res_reschedule(ResHost &t, const std::vector<double> &cost, std::string &err) {
+    const int64_t ntile = (int64_t)t.tiles.size();
+    const int32_t ncta = t.ncta, Rf = t.rf;
+    if ((int64_t)cost.size() != ntile || ncta < 1 || Rf < 1) {
+        err = "internal: res_reschedule arguments";
+        return EPHC_ESTATE;
+    }
+    try {
+        double total = 0.0;
+        for (double c : cost) total += std::max(c, 0.0);
+        t.cta_ptr.assign((size_t)ncta + 1, 0);
+        t.runs.clear();
+        t.slot_off.clear();
+        t.slot_row0.clear();
+        t.slot_rows.clear();
+        int64_t rows = 0;
+        auto new_slot = [&](int32_t row0, int32_t nrows_) {
+            const int32_t sl = (int32_t)t.slot_off.size();
+            t.slot_off.push_back(rows);
+            t.slot_row0.push_back(row0);
+            t.slot_rows.push_back(nrows_);
+            rows += nrows_;
+            return sl;
+        };
+        int32_t cta = 0, cur_strip = -1;
+        double done = 0.0;
+        for (int64_t i = 0; i < ntile; ++i) {
+            ResTile &D = t.tiles[i];
+            const double wk = std::max(cost[i], 0.0);
+            bool cut = false;
+            while (cta + 1 < ncta && done + 0.5 * wk > total * (double)(cta + 1) / ncta) {
+                ++cta;
+                t.cta_ptr[cta] = (int32_t)i;
+                cut = true;
+            }
+            if (cut || D.a_row0 != cur_strip || i == 0) {
+                if (!t.runs.empty()) t.tiles[i - 1].flags |= 2;  // the previous tile was the last of its run
+                t.runs.push_back(ResRun{(int32_t)i, 0, D.a_row0, D.a_rows, new_slot(D.a_row0, D.a_rows), cta});
+                cur_strip = D.a_row0;
+                D.flags = 1;
+            } else {
+                D.flags = 0;
+            }
+            ResRun &run = t.runs.back();
+            run.nt++;
+            D.a_slot = run.a_slot;
+            D.a_off = (uint32_t)t.slot_off[run.a_slot];
+            D.b_slot = -1;
+            D.b_off = 0;
+            if (D.b_rows > 0) {
+                D.b_slot = new_slot(D.b_row0, D.b_rows);
+                D.b_off = (uint32_t)t.slot_off[D.b_slot];
+            }
+            done += wk;
+        }
+        if (ntile > 0) t.tiles[ntile - 1].flags |= 2;
+        while (cta + 1 <= ncta) t.cta_ptr[++cta] = (int32_t)ntile;  // shares left without tiles
+        t.part_rows = rows;
+        if (rows > 0xffffffffLL) {
+            err = "resident-tile store: partial-sum buffer exceeds 2^32 rows";
+            return EPHC_ELIMIT;
+        }
+        t.blk_ent_ptr.assign((size_t)t.nblk + 1, 0);
+        const int64_t nslot = (int64_t)t.slot_off.size();
+        for (int64_t sl = 0; sl < nslot; ++sl)
+            for (int32_t b = t.slot_row0[sl] / Rf; b * Rf < t.slot_row0[sl] + t.slot_rows[sl]; ++b) t.blk_ent_ptr[b + 1]++;
+        for (int32_t b = 0; b < t.nblk; ++b) t.blk_ent_ptr[b + 1] += t.blk_ent_ptr[b];
+        t.blk_ent_off.assign((size_t)t.blk_ent_ptr[t.nblk], 0);
+        std::vector<int32_t> cur(t.blk_ent_ptr.begin(), t.blk_ent_ptr.end() - 1);
+        for (int64_t sl = 0; sl < nslot; ++sl)
+            for (int32_t b = t.slot_row0[sl] / Rf; b * Rf < t.slot_row0[sl] + t.slot_rows[sl]; ++b)
+                t.blk_ent_off[cur[b]++] = t.slot_off[sl] + (t.blk_row0[b] - t.slot_row0[sl]);
+    } catch (const std::bad_alloc &) {
+        err = "host allocation failed (resident-tile schedule)";
+        return EPHC_ENOMEM;
+    }
     return EPHC_OK;
 }
 

@@ -39,6 +39,7 @@ struct ResParams {
     const double *fc;       // f in compact row order (padded to an even number of rows)
     const double *N;
     double *part;
+    long long *tile_cycles; // calibration (null otherwise): cycles the consumers spent on every tile, in storage order
 #ifdef EPHC_RES_TIMING
     long long *dbg;         // per CTA: cycles spent in 8 sections (working builds only)
 #endif
@@ -238,6 +239,7 @@ __global__ void __launch_bounds__(NL + kResProducerThreads, CTAS) res_kernel(con
 #endif
     const int lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NL / 32;
+    long long cyc0 = P.tile_cycles != nullptr ? clock64() : 0;
     for (int i = 0; i < n; ++i) {
         const int b = i & 1;
         unsigned char *buf = buf_of(b);
@@ -402,6 +404,11 @@ __global__ void __launch_bounds__(NL + kResProducerThreads, CTAS) res_kernel(con
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         __syncwarp();
         if (lane == 0) mbar_arrive(&sEmpty[b]);
+        if (P.tile_cycles != nullptr && tid == 0) {  // from the end of the previous tile to the end of this one (waits included)
+            const long long cyc1 = clock64();
+            P.tile_cycles[i0 + i] = cyc1 - cyc0;
+            cyc0 = cyc1;
+        }
         EPHC_TICK(7)
     }
 #ifdef EPHC_RES_TIMING

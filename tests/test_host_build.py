@@ -209,6 +209,10 @@ def test_res_store_holds_every_weight_once(prob, rows, fine, smem, hcap, mode, m
     for k, v in (("EPHC_RES_SMEM", smem), ("EPHC_RES_HCAP", hcap), ("EPHC_RES_MODE", mode)):
         if v is not None:
             monkeypatch.setenv(k, str(v))
+    if mode in (1, 4, 6):
+        # the schedule re-cut that device handles do from measured tile times (res_reschedule), here with pseudo-random
+        # costs: the export below checks runs, flags, slots and slot lists of the new shares
+        monkeypatch.setenv("EPHC_RES_TEST_RECUT", str(mode))
     L = oracle.OracleList(prob)
     h = ephc.build_channels(prob, flags=ephc.HOST_ONLY)
     t = h.export_res()        # also checks the tile images: slabs of both phases, padding, gather lists, slots, coverage
