@@ -383,8 +383,11 @@ static int make_res_store(ephc_handle *h) {
     const ephc_problem q = problem_view(h);
     std::string err;
     ResHost xh;
-    // Launch mode: two CTAs of 8 consumer warps per SM overlap best; when the rows of a half-size tile would carry fewer
-    // than about six entries (sparse, few channels per pair), one CTA of 16 warps with tiles twice as large wins.
+    // Launch mode (measured on B200 with the calibrated schedule, collision call in us for modes 0 / 1 / 2 / 3):
+    //   many channels per pair (large cell: 285 / 297 / 290 / 288): two CTAs of 8 consumer warps per SM;
+    //   few channels per pair: ONE CTA per SM with tiles twice as large and shares calibrated on the device --
+    //   8 consumer warps when the rows of a tile are long (GaAs-like: 1534 / 1559 / 1440 / 1481), 12 when a half-size
+    //   tile's rows would carry fewer than about six entries (Si-like: 105 / 98.9 / 99.6 / 97.1).
     h->x_mode = kResDefaultMode;
     {
         int64_t nrows = 0;
@@ -392,7 +395,7 @@ static int make_res_store(ephc_handle *h) {
         const double per_pair = (double)h->can.nw / (double)std::max<int64_t>(1, h->can.npair_active);
         const double rho = (double)h->can.nw / (0.5 * (double)nrows * (double)nrows + 1.0);
         const double fit = 44000.0 / (15.5 + 8.0 * h->d.nnu / std::max(1.0, per_pair));
-        if (per_pair < 64.0 && std::sqrt(rho * fit) < 6.0) h->x_mode = 1;
+        if (per_pair < 64.0) h->x_mode = std::sqrt(rho * fit) < 6.0 ? 3 : 2;
     }
     if (const char *e = std::getenv("EPHC_RES_MODE")) h->x_mode = std::min(kResNModes - 1, std::max(0, std::atoi(e)));
     const ResMode &md = kResModes[h->x_mode];
