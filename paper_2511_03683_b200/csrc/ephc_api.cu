@@ -2100,7 +2100,24 @@ extern "C" int ephc_transport_iters(ephc_handle *h, const double *F_dev, const d
             if (!rdbg) cudaMalloc((void **)&rdbg, 4 * 8 * 1024);
             R.dbg = rdbg;
 #endif
-            row_iter_kernel<<<(unsigned)std::max(h->r_nstrip, 1), kRowThreads, row_smem_bytes(h->r_Rb, h->r_Ra), s>>>(R);
+            if (it > 0 && std::getenv("EPHC_ROW_NO_PDL") == nullptr) {
+                // programmatic dependent launch: iteration it may take an SM as soon as a CTA of iteration it - 1 leaves it
+                // (the kernel itself waits for the previous launch to complete before it reads F)
+                cudaLaunchConfig_t cfg;
+                std::memset(&cfg, 0, sizeof(cfg));
+                cfg.gridDim = dim3((unsigned)std::max(h->r_nstrip, 1));
+                cfg.blockDim = dim3(kRowThreads);
+                cfg.dynamicSmemBytes = row_smem_bytes(h->r_Rb, h->r_Ra);
+                cfg.stream = s;
+                cudaLaunchAttribute attr[1];
+                attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                attr[0].val.programmaticStreamSerializationAllowed = 1;
+                cfg.attrs = attr;
+                cfg.numAttrs = 1;
+                CUDA_TRY(cudaLaunchKernelEx(&cfg, row_iter_kernel, R));
+            } else {
+                row_iter_kernel<<<(unsigned)std::max(h->r_nstrip, 1), kRowThreads, row_smem_bytes(h->r_Rb, h->r_Ra), s>>>(R);
+            }
             h->launches++;
 #ifdef EPHC_ROW_TIMING
             if (it == niter / 2 && std::getenv("EPHC_ROW_TIMING_PRINT")) {

@@ -212,6 +212,11 @@ __global__ void __launch_bounds__(kRowThreads, 1024 / kRowThreads) row_iter_kern
     const int sub = lane / kRowGroup, gl = lane % kRowGroup;
     constexpr int GPW = 32 / kRowGroup;  // row groups per warp
 
+    // Chained iterations are launched with programmatic stream serialization: the next launch may take an SM as soon as
+    // this CTA leaves it, and waits here until the previous launch has completed and its F is visible (plain launches:
+    // both instructions do nothing).
+    asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
     // states outside the window receive no contribution: F' = tau v (grid-stride over all states)
     if (P.out != nullptr)
         for (int64_t s = (int64_t)blockIdx.x * kRowThreads + tid; s < P.ns; s += (int64_t)gridDim.x * kRowThreads)
