@@ -2132,6 +2132,16 @@ extern "C" int ephc_transport_iters(ephc_handle *h, const double *F_dev, const d
                 }
                 std::fprintf(stderr, "row timing (ns): entry spread %llu, first entry -> last exit %llu, exit spread %llu; per CTA prologue %.0f loop %.0f epilogue %.0f\n",
                              e1 - e0, x1 - e0, x1 - x0, pro / h->r_nstrip, loop / h->r_nstrip, epi / h->r_nstrip);
+                {   // the slowest and fastest strips (is the spread tied to the strip?)
+                    std::vector<std::pair<unsigned long long, int>> tt;
+                    for (int k = 0; k < h->r_nstrip; ++k) tt.push_back({hd[4 * k + 3] - hd[4 * k], k});
+                    std::sort(tt.begin(), tt.end());
+                    std::fprintf(stderr, "row timing fastest:");
+                    for (int k = 0; k < 4; ++k) std::fprintf(stderr, " %d:%llu", tt[k].second, tt[k].first);
+                    std::fprintf(stderr, "  slowest:");
+                    for (int k = 0; k < 6; ++k) std::fprintf(stderr, " %d:%llu", tt[tt.size() - 1 - k].second, tt[tt.size() - 1 - k].first);
+                    std::fprintf(stderr, "\n");
+                }
             }
 #endif
         }
